@@ -1,0 +1,210 @@
+"""ctypes/numpy wrapper around oracle/semoracle.c.
+
+TEST INFRASTRUCTURE ONLY (see the header of semoracle.c): imported by tests/,
+__graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs.  The product
+package (paper_2501_13240_b200) never imports this module.
+
+Every function takes and returns host numpy arrays (fp64 / int32), laid out as the C file
+states: local node l = e*Np + k*n1^2 + j*n1 + i ("(ijk) ordering").
+"""
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "semoracle.c")
+_LIB = os.path.join(_HERE, "libsemoracle.so")
+_lib = None
+
+
+def build(force=False):
+    """Compile semoracle.c -> libsemoracle.so (gcc -O2, OpenMP, no FP contraction)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-ffp-contract=off", "-fPIC", "-shared",
+               "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+class _Op(C.Structure):
+    _fields_ = [("E", C.c_int64), ("N", C.c_int32), ("pad_", C.c_int32), ("n", C.c_int64),
+                ("n_unique", C.c_int64), ("geo", C.c_void_p), ("D", C.c_void_p), ("gid", C.c_void_p),
+                ("mask", C.c_void_p), ("invmult", C.c_void_p), ("lam", C.c_double)]
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = C.CDLL(_LIB)
+        _lib.orc_min_spacing.restype = C.c_double
+        _lib.orc_dot.restype = C.c_double
+        _lib.orc_geo.restype = C.c_int64
+        _lib.orc_numbering.restype = C.c_int64
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p) if a is not None else None
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def num_threads():
+    return int(lib().orc_num_threads())
+
+
+def gll(N):
+    """c-1: (xi, rho), each [N+1]."""
+    xi = np.zeros(N + 1); rho = np.zeros(N + 1)
+    assert lib().orc_gll(C.c_int(N), _p(xi), _p(rho)) == 0
+    return xi, rho
+
+
+def dhat(N, xi=None):
+    """c-2: D[i, j] = l'_j(xi_i), [N+1, N+1]."""
+    if xi is None:
+        xi = gll(N)[0]
+    D = np.zeros((N + 1, N + 1))
+    assert lib().orc_dhat(C.c_int(N), _p(_f64(xi)), _p(D)) == 0
+    return D
+
+
+def geo_factors(E, N, x, y, z):
+    """c-3: geo [E, 7, Np]; raises ValueError on a non-positive Jacobian."""
+    xi, rho = gll(N); D = dhat(N, xi)
+    Np = (N + 1) ** 3
+    x, y, z = _f64(x), _f64(y), _f64(z)
+    geo = np.zeros((E, 7, Np))
+    bad = lib().orc_geo(C.c_int64(E), C.c_int(N), _p(x), _p(y), _p(z), _p(D), _p(rho), _p(geo))
+    if bad >= 0:
+        raise ValueError(f"non-positive Jacobian in element {bad}")
+    return geo
+
+
+def axhelm(E, N, geo, lam, u, lam0=None, lam1=None, D=None):
+    """c-4: w = D^T G D u + lam B u on every element."""
+    if D is None:
+        D = dhat(N)
+    u = _f64(u); w = np.zeros_like(u)
+    l0 = _f64(lam0) if lam0 is not None else None
+    l1 = _f64(lam1) if lam1 is not None else None
+    lib().orc_axhelm(C.c_int64(E), C.c_int(N), _p(geo), _p(_f64(D)), C.c_double(lam), _p(l0), _p(l1), _p(u), _p(w))
+    return w
+
+
+def min_spacing(E, N, x, y, z):
+    return float(lib().orc_min_spacing(C.c_int64(E), C.c_int(N), _p(_f64(x)), _p(_f64(y)), _p(_f64(z))))
+
+
+def numbering(E, N, x, y, z, period, tol=None):
+    """c-6: (gid int32 [n], n_unique).  tol defaults to 1e-8 * min node spacing."""
+    x, y, z = _f64(x), _f64(y), _f64(z)
+    if tol is None:
+        tol = 1e-8 * min_spacing(E, N, x, y, z)
+    per = _f64(period)
+    gid = np.zeros(E * (N + 1) ** 3, dtype=np.int32)
+    nu = lib().orc_numbering(C.c_int64(E), C.c_int(N), _p(x), _p(y), _p(z), _p(per), C.c_double(tol), _p(gid))
+    if nu < 0:
+        raise ValueError("coordinate matching is not an equivalence relation at this tolerance")
+    return gid, int(nu)
+
+
+def gs(gid, n_unique, w):
+    """c-7: QQ^T w (returns a new array)."""
+    out = _f64(w).copy()
+    lib().orc_gs(C.c_int64(out.size), _p(gid), C.c_int64(n_unique), _p(out))
+    return out
+
+
+def dirichlet_mask(E, N, face_tag, tags, gid, n_unique):
+    mask = np.zeros(E * (N + 1) ** 3)
+    ft = np.ascontiguousarray(face_tag, dtype=np.int32)
+    lib().orc_mask(C.c_int64(E), C.c_int(N), _p(ft), C.c_uint32(tags), _p(gid), C.c_int64(n_unique), _p(mask))
+    return mask
+
+
+def diag_local(E, N, geo, lam, D=None):
+    if D is None:
+        D = dhat(N)
+    d = np.zeros(E * (N + 1) ** 3)
+    lib().orc_diag_local(C.c_int64(E), C.c_int(N), _p(geo), _p(_f64(D)), C.c_double(lam), _p(d))
+    return d
+
+
+def minmax_hist(v, nbins, lo, hi):
+    v = _f64(v); mm = np.zeros(2); h = np.zeros(nbins, dtype=np.uint64)
+    lib().orc_minmax_hist(C.c_int64(v.size), _p(v), C.c_int(nbins), C.c_double(lo), C.c_double(hi), _p(mm), _p(h))
+    return mm[0], mm[1], h
+
+
+def vmag(vx, vy, vz):
+    vx, vy, vz = _f64(vx), _f64(vy), _f64(vz); out = np.zeros_like(vx)
+    lib().orc_vmag(C.c_int64(vx.size), _p(vx), _p(vy), _p(vz), _p(out))
+    return out
+
+
+class Problem:
+    """Mesh + operator state of the oracle: geo, numbering, mask, invmult, dinv (c-3 .. c-8)."""
+
+    def __init__(self, E, N, x, y, z, face_tag, period, lam=0.0, dirichlet_tags=0, gid=None):
+        self.E, self.N, self.Np = E, N, (N + 1) ** 3
+        self.n = E * self.Np
+        self.xi, self.rho = gll(N)
+        self.D = dhat(N, self.xi)
+        self.geo = geo_factors(E, N, x, y, z)
+        if gid is None:
+            self.gid, self.n_unique = numbering(E, N, x, y, z, period)
+        else:
+            self.gid = np.ascontiguousarray(gid, dtype=np.int32); self.n_unique = int(self.gid.max()) + 1
+        self.face_tag = np.ascontiguousarray(face_tag, dtype=np.int32)
+        self.invmult = np.zeros(self.n)
+        lib().orc_invmult(C.c_int64(self.n), _p(self.gid), C.c_int64(self.n_unique), _p(self.invmult))
+        self.set_operator(lam, dirichlet_tags)
+
+    def set_operator(self, lam, dirichlet_tags):
+        self.lam, self.tags = float(lam), int(dirichlet_tags)
+        self.mask = dirichlet_mask(self.E, self.N, self.face_tag, self.tags, self.gid, self.n_unique)
+        self._op = _Op(self.E, self.N, 0, self.n, self.n_unique, _p(self.geo), _p(self.D), _p(self.gid),
+                       _p(self.mask), _p(self.invmult), self.lam)
+        self.dinv = np.zeros(self.n)
+        lib().orc_dinv(C.byref(self._op), _p(self.dinv))
+
+    def apply_A(self, v):
+        v = _f64(v); out = np.zeros(self.n); tmp = np.zeros(self.n)
+        lib().orc_apply_A(C.byref(self._op), _p(v), _p(out), _p(tmp))
+        return out
+
+    def dot(self, a, b):
+        return float(lib().orc_dot(C.byref(self._op), _p(_f64(a)), _p(_f64(b))))
+
+    def assemble_rhs(self, f):
+        b = np.zeros(self.n)
+        lib().orc_assemble_rhs(C.byref(self._op), _p(_f64(f)), _p(b))
+        return b
+
+    def cheb_jacobi(self, k, lmax, r):
+        z = np.zeros(self.n); work = np.zeros(4 * self.n)
+        lib().orc_cheb_jacobi(C.byref(self._op), C.c_int(k), C.c_double(lmax), _p(self.dinv), _p(_f64(r)), _p(z), _p(work))
+        return z
+
+    def lanczos_lmax(self, v0, steps=10):
+        """largest Ritz value of D^-1/2 A D^-1/2 after `steps` Lanczos steps, times 1.1 (c-10)."""
+        a = np.zeros(steps); b = np.zeros(steps)
+        m = lib().orc_lanczos(C.byref(self._op), _p(self.dinv), _p(_f64(v0)), C.c_int(steps), _p(a), _p(b))
+        T = np.diag(a[:m]) + np.diag(b[:m - 1], 1) + np.diag(b[:m - 1], -1)
+        return 1.1 * float(np.linalg.eigvalsh(T)[-1])
+
+    def pcg(self, b, x0=None, precond=1, cheb_k=2, lmax=0.0, rtol=1e-10, atol=0.0, maxit=10000, hist_len=0):
+        """c-9.  Returns dict(x, iters, status, r0, rn, hist)."""
+        x = np.zeros(self.n) if x0 is None else _f64(x0).copy()
+        hist = np.zeros(max(hist_len, 1)); out3 = np.zeros(3)
+        st = lib().orc_pcg(C.byref(self._op), C.c_int(precond), C.c_int(cheb_k), C.c_double(lmax), _p(self.dinv),
+                           _p(_f64(b)), _p(x), C.c_double(rtol), C.c_double(atol), C.c_int(maxit),
+                           C.c_int(1 if x0 is None else 0), _p(hist), C.c_int(hist_len), _p(out3))
+        it = int(out3[0])
+        return dict(x=x, iters=it, status=int(st), r0=out3[1], rn=out3[2], hist=hist[:min(hist_len, it + 1)])
