@@ -1,0 +1,213 @@
+/*
+ * semb200.h — C ABI of libsemb200.so: the B200-native (sm_100a, fp64) spectral-element
+ * Poisson/Helmholtz hot path of arxiv/paper_2501_13240 (NekRS runs of Rayleigh-Benard convection).
+ *
+ * The call list follows BASELINE.json:north_star — mesh/setup(E, N, coords, boundary tags),
+ * apply_axhelm, gather_scatter, pcg_solve, export_field — and the paper's hand-off protocol
+ * (§3.1, Listing 2: register device pointers once, set state/cycle and
+ * state/time and publish per analysis step, close at exit; PAPER.md:L128 zero-copy; L171-177 the
+ * consumer must know which memory space a pointer lives in).
+ *
+ * Conventions
+ *   - Every function returns int: 0 = SEMB_OK, < 0 an error, > 0 a status with valid outputs.
+ *   - "device" pointers are CUDA device memory of the current device, OWNED BY THE CALLER, never
+ *     freed or retained beyond the call unless the call says so (semb_publish_field retains the
+ *     pointer, not the memory).  "host" pointers are ordinary host memory.
+ *   - Mesh-derived arrays are owned by the handle until semb_destroy.
+ *   - All work is enqueued on the caller's stream (a cudaStream_t passed as void*; NULL = default
+ *     stream).  Only semb_setup, semb_pcg_solve, semb_estimate_lmax and the *_host calls synchronise.
+ *   - Layout ("(ijk) ordering on [-1,1]^3"): local node l = e*Np + k*n1*n1 + j*n1 + i,
+ *     n1 = N+1, Np = n1^3, i fastest; n = E*Np local nodes; all fields fp64, indices int32.
+ *   - There is no CPU fallback: with no CUDA device every compute call returns SEMB_ECUDA.
+ */
+#ifndef SEMB200_H
+#define SEMB200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define SEMB_API __attribute__((visibility("default")))
+#else
+#define SEMB_API
+#endif
+
+#define SEMB_OK          0
+#define SEMB_MAXIT       1   /* pcg_solve: maxit reached, outputs valid                     */
+#define SEMB_EINVAL     -1   /* bad argument                                                */
+#define SEMB_ENOMEM     -2   /* allocation failed                                           */
+#define SEMB_ECUDA      -3   /* CUDA runtime error (see semb_last_error)                    */
+#define SEMB_EGEOM      -4   /* non-positive Jacobian (semb_last_error names the element)   */
+#define SEMB_EBREAKDOWN -5   /* PCG breakdown: p.Ap <= 0 or not finite                      */
+#define SEMB_EMATCH     -6   /* coordinate matching is not an equivalence at this tolerance */
+#define SEMB_ENOTFOUND  -7   /* export_field: no such field                                 */
+
+#define SEMB_MAX_N      10   /* PAPER.md:L204 §4.1: polynomial order p <= 10                */
+
+typedef struct semb_mesh* semb_handle;
+
+/* Optional allocator for every device buffer the library owns (so that e.g. torch's caching
+ * allocator owns all memory).  NULL => cudaMalloc/cudaFree. */
+typedef struct {
+    void* (*alloc)(size_t bytes, void* user);
+    void  (*free)(void* ptr, void* user);
+    void*  user;
+} semb_allocator;
+
+/* ---- basis (host) ------------------------------------------------------------------------
+ * GLL nodes xi[N+1], weights rho[N+1] and the derivative matrix D[(N+1)*(N+1)], D[i*n1+j] =
+ * l'_j(xi_i) (PAPER.md:L85 GLL quadrature; L100 "(p+1)x(p+1) operator matrices identical for
+ * all elements").  The diagonal is minus the off-diagonal row sum (reading R2).
+ * Host pointers; any may be NULL.  1 <= N <= SEMB_MAX_N else SEMB_EINVAL. */
+SEMB_API int semb_gll(int N, double* xi, double* rho, double* D);
+
+/* ---- setup (PAPER.md:L85, L100 chain rule for deformed elements, L102 inter-element exchange) --
+ * x, y, z     device [n]   node coordinates, layout above.
+ * face_tag    HOST   [E*6] faces r-,r+,s-,s+,t-,t+ ; 0 = none/interior/periodic, 1..31 = user id.
+ * period      HOST   [3]   0 = not periodic, else the period length in that direction.
+ * gid_or_null device [n]   optional caller-supplied global ids (int32, any labels >= 0 that are
+ *                          equal exactly on coincident nodes); skips coordinate matching.  The
+ *                          library still renumbers to canonical first-touch ids.
+ * Computes (device, handle-owned): geometric factors G_rr,G_rs,G_rt,G_ss,G_st,G_tt,B per node,
+ * canonical global ids, gather lists, inverse multiplicity.  Synchronises the stream.
+ * Errors: SEMB_EINVAL, SEMB_ENOMEM, SEMB_ECUDA, SEMB_EGEOM, SEMB_EMATCH (*out = NULL on error). */
+SEMB_API int semb_setup(int64_t E, int N, const double* x, const double* y, const double* z,
+               const int32_t* face_tag, const double* period, const int32_t* gid_or_null,
+               const semb_allocator* alloc_or_null, void* stream, semb_handle* out);
+
+/* Frees everything the handle owns ("close").  NULL is a no-op. */
+SEMB_API int semb_destroy(semb_handle h);
+
+/* Message of the last error on this handle (or of the last failed semb_setup if h == NULL).
+ * The string is owned by the library. */
+SEMB_API const char* semb_last_error(semb_handle h);
+
+typedef struct {
+    int64_t E; int32_t N; int32_t n1; int64_t Np; int64_t n;
+    int64_t n_unique;      /* number of global nodes                                        */
+    int64_t n_shared;      /* local nodes whose global node has >= 2 copies                 */
+    int64_t n_gs;          /* global nodes with >= 2 copies                                  */
+    double  tol;           /* matching tolerance used (1e-8 * smallest node spacing)        */
+    const int32_t* gid;       /* device [n]  canonical global ids                            */
+    const double*  geo;       /* device [E][7][Np]: G_rr,G_rs,G_rt,G_ss,G_st,G_tt,B          */
+    const double*  invmult;   /* device [n]  1 / multiplicity                                */
+    const int32_t* gs_offsets;/* device [n_gs+1] CSR offsets into gs_ids                     */
+    const int32_t* gs_ids;    /* device [n_shared] local ids, classes by gid, members ascending */
+} semb_info;
+SEMB_API int semb_mesh_info(semb_handle h, semb_info* out);
+
+/* ---- the local operator (north_star: per element w = D^T G D u + lambda B u) ----
+ * u, w   device [nfields][n], w != u.  lambda == 0 and no coefficient fields selects the
+ *        6-factor Poisson kernel (64 B/node), otherwise the 7-factor Helmholtz kernel (72 B/node).
+ * lambda0_or_null, lambda1_or_null  device [n]: per-node coefficients, w = D^T(lambda0 G)D u +
+ *        lambda1 B u (reading R3); with lambda1 == NULL the scalar lambda multiplies B.
+ * Element-local: no assembly, no mask.  Asynchronous on stream. */
+SEMB_API int semb_apply_axhelm(semb_handle h, double lambda, const double* lambda0_or_null,
+                      const double* lambda1_or_null, const double* u, double* w, int nfields,
+                      void* stream);
+
+/* ---- direct-stiffness summation QQ^T -------------------------------------
+ * w device [nfields][n], in place: every copy of a global node receives the sum of all copies,
+ * summed in ascending local index (deterministic, no atomics). */
+SEMB_API int semb_gather_scatter(semb_handle h, double* w, int nfields, void* stream);
+
+/* w[l] = 0 at every local node whose global node lies on a face whose tag t has bit t set in
+ * dirichlet_tags (PAPER.md:L238 isothermal / no-slip plates). */
+SEMB_API int semb_apply_mask(semb_handle h, uint32_t dirichlet_tags, double* w, int nfields, void* stream);
+
+/* b = M QQ^T (B o f): right-hand side from nodal values f (device [n]); b device [n], b != f. */
+SEMB_API int semb_assemble_rhs(semb_handle h, uint32_t dirichlet_tags, const double* f, double* b, void* stream);
+
+/* out = M QQ^T A_L (M v): the assembled masked operator (v, out device [n], out != v). */
+SEMB_API int semb_apply_operator(semb_handle h, double lambda, uint32_t dirichlet_tags, const double* v,
+                        double* out, void* stream);
+
+/* dinv_out device [n] = 1 / (QQ^T diag(D^T G D + lambda B)), 1 at masked nodes (Jacobi). */
+SEMB_API int semb_jacobi_diag(semb_handle h, double lambda, uint32_t dirichlet_tags, double* dinv_out, void* stream);
+
+/* ---- PCG (the pressure Poisson solve; north_star: Jacobi / Chebyshev-Jacobi PCG) ----- */
+typedef struct {
+    double   lambda;          /* operator D^T G D + lambda B                                     */
+    uint32_t dirichlet_tags;  /* bit t set => faces tagged t are Dirichlet (homogeneous)         */
+    int32_t  precond;         /* 0 none, 1 Jacobi, 2 Chebyshev-Jacobi                            */
+    int32_t  cheb_degree;     /* k operator applications per preconditioner application          */
+    double   cheb_lmax;       /* upper bound of spec(D^-1 A); <= 0 => 10-step Lanczos x 1.1      */
+    double   rtol, atol;      /* stop when ||r|| <= max(rtol ||b||, atol) (unique-node 2-norm)   */
+    int32_t  maxit;
+    int32_t  x0_is_zero;      /* 1: ignore the contents of x and start from 0                    */
+    int32_t  check_every;     /* iterations enqueued between host polls of the stop flag; <= 0 => 16.
+                                 The iteration count returned is exact regardless.               */
+    int32_t  reserved;
+} semb_pcg_opts;
+
+typedef struct {
+    int32_t iters;            /* iterations performed                                            */
+    int32_t status;           /* same as the return value                                        */
+    double  b_norm, r0_norm, r_norm, lmax_used;
+    double* hist_host_or_null;/* in: host buffer [hist_len] for ||r_it||, it = 0..; may be NULL   */
+    int32_t hist_len;
+    int32_t reserved;
+} semb_pcg_stats;
+
+/* b device [n]: assembled, masked right-hand side.  x device [n]: in = initial guess (continuous,
+ * zero at Dirichlet nodes) unless x0_is_zero, out = solution.  Returns SEMB_OK (converged),
+ * SEMB_MAXIT, SEMB_EBREAKDOWN, or an error.  Synchronises only to poll the stop flag. */
+SEMB_API int semb_pcg_solve(semb_handle h, const semb_pcg_opts* opts, const double* b, double* x,
+                   semb_pcg_stats* stats, void* stream);
+
+/* 1.1 x the largest Ritz value of D^-1/2 A D^-1/2 after `steps` Lanczos steps from the continuous,
+ * masked start vector v0 (device [n]). */
+SEMB_API int semb_estimate_lmax(semb_handle h, double lambda, uint32_t dirichlet_tags, const double* v0,
+                       int steps, double* lmax_out, void* stream);
+
+/* z = Chebyshev-Jacobi(k) preconditioner applied to r (device [n] each, z != r). */
+SEMB_API int semb_cheb_jacobi(semb_handle h, double lambda, uint32_t dirichlet_tags, int k, double lmax,
+                     const double* r, double* z, void* stream);
+
+/* ---- in-situ hand-off ---------------------------------------- */
+#define SEMB_F64          1
+#define SEMB_MEM_HOST     0
+#define SEMB_MEM_DEVICE   1
+
+typedef struct {
+    const char* name;    /* owned by the handle                                    */
+    void*       ptr;     /* for a registered field: exactly the pointer registered */
+    int32_t     dtype;   /* SEMB_F64                                               */
+    int32_t     memspace;/* SEMB_MEM_DEVICE                    */
+    int64_t     count, stride;   /* elements; stride in elements                   */
+    int64_t     cycle;   /* state/cycle of the last publish_state  */
+    double      time;    /* state/time                            */
+} semb_field_desc;
+
+/* Register a device array under a name once.  Names "velocity_x|y|z" additionally
+ * define the derived field "velocity_magnitude" (library-owned buffer, allocated here, not later). */
+SEMB_API int semb_publish_field(semb_handle h, const char* name, double* dev_ptr, int64_t count);
+/* Per analysis step: records cycle/time and refreshes derived fields with one
+ * kernel on stream.  Steps that do no analysis simply do not call it. */
+SEMB_API int semb_publish_state(semb_handle h, int64_t cycle, double time, void* stream);
+/* No copy, no allocation, no synchronisation, no launch. */
+SEMB_API int semb_export_field(semb_handle h, const char* name, semb_field_desc* out);
+/* In-device consumer: min, max and an nbins histogram of the field over [lo, hi] (values outside go
+ * to the end bins); bin = min(nbins-1, floor((v - lo) * (nbins / (hi - lo)))).
+ * minmax_dev device [2], hist_dev device [nbins] (uint64).  Results stay on the device.
+ * If lo >= hi the range [min, max] found by the first pass is used (two passes). */
+SEMB_API int semb_field_minmax_hist(const semb_field_desc* f, int nbins, double lo, double hi,
+                           double* minmax_dev, uint64_t* hist_dev, void* stream);
+
+/* ---- convenience: the same calls with HOST buffers (copies inside; used for end-to-end timing) */
+SEMB_API int semb_apply_axhelm_host(semb_handle h, double lambda, const double* u_host, double* w_host);
+
+/* Blocking copy of `bytes` bytes from device memory (e.g. a semb_info view) to host memory. */
+SEMB_API int semb_read_device(const void* dev, void* host, size_t bytes);
+
+/* Library version and the compute capability it was built for ("sm_100a"). */
+SEMB_API const char* semb_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SEMB200_H */

@@ -1,0 +1,103 @@
+// In-situ hand-off (§2.3 zero-copy; L138-159 §3.1 Listing 2: device pointers registered once,
+// state/cycle + state/time + publish per analysis step) and the in-device consumer north_star names:
+// min / max / histogram of a field, plus the derived field velocity_magnitude.
+#include <math.h>
+
+#include "semb_internal.h"
+
+// |v| = sqrt(fma(vz, vz, fma(vy, vy, vx*vx)))  (reading R11: the fma form is part of the definition)
+__global__ void k_vmag(int64_t n, const double* __restrict__ vx, const double* __restrict__ vy,
+                       const double* __restrict__ vz, double* __restrict__ out)
+{
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
+        const double a = vx[l], b = vy[l], c = vz[l];
+        out[l] = sqrt(fma(c, c, fma(b, b, __dmul_rn(a, a))));
+    }
+}
+
+int semb_vmag_launch(const double* vx, const double* vy, const double* vz, double* out, int64_t n, cudaStream_t s)
+{
+    int64_t b = (n + 1023) / 1024; if (b > 148 * 8) b = 148 * 8; if (b < 1) b = 1;
+    k_vmag<<<(unsigned)b, 256, 0, s>>>(n, vx, vy, vz, out);
+    return cudaGetLastError() == cudaSuccess ? SEMB_OK : SEMB_ECUDA;
+}
+
+__device__ __forceinline__ unsigned long long enc(double v)
+{
+    unsigned long long u = (unsigned long long)__double_as_longlong(v);
+    return (u & 0x8000000000000000ull) ? ~u : (u | 0x8000000000000000ull);
+}
+__device__ __forceinline__ double dec(unsigned long long o)
+{
+    unsigned long long u = (o & 0x8000000000000000ull) ? (o & 0x7fffffffffffffffull) : ~o;
+    return __longlong_as_double((long long)u);
+}
+
+__global__ void k_mm_init(unsigned long long* mm) { mm[0] = ~0ull; mm[1] = 0ull; }
+__global__ void k_mm_decode(unsigned long long* mm)
+{
+    const double a = dec(mm[0]), b = dec(mm[1]);
+    ((double*)mm)[0] = a; ((double*)mm)[1] = b;
+}
+
+__global__ void __launch_bounds__(256)
+k_minmax(int64_t n, int64_t stride, const double* __restrict__ v, unsigned long long* __restrict__ mm)
+{
+    double mn = INFINITY, mx = -INFINITY;
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
+        const double a = v[l * stride];
+        mn = fmin(mn, a); mx = fmax(mx, a);
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        mn = fmin(mn, __shfl_xor_sync(0xffffffffu, mn, o));
+        mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    }
+    __shared__ double smn[8], smx[8];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane == 0) { smn[wid] = mn; smx[wid] = mx; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 8; ++w) { mn = fmin(mn, smn[w]); mx = fmax(mx, smx[w]); }
+        atomicMin(&mm[0], enc(mn)); atomicMax(&mm[1], enc(mx));
+    }
+}
+
+// bin = min(nbins-1, floor((v - lo) * scale)), scale = nbins / (hi - lo); v < lo -> bin 0.
+// The subtraction and the multiplication are rounded separately (no fused multiply-add).
+__global__ void __launch_bounds__(256)
+k_hist(int64_t n, int64_t stride, const double* __restrict__ v, int nbins, double lo, double hi,
+       const double* __restrict__ range_dev, unsigned long long* __restrict__ hist)
+{
+    extern __shared__ unsigned int sh[];
+    for (int b = threadIdx.x; b < nbins; b += blockDim.x) sh[b] = 0u;
+    if (range_dev) { lo = range_dev[0]; hi = range_dev[1]; }
+    const double scale = __ddiv_rn((double)nbins, __dsub_rn(hi, lo));
+    __syncthreads();
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
+        const double t = __dsub_rn(v[l * stride], lo);
+        const double sc = __dmul_rn(t, scale);
+        long long b = (sc < 0.0) ? 0ll : (long long)floor(sc);
+        if (b > nbins - 1) b = nbins - 1;
+        atomicAdd(&sh[b], 1u);
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < nbins; b += blockDim.x) if (sh[b]) atomicAdd(&hist[b], (unsigned long long)sh[b]);
+}
+
+int semb_minmax_hist_launch(const double* v, int64_t n, int64_t stride, int nbins, double lo, double hi,
+                            double* minmax_dev, uint64_t* hist_dev, cudaStream_t s)
+{
+    if (nbins < 1 || nbins > 8192 || n < 1 || stride < 1) return SEMB_EINVAL;
+    // each block's shared counters are 32-bit: keep every block's share of the input below 2^32
+    int64_t blocks = (n + 2047) / 2048; if (blocks > 148 * 8) blocks = 148 * 8; if (blocks < 1) blocks = 1;
+    unsigned long long* mm = (unsigned long long*)minmax_dev;
+    k_mm_init<<<1, 1, 0, s>>>(mm);
+    k_minmax<<<(unsigned)blocks, 256, 0, s>>>(n, stride, v, mm);
+    k_mm_decode<<<1, 1, 0, s>>>(mm);
+    if (cudaMemsetAsync(hist_dev, 0, sizeof(uint64_t) * nbins, s) != cudaSuccess) return SEMB_ECUDA;
+    const bool own_range = !(lo < hi);
+    k_hist<<<(unsigned)blocks, 256, sizeof(unsigned int) * nbins, s>>>(n, stride, v, nbins, lo, hi,
+                                                                      own_range ? minmax_dev : nullptr,
+                                                                      (unsigned long long*)hist_dev);
+    return cudaGetLastError() == cudaSuccess ? SEMB_OK : SEMB_ECUDA;
+}

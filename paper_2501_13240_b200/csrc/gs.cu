@@ -1,0 +1,41 @@
+// gather-scatter QQ^T (direct-stiffness summation; §2.2 "surface-element data exchange ...
+// complete residual on subdomain surface") as a sorted-offset segmented sum, and the Dirichlet mask
+// (§4.1).  No atomics: one thread owns one global node, sums its copies in ascending local
+// index and writes the sum back to every copy, so the result is deterministic.
+#include "semb_internal.h"
+
+__global__ void k_gs(int64_t n_gs, int64_t n, const int32_t* __restrict__ off, const int32_t* __restrict__ ids,
+                     double* __restrict__ w)
+{
+    const int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (g >= n_gs) return;
+    double* __restrict__ wf = w + blockIdx.y * n;
+    const int32_t a = off[g], b = off[g + 1];
+    double s = 0.0;
+    for (int32_t t = a; t < b; ++t) s += wf[ids[t]];
+    for (int32_t t = a; t < b; ++t) wf[ids[t]] = s;
+}
+
+int semb_gs_launch(semb_mesh* h, double* w, int nfields, cudaStream_t s)
+{
+    if (h->n_gs == 0) return SEMB_OK;
+    dim3 grid((unsigned)((h->n_gs + 255) / 256), (unsigned)nfields);
+    k_gs<<<grid, 256, 0, s>>>(h->n_gs, h->n, h->gs_off, h->gs_ids, w);
+    SEMB_CUDA(h, cudaGetLastError());
+    return SEMB_OK;
+}
+
+__global__ void k_mask(int64_t c, int64_t n, const int32_t* __restrict__ list, double* __restrict__ w)
+{
+    const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (t < c) w[blockIdx.y * n + list[t]] = 0.0;
+}
+
+int semb_mask_launch(semb_mesh* h, const semb_mask_entry& m, double* w, int nfields, cudaStream_t s)
+{
+    if (m.count == 0) return SEMB_OK;
+    dim3 grid((unsigned)((m.count + 255) / 256), (unsigned)nfields);
+    k_mask<<<grid, 256, 0, s>>>(m.count, h->n, m.list, w);
+    SEMB_CUDA(h, cudaGetLastError());
+    return SEMB_OK;
+}

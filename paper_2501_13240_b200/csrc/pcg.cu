@@ -1,0 +1,396 @@
+// Preconditioned conjugate gradients on the assembled, masked operator A = M QQ^T A_L M with Jacobi or
+// Chebyshev-Jacobi preconditioning (BASELINE.json:north_star; §2.2: the pressure Poisson
+// solve is the stiffest sub-step, Chebyshev-accelerated smoothers).  Vectors live in local (redundant)
+// storage and are continuous; <a,b> = sum_l a_l b_l / mult_l.
+//
+// alpha, beta, the residual norm, the iteration counter and the stop flag stay in device memory
+// (semb_scalars).  Every kernel of the loop returns at once when the stop flag is set, so the host can
+// enqueue `check_every` iterations between polls and the iteration count is still exact.
+#include <math.h>
+#include <string.h>
+
+#include "reduce.cuh"
+#include "semb_internal.h"
+
+#define VEC_BLOCK 256
+static inline unsigned vec_grid(int64_t n)
+{
+    int64_t b = (n + VEC_BLOCK * 4 - 1) / (VEC_BLOCK * 4);
+    if (b < 1) b = 1;
+    if (b > 148 * 8) b = 148 * 8;
+    return (unsigned)b;
+}
+#define GSTRIDE(l, n) for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < (n); l += (int64_t)gridDim.x * blockDim.x)
+#define STOPPED(scal) (*(volatile int32_t*)&(scal)->done)
+
+// r = b (x = 0) or r = b - q (q = A x0);  bb, rr, rz
+__global__ void __launch_bounds__(VEC_BLOCK)
+k_pcg_init(int64_t n, const double* __restrict__ b, const double* __restrict__ q, double* __restrict__ x,
+           double* __restrict__ r, const double* __restrict__ invmult, const double* __restrict__ dinv,
+           semb_scalars* __restrict__ scal, double* __restrict__ partials, double* __restrict__ hist)
+{
+    __shared__ double red[32];
+    double bb = 0.0, rr = 0.0, rz = 0.0;
+    GSTRIDE(l, n) {
+        const double bl = b[l], w = invmult[l];
+        double rl = bl;
+        if (q) rl -= q[l]; else x[l] = 0.0;
+        r[l] = rl;
+        bb += bl * bl * w; rr += rl * rl * w;
+        rz += (dinv ? dinv[l] : 1.0) * rl * rl * w;
+    }
+    double v[3] = { block_sum(bb, red), block_sum(rr, red), block_sum(rz, red) }, tot[3];
+    if (grid_sum<3>(v, partials, &scal->ticket[1], tot, red) && threadIdx.x == 0) {
+        scal->bnorm = sqrt(tot[0]); scal->rr = tot[1]; scal->rnorm = sqrt(tot[1]); scal->r0norm = scal->rnorm;
+        scal->target = fmax(scal->rtol * scal->bnorm, scal->atol);
+        scal->rho_old = 0.0; scal->rho_new = tot[2]; scal->rz = tot[2]; scal->beta = 0.0; scal->alpha = 0.0;
+        scal->iter = 0; scal->status = SEMB_MAXIT;
+        scal->done = 0;
+        if (hist) hist[0] = scal->rnorm;
+        if (scal->rnorm <= scal->target) { scal->done = 1; scal->status = SEMB_OK; }
+    }
+}
+
+// p = z + beta p,  z = dinv o r (Jacobi), r (none) or a given z (Chebyshev)
+__global__ void __launch_bounds__(VEC_BLOCK)
+k_update_p(int64_t n, const double* __restrict__ zsrc, const double* __restrict__ dinv, double* __restrict__ p,
+           const semb_scalars* __restrict__ scal)
+{
+    if (STOPPED(scal)) return;
+    const double beta = scal->beta;
+    if (beta == 0.0) { GSTRIDE(l, n) p[l] = dinv ? dinv[l] * zsrc[l] : zsrc[l]; }
+    else             { GSTRIDE(l, n) p[l] = (dinv ? dinv[l] * zsrc[l] : zsrc[l]) + beta * p[l]; }
+}
+
+// x += alpha p; r -= alpha q; rr = <r,r>, rz = <r, dinv r>; the last block closes the iteration
+template <bool FUSED_Z>
+__global__ void __launch_bounds__(VEC_BLOCK)
+k_update_xr(int64_t n, const double* __restrict__ p, const double* __restrict__ q, double* __restrict__ x,
+            double* __restrict__ r, const double* __restrict__ invmult, const double* __restrict__ dinv,
+            semb_scalars* __restrict__ scal, double* __restrict__ partials, double* __restrict__ hist, int hist_cap)
+{
+    __shared__ double red[32];
+    if (STOPPED(scal)) return;
+    const double alpha = scal->alpha;
+    double rr = 0.0, rz = 0.0;
+    GSTRIDE(l, n) {
+        x[l] += alpha * p[l];
+        const double rl = r[l] - alpha * q[l];
+        r[l] = rl;
+        const double t = rl * rl * invmult[l];
+        rr += t;
+        if (FUSED_Z) rz += (dinv ? dinv[l] : 1.0) * t;
+    }
+    double v[2] = { block_sum(rr, red), block_sum(rz, red) }, tot[2];
+    if (grid_sum<2>(v, partials, &scal->ticket[2], tot, red) && threadIdx.x == 0) {
+        const int it = scal->iter + 1;
+        scal->iter = it;
+        scal->rr = tot[0]; scal->rnorm = sqrt(tot[0]);
+        if (hist && it < hist_cap) hist[it] = scal->rnorm;
+        scal->rho_old = scal->rho_new;
+        if (FUSED_Z) { scal->rho_new = tot[1]; scal->rz = tot[1]; scal->beta = tot[1] / scal->rho_old; }
+        if (scal->rnorm <= scal->target) { scal->done = 1; scal->status = SEMB_OK; }
+        else if (it >= scal->maxit) { scal->done = 1; scal->status = SEMB_MAXIT; }
+    }
+}
+
+// rho_new = <r,z>, beta = rho_new / rho_old (0 in the first iteration)   [Chebyshev path]
+__global__ void __launch_bounds__(VEC_BLOCK)
+k_dot_rz(int64_t n, const double* __restrict__ r, const double* __restrict__ z, const double* __restrict__ invmult,
+         semb_scalars* __restrict__ scal, double* __restrict__ partials)
+{
+    __shared__ double red[32];
+    if (STOPPED(scal)) return;
+    double s = 0.0;
+    GSTRIDE(l, n) s += r[l] * z[l] * invmult[l];
+    double v[1] = { block_sum(s, red) }, tot[1];
+    if (grid_sum<1>(v, partials, &scal->ticket[3], tot, red) && threadIdx.x == 0) {
+        scal->rho_new = tot[0]; scal->rz = tot[0];
+        scal->beta = (scal->iter == 0) ? 0.0 : tot[0] / scal->rho_old;
+    }
+}
+
+// plain weighted dot product into scal->aux (Lanczos, tests)
+__global__ void __launch_bounds__(VEC_BLOCK)
+k_dot_aux(int64_t n, const double* __restrict__ a, const double* __restrict__ b, const double* __restrict__ invmult,
+          semb_scalars* __restrict__ scal, double* __restrict__ partials)
+{
+    __shared__ double red[32];
+    double s = 0.0;
+    GSTRIDE(l, n) s += a[l] * b[l] * invmult[l];
+    double v[1] = { block_sum(s, red) }, tot[1];
+    if (grid_sum<1>(v, partials, &scal->ticket[4], tot, red) && threadIdx.x == 0) scal->aux = tot[0];
+}
+
+// ---- Chebyshev-Jacobi(k), 1st-kind recurrence on [0.1 lmax, lmax] (reading R9):
+// z = 0; res = r; d = dinv o res / theta; k x { z += d; res -= A d; d = c1 d + c2 dinv o res }; z += d
+__global__ void __launch_bounds__(VEC_BLOCK)
+k_cheb_init(int64_t n, const double* __restrict__ r, const double* __restrict__ dinv, double itheta,
+            double* __restrict__ res, double* __restrict__ d, double* __restrict__ z, int last,
+            const semb_scalars* __restrict__ scal)
+{
+    if (scal && STOPPED(scal)) return;
+    GSTRIDE(l, n) {
+        const double rl = r[l], dl = dinv[l] * rl * itheta;
+        res[l] = rl; d[l] = dl; z[l] = last ? dl : 0.0;
+    }
+}
+__global__ void __launch_bounds__(VEC_BLOCK)
+k_cheb_step(int64_t n, const double* __restrict__ Ad, const double* __restrict__ dinv, double c1, double c2,
+            double* __restrict__ res, double* __restrict__ d, double* __restrict__ z, int last,
+            const semb_scalars* __restrict__ scal)
+{
+    if (scal && STOPPED(scal)) return;
+    GSTRIDE(l, n) {
+        const double dl = d[l];
+        double zl = z[l] + dl;
+        const double rl = res[l] - Ad[l];
+        const double dn = c1 * dl + c2 * (dinv[l] * rl);
+        res[l] = rl; d[l] = dn;
+        if (last) zl += dn;
+        z[l] = zl;
+    }
+}
+
+// ---- small vector kernels for Lanczos / operator application
+__global__ void k_copy(int64_t n, const double* __restrict__ a, double* __restrict__ out) { GSTRIDE(l, n) out[l] = a[l]; }
+__global__ void k_scale(int64_t n, double c, const double* __restrict__ a, double* __restrict__ out) { GSTRIDE(l, n) out[l] = c * a[l]; }
+__global__ void k_sqrt_scale(int64_t n, const double* __restrict__ dinv, const double* __restrict__ a, double* __restrict__ out)
+{ GSTRIDE(l, n) out[l] = sqrt(dinv[l]) * a[l]; }
+// w = sqrt(dinv) w - bprev vold
+__global__ void k_lanczos_a(int64_t n, const double* __restrict__ dinv, double bprev, const double* __restrict__ vold, double* __restrict__ w)
+{ GSTRIDE(l, n) w[l] = sqrt(dinv[l]) * w[l] - bprev * vold[l]; }
+__global__ void k_axpy(int64_t n, double a, const double* __restrict__ x, double* __restrict__ y) { GSTRIDE(l, n) y[l] += a * x[l]; }
+
+int semb_ensure_work(semb_mesh* h, int64_t vecs)
+{
+    if (!h->scal) {
+        h->scal = (semb_scalars*)semb_dev_alloc(h, sizeof(semb_scalars));
+        h->partials = (double*)semb_dev_alloc(h, sizeof(double) * 4 * SEMB_MAX_BLOCKS);
+        if (!h->scal || !h->partials) return semb_fail(h, SEMB_ENOMEM, "solver scalars");
+        SEMB_CUDA(h, cudaMemset(h->scal, 0, sizeof(semb_scalars)));
+        SEMB_CUDA(h, cudaMallocHost((void**)&h->scal_host, sizeof(semb_scalars)));
+    }
+    if (vecs > h->work_vecs) {
+        if (h->work) semb_dev_free(h, h->work);
+        h->work = (double*)semb_dev_alloc(h, sizeof(double) * (size_t)vecs * (size_t)h->n);
+        if (!h->work) { h->work_vecs = 0; return semb_fail(h, SEMB_ENOMEM, "solver workspace: %lld vectors", (long long)vecs); }
+        h->work_vecs = vecs;
+    }
+    return SEMB_OK;
+}
+
+// out = M QQ^T A_L (M v); tmp: one work vector
+static int apply_A(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* v_masked, double* out,
+                   semb_scalars* scal, cudaStream_t s)
+{
+    int rc = semb_axhelm_launch(h, lambda, nullptr, nullptr, v_masked, out, 1, scal, s); if (rc) return rc;
+    rc = semb_gs_launch(h, out, 1, s); if (rc) return rc;
+    return semb_mask_launch(h, m, out, 1, s);
+}
+
+int semb_operator_run(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* v, double* out, cudaStream_t s)
+{
+    int rc = semb_ensure_work(h, 1); if (rc) return rc;
+    double* tmp = h->work;
+    k_copy<<<vec_grid(h->n), VEC_BLOCK, 0, s>>>(h->n, v, tmp);
+    rc = semb_mask_launch(h, m, tmp, 1, s); if (rc) return rc;
+    return apply_A(h, lambda, m, tmp, out, nullptr, s);
+}
+
+struct cheb_coef { double itheta; double c1[16], c2[16]; };
+static cheb_coef cheb_coefficients(int k, double lmax)
+{
+    cheb_coef c;
+    const double lmin = 0.1 * lmax, theta = 0.5 * (lmax + lmin), delta = 0.5 * (lmax - lmin), sigma = theta / delta;
+    double rho = 1.0 / sigma;
+    c.itheta = 1.0 / theta;
+    for (int it = 0; it < k && it < 16; ++it) {
+        const double rho1 = 1.0 / (2.0 * sigma - rho);
+        c.c1[it] = rho1 * rho; c.c2[it] = 2.0 * rho1 / delta;
+        rho = rho1;
+    }
+    return c;
+}
+
+// z = Cheb_k(r);  res, d, Ad: work vectors
+static int cheb_apply(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* dinv, int k, const cheb_coef& c,
+                      const double* r, double* z, double* res, double* d, double* Ad, semb_scalars* scal, cudaStream_t s)
+{
+    const int64_t n = h->n;
+    k_cheb_init<<<vec_grid(n), VEC_BLOCK, 0, s>>>(n, r, dinv, c.itheta, res, d, z, k == 0, scal);
+    for (int it = 0; it < k; ++it) {
+        int rc = semb_axhelm_launch(h, lambda, nullptr, nullptr, d, Ad, 1, nullptr, s); if (rc) return rc;
+        rc = semb_gs_launch(h, Ad, 1, s); if (rc) return rc;
+        rc = semb_mask_launch(h, m, Ad, 1, s); if (rc) return rc;
+        k_cheb_step<<<vec_grid(n), VEC_BLOCK, 0, s>>>(n, Ad, dinv, c.c1[it], c.c2[it], res, d, z, it == k - 1, scal);
+    }
+    SEMB_CUDA(h, cudaGetLastError());
+    return SEMB_OK;
+}
+
+int semb_cheb_run(semb_mesh* h, double lambda, uint32_t tags, int k, double lmax, const double* r, double* z, cudaStream_t s)
+{
+    if (k < 0 || k > 16 || !(lmax > 0.0)) return semb_fail(h, SEMB_EINVAL, "cheb_jacobi: k=%d lmax=%g", k, lmax);
+    semb_mask_entry m; double* dinv;
+    int rc = semb_get_mask(h, tags, &m, s); if (rc) return rc;
+    rc = semb_get_dinv(h, lambda, tags, &dinv, s); if (rc) return rc;
+    rc = semb_ensure_work(h, 3); if (rc) return rc;
+    const int64_t n = h->n;
+    return cheb_apply(h, lambda, m, dinv, k, cheb_coefficients(k, lmax), r, z, h->work, h->work + n, h->work + 2 * n, nullptr, s);
+}
+
+// largest eigenvalue of the symmetric tridiagonal (a[0..m), b[0..m-1)) by bisection on the Sturm count
+static double tridiag_lmax(int m, const double* a, const double* b)
+{
+    double lo = a[0], hi = a[0];
+    for (int i = 0; i < m; ++i) {
+        const double rad = (i > 0 ? fabs(b[i - 1]) : 0.0) + (i + 1 < m ? fabs(b[i]) : 0.0);
+        if (a[i] - rad < lo) lo = a[i] - rad;
+        if (a[i] + rad > hi) hi = a[i] + rad;
+    }
+    for (int it = 0; it < 200 && hi - lo > 1e-15 * fmax(fabs(hi), fabs(lo)); ++it) {
+        const double mid = 0.5 * (lo + hi);
+        int below = 0; double q = a[0] - mid;               // number of eigenvalues < mid
+        if (q < 0.0) ++below;
+        for (int i = 1; i < m; ++i) {
+            if (q == 0.0) q = 1e-300;
+            q = a[i] - mid - b[i - 1] * b[i - 1] / q;
+            if (q < 0.0) ++below;
+        }
+        if (below == m) hi = mid; else lo = mid;
+    }
+    return 0.5 * (lo + hi);
+}
+
+static int dot_to_host(semb_mesh* h, const double* a, const double* b, double* out, cudaStream_t s)
+{
+    k_dot_aux<<<vec_grid(h->n), VEC_BLOCK, 0, s>>>(h->n, a, b, h->invmult, h->scal, h->partials);
+    SEMB_CUDA(h, cudaMemcpyAsync(h->scal_host, h->scal, sizeof(semb_scalars), cudaMemcpyDeviceToHost, s));
+    SEMB_CUDA(h, cudaStreamSynchronize(s));
+    *out = h->scal_host->aux;
+    return SEMB_OK;
+}
+
+// Lanczos on D^-1/2 A D^-1/2: v = v0/||v0||; per step  t = D^-1/2 v; w = D^-1/2 A t - beta_{j-1} v_{j-1};
+// alpha_j = <w,v>; w -= alpha_j v; beta_j = ||w||; v_{j+1} = w / beta_j.   lmax = 1.1 x largest Ritz value.
+int semb_lanczos_run(semb_mesh* h, double lambda, uint32_t tags, const double* v0, int steps, double* lmax, cudaStream_t s)
+{
+    if (steps < 1 || steps > 64) return semb_fail(h, SEMB_EINVAL, "lanczos steps=%d", steps);
+    semb_mask_entry m; double* dinv;
+    int rc = semb_get_mask(h, tags, &m, s); if (rc) return rc;
+    rc = semb_get_dinv(h, lambda, tags, &dinv, s); if (rc) return rc;
+    rc = semb_ensure_work(h, 4); if (rc) return rc;
+    const int64_t n = h->n; const unsigned G = vec_grid(n);
+    double *v = h->work, *vold = v + n, *w = v + 2 * n, *t = v + 3 * n;
+    double nrm2, a[64], b[64];
+    rc = dot_to_host(h, v0, v0, &nrm2, s); if (rc) return rc;
+    k_scale<<<G, VEC_BLOCK, 0, s>>>(n, 1.0 / sqrt(nrm2), v0, v);
+    SEMB_CUDA(h, cudaMemsetAsync(vold, 0, sizeof(double) * (size_t)n, s));
+    double bprev = 0.0; int msteps = 0;
+    for (int j = 0; j < steps; ++j) {
+        k_sqrt_scale<<<G, VEC_BLOCK, 0, s>>>(n, dinv, v, t);
+        rc = apply_A(h, lambda, m, t, w, nullptr, s); if (rc) return rc;
+        k_lanczos_a<<<G, VEC_BLOCK, 0, s>>>(n, dinv, bprev, vold, w);
+        rc = dot_to_host(h, w, v, &a[j], s); if (rc) return rc;
+        k_axpy<<<G, VEC_BLOCK, 0, s>>>(n, -a[j], v, w);
+        double bb; rc = dot_to_host(h, w, w, &bb, s); if (rc) return rc;
+        b[j] = sqrt(bb);
+        msteps = j + 1;
+        if (!(b[j] > 0.0)) break;
+        k_copy<<<G, VEC_BLOCK, 0, s>>>(n, v, vold);
+        k_scale<<<G, VEC_BLOCK, 0, s>>>(n, 1.0 / b[j], w, v);
+        bprev = b[j];
+    }
+    SEMB_CUDA(h, cudaGetLastError());
+    *lmax = 1.1 * tridiag_lmax(msteps, a, b);
+    return SEMB_OK;
+}
+
+int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* x, semb_pcg_stats* st, cudaStream_t s)
+{
+    const int64_t n = h->n; const unsigned G = vec_grid(n);
+    if (o->precond < 0 || o->precond > 2 || o->maxit < 0 || (o->precond == 2 && (o->cheb_degree < 0 || o->cheb_degree > 16)))
+        return semb_fail(h, SEMB_EINVAL, "pcg: precond=%d cheb_degree=%d maxit=%d", o->precond, o->cheb_degree, o->maxit);
+    semb_mask_entry m; double* dinv = nullptr;
+    int rc = semb_get_mask(h, o->dirichlet_tags, &m, s); if (rc) return rc;
+    if (o->precond >= 1) { rc = semb_get_dinv(h, o->lambda, o->dirichlet_tags, &dinv, s); if (rc) return rc; }
+    rc = semb_ensure_work(h, o->precond == 2 ? 6 : 3); if (rc) return rc;
+    double *r = h->work, *p = r + n, *q = r + 2 * n;
+    double *z = nullptr, *res = nullptr, *d = nullptr;
+    if (o->precond == 2) { z = r + 3 * n; res = r + 4 * n; d = r + 5 * n; }
+
+    double lmax = o->cheb_lmax;
+    cheb_coef cc{};
+    if (o->precond == 2) {
+        if (!(lmax > 0.0)) {
+            // start vector of the estimator: the right-hand side (continuous, masked)
+            rc = semb_lanczos_run(h, o->lambda, o->dirichlet_tags, b, 10, &lmax, s); if (rc) return rc;
+            r = h->work; p = r + n; q = r + 2 * n; z = r + 3 * n; res = r + 4 * n; d = r + 5 * n;
+        }
+        cc = cheb_coefficients(o->cheb_degree, lmax);
+    }
+    // history buffer
+    const int want_hist = (st && st->hist_host_or_null && st->hist_len > 0) ? st->hist_len : 0;
+    if (want_hist > h->hist_cap) {
+        if (h->hist_dev) semb_dev_free(h, h->hist_dev);
+        h->hist_dev = (double*)semb_dev_alloc(h, sizeof(double) * (size_t)want_hist);
+        if (!h->hist_dev) { h->hist_cap = 0; return semb_fail(h, SEMB_ENOMEM, "residual history"); }
+        h->hist_cap = want_hist;
+    }
+    double* hist = want_hist ? h->hist_dev : nullptr;
+
+    semb_scalars init; memset(&init, 0, sizeof(init));
+    init.rtol = o->rtol; init.atol = o->atol; init.maxit = o->maxit; init.status = SEMB_MAXIT;
+    SEMB_CUDA(h, cudaMemcpyAsync(h->scal, &init, sizeof(init), cudaMemcpyHostToDevice, s));
+
+    const double* dz = (o->precond == 1) ? dinv : nullptr;      // fused z = dinv o r
+    if (!o->x0_is_zero) {
+        rc = apply_A(h, o->lambda, m, x, q, nullptr, s); if (rc) return rc;
+        k_pcg_init<<<G, VEC_BLOCK, 0, s>>>(n, b, q, x, r, h->invmult, dz, h->scal, h->partials, hist);
+    } else {
+        k_pcg_init<<<G, VEC_BLOCK, 0, s>>>(n, b, nullptr, x, r, h->invmult, dz, h->scal, h->partials, hist);
+    }
+    SEMB_CUDA(h, cudaGetLastError());
+
+    const int check = o->check_every > 0 ? o->check_every : 16;
+    bool finished = (o->maxit == 0);
+    for (int it0 = 0; it0 < o->maxit && !finished; it0 += check) {
+        const int mbatch = (o->maxit - it0 < check) ? o->maxit - it0 : check;
+        for (int i = 0; i < mbatch; ++i) {
+            if (o->precond == 2) {
+                rc = cheb_apply(h, o->lambda, m, dinv, o->cheb_degree, cc, r, z, res, d, q, h->scal, s); if (rc) return rc;
+                k_dot_rz<<<G, VEC_BLOCK, 0, s>>>(n, r, z, h->invmult, h->scal, h->partials);
+                k_update_p<<<G, VEC_BLOCK, 0, s>>>(n, z, nullptr, p, h->scal);
+            } else {
+                k_update_p<<<G, VEC_BLOCK, 0, s>>>(n, r, dz, p, h->scal);
+            }
+            rc = semb_axhelm_launch(h, o->lambda, nullptr, nullptr, p, q, 1, h->scal, s); if (rc) return rc;
+            rc = semb_gs_launch(h, q, 1, s); if (rc) return rc;
+            rc = semb_mask_launch(h, m, q, 1, s); if (rc) return rc;
+            if (o->precond == 2) k_update_xr<false><<<G, VEC_BLOCK, 0, s>>>(n, p, q, x, r, h->invmult, nullptr, h->scal, h->partials, hist, want_hist);
+            else                 k_update_xr<true><<<G, VEC_BLOCK, 0, s>>>(n, p, q, x, r, h->invmult, dz, h->scal, h->partials, hist, want_hist);
+        }
+        SEMB_CUDA(h, cudaGetLastError());
+        SEMB_CUDA(h, cudaMemcpyAsync(h->scal_host, h->scal, sizeof(semb_scalars), cudaMemcpyDeviceToHost, s));
+        SEMB_CUDA(h, cudaStreamSynchronize(s));
+        finished = h->scal_host->done != 0;
+    }
+    if (o->maxit == 0 || !finished) {
+        SEMB_CUDA(h, cudaMemcpyAsync(h->scal_host, h->scal, sizeof(semb_scalars), cudaMemcpyDeviceToHost, s));
+        SEMB_CUDA(h, cudaStreamSynchronize(s));
+    }
+    const semb_scalars& S = *h->scal_host;
+    int status = S.status;
+    if (st) {
+        st->iters = S.iter; st->status = status; st->b_norm = S.bnorm; st->r0_norm = S.r0norm; st->r_norm = S.rnorm;
+        st->lmax_used = lmax;
+        if (want_hist) {
+            const int cnt = (S.iter + 1 < want_hist) ? S.iter + 1 : want_hist;
+            SEMB_CUDA(h, cudaMemcpyAsync(st->hist_host_or_null, hist, sizeof(double) * cnt, cudaMemcpyDeviceToHost, s));
+            SEMB_CUDA(h, cudaStreamSynchronize(s));
+        }
+    }
+    if (status == SEMB_EBREAKDOWN) return semb_fail(h, SEMB_EBREAKDOWN, "pcg breakdown: p.Ap = %g at iteration %d", S.pAp, S.iter + 1);
+    return status;
+}

@@ -1,0 +1,115 @@
+// Internal declarations of libsemb200.so (not part of the ABI).  CUDA C++ for sm_100a only.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <map>
+#include <string>
+#include <utility>
+#include <vector>
+
+#include "../../include/semb200.h"
+
+#define SEMB_MAXN1 (SEMB_MAX_N + 1)
+
+// Device-resident scalars of the Krylov loop (alpha, beta, ... never visit the host; north_star:
+// "fused PCG vector updates and dot-product reductions").  One copy lives in device memory, a pinned host
+// mirror receives it when the host polls the stop flag.
+struct semb_scalars {
+    double rho_old, rho_new, pAp, alpha, beta, rr, rz, rnorm, bnorm, r0norm, target, rtol, atol, aux;
+    int32_t iter, done, status, maxit;
+    uint32_t ticket[8];
+};
+
+struct semb_mask_entry {
+    int32_t* list = nullptr;   // device: local ids of Dirichlet nodes, ascending
+    int64_t  count = 0;
+};
+
+struct semb_field_entry {
+    std::string name;
+    double* ptr = nullptr;
+    int64_t count = 0;
+    bool derived = false;
+};
+
+struct semb_mesh {
+    int64_t E = 0; int N = 0, n1 = 0; int64_t Np = 0, n = 0;
+    int64_t n_unique = 0, n_shared = 0, n_gs = 0;
+    double tol = 0.0;
+    bool has_alloc = false; semb_allocator alloc{};
+    double xi[SEMB_MAXN1], rho[SEMB_MAXN1], D[SEMB_MAXN1 * SEMB_MAXN1];   // host copies
+    // handle-owned device arrays
+    double*  geo = nullptr;        // [E][7][Np]  canonical layout (semb_info.geo)
+    double*  geoK = nullptr;       // kernel-native layout of the same data (axhelm.cu), may alias geo
+    int32_t* gid = nullptr;        // [n]
+    double*  invmult = nullptr;    // [n]
+    int32_t* gs_off = nullptr;     // [n_gs+1]
+    int32_t* gs_ids = nullptr;     // [n_shared]
+    std::vector<int32_t> face_tag; // host [E*6]
+    int32_t* face_tag_dev = nullptr;
+    std::map<uint32_t, semb_mask_entry> masks;
+    std::map<std::pair<uint32_t, double>, double*> dinvs;
+    // solver workspace
+    double* work = nullptr; int64_t work_vecs = 0;
+    double* partials = nullptr;         // block partial sums [4][SEMB_MAX_BLOCKS]
+    semb_scalars* scal = nullptr;       // device
+    semb_scalars* scal_host = nullptr;  // pinned mirror
+    double* hist_dev = nullptr; int hist_cap = 0;
+    // export
+    std::vector<semb_field_entry> fields;
+    int64_t cycle = 0; double time = 0.0;
+    std::string err;
+};
+
+// ---- helpers -------------------------------------------------------------------------------
+int  semb_fail(semb_mesh* h, int code, const char* fmt, ...);
+void* semb_dev_alloc(semb_mesh* h, size_t bytes);
+void  semb_dev_free(semb_mesh* h, void* p);
+
+#define SEMB_CUDA(h, call)                                                                     \
+    do { cudaError_t e_ = (call);                                                              \
+         if (e_ != cudaSuccess) return semb_fail((h), SEMB_ECUDA, "%s:%d %s: %s", __FILE__,    \
+                                                 __LINE__, #call, cudaGetErrorString(e_)); } while (0)
+
+#define SEMB_MAX_BLOCKS 4096   // upper bound on the grid of any kernel that writes block partials
+
+// ---- basis.cpp
+void semb_basis_host(int N, double* xi, double* rho, double* D);
+
+// ---- setup.cu
+int semb_setup_geo(semb_mesh* h, const double* x, const double* y, const double* z, cudaStream_t s);
+int semb_setup_numbering(semb_mesh* h, const double* x, const double* y, const double* z,
+                         const double* period, const int32_t* gid_in, cudaStream_t s);
+int semb_get_mask(semb_mesh* h, uint32_t tags, semb_mask_entry* out, cudaStream_t s);
+int semb_get_dinv(semb_mesh* h, double lambda, uint32_t tags, double** out, cudaStream_t s);
+int semb_diag_local(semb_mesh* h, double lambda, double* d, cudaStream_t s);
+
+// ---- axhelm.cu
+int semb_axhelm_upload_basis(semb_mesh* h);
+int semb_axhelm_prepare_geo(semb_mesh* h, cudaStream_t s);
+// dot_partials != NULL: also writes per-block partial sums of sum_l u_l w_l and (last block) their total
+// into *dot_total (device).
+// scal != NULL (PCG): the kernel early-exits when scal->done, and its last block leaves
+// scal->pAp = sum_l u_l w_l and scal->alpha = scal->rho_new / scal->pAp (breakdown -> status, done).
+int semb_axhelm_launch(semb_mesh* h, double lambda, const double* lam0, const double* lam1,
+                       const double* u, double* w, int nfields, semb_scalars* scal, cudaStream_t s);
+
+// ---- gs.cu
+int semb_gs_launch(semb_mesh* h, double* w, int nfields, cudaStream_t s);
+int semb_mask_launch(semb_mesh* h, const semb_mask_entry& m, double* w, int nfields, cudaStream_t s);
+
+// ---- pcg.cu
+int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* x, semb_pcg_stats* st,
+                 cudaStream_t s);
+int semb_lanczos_run(semb_mesh* h, double lambda, uint32_t tags, const double* v0, int steps, double* lmax,
+                     cudaStream_t s);
+int semb_cheb_run(semb_mesh* h, double lambda, uint32_t tags, int k, double lmax, const double* r, double* z,
+                  cudaStream_t s);
+int semb_operator_run(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* v, double* out,
+                      cudaStream_t s);
+int semb_ensure_work(semb_mesh* h, int64_t vecs);
+
+// ---- export.cu
+int semb_vmag_launch(const double* vx, const double* vy, const double* vz, double* out, int64_t n, cudaStream_t s);
+int semb_minmax_hist_launch(const double* v, int64_t n, int64_t stride, int nbins, double lo, double hi,
+                            double* minmax_dev, uint64_t* hist_dev, cudaStream_t s);

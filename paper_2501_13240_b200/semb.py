@@ -1,0 +1,232 @@
+"""Thin ctypes binding over libsemb200.so (include/semb200.h): argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels; torch supplies device memory
+(`tensor.data_ptr()`) and the stream (`torch.cuda.current_stream().cuda_stream`).  There is no
+CPU fallback: loading fails loudly when the library is missing, and every compute call raises
+SembError when the library reports an error (e.g. no CUDA device).
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsemb200.so")
+
+SEMB_OK, SEMB_MAXIT = 0, 1
+ERRORS = {-1: "SEMB_EINVAL", -2: "SEMB_ENOMEM", -3: "SEMB_ECUDA", -4: "SEMB_EGEOM", -5: "SEMB_EBREAKDOWN",
+          -6: "SEMB_EMATCH", -7: "SEMB_ENOTFOUND"}
+
+# every symbol include/semb200.h declares (tests check that the library exports all of them)
+SYMBOLS = ["semb_gll", "semb_setup", "semb_destroy", "semb_last_error", "semb_mesh_info", "semb_apply_axhelm",
+           "semb_gather_scatter", "semb_apply_mask", "semb_assemble_rhs", "semb_apply_operator", "semb_jacobi_diag",
+           "semb_pcg_solve", "semb_estimate_lmax", "semb_cheb_jacobi", "semb_publish_field", "semb_publish_state",
+           "semb_export_field", "semb_field_minmax_hist", "semb_apply_axhelm_host", "semb_read_device", "semb_version"]
+
+
+class SembError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"{ERRORS.get(code, code)}: {msg}")
+        self.code = code
+
+
+class Info(C.Structure):
+    _fields_ = [("E", C.c_int64), ("N", C.c_int32), ("n1", C.c_int32), ("Np", C.c_int64), ("n", C.c_int64),
+                ("n_unique", C.c_int64), ("n_shared", C.c_int64), ("n_gs", C.c_int64), ("tol", C.c_double),
+                ("gid", C.c_void_p), ("geo", C.c_void_p), ("invmult", C.c_void_p), ("gs_offsets", C.c_void_p),
+                ("gs_ids", C.c_void_p)]
+
+
+class PcgOpts(C.Structure):
+    _fields_ = [("lam", C.c_double), ("dirichlet_tags", C.c_uint32), ("precond", C.c_int32),
+                ("cheb_degree", C.c_int32), ("cheb_lmax", C.c_double), ("rtol", C.c_double), ("atol", C.c_double),
+                ("maxit", C.c_int32), ("x0_is_zero", C.c_int32), ("check_every", C.c_int32), ("reserved", C.c_int32)]
+
+
+class PcgStats(C.Structure):
+    _fields_ = [("iters", C.c_int32), ("status", C.c_int32), ("b_norm", C.c_double), ("r0_norm", C.c_double),
+                ("r_norm", C.c_double), ("lmax_used", C.c_double), ("hist", C.c_void_p), ("hist_len", C.c_int32),
+                ("reserved", C.c_int32)]
+
+
+class FieldDesc(C.Structure):
+    _fields_ = [("name", C.c_char_p), ("ptr", C.c_void_p), ("dtype", C.c_int32), ("memspace", C.c_int32),
+                ("count", C.c_int64), ("stride", C.c_int64), ("cycle", C.c_int64), ("time", C.c_double)]
+
+
+_lib = None
+
+
+def lib():
+    """Load libsemb200.so (build it with `python -m paper_2501_13240_b200.build`)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2501_13240_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.semb_last_error.restype = C.c_char_p
+        L.semb_last_error.argtypes = [C.c_void_p]
+        L.semb_version.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def version():
+    return lib().semb_version().decode()
+
+
+def gll(N):
+    """(xi, rho, D) of order N from the library (host)."""
+    xi = np.zeros(N + 1); rho = np.zeros(N + 1); D = np.zeros((N + 1, N + 1))
+    rc = lib().semb_gll(C.c_int(N), xi.ctypes.data_as(C.c_void_p), rho.ctypes.data_as(C.c_void_p),
+                        D.ctypes.data_as(C.c_void_p))
+    if rc:
+        raise SembError(rc, f"semb_gll(N={N})")
+    return xi, rho, D
+
+
+def _stream():
+    import torch
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _dp(t):
+    """device pointer of a contiguous CUDA tensor (or None)."""
+    if t is None:
+        return None
+    assert t.is_cuda and t.is_contiguous(), "expected a contiguous CUDA tensor"
+    return C.c_void_p(t.data_ptr())
+
+
+class Mesh:
+    """Handle of one mesh on the current CUDA device (semb_setup ... semb_destroy)."""
+
+    def __init__(self, E, N, x, y, z, face_tag, period, gid=None):
+        import torch
+        assert x.dtype == torch.float64 and y.dtype == torch.float64 and z.dtype == torch.float64
+        self._h = C.c_void_p()
+        ft = np.ascontiguousarray(face_tag, dtype=np.int32)
+        per = np.ascontiguousarray(period, dtype=np.float64)
+        assert ft.size == 6 * E and x.numel() == E * (N + 1) ** 3
+        rc = lib().semb_setup(C.c_int64(E), C.c_int(N), _dp(x), _dp(y), _dp(z), ft.ctypes.data_as(C.c_void_p),
+                              per.ctypes.data_as(C.c_void_p), _dp(gid), None, _stream(), C.byref(self._h))
+        if rc:
+            raise SembError(rc, lib().semb_last_error(None).decode())
+        self.info = Info()
+        self._check(lib().semb_mesh_info(self._h, C.byref(self.info)))
+        self.E, self.N, self.n, self.Np = int(self.info.E), int(self.info.N), int(self.info.n), int(self.info.Np)
+        self.n_unique, self.n_shared, self.n_gs = int(self.info.n_unique), int(self.info.n_shared), int(self.info.n_gs)
+        self._keep = []
+
+    def _check(self, rc):
+        if rc < 0:
+            raise SembError(rc, lib().semb_last_error(self._h).decode())
+        return rc
+
+    def close(self):
+        if self._h:
+            lib().semb_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- read-only views of handle-owned arrays (copied to host for tests) -------------------
+    def _to_host(self, ptr, count, dtype):
+        out = np.empty(count, dtype=dtype)
+        if count:
+            self._check(lib().semb_read_device(C.c_void_p(ptr), out.ctypes.data_as(C.c_void_p), C.c_size_t(out.nbytes)))
+        return out
+
+    def gid_host(self):
+        return self._to_host(self.info.gid, self.n, np.int32)
+
+    def geo_host(self):
+        return self._to_host(self.info.geo, self.n * 7, np.float64).reshape(self.E, 7, self.Np)
+
+    def invmult_host(self):
+        return self._to_host(self.info.invmult, self.n, np.float64)
+
+    def gs_lists_host(self):
+        return (self._to_host(self.info.gs_offsets, self.n_gs + 1, np.int32),
+                self._to_host(self.info.gs_ids, self.n_shared, np.int32))
+
+    # ---- the hot path ------------------------------------------------------------------------
+    def apply_axhelm(self, u, w, lam=0.0, lam0=None, lam1=None, nfields=1):
+        self._check(lib().semb_apply_axhelm(self._h, C.c_double(lam), _dp(lam0), _dp(lam1), _dp(u), _dp(w),
+                                            C.c_int(nfields), _stream()))
+        return w
+
+    def gather_scatter(self, w, nfields=1):
+        self._check(lib().semb_gather_scatter(self._h, _dp(w), C.c_int(nfields), _stream()))
+        return w
+
+    def apply_mask(self, w, tags, nfields=1):
+        self._check(lib().semb_apply_mask(self._h, C.c_uint32(tags), _dp(w), C.c_int(nfields), _stream()))
+        return w
+
+    def assemble_rhs(self, f, b, tags):
+        self._check(lib().semb_assemble_rhs(self._h, C.c_uint32(tags), _dp(f), _dp(b), _stream()))
+        return b
+
+    def apply_operator(self, v, out, lam, tags):
+        self._check(lib().semb_apply_operator(self._h, C.c_double(lam), C.c_uint32(tags), _dp(v), _dp(out), _stream()))
+        return out
+
+    def jacobi_diag(self, dinv_out, lam, tags):
+        self._check(lib().semb_jacobi_diag(self._h, C.c_double(lam), C.c_uint32(tags), _dp(dinv_out), _stream()))
+        return dinv_out
+
+    def pcg_solve(self, b, x, lam=0.0, tags=0, precond=1, cheb_degree=2, cheb_lmax=0.0, rtol=1e-10, atol=0.0,
+                  maxit=10000, x0_is_zero=True, check_every=0, hist_len=0):
+        """Returns dict(iters, status, b_norm, r0_norm, r_norm, lmax_used, hist)."""
+        o = PcgOpts(lam, tags, precond, cheb_degree, cheb_lmax, rtol, atol, maxit, 1 if x0_is_zero else 0, check_every, 0)
+        hist = np.zeros(max(hist_len, 1))
+        st = PcgStats()
+        st.hist = hist.ctypes.data_as(C.c_void_p).value if hist_len > 0 else None
+        st.hist_len = hist_len
+        rc = self._check(lib().semb_pcg_solve(self._h, C.byref(o), _dp(b), _dp(x), C.byref(st), _stream()))
+        return dict(iters=int(st.iters), status=int(rc), b_norm=st.b_norm, r0_norm=st.r0_norm, r_norm=st.r_norm,
+                    lmax_used=st.lmax_used, hist=hist[:min(hist_len, st.iters + 1)])
+
+    def estimate_lmax(self, v0, lam, tags, steps=10):
+        out = C.c_double(0.0)
+        self._check(lib().semb_estimate_lmax(self._h, C.c_double(lam), C.c_uint32(tags), _dp(v0), C.c_int(steps),
+                                             C.byref(out), _stream()))
+        return out.value
+
+    def cheb_jacobi(self, r, z, lam, tags, k, lmax):
+        self._check(lib().semb_cheb_jacobi(self._h, C.c_double(lam), C.c_uint32(tags), C.c_int(k), C.c_double(lmax),
+                                           _dp(r), _dp(z), _stream()))
+        return z
+
+    # ---- in-situ hand-off --------------------------------------------------------------------
+    def publish_field(self, name, t):
+        self._keep.append(t)
+        self._check(lib().semb_publish_field(self._h, name.encode(), _dp(t), C.c_int64(t.numel())))
+
+    def publish_state(self, cycle, time):
+        self._check(lib().semb_publish_state(self._h, C.c_int64(cycle), C.c_double(time), _stream()))
+
+    def export_field(self, name):
+        d = FieldDesc()
+        self._check(lib().semb_export_field(self._h, name.encode(), C.byref(d)))
+        return d
+
+    def apply_axhelm_host(self, u_host, w_host, lam=0.0):
+        """End-to-end call with HOST numpy buffers (copies inside the library)."""
+        self._check(lib().semb_apply_axhelm_host(self._h, C.c_double(lam), u_host.ctypes.data_as(C.c_void_p),
+                                                 w_host.ctypes.data_as(C.c_void_p)))
+        return w_host
+
+
+def field_minmax_hist(desc, nbins, lo, hi, minmax_dev, hist_dev):
+    """In-device consumer: minmax_dev (float64[2]) and hist_dev (int64/uint64[nbins]) CUDA tensors."""
+    rc = lib().semb_field_minmax_hist(C.byref(desc), C.c_int(nbins), C.c_double(lo), C.c_double(hi), _dp(minmax_dev),
+                                      _dp(hist_dev), _stream())
+    if rc:
+        raise SembError(rc, "semb_field_minmax_hist")
