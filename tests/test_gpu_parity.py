@@ -94,8 +94,12 @@ def test_numbering_bit_exact(cases, name):
 def test_geometric_factors(cases, name):
     m, P, G = cases(name)
     geo = G.geo_host()
-    for g in range(7):
-        assert normwise(geo[:, g], P.geo[:, g]) <= TOL, f"factor {g}"
+    # the six G factors are one symmetric tensor: errors are measured against its largest entry (on affine
+    # meshes the cross terms are pure rounding noise around 0, so a per-factor norm would compare noise with noise)
+    scale = np.abs(P.geo[:, :6]).max()
+    for g in range(6):
+        assert np.abs(geo[:, g] - P.geo[:, g]).max() <= TOL * scale, f"factor {g}"
+    assert normwise(geo[:, 6], P.geo[:, 6]) <= TOL
 
 
 def test_caller_supplied_gid(torch_cuda, semb, orc, xi_of):
