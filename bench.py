@@ -1,0 +1,272 @@
+#!/usr/bin/env python
+"""bench.py — headline benchmark of the SEM hot path on B200 (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path over the synthetic batch: ONE Jacobi-PCG pressure iteration
+(axhelm with fused p.Ap -> gather-scatter -> Dirichlet mask -> fused x/r update with the ||r||^2 and r.z
+reductions -> Jacobi + direction update) on the 64^3-element deformed box of BASELINE.json configs[3]
+(N = 7, fp64, 134 217 728 local nodes, lambda = 0).  K steps = one semb_pcg_solve call with maxit = K and
+rtol = 0 (it cannot stop early), bracketed by CUDA events on the launching stream.
+
+    value     = local nodes processed per second by the whole step (GDOF/s), all ranks
+    roofline  = the dominant kernel (axhelm): 64 B/node algorithmic bytes / its mean device time measured with
+                CUDA event pairs around its launches INSIDE the timed solve, against MEASURED_PEAKS.json hbm_gbs
+    pcg_iter  = the whole iteration against the fixed 171.6 B/node model
+    e2e       = the same K iterations through semb_pcg_solve_host: b from pinned host memory, x back to it
+    cpu_baseline = the oracle (oracle/semoracle.c, as it stands) timed on this box's host cores
+
+`--impl reference` times the oracle alone, same metric/unit/config.  Multi-GPU: replicas only:
+each rank runs the same workload on its own GPU, value = sum over ranks / max-over-ranks time.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2501_13240_b200 import inputs as I  # noqa: E402
+
+METRIC = "SEM Jacobi-PCG pressure-iteration throughput (axhelm+gather-scatter+mask+Jacobi+fused updates), N=7 fp64"
+UNIT = "GDOF/s"
+B_AXHELM = 64.0          # algorithmic bytes per node, Poisson axhelm
+B_AXHELM_HELM = 72.0
+B_ITER = 171.6           # algorithmic bytes per node per Jacobi-PCG iteration, N = 7, Poisson
+WORKLOADS = {            # name -> elements per direction of the deformed box (BASELINE.json configs[3] / configs[1])
+    "cfg3_box64_deformed_N7": 64,
+    "cfg1_box16_deformed_N7": 16,
+    "box32_deformed_N7": 32,
+}
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 100 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.p = index, None
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            out, _ = self.p.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill(); out, _ = self.p.communicate()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [t.strip() for t in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def build_problem(torch, semb, ne):
+    """64^3 (or ne^3) deformed box, N = 7: mesh on the host, coordinates to the device, setup, rhs."""
+    xi = semb.gll(7)[0]
+    m = I.box_mesh(ne, ne, ne, 7, xi, deform=0.05, name=f"box{ne}_deformed")
+    x, y, z = (torch.from_numpy(a).cuda() for a in (m.x, m.y, m.z))
+    G = semb.Mesh(m.E, m.N, x, y, z, m.face_tag, m.period)
+    del x, y, z
+    torch.cuda.empty_cache()
+    return m, G
+
+
+def oracle_sample(steps, warmup):
+    """The oracle's Jacobi-PCG iteration on the 16^3-element member of the same deformed-box family."""
+    from oracle import semoracle as O
+    O.build()
+    ne = 16
+    xi = O.gll(7)[0]
+    m = I.box_mesh(ne, ne, ne, 7, xi, deform=0.05)
+    P = O.Problem(m.E, m.N, m.x, m.y, m.z, m.face_tag, m.period, lam=0.0, dirichlet_tags=0b10)
+    b = P.assemble_rhs(I.uniform(I.seed_for(3, 2), m.n))
+    if warmup > 0:
+        P.pcg(b, precond=1, rtol=0.0, maxit=warmup)
+    t0 = time.perf_counter()
+    r = P.pcg(b, precond=1, rtol=0.0, maxit=steps)
+    dt = time.perf_counter() - t0
+    assert r["iters"] == steps
+    return dict(n=m.n, seconds=dt, steps=steps, cores=O.num_threads(),
+                sample=f"{steps} Jacobi-PCG iterations of oracle/semoracle.c on the 16^3-element deformed box "
+                       f"(N=7, {m.n} local nodes = 1/64 of the workload), OpenMP over elements in axhelm only")
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    s = oracle_sample(max(args.steps, 1), args.warmup)
+    val = s["n"] * s["steps"] / s["seconds"] / 1e9
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * s["seconds"] / s["steps"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "sample": s["sample"]},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": s["cores"], "kind": "oracle", "sample": s["sample"]},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg3_box64_deformed_N7", choices=list(WORKLOADS))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_2501_13240_b200 import semb
+    semb.lib()                                         # fails loudly if the CUDA library is missing
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    K, W = max(args.steps, 1), max(args.warmup, 0)
+    peak, peak_src = measured_peak()
+
+    ne = WORKLOADS[args.workload]
+    m, G = build_problem(torch, semb, ne)
+    n = m.n
+    f = torch.from_numpy(I.uniform(I.seed_for(3, 2), n)).cuda()
+    b = torch.empty_like(f)
+    G.assemble_rhs(f, b, 0b10)
+    x = torch.zeros_like(b)
+    del f
+    solve = dict(lam=0.0, tags=0b10, precond=1, rtol=0.0, atol=0.0)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- warm-up, then exactly K timed steps
+    if W > 0:
+        G.pcg_solve(b, x, maxit=W, check_every=W, **solve)
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    st = G.pcg_solve(b, x, maxit=K, check_every=K, profile=True, **solve)
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1)
+    assert st["iters"] == K, st
+    if dist is not None:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    ms_step = ms / K
+    value = world * n * K / (ms * 1e-3) / 1e9
+    ax_ms = st["axhelm_ms"]
+    ax_gbs = B_AXHELM * n / (ax_ms * 1e-3) / 1e9
+
+    # ---- axhelm alone, Poisson and Helmholtz (BASELINE.json configs[3] "roofline sweep"); not the headline
+    u = torch.from_numpy(I.uniform(I.seed_for(3, 1), n)).cuda()
+    w = torch.empty_like(u)
+    sweep = {}
+    for name, lam, nbytes in (("poisson", 0.0, B_AXHELM), ("helmholtz", 1e4, B_AXHELM_HELM)):
+        for _ in range(5):
+            G.apply_axhelm(u, w, lam=lam)
+        reps = 20
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(); a0.record()
+        for _ in range(reps):
+            G.apply_axhelm(u, w, lam=lam)
+        a1.record(); torch.cuda.synchronize()
+        t = a0.elapsed_time(a1) / reps
+        sweep[name] = {"ms": t, "gdofs": n / (t * 1e-3) / 1e9, "gbs": nbytes * n / (t * 1e-3) / 1e9,
+                       "frac_of_measured_peak": nbytes * n / (t * 1e-3) / 1e9 / peak,
+                       "frac_of_8TBs": nbytes * n / (t * 1e-3) / 8e12}
+    del u, w
+
+    # ---- end to end through the C ABI with HOST buffers (pinned): b H2D, K iterations, x D2H
+    e2e = None
+    if not args.no_e2e:
+        bh = b.cpu().pin_memory(); xh = torch.empty_like(bh).pin_memory()
+        G.pcg_solve_host(bh, xh, maxit=1, check_every=1, **solve)                      # warm-up (allocates staging)
+        barrier()
+        h0, h1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        h0.record()
+        G.pcg_solve_host(bh, xh, maxit=K, check_every=K, **solve)
+        h1.record(); barrier()
+        hms = h0.elapsed_time(h1)
+        if dist is not None:
+            t = torch.tensor([hms], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX); hms = float(t.item())
+        e2e = {"value": world * n * K / (hms * 1e-3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": 8 * n / K,
+               "d2h_bytes_per_step": 8 * n / K, "note": "one call = b host->device, K iterations, x device->host"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "E": m.E, "N": 7, "local_nodes": n, "lambda": 0.0,
+                   "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "l2": "inputs larger than L2 (every vector is %.2f GB)" % (8 * n / 1e9)},
+        "roofline": {"bound": "hbm", "kernel": "axhelm (Poisson, fused p.Ap)", "achieved": ax_gbs, "peak": peak,
+                     "unit": "GB/s", "frac": ax_gbs / peak, "traffic": None, "peak_source": peak_src,
+                     "bytes_per_node": B_AXHELM, "ms": ax_ms, "timed_launches": st["profiled"],
+                     "frac_of_8TBs": ax_gbs / 8000.0, "gdofs": n / (ax_ms * 1e-3) / 1e9},
+        "pcg_iter": {"ms": ms_step, "model_bytes_per_node": B_ITER, "gbs": B_ITER * n / (ms_step * 1e-3) / 1e9,
+                     "frac_of_measured_peak": B_ITER * n / (ms_step * 1e-3) / 1e9 / peak,
+                     "frac_of_8TBs": B_ITER * n / (ms_step * 1e-3) / 8e12},
+        "axhelm_sweep": sweep,
+        "e2e": e2e, "gpu_launches": st["launches"], "clocks": clocks,
+    }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        s = oracle_sample(60, 2)
+        line["cpu_baseline"] = {"value": s["n"] * s["steps"] / s["seconds"] / 1e9, "unit": UNIT, "cores": s["cores"],
+                                "kind": "oracle", "sample": s["sample"]}
+    if rank == 0:
+        print(json.dumps(line))
+    G.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

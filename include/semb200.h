@@ -141,7 +141,8 @@ typedef struct {
     int32_t  x0_is_zero;      /* 1: ignore the contents of x and start from 0                    */
     int32_t  check_every;     /* iterations enqueued between host polls of the stop flag; <= 0 => 16.
                                  The iteration count returned is exact regardless.               */
-    int32_t  reserved;
+    int32_t  profile;         /* 1: bracket every axhelm launch of the loop with CUDA events on the stream
+                                 (no synchronisation added) and report their mean in stats.axhelm_ms     */
 } semb_pcg_opts;
 
 typedef struct {
@@ -150,7 +151,9 @@ typedef struct {
     double  b_norm, r0_norm, r_norm, lmax_used;
     double* hist_host_or_null;/* in: host buffer [hist_len] for ||r_it||, it = 0..; may be NULL   */
     int32_t hist_len;
-    int32_t reserved;
+    int32_t profiled;         /* number of axhelm launches that were timed (opts.profile)            */
+    double  axhelm_ms;        /* mean device time of those launches, milliseconds                    */
+    int64_t launches;         /* kernels this call launched                                          */
 } semb_pcg_stats;
 
 /* b device [n]: assembled, masked right-hand side.  x device [n]: in = initial guess (continuous,
@@ -200,6 +203,10 @@ SEMB_API int semb_field_minmax_hist(const semb_field_desc* f, int nbins, double 
 
 /* ---- convenience: the same calls with HOST buffers (copies inside; used for end-to-end timing) */
 SEMB_API int semb_apply_axhelm_host(semb_handle h, double lambda, const double* u_host, double* w_host);
+/* pcg_solve with b and x in HOST memory (pinned memory makes the copies asynchronous): b is copied to the
+ * device, the solve runs, x is copied back; the device staging buffers belong to the handle. */
+SEMB_API int semb_pcg_solve_host(semb_handle h, const semb_pcg_opts* opts, const double* b_host, double* x_host,
+                                 semb_pcg_stats* stats, void* stream);
 
 /* Blocking copy of `bytes` bytes from device memory (e.g. a semb_info view) to host memory. */
 SEMB_API int semb_read_device(const void* dev, void* host, size_t bytes);

@@ -58,8 +58,9 @@ int semb_destroy(semb_handle h)
     semb_dev_free(h, h->gs_off); semb_dev_free(h, h->gs_ids); semb_dev_free(h, h->face_tag_dev);
     for (auto& kv : h->masks) semb_dev_free(h, kv.second.list);
     for (auto& kv : h->dinvs) semb_dev_free(h, kv.second);
-    semb_dev_free(h, h->work); semb_dev_free(h, h->partials); semb_dev_free(h, h->scal); semb_dev_free(h, h->hist_dev);
+    semb_dev_free(h, h->work); semb_dev_free(h, h->partials); semb_dev_free(h, h->scal); semb_dev_free(h, h->hist_dev); semb_dev_free(h, h->stage);
     if (h->scal_host) cudaFreeHost(h->scal_host);
+    for (cudaEvent_t ev : h->prof_ev) cudaEventDestroy(ev);
     for (auto& f : h->fields) if (f.derived) semb_dev_free(h, f.ptr);
     delete h;
     return SEMB_OK;
@@ -274,6 +275,28 @@ int semb_apply_axhelm_host(semb_handle h, double lambda, const double* u_host, d
     rc = semb_axhelm_launch(h, lambda, nullptr, nullptr, h->work, h->work + h->n, 1, nullptr, 0); if (rc) return rc;
     SEMB_CUDA(h, cudaMemcpy(w_host, h->work + h->n, bytes, cudaMemcpyDeviceToHost));
     return SEMB_OK;
+}
+
+int semb_pcg_solve_host(semb_handle h, const semb_pcg_opts* o, const double* b_host, double* x_host,
+                        semb_pcg_stats* st, void* stream)
+{
+    if (!h) return SEMB_EINVAL;
+    if (!o || !b_host || !x_host) return semb_fail(h, SEMB_EINVAL, "pcg_solve_host: bad argument");
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t bytes = sizeof(double) * (size_t)h->n;
+    if (!h->stage) {
+        h->stage = (double*)semb_dev_alloc(h, 2 * bytes);
+        if (!h->stage) return semb_fail(h, SEMB_ENOMEM, "host-call staging buffers");
+    }
+    double *b = h->stage, *x = h->stage + h->n;
+    SEMB_CUDA(h, cudaMemcpyAsync(b, b_host, bytes, cudaMemcpyHostToDevice, s));
+    if (!o->x0_is_zero) SEMB_CUDA(h, cudaMemcpyAsync(x, x_host, bytes, cudaMemcpyHostToDevice, s));
+    const int rc = semb_pcg_run(h, o, b, x, st, s);
+    if (st) st->status = rc;
+    if (rc < 0) return rc;
+    SEMB_CUDA(h, cudaMemcpyAsync(x_host, x, bytes, cudaMemcpyDeviceToHost, s));
+    SEMB_CUDA(h, cudaStreamSynchronize(s));
+    return rc;
 }
 
 }  // extern "C"

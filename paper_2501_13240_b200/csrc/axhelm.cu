@@ -104,6 +104,7 @@ static int launch_slab(semb_mesh* h, bool helm, double lambda, const double* lam
     if (helm) k_axhelm_slab<n1, true><<<(unsigned)blocks, n1 * n1, 0, s>>>(h->E, h->n, h->geoK, lambda, lam0, lam1, u, w, nfields, scal, h->partials);
     else      k_axhelm_slab<n1, false><<<(unsigned)blocks, n1 * n1, 0, s>>>(h->E, h->n, h->geoK, lambda, lam0, lam1, u, w, nfields, scal, h->partials);
     SEMB_CUDA(h, cudaGetLastError());
+    h->launches += 1;
     return SEMB_OK;
 }
 

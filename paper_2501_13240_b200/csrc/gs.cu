@@ -21,6 +21,7 @@ int semb_gs_launch(semb_mesh* h, double* w, int nfields, cudaStream_t s)
     if (h->n_gs == 0) return SEMB_OK;
     dim3 grid((unsigned)((h->n_gs + 255) / 256), (unsigned)nfields);
     k_gs<<<grid, 256, 0, s>>>(h->n_gs, h->n, h->gs_off, h->gs_ids, w);
+    h->launches += 1;
     SEMB_CUDA(h, cudaGetLastError());
     return SEMB_OK;
 }
@@ -36,6 +37,7 @@ int semb_mask_launch(semb_mesh* h, const semb_mask_entry& m, double* w, int nfie
     if (m.count == 0) return SEMB_OK;
     dim3 grid((unsigned)((m.count + 255) / 256), (unsigned)nfields);
     k_mask<<<grid, 256, 0, s>>>(m.count, h->n, m.list, w);
+    h->launches += 1;
     SEMB_CUDA(h, cudaGetLastError());
     return SEMB_OK;
 }

@@ -219,6 +219,7 @@ static int cheb_apply(semb_mesh* h, double lambda, const semb_mask_entry& m, con
 {
     const int64_t n = h->n;
     k_cheb_init<<<vec_grid(n), VEC_BLOCK, 0, s>>>(n, r, dinv, c.itheta, res, d, z, k == 0, scal);
+    h->launches += 1 + k;
     for (int it = 0; it < k; ++it) {
         int rc = semb_axhelm_launch(h, lambda, nullptr, nullptr, d, Ad, 1, nullptr, s); if (rc) return rc;
         rc = semb_gs_launch(h, Ad, 1, s); if (rc) return rc;
@@ -310,6 +311,7 @@ int semb_lanczos_run(semb_mesh* h, double lambda, uint32_t tags, const double* v
 int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* x, semb_pcg_stats* st, cudaStream_t s)
 {
     const int64_t n = h->n; const unsigned G = vec_grid(n);
+    const int64_t launches0 = h->launches;
     if (o->precond < 0 || o->precond > 2 || o->maxit < 0 || (o->precond == 2 && (o->cheb_degree < 0 || o->cheb_degree > 16)))
         return semb_fail(h, SEMB_EINVAL, "pcg: precond=%d cheb_degree=%d maxit=%d", o->precond, o->cheb_degree, o->maxit);
     semb_mask_entry m; double* dinv = nullptr;
@@ -353,6 +355,12 @@ int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* 
     }
     SEMB_CUDA(h, cudaGetLastError());
 
+    h->launches += 1;
+    // optional event pairs around the axhelm launches of the first iterations (no synchronisation added)
+    const int nprof = o->profile ? (o->maxit < 64 ? o->maxit : 64) : 0;
+    while ((int)h->prof_ev.size() < 2 * nprof) {
+        cudaEvent_t ev; SEMB_CUDA(h, cudaEventCreate(&ev)); h->prof_ev.push_back(ev);
+    }
     const int check = o->check_every > 0 ? o->check_every : 16;
     bool finished = (o->maxit == 0);
     for (int it0 = 0; it0 < o->maxit && !finished; it0 += check) {
@@ -362,14 +370,20 @@ int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* 
                 rc = cheb_apply(h, o->lambda, m, dinv, o->cheb_degree, cc, r, z, res, d, q, h->scal, s); if (rc) return rc;
                 k_dot_rz<<<G, VEC_BLOCK, 0, s>>>(n, r, z, h->invmult, h->scal, h->partials);
                 k_update_p<<<G, VEC_BLOCK, 0, s>>>(n, z, nullptr, p, h->scal);
+                h->launches += 2;
             } else {
                 k_update_p<<<G, VEC_BLOCK, 0, s>>>(n, r, dz, p, h->scal);
+                h->launches += 1;
             }
+            const int itn = it0 + i;
+            if (itn < nprof) SEMB_CUDA(h, cudaEventRecord(h->prof_ev[2 * itn], s));
             rc = semb_axhelm_launch(h, o->lambda, nullptr, nullptr, p, q, 1, h->scal, s); if (rc) return rc;
+            if (itn < nprof) SEMB_CUDA(h, cudaEventRecord(h->prof_ev[2 * itn + 1], s));
             rc = semb_gs_launch(h, q, 1, s); if (rc) return rc;
             rc = semb_mask_launch(h, m, q, 1, s); if (rc) return rc;
             if (o->precond == 2) k_update_xr<false><<<G, VEC_BLOCK, 0, s>>>(n, p, q, x, r, h->invmult, nullptr, h->scal, h->partials, hist, want_hist);
             else                 k_update_xr<true><<<G, VEC_BLOCK, 0, s>>>(n, p, q, x, r, h->invmult, dz, h->scal, h->partials, hist, want_hist);
+            h->launches += 1;
         }
         SEMB_CUDA(h, cudaGetLastError());
         SEMB_CUDA(h, cudaMemcpyAsync(h->scal_host, h->scal, sizeof(semb_scalars), cudaMemcpyDeviceToHost, s));
@@ -385,6 +399,14 @@ int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* 
     if (st) {
         st->iters = S.iter; st->status = status; st->b_norm = S.bnorm; st->r0_norm = S.r0norm; st->r_norm = S.rnorm;
         st->lmax_used = lmax;
+        st->launches = h->launches - launches0;
+        st->profiled = 0; st->axhelm_ms = 0.0;
+        const int np_ = S.iter < nprof ? S.iter : nprof;
+        if (np_ > 0) {
+            double tot = 0.0;
+            for (int i = 0; i < np_; ++i) { float ms = 0.f; SEMB_CUDA(h, cudaEventElapsedTime(&ms, h->prof_ev[2 * i], h->prof_ev[2 * i + 1])); tot += ms; }
+            st->profiled = np_; st->axhelm_ms = tot / np_;
+        }
         if (want_hist) {
             const int cnt = (S.iter + 1 < want_hist) ? S.iter + 1 : want_hist;
             SEMB_CUDA(h, cudaMemcpyAsync(st->hist_host_or_null, hist, sizeof(double) * cnt, cudaMemcpyDeviceToHost, s));

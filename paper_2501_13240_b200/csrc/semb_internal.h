@@ -55,6 +55,9 @@ struct semb_mesh {
     semb_scalars* scal = nullptr;       // device
     semb_scalars* scal_host = nullptr;  // pinned mirror
     double* hist_dev = nullptr; int hist_cap = 0;
+    double* stage = nullptr;            // device staging of the *_host entry points [2][n]
+    int64_t launches = 0;               // kernels launched through this handle (bench.py reports it)
+    std::vector<cudaEvent_t> prof_ev;   // event pairs around axhelm launches (opts.profile)
     // export
     std::vector<semb_field_entry> fields;
     int64_t cycle = 0; double time = 0.0;

@@ -21,7 +21,7 @@ ERRORS = {-1: "SEMB_EINVAL", -2: "SEMB_ENOMEM", -3: "SEMB_ECUDA", -4: "SEMB_EGEO
 SYMBOLS = ["semb_gll", "semb_setup", "semb_destroy", "semb_last_error", "semb_mesh_info", "semb_apply_axhelm",
            "semb_gather_scatter", "semb_apply_mask", "semb_assemble_rhs", "semb_apply_operator", "semb_jacobi_diag",
            "semb_pcg_solve", "semb_estimate_lmax", "semb_cheb_jacobi", "semb_publish_field", "semb_publish_state",
-           "semb_export_field", "semb_field_minmax_hist", "semb_apply_axhelm_host", "semb_read_device", "semb_version"]
+           "semb_export_field", "semb_field_minmax_hist", "semb_apply_axhelm_host", "semb_pcg_solve_host", "semb_read_device", "semb_version"]
 
 
 class SembError(RuntimeError):
@@ -40,13 +40,13 @@ class Info(C.Structure):
 class PcgOpts(C.Structure):
     _fields_ = [("lam", C.c_double), ("dirichlet_tags", C.c_uint32), ("precond", C.c_int32),
                 ("cheb_degree", C.c_int32), ("cheb_lmax", C.c_double), ("rtol", C.c_double), ("atol", C.c_double),
-                ("maxit", C.c_int32), ("x0_is_zero", C.c_int32), ("check_every", C.c_int32), ("reserved", C.c_int32)]
+                ("maxit", C.c_int32), ("x0_is_zero", C.c_int32), ("check_every", C.c_int32), ("profile", C.c_int32)]
 
 
 class PcgStats(C.Structure):
     _fields_ = [("iters", C.c_int32), ("status", C.c_int32), ("b_norm", C.c_double), ("r0_norm", C.c_double),
                 ("r_norm", C.c_double), ("lmax_used", C.c_double), ("hist", C.c_void_p), ("hist_len", C.c_int32),
-                ("reserved", C.c_int32)]
+                ("profiled", C.c_int32), ("axhelm_ms", C.c_double), ("launches", C.c_int64)]
 
 
 class FieldDesc(C.Structure):
@@ -182,16 +182,27 @@ class Mesh:
         return dinv_out
 
     def pcg_solve(self, b, x, lam=0.0, tags=0, precond=1, cheb_degree=2, cheb_lmax=0.0, rtol=1e-10, atol=0.0,
-                  maxit=10000, x0_is_zero=True, check_every=0, hist_len=0):
+                  maxit=10000, x0_is_zero=True, check_every=0, hist_len=0, profile=False):
         """Returns dict(iters, status, b_norm, r0_norm, r_norm, lmax_used, hist)."""
-        o = PcgOpts(lam, tags, precond, cheb_degree, cheb_lmax, rtol, atol, maxit, 1 if x0_is_zero else 0, check_every, 0)
+        o = PcgOpts(lam, tags, precond, cheb_degree, cheb_lmax, rtol, atol, maxit, 1 if x0_is_zero else 0, check_every, 1 if profile else 0)
         hist = np.zeros(max(hist_len, 1))
         st = PcgStats()
         st.hist = hist.ctypes.data_as(C.c_void_p).value if hist_len > 0 else None
         st.hist_len = hist_len
         rc = self._check(lib().semb_pcg_solve(self._h, C.byref(o), _dp(b), _dp(x), C.byref(st), _stream()))
         return dict(iters=int(st.iters), status=int(rc), b_norm=st.b_norm, r0_norm=st.r0_norm, r_norm=st.r_norm,
-                    lmax_used=st.lmax_used, hist=hist[:min(hist_len, st.iters + 1)])
+                    lmax_used=st.lmax_used, hist=hist[:min(hist_len, st.iters + 1)], axhelm_ms=st.axhelm_ms,
+                    profiled=int(st.profiled), launches=int(st.launches))
+
+    def pcg_solve_host(self, b_host, x_host, lam=0.0, tags=0, precond=1, cheb_degree=2, cheb_lmax=0.0, rtol=1e-10,
+                       atol=0.0, maxit=10000, check_every=0):
+        """pcg_solve with HOST buffers (torch CPU tensors, ideally pinned, or numpy arrays)."""
+        def hp(a):
+            return C.c_void_p(a.data_ptr()) if hasattr(a, "data_ptr") else a.ctypes.data_as(C.c_void_p)
+        o = PcgOpts(lam, tags, precond, cheb_degree, cheb_lmax, rtol, atol, maxit, 1, check_every, 0)
+        st = PcgStats()
+        rc = self._check(lib().semb_pcg_solve_host(self._h, C.byref(o), hp(b_host), hp(x_host), C.byref(st), _stream()))
+        return dict(iters=int(st.iters), status=int(rc), r_norm=st.r_norm, b_norm=st.b_norm, launches=int(st.launches))
 
     def estimate_lmax(self, v0, lam, tags, steps=10):
         out = C.c_double(0.0)
