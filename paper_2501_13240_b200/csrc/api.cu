@@ -58,7 +58,7 @@ int semb_destroy(semb_handle h)
     semb_dev_free(h, h->gs_off); semb_dev_free(h, h->gs_ids); semb_dev_free(h, h->face_tag_dev);
     for (auto& kv : h->masks) semb_dev_free(h, kv.second.list);
     for (auto& kv : h->dinvs) semb_dev_free(h, kv.second);
-    semb_dev_free(h, h->work); semb_dev_free(h, h->partials); semb_dev_free(h, h->scal); semb_dev_free(h, h->hist_dev); semb_dev_free(h, h->stage);
+    semb_dev_free(h, h->work); semb_dev_free(h, h->partials); semb_dev_free(h, h->ax_dot); semb_dev_free(h, h->scal); semb_dev_free(h, h->hist_dev); semb_dev_free(h, h->stage);
     if (h->scal_host) cudaFreeHost(h->scal_host);
     for (cudaEvent_t ev : h->prof_ev) cudaEventDestroy(ev);
     for (auto& f : h->fields) if (f.derived) semb_dev_free(h, f.ptr);

@@ -1,0 +1,227 @@
+// axhelm device kernels (sm_100a, fp64):  w = D^T G D u + lambda B u  per hexahedral element
+// (BASELINE.json:north_star; §2.2 "matrix-free ... tensor-product contractions with
+// (p+1)x(p+1) operator matrices identical for all elements").
+//
+//   u_r = sum_m D_im u(m,j,k)   u_s = sum_m D_jm u(i,m,k)   u_t = sum_m D_km u(i,j,m)
+//   g_r = G_rr u_r + G_rs u_s + G_rt u_t,  g_s = G_rs u_r + G_ss u_s + G_st u_t,  g_t = G_rt u_r + G_st u_s + G_tt u_t
+//   w(i,j,k) = sum_m D_mi g_r(m,j,k) + sum_m D_mj g_s(i,m,k) + sum_m D_mk g_t(i,j,m) + lambda B u
+//
+// k_axhelm_line ("line" kernel, the production path).  One block of n1 x n1 threads per element.  Every one
+// of the six contractions is done by a thread that holds a WHOLE line of n1 nodes in registers, so its n1 x n1
+// multiply-adds take D from the constant bank (compile-time indices -> DFMA with a c[][] operand) and touch
+// shared memory only to transpose between the three line orientations:
+//     thread (a,b) owns   t-line (i=a, j=b, k=*)   -- also the layout of every global load/store (coalesced)
+//                         r-line (i=*, j=a, k=b)
+//                         s-line (i=a, j=*, k=b)
+// Shared-memory traffic is 8 transposes x 16 B + 8 B = 136 B per node (about 1.06 wavefronts per node,
+// conflict-free for n1 = 8 through the XOR swizzle below), against 3.7 wavefronts per node of the slab kernel
+// that ncu showed to be bound by the shared-memory pipe (profiles/r1_v1_axhelm_full.md).
+#pragma once
+#include "reduce.cuh"
+#include "semb_internal.h"
+
+// D for every order 1..SEMB_MAX_N, row-major n1 x n1 at c_D[N]; filled at setup.
+__constant__ double c_D[SEMB_MAX_N + 1][SEMB_MAXN1 * SEMB_MAXN1];
+
+// ---- shared-memory layout of one element tile, index (k,j,i) -> double slot -------------------------------
+// All three line orientations read/write it with 64-bit accesses; a half-warp (16 lanes) is conflict-free iff
+// its 16 slots are distinct mod 16.
+template <int n1> struct ax_tile {
+    // padded strides found by exhaustive search (fewest wavefronts over the three orientations)
+    static constexpr int P1 = (n1 == 10) ? 10 : n1;
+    static constexpr int P2 = (n1 == 4) ? 19 : (n1 == 10) ? 101 : n1 * n1;
+    static constexpr int size = n1 * P2;
+    __device__ static __forceinline__ int idx(int k, int j, int i) { return k * P2 + j * P1 + i; }
+};
+// n1 = 8: XOR swizzle, conflict-free in all three orientations without padding:
+//   slot mod 16 = ((j^k)&1)*8 + (i ^ (((j>>1)&3) | ((k&1)<<2)))
+template <> struct ax_tile<8> {
+    static constexpr int size = 512;
+    __device__ static __forceinline__ int idx(int k, int j, int i)
+    {
+        return k * 64 + ((j ^ (k & 1)) << 3) + (i ^ (((j >> 1) & 3) | ((k & 1) << 2)));
+    }
+};
+
+// PCG epilogue shared by the kernels: grid-wide sum of u.w (= p.Ap before assembly, valid because p is
+// continuous and zero at masked nodes: SURVEY.md §8 a-6), then alpha = rho / p.Ap in the last block.
+__device__ __forceinline__ void ax_finish_dot(double dot, semb_scalars* __restrict__ scal, double* __restrict__ partials, double* red)
+{
+    double v[1] = { block_sum(dot, red) }, tot[1];
+    if (grid_sum<1>(v, partials, &scal->ticket[0], tot, red) && threadIdx.x == 0) {
+        const double gamma = tot[0];
+        scal->pAp = gamma;
+        if (!(gamma > 0.0) || !isfinite(gamma)) { scal->status = SEMB_EBREAKDOWN; scal->done = 1; }
+        else scal->alpha = scal->rho_new / gamma;
+    }
+}
+
+// ---- even-odd form of the line contractions ------------------------------------------------------------
+// D (and D^T) are centro-antisymmetric, A[N-i][N-m] = -A[i][m], so with e_m = x_m + x_{N-m}, o_m = x_m - x_{N-m}
+// (m < h = n1/2),  P_im = (A_im + A_i,N-m)/2,  M_im = (A_im - A_i,N-m)/2:
+//     y_i = sum_m M_im o_m + a_i,   y_{N-i} = sum_m M_im o_m - a_i,   a_i = sum_m P_im e_m (+ A_ih x_h, n1 odd)
+// and, for odd n1, the middle row y_h = sum_m M_hm o_m.  That is n1^2/2 multiply-adds plus 2 n1 additions per
+// line instead of n1^2, and only n1^2/2 distinct constants, all at compile-time offsets of the constant bank.
+#define SEMB_EO_H  ((SEMB_MAXN1) / 2)          // max h
+#define SEMB_EO_H2 ((SEMB_MAXN1 + 1) / 2)      // max number of rows i <= h
+struct ax_eo_tab { double P[SEMB_EO_H2 * SEMB_EO_H], M[SEMB_EO_H2 * SEMB_EO_H], mid[SEMB_EO_H2]; };
+__constant__ ax_eo_tab c_EO[SEMB_MAX_N + 1][2];      // [N][0] for D, [N][1] for D^T
+
+// host: fill the two tables of order N from D (row-major n1 x n1)
+static inline void ax_eo_build(int n1, const double* D, ax_eo_tab tab[2])
+{
+    const int N = n1 - 1, h = n1 / 2, h2 = (n1 + 1) / 2;
+    for (int tr = 0; tr < 2; ++tr) {
+        ax_eo_tab& T = tab[tr];
+        for (auto& v : T.P) v = 0.0;
+        for (auto& v : T.M) v = 0.0;
+        for (auto& v : T.mid) v = 0.0;
+        for (int i = 0; i < h2; ++i) {
+            for (int m = 0; m < h; ++m) {
+                const double x = tr ? D[m * n1 + i] : D[i * n1 + m], y = tr ? D[(N - m) * n1 + i] : D[i * n1 + (N - m)];
+                T.P[i * SEMB_EO_H + m] = 0.5 * (x + y);
+                T.M[i * SEMB_EO_H + m] = 0.5 * (x - y);
+            }
+            if (n1 & 1) T.mid[i] = tr ? D[h * n1 + i] : D[i * n1 + h];
+        }
+    }
+}
+
+template <int n1, int TR>
+__device__ __forceinline__ void ax_line(const double (&x)[n1], double (&y)[n1])
+{
+    constexpr int N = n1 - 1, h = n1 / 2;
+    constexpr bool odd = n1 & 1;
+    const ax_eo_tab& T = c_EO[N][TR];
+    double e[h > 0 ? h : 1], o[h > 0 ? h : 1];
+#pragma unroll
+    for (int m = 0; m < h; ++m) { e[m] = x[m] + x[N - m]; o[m] = x[m] - x[N - m]; }
+#pragma unroll
+    for (int i = 0; i < h; ++i) {
+        double a = odd ? T.mid[i] * x[h] : 0.0, s = 0.0;
+#pragma unroll
+        for (int m = 0; m < h; ++m) { a += T.P[i * SEMB_EO_H + m] * e[m]; s += T.M[i * SEMB_EO_H + m] * o[m]; }
+        y[i] = s + a; y[N - i] = s - a;
+    }
+    if (odd) {
+        double s = 0.0;
+#pragma unroll
+        for (int m = 0; m < h; ++m) s += T.M[h * SEMB_EO_H + m] * o[m];
+        y[h] = s;
+    }
+}
+
+// MODE bit 0: Helmholtz term lambda*B*u (7th factor);  bit 1: per-node coefficient fields lam0 / lam1.
+// One block per (element, field): grid = E * nfields.  dot_out != NULL: block b writes its partial sum of
+// u.w to dot_out[b] (fixed summation order; reduced by k_ax_dot_finish).
+template <int n1, int MODE, int MINB>
+__global__ void __launch_bounds__(n1 * n1, MINB)
+k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambda,
+              const double* __restrict__ lam0, const double* __restrict__ lam1,
+              const double* __restrict__ u, double* __restrict__ w,
+              const semb_scalars* __restrict__ scal, double* __restrict__ dot_out)
+{
+    constexpr int n2 = n1 * n1, Np = n1 * n1 * n1;
+    constexpr bool HELM = MODE & 1, VAR = MODE & 2;
+    constexpr int NG = HELM ? 7 : 6;
+    using T = ax_tile<n1>;
+    __shared__ double Su[T::size], Sr[T::size], Ss[T::size];
+    if (scal && *(volatile const int32_t*)&scal->done) return;
+    const int a = threadIdx.x % n1, b = threadIdx.x / n1;
+    const int64_t e = blockIdx.x % E, f = blockIdx.x / E;
+    const double* __restrict__ ue = u + f * n + e * Np + threadIdx.x;
+    double* __restrict__ we = w + f * n + e * Np + threadIdx.x;
+    const double* __restrict__ g = geo + e * 7 * (int64_t)Np + threadIdx.x;
+    // ---- global loads, t-line layout: lane -> consecutive nodes of plane k (coalesced 64-bit)
+    double ru[n1], G[NG][n1];
+#pragma unroll
+    for (int k = 0; k < n1; ++k) ru[k] = ue[k * n2];
+#pragma unroll
+    for (int k = 0; k < n1; ++k) {
+#pragma unroll
+        for (int c = 0; c < NG; ++c) G[c][k] = __ldg(g + c * Np + k * n2);
+    }
+#pragma unroll
+    for (int k = 0; k < n1; ++k) Su[T::idx(k, b, a)] = ru[k];
+    __syncthreads();
+    // ---- forward contractions, one line per orientation
+    {
+        double ln[n1], out[n1];
+#pragma unroll
+        for (int i = 0; i < n1; ++i) ln[i] = Su[T::idx(b, a, i)];
+        ax_line<n1, 0>(ln, out);
+#pragma unroll
+        for (int i = 0; i < n1; ++i) Sr[T::idx(b, a, i)] = out[i];
+#pragma unroll
+        for (int j = 0; j < n1; ++j) ln[j] = Su[T::idx(b, j, a)];
+        ax_line<n1, 0>(ln, out);
+#pragma unroll
+        for (int j = 0; j < n1; ++j) Ss[T::idx(b, j, a)] = out[j];
+    }
+    double ut[n1];
+    ax_line<n1, 0>(ru, ut);
+    __syncthreads();
+    // ---- geometric factors at the nodes of the t-line
+    double gt[n1];
+#pragma unroll
+    for (int k = 0; k < n1; ++k) {
+        const int s = T::idx(k, b, a);
+        const double ur = Sr[s], us = Ss[s];
+        double Grr = G[0][k], Grs = G[1][k], Grt = G[2][k], Gss = G[3][k], Gst = G[4][k], Gtt = G[5][k];
+        if (VAR && lam0) { const double c = lam0[e * Np + k * n2 + threadIdx.x]; Grr *= c; Grs *= c; Grt *= c; Gss *= c; Gst *= c; Gtt *= c; }
+        Sr[s] = Grr * ur + Grs * us + Grt * ut[k];
+        Ss[s] = Grs * ur + Gss * us + Gst * ut[k];
+        gt[k] = Grt * ur + Gst * us + Gtt * ut[k];
+    }
+    __syncthreads();
+    // ---- transposed contractions
+    {
+        double ln[n1], out[n1];
+#pragma unroll
+        for (int i = 0; i < n1; ++i) ln[i] = Sr[T::idx(b, a, i)];
+        ax_line<n1, 1>(ln, out);
+#pragma unroll
+        for (int i = 0; i < n1; ++i) Sr[T::idx(b, a, i)] = out[i];
+#pragma unroll
+        for (int j = 0; j < n1; ++j) ln[j] = Ss[T::idx(b, j, a)];
+        ax_line<n1, 1>(ln, out);
+#pragma unroll
+        for (int j = 0; j < n1; ++j) Ss[T::idx(b, j, a)] = out[j];
+    }
+    double wt[n1];
+    ax_line<n1, 1>(gt, wt);
+    if (HELM) {
+#pragma unroll
+        for (int k = 0; k < n1; ++k) {
+            const double lam = (VAR && lam1) ? lam1[e * Np + k * n2 + threadIdx.x] : lambda;
+            wt[k] += lam * G[NG - 1][k] * ru[k];
+        }
+    }
+    __syncthreads();
+    double dot = 0.0;
+#pragma unroll
+    for (int k = 0; k < n1; ++k) {
+        const int s = T::idx(k, b, a);
+        const double wv = wt[k] + Sr[s] + Ss[s];
+        we[k * n2] = wv;
+        dot += ru[k] * wv;
+    }
+    if (dot_out) {
+        __shared__ double red[32];
+        dot = block_sum(dot, red);
+        if (threadIdx.x == 0) dot_out[blockIdx.x] = dot;
+    }
+}
+
+// Sum of the per-block partials dot_in[0..count) in a fixed order (two stages, last block by ticket), then
+// the PCG scalars: p.Ap, alpha = rho / p.Ap, breakdown detection.
+__global__ void __launch_bounds__(256)
+k_ax_dot_finish(int64_t count, const double* __restrict__ dot_in, semb_scalars* __restrict__ scal, double* __restrict__ partials)
+{
+    __shared__ double red[32];
+    if (*(volatile int32_t*)&scal->done) return;
+    double s = 0.0;
+    const int64_t per = (count + gridDim.x - 1) / gridDim.x, lo = blockIdx.x * per, hi = (lo + per < count) ? lo + per : count;
+    for (int64_t q = lo + threadIdx.x; q < hi; q += blockDim.x) s += dot_in[q];
+    ax_finish_dot(s, scal, partials, red);
+}

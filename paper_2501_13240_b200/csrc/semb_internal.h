@@ -52,6 +52,7 @@ struct semb_mesh {
     // solver workspace
     double* work = nullptr; int64_t work_vecs = 0;
     double* partials = nullptr;         // block partial sums [4][SEMB_MAX_BLOCKS]
+    double* ax_dot = nullptr;           // per-element partials of p.Ap written by axhelm [E]
     semb_scalars* scal = nullptr;       // device
     semb_scalars* scal_host = nullptr;  // pinned mirror
     double* hist_dev = nullptr; int hist_cap = 0;
