@@ -2,14 +2,15 @@
 """bench.py — headline benchmark of the SEM hot path on B200 (BASELINE.json metric).
 
 A "step" is one pass of the whole hot path over the synthetic batch: ONE Jacobi-PCG pressure iteration
-(axhelm with fused p.Ap -> gather-scatter -> Dirichlet mask -> fused x/r update with the ||r||^2 and r.z
-reductions -> Jacobi + direction update) on the 64^3-element deformed box of BASELINE.json configs[3]
+(axhelm with the fused x / Jacobi + direction updates and p.Ap -> gather-scatter -> Dirichlet mask -> r update with
+the ||r||^2 and r.z reductions) on the 64^3-element deformed box of BASELINE.json configs[3]
 (N = 7, fp64, 134 217 728 local nodes, lambda = 0).  K steps = one semb_pcg_solve call with maxit = K and
 rtol = 0 (it cannot stop early), bracketed by CUDA events on the launching stream.
 
     value     = local nodes processed per second by the whole step (GDOF/s), all ranks
-    roofline  = the dominant kernel (axhelm): 64 B/node algorithmic bytes / its mean device time measured with
-                CUDA event pairs around its launches INSIDE the timed solve, against MEASURED_PEAKS.json hbm_gbs
+    roofline  = the dominant kernel (the PCG-fused axhelm launch): 104 B/node algorithmic bytes / its mean device
+                time measured with CUDA event pairs around its launches INSIDE the timed solve, against
+                MEASURED_PEAKS.json hbm_gbs; axhelm_sweep = the stand-alone operator at 64 / 72 B/node
     pcg_iter  = the whole iteration against the fixed 171.6 B/node model
     e2e       = the same K iterations through semb_pcg_solve_host: b from pinned host memory, x back to it
     cpu_baseline = the oracle (oracle/semoracle.c, as it stands) timed on this box's host cores
@@ -35,6 +36,7 @@ METRIC = "SEM Jacobi-PCG pressure-iteration throughput (axhelm+gather-scatter+ma
 UNIT = "GDOF/s"
 B_AXHELM = 64.0          # algorithmic bytes per node, Poisson axhelm
 B_AXHELM_HELM = 72.0
+B_AXHELM_PCG = 104.0     # the PCG-fused launch: reads r, dinv, p, x (32) + G (48), writes p, x, q (24)
 B_ITER = 171.6           # algorithmic bytes per node per Jacobi-PCG iteration, N = 7, Poisson
 WORKLOADS = {            # name -> elements per direction of the deformed box (BASELINE.json configs[3] / configs[1])
     "cfg3_box64_deformed_N7": 64,
@@ -90,6 +92,21 @@ class ClockSampler:
                     reasons.add(nme)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def aggregate(ms_local, nodes_local, steps, dist=None, device=None):
+    """Whole-job figure from per-rank device times (replicas only): every rank processed
+    nodes_local x steps node updates in ms_local milliseconds; the job took the MAX over ranks and processed the
+    SUM over ranks.  Returns (ms, value in GDOF/s).  `dist` = an initialised torch.distributed module or None."""
+    import torch
+    ms, total = float(ms_local), float(nodes_local) * steps
+    if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        c = torch.tensor([total], dtype=torch.float64, device=device)
+        dist.all_reduce(c, op=dist.ReduceOp.SUM)
+        ms, total = float(t.item()), float(c.item())
+    return ms, total / (ms * 1e-3) / 1e9
 
 
 def build_problem(torch, semb, ne):
@@ -195,14 +212,10 @@ def main():
     clocks = sampler.stop()
     ms = e0.elapsed_time(e1)
     assert st["iters"] == K, st
-    if dist is not None:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms, value = aggregate(ms, n, K, dist, "cuda")
     ms_step = ms / K
-    value = world * n * K / (ms * 1e-3) / 1e9
     ax_ms = st["axhelm_ms"]
-    ax_gbs = B_AXHELM * n / (ax_ms * 1e-3) / 1e9
+    ax_gbs = B_AXHELM_PCG * n / (ax_ms * 1e-3) / 1e9
 
     # ---- axhelm alone, Poisson and Helmholtz (BASELINE.json configs[3] "roofline sweep"); not the headline
     u = torch.from_numpy(I.uniform(I.seed_for(3, 1), n)).cuda()
@@ -234,10 +247,8 @@ def main():
         G.pcg_solve_host(bh, xh, maxit=K, check_every=K, **solve)
         h1.record(); barrier()
         hms = h0.elapsed_time(h1)
-        if dist is not None:
-            t = torch.tensor([hms], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX); hms = float(t.item())
-        e2e = {"value": world * n * K / (hms * 1e-3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": 8 * n / K,
+        hms, e2e_value = aggregate(hms, n, K, dist, "cuda")
+        e2e = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 8 * n / K,
                "d2h_bytes_per_step": 8 * n / K, "note": "one call = b host->device, K iterations, x device->host"}
 
     line = {
@@ -247,9 +258,9 @@ def main():
         "config": {"workload": args.workload, "E": m.E, "N": 7, "local_nodes": n, "lambda": 0.0,
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": "inputs larger than L2 (every vector is %.2f GB)" % (8 * n / 1e9)},
-        "roofline": {"bound": "hbm", "kernel": "axhelm (Poisson, fused p.Ap)", "achieved": ax_gbs, "peak": peak,
+        "roofline": {"bound": "hbm", "kernel": "k_axhelm_line<8,4,4>: axhelm (Poisson) with the fused PCG prologue (x += alpha p, p = dinv r + beta p) and p.Ap epilogue", "achieved": ax_gbs, "peak": peak,
                      "unit": "GB/s", "frac": ax_gbs / peak, "traffic": None, "peak_source": peak_src,
-                     "bytes_per_node": B_AXHELM, "ms": ax_ms, "timed_launches": st["profiled"],
+                     "bytes_per_node": B_AXHELM_PCG, "ms": ax_ms, "timed_launches": st["profiled"],
                      "frac_of_8TBs": ax_gbs / 8000.0, "gdofs": n / (ax_ms * 1e-3) / 1e9},
         "pcg_iter": {"ms": ms_step, "model_bytes_per_node": B_ITER, "gbs": B_ITER * n / (ms_step * 1e-3) / 1e9,
                      "frac_of_measured_peak": B_ITER * n / (ms_step * 1e-3) / 1e9 / peak,

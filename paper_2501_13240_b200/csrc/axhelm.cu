@@ -27,16 +27,21 @@ template <int n1> struct ax_minb { static constexpr int v = (n1 <= 4) ? 16 : (n1
 
 template <int n1>
 static int launch_line(semb_mesh* h, int mode, double lambda, const double* lam0, const double* lam1,
-                       const double* u, double* w, int nfields, semb_scalars* scal, cudaStream_t s)
+                       const double* u, double* w, int nfields, semb_scalars* scal, const ax_pcg_args& pcg, cudaStream_t s)
 {
     constexpr int MB = ax_minb<n1>::v;
     const unsigned grid = (unsigned)(h->E * nfields);
     double* dot = scal ? h->ax_dot : nullptr;
+#define SEMB_AX_LAUNCH(M) k_axhelm_line<n1, M, MB><<<grid, n1 * n1, 0, s>>>(h->E, h->n, h->geoK, lambda, lam0, lam1, u, w, scal, dot, pcg)
     switch (mode) {
-        case 0: k_axhelm_line<n1, 0, MB><<<grid, n1 * n1, 0, s>>>(h->E, h->n, h->geoK, lambda, lam0, lam1, u, w, scal, dot); break;
-        case 1: k_axhelm_line<n1, 1, MB><<<grid, n1 * n1, 0, s>>>(h->E, h->n, h->geoK, lambda, lam0, lam1, u, w, scal, dot); break;
-        default: k_axhelm_line<n1, 3, MB><<<grid, n1 * n1, 0, s>>>(h->E, h->n, h->geoK, lambda, lam0, lam1, u, w, scal, dot); break;
+        case 0: SEMB_AX_LAUNCH(0); break;
+        case 1: SEMB_AX_LAUNCH(1); break;
+        case 3: SEMB_AX_LAUNCH(3); break;
+        case 4: SEMB_AX_LAUNCH(4); break;
+        case 5: SEMB_AX_LAUNCH(5); break;
+        default: return semb_fail(h, SEMB_EINVAL, "axhelm: unsupported mode %d", mode);
     }
+#undef SEMB_AX_LAUNCH
     h->launches += 1;
     if (scal) {
         // p.Ap = sum of the per-element partials, alpha = rho / p.Ap (fixed order: bit-reproducible)
@@ -49,26 +54,41 @@ static int launch_line(semb_mesh* h, int mode, double lambda, const double* lam0
     return SEMB_OK;
 }
 
-int semb_axhelm_launch(semb_mesh* h, double lambda, const double* lam0, const double* lam1,
-                       const double* u, double* w, int nfields, semb_scalars* scal, cudaStream_t s)
+static int axhelm_dispatch(semb_mesh* h, int mode, double lambda, const double* lam0, const double* lam1,
+                           const double* u, double* w, int nfields, semb_scalars* scal, const ax_pcg_args& pcg, cudaStream_t s)
 {
-    const int mode = (lam0 || lam1) ? 3 : (lambda != 0.0) ? 1 : 0;
     if (scal && nfields != 1) return semb_fail(h, SEMB_EINVAL, "axhelm: fused p.Ap needs nfields == 1");
     if (scal && !h->ax_dot) {
         h->ax_dot = (double*)semb_dev_alloc(h, sizeof(double) * (size_t)h->E);
         if (!h->ax_dot) return semb_fail(h, SEMB_ENOMEM, "axhelm: p.Ap partials");
     }
     switch (h->n1) {
-        case 2:  return launch_line<2>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, s);
-        case 3:  return launch_line<3>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, s);
-        case 4:  return launch_line<4>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, s);
-        case 5:  return launch_line<5>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, s);
-        case 6:  return launch_line<6>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, s);
-        case 7:  return launch_line<7>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, s);
-        case 8:  return launch_line<8>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, s);
-        case 9:  return launch_line<9>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, s);
-        case 10: return launch_line<10>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, s);
-        case 11: return launch_line<11>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, s);
+        case 2:  return launch_line<2>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, pcg, s);
+        case 3:  return launch_line<3>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, pcg, s);
+        case 4:  return launch_line<4>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, pcg, s);
+        case 5:  return launch_line<5>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, pcg, s);
+        case 6:  return launch_line<6>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, pcg, s);
+        case 7:  return launch_line<7>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, pcg, s);
+        case 8:  return launch_line<8>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, pcg, s);
+        case 9:  return launch_line<9>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, pcg, s);
+        case 10: return launch_line<10>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, pcg, s);
+        case 11: return launch_line<11>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, pcg, s);
     }
     return semb_fail(h, SEMB_EINVAL, "unsupported order N=%d", h->N);
+}
+
+int semb_axhelm_launch(semb_mesh* h, double lambda, const double* lam0, const double* lam1,
+                       const double* u, double* w, int nfields, semb_scalars* scal, cudaStream_t s)
+{
+    const int mode = (lam0 || lam1) ? 3 : (lambda != 0.0) ? 1 : 0;
+    return axhelm_dispatch(h, mode, lambda, lam0, lam1, u, w, nfields, scal, ax_pcg_args{nullptr, nullptr, nullptr, nullptr}, s);
+}
+
+// PCG-fused form (pcg.cu): x += alpha p_old (if pending), p = dinv o zsrc + beta p_old, q = A_L p, partial p.q;
+// then p.Ap and alpha.  dinv may be NULL (z = zsrc).
+int semb_axhelm_pcg_launch(semb_mesh* h, double lambda, const double* zsrc, const double* dinv, double* p, double* x,
+                           double* q, semb_scalars* scal, cudaStream_t s)
+{
+    const int mode = 4 | ((lambda != 0.0) ? 1 : 0);
+    return axhelm_dispatch(h, mode, lambda, nullptr, nullptr, nullptr, q, 1, scal, ax_pcg_args{zsrc, dinv, p, x}, s);
 }

@@ -51,8 +51,8 @@ __device__ __forceinline__ void ax_finish_dot(double dot, semb_scalars* __restri
     if (grid_sum<1>(v, partials, &scal->ticket[0], tot, red) && threadIdx.x == 0) {
         const double gamma = tot[0];
         scal->pAp = gamma;
-        if (!(gamma > 0.0) || !isfinite(gamma)) { scal->status = SEMB_EBREAKDOWN; scal->done = 1; }
-        else scal->alpha = scal->rho_new / gamma;
+        if (!(gamma > 0.0) || !isfinite(gamma)) { scal->status = SEMB_EBREAKDOWN; scal->done = 1; scal->x_pending = 0; }
+        else { scal->alpha = scal->rho_new / gamma; scal->x_pending = 1; }   // x += alpha p is applied by the next fused axhelm
     }
 }
 
@@ -111,31 +111,64 @@ __device__ __forceinline__ void ax_line(const double (&x)[n1], double (&y)[n1])
     }
 }
 
-// MODE bit 0: Helmholtz term lambda*B*u (7th factor);  bit 1: per-node coefficient fields lam0 / lam1.
+// MODE bit 0: Helmholtz term lambda*B*u (7th factor);  bit 1: per-node coefficient fields lam0 / lam1;
+// bit 2: PCG-fused prologue (nfields = 1): before the operator is applied the thread updates its own nodes
+//     x += alpha * p_old  (the x-update of the PREVIOUS iteration, pending in scal)   and
+//     p  = z + beta * p_old,  z = dinv o zsrc  (Jacobi), zsrc (none / Chebyshev's z)
+// writes x and p back and applies the operator to the new p, so p is read once per iteration instead of three
+// times (SURVEY.md §8 a-6 (iii),(iv) folded into (i)).  u is then unused; p_io is both input and output.
 // One block per (element, field): grid = E * nfields.  dot_out != NULL: block b writes its partial sum of
 // u.w to dot_out[b] (fixed summation order; reduced by k_ax_dot_finish).
+struct ax_pcg_args { const double* zsrc; const double* dinv; double* p_io; double* x; };
+
 template <int n1, int MODE, int MINB>
 __global__ void __launch_bounds__(n1 * n1, MINB)
 k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambda,
               const double* __restrict__ lam0, const double* __restrict__ lam1,
               const double* __restrict__ u, double* __restrict__ w,
-              const semb_scalars* __restrict__ scal, double* __restrict__ dot_out)
+              const semb_scalars* __restrict__ scal, double* __restrict__ dot_out, ax_pcg_args pcg)
 {
     constexpr int n2 = n1 * n1, Np = n1 * n1 * n1;
-    constexpr bool HELM = MODE & 1, VAR = MODE & 2;
+    constexpr bool HELM = MODE & 1, VAR = MODE & 2, FUSE = MODE & 4;
     constexpr int NG = HELM ? 7 : 6;
     using T = ax_tile<n1>;
     __shared__ double Su[T::size], Sr[T::size], Ss[T::size];
     if (scal && *(volatile const int32_t*)&scal->done) return;
     const int a = threadIdx.x % n1, b = threadIdx.x / n1;
     const int64_t e = blockIdx.x % E, f = blockIdx.x / E;
-    const double* __restrict__ ue = u + f * n + e * Np + threadIdx.x;
     double* __restrict__ we = w + f * n + e * Np + threadIdx.x;
     const double* __restrict__ g = geo + e * 7 * (int64_t)Np + threadIdx.x;
-    // ---- global loads, t-line layout: lane -> consecutive nodes of plane k (coalesced 64-bit)
     double ru[n1], G[NG][n1];
+    if (FUSE) {
+        const int64_t l0 = e * Np + threadIdx.x;
+        const double beta = scal->beta, alpha = scal->alpha;
+        const bool pend = scal->x_pending != 0, first = (beta == 0.0);
+        double z[n1], po[n1];
 #pragma unroll
-    for (int k = 0; k < n1; ++k) ru[k] = ue[k * n2];
+        for (int k = 0; k < n1; ++k) z[k] = pcg.zsrc[l0 + k * n2];
+        if (pcg.dinv) {
+#pragma unroll
+            for (int k = 0; k < n1; ++k) z[k] *= pcg.dinv[l0 + k * n2];
+        }
+        if (pend || !first) {
+#pragma unroll
+            for (int k = 0; k < n1; ++k) po[k] = pcg.p_io[l0 + k * n2];
+        }
+        if (pend) {
+#pragma unroll
+            for (int k = 0; k < n1; ++k) pcg.x[l0 + k * n2] += alpha * po[k];
+        }
+#pragma unroll
+        for (int k = 0; k < n1; ++k) {
+            ru[k] = first ? z[k] : z[k] + beta * po[k];
+            pcg.p_io[l0 + k * n2] = ru[k];
+        }
+    } else {
+        const double* __restrict__ ue = u + f * n + e * Np + threadIdx.x;
+#pragma unroll
+        for (int k = 0; k < n1; ++k) ru[k] = ue[k * n2];
+    }
+    // ---- global loads, t-line layout: lane -> consecutive nodes of plane k (coalesced 64-bit)
 #pragma unroll
     for (int k = 0; k < n1; ++k) {
 #pragma unroll

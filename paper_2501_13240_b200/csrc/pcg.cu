@@ -51,30 +51,19 @@ k_pcg_init(int64_t n, const double* __restrict__ b, const double* __restrict__ q
     }
 }
 
-// p = z + beta p,  z = dinv o r (Jacobi), r (none) or a given z (Chebyshev)
-__global__ void __launch_bounds__(VEC_BLOCK)
-k_update_p(int64_t n, const double* __restrict__ zsrc, const double* __restrict__ dinv, double* __restrict__ p,
-           const semb_scalars* __restrict__ scal)
-{
-    if (STOPPED(scal)) return;
-    const double beta = scal->beta;
-    if (beta == 0.0) { GSTRIDE(l, n) p[l] = dinv ? dinv[l] * zsrc[l] : zsrc[l]; }
-    else             { GSTRIDE(l, n) p[l] = (dinv ? dinv[l] * zsrc[l] : zsrc[l]) + beta * p[l]; }
-}
-
-// x += alpha p; r -= alpha q; rr = <r,r>, rz = <r, dinv r>; the last block closes the iteration
+// r -= alpha q; rr = <r,r>, rz = <r, dinv r>; the last block closes the iteration.  (x += alpha p and
+// p = z + beta p are done by the next fused axhelm launch, which reads p anyway: axhelm_kernels.cuh MODE bit 2.)
 template <bool FUSED_Z>
 __global__ void __launch_bounds__(VEC_BLOCK)
-k_update_xr(int64_t n, const double* __restrict__ p, const double* __restrict__ q, double* __restrict__ x,
-            double* __restrict__ r, const double* __restrict__ invmult, const double* __restrict__ dinv,
-            semb_scalars* __restrict__ scal, double* __restrict__ partials, double* __restrict__ hist, int hist_cap)
+k_update_r(int64_t n, const double* __restrict__ q, double* __restrict__ r, const double* __restrict__ invmult,
+           const double* __restrict__ dinv, semb_scalars* __restrict__ scal, double* __restrict__ partials,
+           double* __restrict__ hist, int hist_cap)
 {
     __shared__ double red[32];
     if (STOPPED(scal)) return;
     const double alpha = scal->alpha;
     double rr = 0.0, rz = 0.0;
     GSTRIDE(l, n) {
-        x[l] += alpha * p[l];
         const double rl = r[l] - alpha * q[l];
         r[l] = rl;
         const double t = rl * rl * invmult[l];
@@ -92,6 +81,15 @@ k_update_xr(int64_t n, const double* __restrict__ p, const double* __restrict__ 
         if (scal->rnorm <= scal->target) { scal->done = 1; scal->status = SEMB_OK; }
         else if (it >= scal->maxit) { scal->done = 1; scal->status = SEMB_MAXIT; }
     }
+}
+
+// the x-update of the last iteration, still pending when the loop stops
+__global__ void __launch_bounds__(VEC_BLOCK)
+k_final_x(int64_t n, const double* __restrict__ p, double* __restrict__ x, const semb_scalars* __restrict__ scal)
+{
+    if (!scal->x_pending) return;
+    const double alpha = scal->alpha;
+    GSTRIDE(l, n) x[l] += alpha * p[l];
 }
 
 // rho_new = <r,z>, beta = rho_new / rho_old (0 in the first iteration)   [Chebyshev path]
@@ -366,23 +364,21 @@ int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* 
     for (int it0 = 0; it0 < o->maxit && !finished; it0 += check) {
         const int mbatch = (o->maxit - it0 < check) ? o->maxit - it0 : check;
         for (int i = 0; i < mbatch; ++i) {
+            const double* zsrc = r;
             if (o->precond == 2) {
                 rc = cheb_apply(h, o->lambda, m, dinv, o->cheb_degree, cc, r, z, res, d, q, h->scal, s); if (rc) return rc;
                 k_dot_rz<<<G, VEC_BLOCK, 0, s>>>(n, r, z, h->invmult, h->scal, h->partials);
-                k_update_p<<<G, VEC_BLOCK, 0, s>>>(n, z, nullptr, p, h->scal);
-                h->launches += 2;
-            } else {
-                k_update_p<<<G, VEC_BLOCK, 0, s>>>(n, r, dz, p, h->scal);
                 h->launches += 1;
+                zsrc = z;
             }
             const int itn = it0 + i;
             if (itn < nprof) SEMB_CUDA(h, cudaEventRecord(h->prof_ev[2 * itn], s));
-            rc = semb_axhelm_launch(h, o->lambda, nullptr, nullptr, p, q, 1, h->scal, s); if (rc) return rc;
+            rc = semb_axhelm_pcg_launch(h, o->lambda, zsrc, dz, p, x, q, h->scal, s); if (rc) return rc;
             if (itn < nprof) SEMB_CUDA(h, cudaEventRecord(h->prof_ev[2 * itn + 1], s));
             rc = semb_gs_launch(h, q, 1, s); if (rc) return rc;
             rc = semb_mask_launch(h, m, q, 1, s); if (rc) return rc;
-            if (o->precond == 2) k_update_xr<false><<<G, VEC_BLOCK, 0, s>>>(n, p, q, x, r, h->invmult, nullptr, h->scal, h->partials, hist, want_hist);
-            else                 k_update_xr<true><<<G, VEC_BLOCK, 0, s>>>(n, p, q, x, r, h->invmult, dz, h->scal, h->partials, hist, want_hist);
+            if (o->precond == 2) k_update_r<false><<<G, VEC_BLOCK, 0, s>>>(n, q, r, h->invmult, nullptr, h->scal, h->partials, hist, want_hist);
+            else                 k_update_r<true><<<G, VEC_BLOCK, 0, s>>>(n, q, r, h->invmult, dz, h->scal, h->partials, hist, want_hist);
             h->launches += 1;
         }
         SEMB_CUDA(h, cudaGetLastError());
@@ -390,6 +386,7 @@ int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* 
         SEMB_CUDA(h, cudaStreamSynchronize(s));
         finished = h->scal_host->done != 0;
     }
+    if (o->maxit > 0) { k_final_x<<<G, VEC_BLOCK, 0, s>>>(n, p, x, h->scal); h->launches += 1; SEMB_CUDA(h, cudaGetLastError()); }
     if (o->maxit == 0 || !finished) {
         SEMB_CUDA(h, cudaMemcpyAsync(h->scal_host, h->scal, sizeof(semb_scalars), cudaMemcpyDeviceToHost, s));
         SEMB_CUDA(h, cudaStreamSynchronize(s));

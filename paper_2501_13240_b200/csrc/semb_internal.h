@@ -16,7 +16,7 @@
 // mirror receives it when the host polls the stop flag.
 struct semb_scalars {
     double rho_old, rho_new, pAp, alpha, beta, rr, rz, rnorm, bnorm, r0norm, target, rtol, atol, aux;
-    int32_t iter, done, status, maxit;
+    int32_t iter, done, status, maxit, x_pending, pad_;
     uint32_t ticket[8];
 };
 
@@ -97,6 +97,9 @@ int semb_axhelm_prepare_geo(semb_mesh* h, cudaStream_t s);
 // scal->pAp = sum_l u_l w_l and scal->alpha = scal->rho_new / scal->pAp (breakdown -> status, done).
 int semb_axhelm_launch(semb_mesh* h, double lambda, const double* lam0, const double* lam1,
                        const double* u, double* w, int nfields, semb_scalars* scal, cudaStream_t s);
+
+int semb_axhelm_pcg_launch(semb_mesh* h, double lambda, const double* zsrc, const double* dinv, double* p, double* x,
+                           double* q, semb_scalars* scal, cudaStream_t s);
 
 // ---- gs.cu
 int semb_gs_launch(semb_mesh* h, double* w, int nfields, cudaStream_t s);

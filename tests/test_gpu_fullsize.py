@@ -1,0 +1,214 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times.
+
+  * cfg3 (64^3 deformed box, N=7, 134 M local nodes, the bench workload): the oracle cannot number or apply a mesh
+    of this size in seconds, so (i) axhelm is compared on SAMPLED ELEMENTS (elements are independent: the oracle
+    computes G and w for the sampled elements alone, Poisson and Helmholtz), (ii) the numbering is compared
+    bit-exactly with the structured-lattice formula (itself pinned against the oracle's numbering on small boxes in
+    test_oracle_operator.py), (iii) gather-scatter is checked through a property that holds at any size: an
+    integer-valued continuous field sums exactly, QQ^T v = mult * v bitwise, with mult from the lattice.
+  * cfg1 (16^3 deformed box): everything element by element against the oracle.
+  * cfg2 (cylinder O-grid, 73 728 elements, N=7): numbering bit-exact, axhelm and gather-scatter element by element,
+    Chebyshev(2)-Jacobi and Jacobi PCG: first 20 residual-history entries and the ORACLE-VERIFIED true residual
+    ||b - A_oracle x_gpu|| / ||b|| <= 2e-10.
+  * cfg4 (O-grid, 64 000 elements, N=9): numbering, axhelm, gather-scatter, one Helmholtz solve, same bars.
+"""
+import numpy as np
+import pytest
+
+from paper_2501_13240_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-12
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("CUDA device required for -m gpu tests (there is no CPU fallback)")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def semb():
+    from paper_2501_13240_b200 import semb as S
+    S.lib()
+    return S
+
+
+def dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def normwise(a, ref):
+    return np.abs(a - ref).max() / max(np.abs(ref).max(), 1e-300)
+
+
+def geometry_tolerance(orc, m):
+    """Parity bar for outputs that depend on G when BOTH sides recompute G from the coordinates (R16):
+    differentiating coordinates of size c with D (||D||_inf = max row sum) has absolute error <= ~eps ||D||_inf c,
+    against a derivative of size (element half-width) = min node spacing / (xi_1 - xi_0); the ratio is the
+    conditioning of G, identical for the oracle and the GPU, so two correct fp64 evaluations may differ by
+    2 eps kappa.  1e-12 (north_star) wherever that bound is smaller."""
+    xi = orc.gll(m.N)[0]
+    D = orc.dhat(m.N)
+    cmax = max(np.abs(m.x).max(), np.abs(m.y).max(), np.abs(m.z).max())
+    kappa = np.abs(D).sum(axis=1).max() * cmax * (xi[1] - xi[0]) / orc.min_spacing(m.E, m.N, m.x, m.y, m.z)
+    return max(TOL, 2.0 * np.finfo(np.float64).eps * kappa)
+
+
+def lattice_ids(ne, N):
+    """Structured-lattice global index of every local node of an ne^3 box (no periodicity), int64 [n]."""
+    G = ne * N + 1
+    e1 = np.arange(ne, dtype=np.int64)[:, None] * N + np.arange(N + 1, dtype=np.int64)[None, :]     # [ne, n1]
+    shape = (ne, ne, ne, N + 1, N + 1, N + 1)                                                       # ez,ey,ex,k,j,i
+    gx = np.broadcast_to(e1[None, None, :, None, None, :], shape)
+    gy = np.broadcast_to(e1[None, :, None, None, :, None], shape)
+    gz = np.broadcast_to(e1[:, None, None, :, None, None], shape)
+    lat = ((gz * G + gy) * G + gx).reshape(-1)
+    return lat, G
+
+
+def lattice_mult(ne, N):
+    """copies of each local node's global node: 2 per direction in which it lies on an interior element interface"""
+    m1 = np.ones((ne, N + 1), dtype=np.float64)
+    m1[1:, 0] = 2.0
+    m1[:-1, N] = 2.0
+    shape = (ne, ne, ne, N + 1, N + 1, N + 1)
+    mult = (np.broadcast_to(m1[None, None, :, None, None, :], shape) * np.broadcast_to(m1[None, :, None, None, :, None], shape)
+            * np.broadcast_to(m1[:, None, None, :, None, None], shape))
+    return mult.reshape(-1)
+
+
+def first_touch_ids(lat):
+    """canonical ids: classes ordered by their smallest local index (SURVEY c-6)"""
+    uniq, first, inv = np.unique(lat, return_index=True, return_inverse=True)
+    rank = np.empty(len(uniq), dtype=np.int64)
+    rank[np.argsort(first, kind="stable")] = np.arange(len(uniq))
+    return rank[inv].astype(np.int32), len(uniq)
+
+
+def test_cfg3_fullsize_bench_configuration(torch_cuda, semb, orc, xi_of):
+    torch = torch_cuda
+    ne, N = 64, 7
+    m = I.box_mesh(ne, ne, ne, N, semb.gll(N)[0], deform=0.05, name="cfg3")         # exactly bench.build_problem
+    G = semb.Mesh(m.E, m.N, dev(torch, m.x), dev(torch, m.y), dev(torch, m.z), m.face_tag, m.period)
+    try:
+        n, Np = m.n, 512
+        assert n == 134217728
+        # ---- counts (closed forms) and numbering (lattice formula), bit-exact
+        Gd = ne * N + 1
+        assert G.n_unique == Gd ** 3 == 90518849
+        assert G.n_gs == Gd ** 3 - (Gd - ne + 1) ** 3
+        assert G.n_shared == n - (ne * (N - 1) + 2) ** 3
+        lat, _ = lattice_ids(ne, N)
+        gid_ref, nu = first_touch_ids(lat)
+        assert nu == G.n_unique
+        assert np.array_equal(G.gid_host(), gid_ref)
+        del gid_ref
+        # ---- axhelm on sampled elements, Poisson and Helmholtz, the launch bench.py times
+        u = I.uniform(I.seed_for(3, 1), n)
+        ud = dev(torch, u)
+        wd = torch.empty_like(ud)
+        rng = np.random.default_rng(I.seed_for(3, 7))
+        sample = np.unique(np.concatenate([[0, 1, ne - 1, ne * ne - 1, m.E // 2, m.E - 2, m.E - 1], rng.integers(0, m.E, 57)]))
+        idx = (sample[:, None] * Np + np.arange(Np)[None, :]).reshape(-1)
+        geo_s = orc.geo_factors(len(sample), N, m.x[idx], m.y[idx], m.z[idx])
+        for lam in (0.0, 1e4):
+            G.apply_axhelm(ud, wd, lam=lam)
+            w = wd.cpu().numpy()
+            ref = orc.axhelm(len(sample), N, geo_s, lam, u[idx])
+            assert normwise(w[idx], ref) <= TOL, (lam, normwise(w[idx], ref))
+            assert np.isfinite(w).all()
+        # ---- gather-scatter: exact on an integer-valued continuous field, QQ^T v = mult * v
+        v = ((lat * 2654435761) % 1021).astype(np.float64) - 510.0
+        mult = lattice_mult(ne, N)
+        vd = dev(torch, v)
+        G.gather_scatter(vd)
+        assert np.array_equal(vd.cpu().numpy(), v * mult)
+        assert np.array_equal(G.invmult_host(), 1.0 / mult)
+        # ---- mask: exactly the nodes of the z = 0 and z = 1 lattice planes
+        ones = torch.ones(n, dtype=torch.float64, device="cuda")
+        G.apply_mask(ones, 0b10)
+        gz = lat // (Gd * Gd)
+        assert np.array_equal(ones.cpu().numpy() == 0.0, (gz == 0) | (gz == Gd - 1))
+    finally:
+        G.close()
+
+
+def test_cfg1_fullsize_everything_vs_oracle(torch_cuda, semb, orc, xi_of):
+    torch = torch_cuda
+    m, prm = I.config_mesh(1, xi_of)
+    P = orc.Problem(m.E, m.N, m.x, m.y, m.z, m.face_tag, m.period, lam=prm["lam"], dirichlet_tags=0)
+    G = semb.Mesh(m.E, m.N, dev(torch, m.x), dev(torch, m.y), dev(torch, m.z), m.face_tag, m.period)
+    try:
+        assert np.array_equal(G.gid_host(), P.gid)
+        assert normwise(G.geo_host(), P.geo) <= TOL
+        u = I.uniform(I.seed_for(1, 1), 3 * m.n)                       # batched: nfields = 3
+        ud = dev(torch, u); wd = torch.empty_like(ud)
+        G.apply_axhelm(ud, wd, lam=prm["lam"], nfields=3)
+        G.gather_scatter(wd, nfields=3)
+        w = wd.cpu().numpy()
+        for f in range(3):
+            ref = orc.gs(P.gid, P.n_unique, orc.axhelm(m.E, m.N, P.geo, prm["lam"], u[f * m.n:(f + 1) * m.n]))
+            assert normwise(w[f * m.n:(f + 1) * m.n], ref) <= TOL
+    finally:
+        G.close()
+
+
+def _solve_and_verify(torch, G, P, m, b, lam, tags, precond, lmax=0.0):
+    """GPU solve; oracle-verified true residual; first history entries against the oracle's own iteration."""
+    P.set_operator(lam, tags)
+    x = torch.zeros(m.n, dtype=torch.float64, device="cuda")
+    rg = G.pcg_solve(dev(torch, b), x, lam=lam, tags=tags, precond=precond, cheb_degree=2, cheb_lmax=lmax, rtol=1e-10,
+                     maxit=20000, hist_len=32)
+    assert rg["status"] == 0, rg
+    xh = x.cpu().numpy()
+    bn = np.sqrt(P.dot(b, b))
+    r = b - P.apply_A(xh)
+    true_res = np.sqrt(P.dot(r, r)) / bn
+    assert true_res <= 2e-10, (true_res, rg["iters"])
+    assert rg["r_norm"] <= 1e-10 * rg["b_norm"]
+    assert abs(rg["b_norm"] - bn) <= 1e-12 * bn
+    ro = P.pcg(b, precond=precond, cheb_k=2, lmax=lmax, rtol=1e-10, maxit=20, hist_len=21)   # 20 oracle iterations
+    k = min(len(ro["hist"]), len(rg["hist"]), 21)
+    assert k >= 10
+    assert np.abs(rg["hist"][:k] - ro["hist"][:k]).max() <= 1e-9 * ro["hist"][0]
+    return rg, true_res
+
+
+@pytest.mark.parametrize("cfg", [2, 4])
+def test_ogrid_fullsize(torch_cuda, semb, orc, xi_of, cfg):
+    torch = torch_cuda
+    m, prm = I.config_mesh(cfg, xi_of)
+    assert m.E == {2: 73728, 4: 64000}[cfg]
+    P = orc.Problem(m.E, m.N, m.x, m.y, m.z, m.face_tag, m.period, lam=0.0, dirichlet_tags=0b10)
+    G = semb.Mesh(m.E, m.N, dev(torch, m.x), dev(torch, m.y), dev(torch, m.z), m.face_tag, m.period)
+    try:
+        assert G.n_unique == P.n_unique == I.ogrid_unique_nodes(m.meta["n_c"], m.meta["n_r"], m.meta["n_z"], m.N)
+        assert np.array_equal(G.gid_host(), P.gid)
+        tol = geometry_tolerance(orc, m)          # tanh-clustered layers: kappa ~ 4e4, tol ~ 8e-12
+        assert tol <= 2e-11
+        for lam in (0.0, prm["lam"] if prm["lam"] else 1e4):
+            u = I.uniform(I.seed_for(cfg, 1), m.n)
+            ud = dev(torch, u); wd = torch.empty_like(ud)
+            G.apply_axhelm(ud, wd, lam=lam)
+            ref = orc.axhelm(m.E, m.N, P.geo, lam, u)
+            err = normwise(wd.cpu().numpy(), ref)
+            print(f"cfg{cfg} lam={lam}: axhelm normwise error {err:.2e} (bar {tol:.2e})")
+            assert err <= tol
+            G.gather_scatter(wd)
+            assert normwise(wd.cpu().numpy(), orc.gs(P.gid, P.n_unique, ref)) <= tol
+        f = I.divergence_source(m, I.seed_for(cfg, 3))
+        if cfg == 2:       # pressure Poisson, Chebyshev(2)-Jacobi with the oracle's lambda_max, then plain Jacobi
+            b = P.assemble_rhs(f)
+            lmax = P.lanczos_lmax(b, 10)
+            rc, _ = _solve_and_verify(torch, G, P, m, b, 0.0, 0b10, 2, lmax)
+            rj, _ = _solve_and_verify(torch, G, P, m, b, 0.0, 0b10, 1)
+            assert rc["iters"] < rj["iters"]
+        else:              # one velocity-type Helmholtz solve (lambda = 1.5/dt, no-slip on plates and side wall)
+            P.set_operator(prm["lam"], 0b110)
+            b = P.assemble_rhs(f)
+            _solve_and_verify(torch, G, P, m, b, prm["lam"], 0b110, 1)
+    finally:
+        G.close()
