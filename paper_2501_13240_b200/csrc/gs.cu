@@ -26,6 +26,30 @@ int semb_gs_launch(semb_mesh* h, double* w, int nfields, cudaStream_t s)
     return SEMB_OK;
 }
 
+// The same sum for the listed classes only (those with >= 3 members: element edges and corners).  The fused PCG /
+// Chebyshev updates (pcg.cu) do the remaining classes -- one partner each -- in gather form.
+__global__ void k_gs_hi(int64_t n_hi, const int32_t* __restrict__ hi, const int32_t* __restrict__ off,
+                        const int32_t* __restrict__ ids, double* __restrict__ w, const semb_scalars* __restrict__ scal)
+{
+    if (scal && *(volatile const int32_t*)&scal->done) return;
+    const int64_t q = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (q >= n_hi) return;
+    const int32_t g = hi[q];
+    const int32_t a = off[g], b = off[g + 1];
+    double s = 0.0;
+    for (int32_t t = a; t < b; ++t) s += w[ids[t]];
+    for (int32_t t = a; t < b; ++t) w[ids[t]] = s;
+}
+
+int semb_gs_hi_launch(semb_mesh* h, double* w, const semb_scalars* scal, cudaStream_t s)
+{
+    if (h->n_gs_hi == 0) return SEMB_OK;
+    k_gs_hi<<<(unsigned)((h->n_gs_hi + 255) / 256), 256, 0, s>>>(h->n_gs_hi, h->gs_hi, h->gs_off, h->gs_ids, w, scal);
+    h->launches += 1;
+    SEMB_CUDA(h, cudaGetLastError());
+    return SEMB_OK;
+}
+
 __global__ void k_mask(int64_t c, int64_t n, const int32_t* __restrict__ list, double* __restrict__ w)
 {
     const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;

@@ -23,6 +23,42 @@ static inline unsigned vec_grid(int64_t n)
 #define GSTRIDE(l, n) for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < (n); l += (int64_t)gridDim.x * blockDim.x)
 #define STOPPED(scal) (*(volatile int32_t*)&(scal)->done)
 
+// Gather form of QQ^T for a vector that is consumed once (SURVEY.md §8 a-2 folded into a-6): the value of
+// (QQ^T q) at local node l = sum of q over the copies of l's global node.  q itself is not written back, which
+// saves most of the read-modify-write pass of the stand-alone gather-scatter.  A node's code (setup.cu:
+// k_gs_code) names its single partner directly (faces: 73 % of the shared nodes at N = 7; the two-term sum is
+// the same bits on both copies since a + b == b + a); classes with >= 3 members (element edges and corners,
+// 16 % of the nodes) have been summed in place by k_gs_hi just before, in ascending local index like k_gs, and
+// carry their multiplicity as code.  The remaining chain code -> q[partner] is one dependent load; the codes of
+// the NEXT chunk are fetched while the current one is processed, so a chunk exposes a single memory latency
+// like a plain streaming kernel (the first version, which followed per-class records inside this kernel, was
+// latency-bound: ncu DRAM 25-33 %, long-scoreboard stalls).  wgt = 1 / multiplicity (bitwise = invmult[l]).
+#define GS_U 4
+struct gs_lists { const int32_t* code; };
+__device__ __forceinline__ void gs_codes(const gs_lists& L, int64_t l0, int64_t n, int32_t (&c)[GS_U])
+{
+#pragma unroll
+    for (int u = 0; u < GS_U; ++u) { const int64_t l = l0 + u * VEC_BLOCK; c[u] = (l < n) ? __ldg(L.code + l) : -1; }
+}
+// own[u] = q at the node itself (already loaded by the caller, coalesced)
+__device__ __forceinline__ void gs_partners(const double* __restrict__ q, const int32_t (&c)[GS_U], double (&pv)[GS_U])
+{
+#pragma unroll
+    for (int u = 0; u < GS_U; ++u) pv[u] = (c[u] <= -2) ? q[-(c[u] + 2)] : 0.0;
+}
+__device__ __forceinline__ void gs_gathered(const int32_t (&c)[GS_U], const double (&own)[GS_U], const double (&pv)[GS_U],
+                                            double (&qa)[GS_U], double (&wgt)[GS_U])
+{
+#pragma unroll
+    for (int u = 0; u < GS_U; ++u) {
+        if (c[u] <= -2) { qa[u] = own[u] + pv[u]; wgt[u] = 0.5; }
+        else { qa[u] = own[u]; wgt[u] = (c[u] >= 3) ? 1.0 / (double)c[u] : 1.0; }
+    }
+}
+// grid-stride over chunks of GS_U * VEC_BLOCK nodes; thread t of a block handles nodes l0 + u * VEC_BLOCK
+#define GS_STEP ((int64_t)gridDim.x * (GS_U * VEC_BLOCK))
+#define GS_CHUNKS(l0, n) for (int64_t l0 = blockIdx.x * (int64_t)(GS_U * VEC_BLOCK) + threadIdx.x; l0 - threadIdx.x < (n); l0 += GS_STEP)
+
 // r = b (x = 0) or r = b - q (q = A x0);  bb, rr, rz
 __global__ void __launch_bounds__(VEC_BLOCK)
 k_pcg_init(int64_t n, const double* __restrict__ b, const double* __restrict__ q, double* __restrict__ x,
@@ -51,11 +87,12 @@ k_pcg_init(int64_t n, const double* __restrict__ b, const double* __restrict__ q
     }
 }
 
-// r -= alpha q; rr = <r,r>, rz = <r, dinv r>; the last block closes the iteration.  (x += alpha p and
-// p = z + beta p are done by the next fused axhelm launch, which reads p anyway: axhelm_kernels.cuh MODE bit 2.)
+// r -= alpha QQ^T q (q = M A_L p, masked but not yet assembled: the gather-scatter is done here in gather form);
+// rr = <r,r>, rz = <r, dinv r>; the last block closes the iteration.  (x += alpha p and p = z + beta p are done
+// by the next fused axhelm launch, which reads p anyway: axhelm_kernels.cuh MODE bit 2.)
 template <bool FUSED_Z>
-__global__ void __launch_bounds__(VEC_BLOCK)
-k_update_r(int64_t n, const double* __restrict__ q, double* __restrict__ r, const double* __restrict__ invmult,
+__global__ void __launch_bounds__(VEC_BLOCK, 4)
+k_update_r(int64_t n, const double* __restrict__ q, double* __restrict__ r, gs_lists L,
            const double* __restrict__ dinv, semb_scalars* __restrict__ scal, double* __restrict__ partials,
            double* __restrict__ hist, int hist_cap)
 {
@@ -63,12 +100,34 @@ k_update_r(int64_t n, const double* __restrict__ q, double* __restrict__ r, cons
     if (STOPPED(scal)) return;
     const double alpha = scal->alpha;
     double rr = 0.0, rz = 0.0;
-    GSTRIDE(l, n) {
-        const double rl = r[l] - alpha * q[l];
-        r[l] = rl;
-        const double t = rl * rl * invmult[l];
-        rr += t;
-        if (FUSED_Z) rz += (dinv ? dinv[l] : 1.0) * t;
+    int32_t cn[GS_U];
+    gs_codes(L, blockIdx.x * (int64_t)(GS_U * VEC_BLOCK) + threadIdx.x, n, cn);
+    GS_CHUNKS(l0, n) {
+        double qa[GS_U], wgt[GS_U], rv[GS_U], dv[GS_U], own[GS_U], pv[GS_U];
+        int32_t c[GS_U];
+#pragma unroll
+        for (int u = 0; u < GS_U; ++u) c[u] = cn[u];
+        gs_partners(q, c, pv);
+        gs_codes(L, l0 + GS_STEP, n, cn);                       // next chunk's codes, in flight during this one
+#pragma unroll
+        for (int u = 0; u < GS_U; ++u) {
+            const int64_t l = l0 + u * VEC_BLOCK;
+            own[u] = (l < n) ? q[l] : 0.0;
+            rv[u] = (l < n) ? r[l] : 0.0;
+            dv[u] = (FUSED_Z && dinv && l < n) ? dinv[l] : 1.0;
+        }
+        gs_gathered(c, own, pv, qa, wgt);
+#pragma unroll
+        for (int u = 0; u < GS_U; ++u) {
+            const int64_t l = l0 + u * VEC_BLOCK;
+            if (l < n) {
+                const double rl = rv[u] - alpha * qa[u];
+                r[l] = rl;
+                const double t = rl * rl * wgt[u];
+                rr += t;
+                if (FUSED_Z) rz += dv[u] * t;
+            }
+        }
     }
     double v[2] = { block_sum(rr, red), block_sum(rz, red) }, tot[2];
     if (grid_sum<2>(v, partials, &scal->ticket[2], tot, red) && threadIdx.x == 0) {
@@ -133,20 +192,41 @@ k_cheb_init(int64_t n, const double* __restrict__ r, const double* __restrict__ 
         res[l] = rl; d[l] = dl; z[l] = last ? dl : 0.0;
     }
 }
-__global__ void __launch_bounds__(VEC_BLOCK)
-k_cheb_step(int64_t n, const double* __restrict__ Ad, const double* __restrict__ dinv, double c1, double c2,
+// Ad = M A_L d, masked but not assembled: QQ^T is applied here in gather form (gs_gathered)
+__global__ void __launch_bounds__(VEC_BLOCK, 4)
+k_cheb_step(int64_t n, const double* __restrict__ Ad, gs_lists L, const double* __restrict__ dinv, double c1, double c2,
             double* __restrict__ res, double* __restrict__ d, double* __restrict__ z, int last,
             const semb_scalars* __restrict__ scal)
 {
     if (scal && STOPPED(scal)) return;
-    GSTRIDE(l, n) {
-        const double dl = d[l];
-        double zl = z[l] + dl;
-        const double rl = res[l] - Ad[l];
-        const double dn = c1 * dl + c2 * (dinv[l] * rl);
-        res[l] = rl; d[l] = dn;
-        if (last) zl += dn;
-        z[l] = zl;
+    int32_t cn[GS_U];
+    gs_codes(L, blockIdx.x * (int64_t)(GS_U * VEC_BLOCK) + threadIdx.x, n, cn);
+    GS_CHUNKS(l0, n) {
+        double qa[GS_U], wgt[GS_U], dl[GS_U], zl[GS_U], rl[GS_U], dv[GS_U], own[GS_U], pv[GS_U];
+        int32_t c[GS_U];
+#pragma unroll
+        for (int u = 0; u < GS_U; ++u) c[u] = cn[u];
+        gs_partners(Ad, c, pv);
+        gs_codes(L, l0 + GS_STEP, n, cn);
+#pragma unroll
+        for (int u = 0; u < GS_U; ++u) {
+            const int64_t l = l0 + u * VEC_BLOCK;
+            own[u] = 0.0;
+            if (l < n) { own[u] = Ad[l]; dl[u] = d[l]; zl[u] = z[l]; rl[u] = res[l]; dv[u] = dinv[l]; }
+        }
+        gs_gathered(c, own, pv, qa, wgt);
+#pragma unroll
+        for (int u = 0; u < GS_U; ++u) {
+            const int64_t l = l0 + u * VEC_BLOCK;
+            if (l < n) {
+                double zn = zl[u] + dl[u];
+                const double rn = rl[u] - qa[u];
+                const double dn = c1 * dl[u] + c2 * (dv[u] * rn);
+                res[l] = rn; d[l] = dn;
+                if (last) zn += dn;
+                z[l] = zn;
+            }
+        }
     }
 }
 
@@ -220,9 +300,9 @@ static int cheb_apply(semb_mesh* h, double lambda, const semb_mask_entry& m, con
     h->launches += 1 + k;
     for (int it = 0; it < k; ++it) {
         int rc = semb_axhelm_launch(h, lambda, nullptr, nullptr, d, Ad, 1, nullptr, s); if (rc) return rc;
-        rc = semb_gs_launch(h, Ad, 1, s); if (rc) return rc;
-        rc = semb_mask_launch(h, m, Ad, 1, s); if (rc) return rc;
-        k_cheb_step<<<vec_grid(n), VEC_BLOCK, 0, s>>>(n, Ad, dinv, c.c1[it], c.c2[it], res, d, z, it == k - 1, scal);
+        rc = semb_mask_launch(h, m, Ad, 1, s); if (rc) return rc;       // every copy of a Dirichlet node is masked => sum 0
+        rc = semb_gs_hi_launch(h, Ad, scal, s); if (rc) return rc;      // edges and corners; faces in k_cheb_step
+        k_cheb_step<<<vec_grid(n), VEC_BLOCK, 0, s>>>(n, Ad, gs_lists{h->gs_code}, dinv, c.c1[it], c.c2[it], res, d, z, it == k - 1, scal);
     }
     SEMB_CUDA(h, cudaGetLastError());
     return SEMB_OK;
@@ -375,10 +455,11 @@ int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* 
             if (itn < nprof) SEMB_CUDA(h, cudaEventRecord(h->prof_ev[2 * itn], s));
             rc = semb_axhelm_pcg_launch(h, o->lambda, zsrc, dz, p, x, q, h->scal, s); if (rc) return rc;
             if (itn < nprof) SEMB_CUDA(h, cudaEventRecord(h->prof_ev[2 * itn + 1], s));
-            rc = semb_gs_launch(h, q, 1, s); if (rc) return rc;
-            rc = semb_mask_launch(h, m, q, 1, s); if (rc) return rc;
-            if (o->precond == 2) k_update_r<false><<<G, VEC_BLOCK, 0, s>>>(n, q, r, h->invmult, nullptr, h->scal, h->partials, hist, want_hist);
-            else                 k_update_r<true><<<G, VEC_BLOCK, 0, s>>>(n, q, r, h->invmult, dz, h->scal, h->partials, hist, want_hist);
+            rc = semb_mask_launch(h, m, q, 1, s); if (rc) return rc;     // every copy of a Dirichlet node is masked => sum 0
+            rc = semb_gs_hi_launch(h, q, h->scal, s); if (rc) return rc; // edges and corners; faces in k_update_r
+            const gs_lists L{h->gs_code};
+            if (o->precond == 2) k_update_r<false><<<G, VEC_BLOCK, 0, s>>>(n, q, r, L, nullptr, h->scal, h->partials, hist, want_hist);
+            else                 k_update_r<true><<<G, VEC_BLOCK, 0, s>>>(n, q, r, L, dz, h->scal, h->partials, hist, want_hist);
             h->launches += 1;
         }
         SEMB_CUDA(h, cudaGetLastError());

@@ -45,6 +45,9 @@ struct semb_mesh {
     double*  invmult = nullptr;    // [n]
     int32_t* gs_off = nullptr;     // [n_gs+1]
     int32_t* gs_ids = nullptr;     // [n_shared]
+    int32_t* gs_code = nullptr;    // [n] gather-form code per node (setup.cu: k_gs_code)
+    int32_t* gs_hi = nullptr;      // [n_gs_hi] indices (into gs_off) of the classes with >= 3 members
+    int64_t  n_gs_hi = 0;
     std::vector<int32_t> face_tag; // host [E*6]
     int32_t* face_tag_dev = nullptr;
     std::map<uint32_t, semb_mask_entry> masks;
@@ -103,6 +106,8 @@ int semb_axhelm_pcg_launch(semb_mesh* h, double lambda, const double* zsrc, cons
 
 // ---- gs.cu
 int semb_gs_launch(semb_mesh* h, double* w, int nfields, cudaStream_t s);
+// QQ^T restricted to the classes with >= 3 members (the rest is done in gather form by the consumer, pcg.cu)
+int semb_gs_hi_launch(semb_mesh* h, double* w, const semb_scalars* scal, cudaStream_t s);
 int semb_mask_launch(semb_mesh* h, const semb_mask_entry& m, double* w, int nfields, cudaStream_t s);
 
 // ---- pcg.cu

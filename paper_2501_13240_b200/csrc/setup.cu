@@ -274,6 +274,28 @@ __global__ void k_invmult(int64_t n_gs, const int32_t* __restrict__ off, const i
     for (int32_t t = a; t < b; ++t) invmult[ids[t]] = v;
 }
 
+// Gather-form code per local node, used by the fused residual / Chebyshev updates (pcg.cu: gs_gathered):
+//   -1        the node has no copy (weight 1);
+//   <= -2     the node has exactly one copy, at local index -(code + 2) (weight 1/2);
+//   >= 3      the node has code copies in all (itself included); such classes (element edges and corners) are
+//             assembled in place by k_gs_hi before the fused kernel runs (weight 1/code).
+__global__ void k_fill_i32(int64_t n, int32_t* __restrict__ a, int32_t v)
+{
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) a[l] = v;
+}
+__global__ void k_gs_code(int64_t n_gs, const int32_t* __restrict__ off, const int32_t* __restrict__ ids, int32_t* __restrict__ code)
+{
+    const int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (g >= n_gs) return;
+    const int32_t a = off[g], b = off[g + 1], m = b - a;
+    if (m == 2) { code[ids[a]] = -(ids[a + 1] + 2); code[ids[a + 1]] = -(ids[a] + 2); return; }
+    for (int32_t t = a; t < b; ++t) code[ids[t]] = m;
+}
+struct gs_hi_pred {
+    const int32_t* off;
+    __device__ bool operator()(int32_t g) const { return off[g + 1] - off[g] >= 3; }
+};
+
 #define GRID1(n) (unsigned)(((n) + 255) / 256)
 static inline unsigned grid_stride_blocks(int64_t n) { int64_t b = (n + 255) / 256; return (unsigned)(b < 148 * 16 ? (b > 0 ? b : 1) : 148 * 16); }
 
@@ -417,13 +439,32 @@ int semb_setup_numbering(semb_mesh* h, const double* x, const double* y, const d
         h->gs_ids = (int32_t*)semb_dev_alloc(h, sizeof(int32_t) * (size_t)(h->n_shared + 1));
         h->gs_off = (int32_t*)semb_dev_alloc(h, sizeof(int32_t) * (size_t)(h->n_gs + 1));
         h->invmult = (double*)semb_dev_alloc(h, sizeof(double) * (size_t)n);
-        if (!h->gs_ids || !h->gs_off || !h->invmult) return semb_fail(h, SEMB_ENOMEM, "gather lists");
+        h->gs_code = (int32_t*)semb_dev_alloc(h, sizeof(int32_t) * (size_t)n);
+        if (!h->gs_ids || !h->gs_off || !h->invmult || !h->gs_code) return semb_fail(h, SEMB_ENOMEM, "gather lists");
         SEMB_CUDA(h, cudaMemcpyAsync(h->gs_ids, ids_c, sizeof(int32_t) * (size_t)h->n_shared, cudaMemcpyDeviceToDevice, s));
         SEMB_CUDA(h, cudaMemcpyAsync(h->gs_off, off_c, sizeof(int32_t) * (size_t)h->n_gs, cudaMemcpyDeviceToDevice, s));
         const int32_t nsh = (int32_t)h->n_shared;
         SEMB_CUDA(h, cudaMemcpyAsync(h->gs_off + h->n_gs, &nsh, sizeof(int32_t), cudaMemcpyHostToDevice, s));
         k_fill<<<grid_stride_blocks(n), 256, 0, s>>>(n, h->invmult, 1.0);
-        if (h->n_gs > 0) k_invmult<<<GRID1(h->n_gs), 256, 0, s>>>(h->n_gs, h->gs_off, h->gs_ids, h->invmult);
+        k_fill_i32<<<grid_stride_blocks(n), 256, 0, s>>>(n, h->gs_code, -1);
+        if (h->n_gs > 0) {
+            k_invmult<<<GRID1(h->n_gs), 256, 0, s>>>(h->n_gs, h->gs_off, h->gs_ids, h->invmult);
+            k_gs_code<<<GRID1(h->n_gs), 256, 0, s>>>(h->n_gs, h->gs_off, h->gs_ids, h->gs_code);
+            // classes with >= 3 members (ascending class index)
+            int32_t* hi_tmp = ids_a;                          // scratch of nc >= n_gs entries, free by now
+            cub::CountingInputIterator<int32_t> cls0(0);
+            size_t tb = 0;
+            cub::DeviceSelect::If(nullptr, tb, cls0, hi_tmp, counts, (int)h->n_gs, gs_hi_pred{h->gs_off}, s);
+            TMP(tmp, char, tb);
+            SEMB_CUDA(h, cub::DeviceSelect::If(tmp, tb, cls0, hi_tmp, counts, (int)h->n_gs, gs_hi_pred{h->gs_off}, s));
+            int64_t nhi = 0;
+            SEMB_CUDA(h, cudaMemcpyAsync(&nhi, counts, sizeof(int64_t), cudaMemcpyDeviceToHost, s));
+            SEMB_CUDA(h, cudaStreamSynchronize(s));
+            h->n_gs_hi = nhi;
+            h->gs_hi = (int32_t*)semb_dev_alloc(h, sizeof(int32_t) * (size_t)(nhi + 1));
+            if (!h->gs_hi) return semb_fail(h, SEMB_ENOMEM, "gather lists (high-multiplicity classes)");
+            SEMB_CUDA(h, cudaMemcpyAsync(h->gs_hi, hi_tmp, sizeof(int32_t) * (size_t)nhi, cudaMemcpyDeviceToDevice, s));
+        }
         SEMB_CUDA(h, cudaGetLastError());
         SEMB_CUDA(h, cudaStreamSynchronize(s));
     }

@@ -187,8 +187,8 @@ def test_ogrid_fullsize(torch_cuda, semb, orc, xi_of, cfg):
     try:
         assert G.n_unique == P.n_unique == I.ogrid_unique_nodes(m.meta["n_c"], m.meta["n_r"], m.meta["n_z"], m.N)
         assert np.array_equal(G.gid_host(), P.gid)
-        tol = geometry_tolerance(orc, m)          # tanh-clustered layers: kappa ~ 4e4, tol ~ 8e-12
-        assert tol <= 2e-11
+        tol = geometry_tolerance(orc, m)          # tanh-clustered layers: kappa ~ 4e4 (N=7), ~ 9e4 (N=9): tol ~ 8e-12 / 4e-11
+        assert tol <= 5e-11
         for lam in (0.0, prm["lam"] if prm["lam"] else 1e4):
             u = I.uniform(I.seed_for(cfg, 1), m.n)
             ud = dev(torch, u); wd = torch.empty_like(ud)
