@@ -2,8 +2,8 @@
 """bench.py — headline benchmark of the SEM hot path on B200 (BASELINE.json metric).
 
 A "step" is one pass of the whole hot path over the synthetic batch: ONE Jacobi-PCG pressure iteration
-(axhelm with the fused x / Jacobi + direction updates and p.Ap -> gather-scatter -> Dirichlet mask -> r update with
-the ||r||^2 and r.z reductions) on the 64^3-element deformed box of BASELINE.json configs[3]
+(axhelm with the fused x / Jacobi + direction updates and p.Ap -> Dirichlet mask -> gather-scatter, done as an
+in-place sum over the edge/corner classes plus a partner gather folded into the r update -> ||r||^2 and r.z reductions) on the 64^3-element deformed box of BASELINE.json configs[3]
 (N = 7, fp64, 134 217 728 local nodes, lambda = 0).  K steps = one semb_pcg_solve call with maxit = K and
 rtol = 0 (it cannot stop early), bracketed by CUDA events on the launching stream.
 
@@ -37,6 +37,7 @@ UNIT = "GDOF/s"
 B_AXHELM = 64.0          # algorithmic bytes per node, Poisson axhelm
 B_AXHELM_HELM = 72.0
 B_AXHELM_PCG = 104.0     # the PCG-fused launch: reads r, dinv, p, x (32) + G (48), writes p, x, q (24)
+NCU_TRAFFIC_AXHELM_PCG = 13.939e9   # dram read + write bytes of one launch on cfg3, ncu --set full (profiles/r1_v3_full.md)
 B_ITER = 171.6           # algorithmic bytes per node per Jacobi-PCG iteration, N = 7, Poisson
 WORKLOADS = {            # name -> elements per direction of the deformed box (BASELINE.json configs[3] / configs[1])
     "cfg3_box64_deformed_N7": 64,
@@ -259,7 +260,7 @@ def main():
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": "inputs larger than L2 (every vector is %.2f GB)" % (8 * n / 1e9)},
         "roofline": {"bound": "hbm", "kernel": "k_axhelm_line<8,4,4>: axhelm (Poisson) with the fused PCG prologue (x += alpha p, p = dinv r + beta p) and p.Ap epilogue", "achieved": ax_gbs, "peak": peak,
-                     "unit": "GB/s", "frac": ax_gbs / peak, "traffic": None, "peak_source": peak_src,
+                     "unit": "GB/s", "frac": ax_gbs / peak, "traffic": NCU_TRAFFIC_AXHELM_PCG if args.workload.startswith("cfg3") else None, "peak_source": peak_src,
                      "bytes_per_node": B_AXHELM_PCG, "ms": ax_ms, "timed_launches": st["profiled"],
                      "frac_of_8TBs": ax_gbs / 8000.0, "gdofs": n / (ax_ms * 1e-3) / 1e9},
         "pcg_iter": {"ms": ms_step, "model_bytes_per_node": B_ITER, "gbs": B_ITER * n / (ms_step * 1e-3) / 1e9,
