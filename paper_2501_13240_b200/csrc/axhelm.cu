@@ -23,7 +23,10 @@ int semb_axhelm_prepare_geo(semb_mesh* h, cudaStream_t) { h->geoK = h->geo; retu
 
 // resident blocks per SM asked of the compiler (register budget): measured on B200, N = 7: 4 blocks x 166
 // registers beat 8 x 128 (the 48 geometric-factor loads of a thread stay in flight without spills).
-template <int n1> struct ax_minb { static constexpr int v = (n1 <= 4) ? 16 : (n1 <= 6) ? 8 : (n1 <= 8) ? 4 : (n1 == 9) ? 4 : 3; };
+#ifndef SEMB_MINB10
+#define SEMB_MINB10 3
+#endif
+template <int n1> struct ax_minb { static constexpr int v = (n1 <= 4) ? 16 : (n1 <= 6) ? 8 : (n1 <= 8) ? 4 : (n1 == 9) ? 4 : (n1 == 10) ? SEMB_MINB10 : 3; };
 
 template <int n1>
 static int launch_line(semb_mesh* h, int mode, double lambda, const double* lam0, const double* lam1,
@@ -32,7 +35,13 @@ static int launch_line(semb_mesh* h, int mode, double lambda, const double* lam0
     constexpr int MB = ax_minb<n1>::v;
     const unsigned grid = (unsigned)(h->E * nfields);
     double* dot = scal ? h->ax_dot : nullptr;
-#define SEMB_AX_LAUNCH(M) k_axhelm_line<n1, M, MB><<<grid, n1 * n1, 0, s>>>(h->E, h->n, h->geoK, lambda, lam0, lam1, u, w, scal, dot, pcg)
+    // L2 prefetch distance in elements: about 8 MB of this launch's traffic ahead of the block that issues it.
+    // Measured on B200 (N = 3, 5, 7, 9, stand-alone and PCG-fused): 4-20 MB ahead is flat (N = 7 Poisson 6.2 -> 7.05 TB/s,
+    // N = 9 4.5 -> 5.7 TB/s), beyond ~30 MB the prefetched lines are evicted before use and the launch gets SLOWER
+    // than without prefetch.
+    const int64_t bytes_per_elem = (int64_t)n1 * n1 * n1 * ((mode & 4) ? 104 : (mode & 2) ? 88 : (mode & 1) ? 72 : 64);
+    const int pf = (int)(((int64_t)8 << 20) / bytes_per_elem);
+#define SEMB_AX_LAUNCH(M) k_axhelm_line<n1, M, MB><<<grid, n1 * n1, 0, s>>>(h->E, h->n, h->geoK, lambda, lam0, lam1, u, w, scal, dot, pcg, pf)
     switch (mode) {
         case 0: SEMB_AX_LAUNCH(0); break;
         case 1: SEMB_AX_LAUNCH(1); break;

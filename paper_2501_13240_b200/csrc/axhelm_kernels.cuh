@@ -121,12 +121,22 @@ __device__ __forceinline__ void ax_line(const double (&x)[n1], double (&y)[n1])
 // u.w to dot_out[b] (fixed summation order; reduced by k_ax_dot_finish).
 struct ax_pcg_args { const double* zsrc; const double* dinv; double* p_io; double* x; };
 
+// L2 prefetch of one contiguous run of doubles (TMA unit, no destination in the SM):
+// cp.async.bulk.prefetch.L2 needs a 16-byte aligned address and size; runs that are only 8-byte aligned (odd n1)
+// are widened inward to the aligned part.  Issued by ONE thread.
+__device__ __forceinline__ void ax_prefetch_l2(const double* ptr, int count)
+{
+    uintptr_t a = (uintptr_t)ptr, b = a + (size_t)count * 8;
+    a = (a + 15) & ~(uintptr_t)15; b &= ~(uintptr_t)15;
+    if (b > a) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" :: "l"(a), "r"((unsigned)(b - a)) : "memory");
+}
+
 template <int n1, int MODE, int MINB>
 __global__ void __launch_bounds__(n1 * n1, MINB)
 k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambda,
               const double* __restrict__ lam0, const double* __restrict__ lam1,
               const double* __restrict__ u, double* __restrict__ w,
-              const semb_scalars* __restrict__ scal, double* __restrict__ dot_out, ax_pcg_args pcg)
+              const semb_scalars* __restrict__ scal, double* __restrict__ dot_out, ax_pcg_args pcg, int pf_dist)
 {
     constexpr int n2 = n1 * n1, Np = n1 * n1 * n1;
     constexpr bool HELM = MODE & 1, VAR = MODE & 2, FUSE = MODE & 4;
@@ -136,6 +146,20 @@ k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambd
     if (scal && *(volatile const int32_t*)&scal->done) return;
     const int a = threadIdx.x % n1, b = threadIdx.x / n1;
     const int64_t e = blockIdx.x % E, f = blockIdx.x / E;
+    // The element that a block pf_dist launches later will work on is pulled into L2 now: DRAM stays busy while
+    // the resident blocks are in their compute phase, and that block's loads hit L2.
+    if (pf_dist > 0 && threadIdx.x == 0 && e + pf_dist < E) {
+        const int64_t ep = e + pf_dist;
+        ax_prefetch_l2(geo + ep * 7 * (int64_t)Np, NG * Np);
+        if (FUSE) {
+            ax_prefetch_l2(pcg.zsrc + ep * Np, Np);
+            if (pcg.dinv) ax_prefetch_l2(pcg.dinv + ep * Np, Np);
+            ax_prefetch_l2(pcg.p_io + ep * Np, Np);
+            ax_prefetch_l2(pcg.x + ep * Np, Np);
+        } else ax_prefetch_l2(u + f * n + ep * Np, Np);
+        if (VAR && lam0) ax_prefetch_l2(lam0 + ep * Np, Np);
+        if (VAR && lam1) ax_prefetch_l2(lam1 + ep * Np, Np);
+    }
     double* __restrict__ we = w + f * n + e * Np + threadIdx.x;
     const double* __restrict__ g = geo + e * 7 * (int64_t)Np + threadIdx.x;
     double ru[n1], G[NG][n1];
