@@ -37,7 +37,7 @@ UNIT = "GDOF/s"
 B_AXHELM = 64.0          # algorithmic bytes per node, Poisson axhelm
 B_AXHELM_HELM = 72.0
 B_AXHELM_PCG = 104.0     # the PCG-fused launch: reads r, dinv, p, x (32) + G (48), writes p, x, q (24)
-NCU_TRAFFIC_AXHELM_PCG = 13.939e9   # dram read + write bytes of one launch on cfg3, ncu --set full (profiles/r1_v3_full.md)
+NCU_TRAFFIC_AXHELM_PCG = 13.943e9   # dram read + write bytes of one launch on cfg3, ncu --set full (profiles/r1_v4_axhelm_full.md)
 B_ITER = 171.6           # algorithmic bytes per node per Jacobi-PCG iteration, N = 7, Poisson
 WORKLOADS = {            # name -> elements per direction of the deformed box (BASELINE.json configs[3] / configs[1])
     "cfg3_box64_deformed_N7": 64,
