@@ -30,16 +30,16 @@ template <int n1> struct ax_minb { static constexpr int v = (n1 <= 4) ? 16 : (n1
 
 template <int n1>
 static int launch_line(semb_mesh* h, int mode, double lambda, const double* lam0, const double* lam1,
-                       const double* u, double* w, int nfields, semb_scalars* scal, const ax_pcg_args& pcg, cudaStream_t s)
+                       const double* u, double* w, int nfields, semb_scalars* scal, bool want_dot, const ax_pcg_args& pcg, cudaStream_t s)
 {
     constexpr int MB = ax_minb<n1>::v;
     const unsigned grid = (unsigned)(h->E * nfields);
-    double* dot = scal ? h->ax_dot : nullptr;
+    double* dot = (scal && want_dot) ? h->ax_dot : nullptr;
     // L2 prefetch distance in elements: about 8 MB of this launch's traffic ahead of the block that issues it.
     // Measured on B200 (N = 3, 5, 7, 9, stand-alone and PCG-fused): 4-20 MB ahead is flat (N = 7 Poisson 6.2 -> 7.05 TB/s,
     // N = 9 4.5 -> 5.7 TB/s), beyond ~30 MB the prefetched lines are evicted before use and the launch gets SLOWER
     // than without prefetch.
-    const int64_t bytes_per_elem = (int64_t)n1 * n1 * n1 * ((mode & 4) ? 104 : (mode & 2) ? 88 : (mode & 1) ? 72 : 64);
+    const int64_t bytes_per_elem = (int64_t)n1 * n1 * n1 * ((mode & 4) ? (pcg.plain ? 80 : 104) : (mode & 2) ? 88 : (mode & 1) ? 72 : 64);
     const int pf = (int)(((int64_t)8 << 20) / bytes_per_elem);
 #define SEMB_AX_LAUNCH(M) k_axhelm_line<n1, M, MB><<<grid, n1 * n1, 0, s>>>(h->E, h->n, h->geoK, lambda, lam0, lam1, u, w, scal, dot, pcg, pf)
     switch (mode) {
@@ -52,7 +52,7 @@ static int launch_line(semb_mesh* h, int mode, double lambda, const double* lam0
     }
 #undef SEMB_AX_LAUNCH
     h->launches += 1;
-    if (scal) {
+    if (dot) {
         // p.Ap = sum of the per-element partials, alpha = rho / p.Ap (fixed order: bit-reproducible)
         int64_t blocks = (h->E + 2047) / 2048;
         if (blocks > 128) blocks = 128;
@@ -64,24 +64,24 @@ static int launch_line(semb_mesh* h, int mode, double lambda, const double* lam0
 }
 
 static int axhelm_dispatch(semb_mesh* h, int mode, double lambda, const double* lam0, const double* lam1,
-                           const double* u, double* w, int nfields, semb_scalars* scal, const ax_pcg_args& pcg, cudaStream_t s)
+                           const double* u, double* w, int nfields, semb_scalars* scal, bool want_dot, const ax_pcg_args& pcg, cudaStream_t s)
 {
     if (scal && nfields != 1) return semb_fail(h, SEMB_EINVAL, "axhelm: fused p.Ap needs nfields == 1");
-    if (scal && !h->ax_dot) {
+    if (scal && want_dot && !h->ax_dot) {
         h->ax_dot = (double*)semb_dev_alloc(h, sizeof(double) * (size_t)h->E);
         if (!h->ax_dot) return semb_fail(h, SEMB_ENOMEM, "axhelm: p.Ap partials");
     }
     switch (h->n1) {
-        case 2:  return launch_line<2>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, pcg, s);
-        case 3:  return launch_line<3>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, pcg, s);
-        case 4:  return launch_line<4>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, pcg, s);
-        case 5:  return launch_line<5>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, pcg, s);
-        case 6:  return launch_line<6>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, pcg, s);
-        case 7:  return launch_line<7>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, pcg, s);
-        case 8:  return launch_line<8>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, pcg, s);
-        case 9:  return launch_line<9>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, pcg, s);
-        case 10: return launch_line<10>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, pcg, s);
-        case 11: return launch_line<11>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, pcg, s);
+        case 2:  return launch_line<2>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
+        case 3:  return launch_line<3>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
+        case 4:  return launch_line<4>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
+        case 5:  return launch_line<5>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
+        case 6:  return launch_line<6>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
+        case 7:  return launch_line<7>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
+        case 8:  return launch_line<8>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
+        case 9:  return launch_line<9>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
+        case 10: return launch_line<10>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
+        case 11: return launch_line<11>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
     }
     return semb_fail(h, SEMB_EINVAL, "unsupported order N=%d", h->N);
 }
@@ -90,7 +90,7 @@ int semb_axhelm_launch(semb_mesh* h, double lambda, const double* lam0, const do
                        const double* u, double* w, int nfields, semb_scalars* scal, cudaStream_t s)
 {
     const int mode = (lam0 || lam1) ? 3 : (lambda != 0.0) ? 1 : 0;
-    return axhelm_dispatch(h, mode, lambda, lam0, lam1, u, w, nfields, scal, ax_pcg_args{nullptr, nullptr, nullptr, nullptr}, s);
+    return axhelm_dispatch(h, mode, lambda, lam0, lam1, u, w, nfields, scal, scal != nullptr, ax_pcg_args{nullptr, nullptr, nullptr, nullptr, 1.0, 0}, s);
 }
 
 // PCG-fused form (pcg.cu): x += alpha p_old (if pending), p = dinv o zsrc + beta p_old, q = A_L p, partial p.q;
@@ -99,5 +99,14 @@ int semb_axhelm_pcg_launch(semb_mesh* h, double lambda, const double* zsrc, cons
                            double* q, semb_scalars* scal, cudaStream_t s)
 {
     const int mode = 4 | ((lambda != 0.0) ? 1 : 0);
-    return axhelm_dispatch(h, mode, lambda, nullptr, nullptr, nullptr, q, 1, scal, ax_pcg_args{zsrc, dinv, p, x}, s);
+    return axhelm_dispatch(h, mode, lambda, nullptr, nullptr, nullptr, q, 1, scal, true, ax_pcg_args{zsrc, dinv, p, x, 1.0, 0}, s);
+}
+
+// First Chebyshev step fused into the operator (pcg.cu: cheb_apply): d = (dinv o r) * scale, written to d, Ad = A_L d.
+// scal (may be NULL) only provides the early exit of a stopped solve.  Algorithmic bytes: r, dinv, 6 G read, d, Ad written = 80.
+int semb_axhelm_scaled_launch(semb_mesh* h, double lambda, const double* r, const double* dinv, double scale, double* d,
+                              double* Ad, semb_scalars* scal, cudaStream_t s)
+{
+    const int mode = 4 | ((lambda != 0.0) ? 1 : 0);
+    return axhelm_dispatch(h, mode, lambda, nullptr, nullptr, nullptr, Ad, 1, scal, false, ax_pcg_args{r, dinv, d, nullptr, scale, 1}, s);
 }

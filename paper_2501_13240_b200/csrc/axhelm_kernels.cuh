@@ -119,7 +119,9 @@ __device__ __forceinline__ void ax_line(const double (&x)[n1], double (&y)[n1])
 // times (SURVEY.md §8 a-6 (iii),(iv) folded into (i)).  u is then unused; p_io is both input and output.
 // One block per (element, field): grid = E * nfields.  dot_out != NULL: block b writes its partial sum of
 // u.w to dot_out[b] (fixed summation order; reduced by k_ax_dot_finish).
-struct ax_pcg_args { const double* zsrc; const double* dinv; double* p_io; double* x; };
+// plain != 0 (first Chebyshev step): no recurrence, p = (dinv o zsrc) * scale is written to p_io and the operator is
+// applied to it; x, alpha, beta are not touched.
+struct ax_pcg_args { const double* zsrc; const double* dinv; double* p_io; double* x; double scale; int plain; };
 
 // L2 prefetch of one contiguous run of doubles (TMA unit, no destination in the SM):
 // cp.async.bulk.prefetch.L2 needs a 16-byte aligned address and size; runs that are only 8-byte aligned (odd n1)
@@ -154,8 +156,7 @@ k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambd
         if (FUSE) {
             ax_prefetch_l2(pcg.zsrc + ep * Np, Np);
             if (pcg.dinv) ax_prefetch_l2(pcg.dinv + ep * Np, Np);
-            ax_prefetch_l2(pcg.p_io + ep * Np, Np);
-            ax_prefetch_l2(pcg.x + ep * Np, Np);
+            if (!pcg.plain) { ax_prefetch_l2(pcg.p_io + ep * Np, Np); ax_prefetch_l2(pcg.x + ep * Np, Np); }
         } else ax_prefetch_l2(u + f * n + ep * Np, Np);
         if (VAR && lam0) ax_prefetch_l2(lam0 + ep * Np, Np);
         if (VAR && lam1) ax_prefetch_l2(lam1 + ep * Np, Np);
@@ -165,14 +166,19 @@ k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambd
     double ru[n1], G[NG][n1];
     if (FUSE) {
         const int64_t l0 = e * Np + threadIdx.x;
-        const double beta = scal->beta, alpha = scal->alpha;
-        const bool pend = scal->x_pending != 0, first = (beta == 0.0);
+        const bool plain = pcg.plain != 0;
+        const double beta = plain ? 0.0 : scal->beta, alpha = plain ? 0.0 : scal->alpha;
+        const bool pend = !plain && scal->x_pending != 0, first = plain || (beta == 0.0);
         double z[n1], po[n1];
 #pragma unroll
         for (int k = 0; k < n1; ++k) z[k] = pcg.zsrc[l0 + k * n2];
         if (pcg.dinv) {
 #pragma unroll
             for (int k = 0; k < n1; ++k) z[k] *= pcg.dinv[l0 + k * n2];
+        }
+        if (plain) {
+#pragma unroll
+            for (int k = 0; k < n1; ++k) z[k] *= pcg.scale;
         }
         if (pend || !first) {
 #pragma unroll

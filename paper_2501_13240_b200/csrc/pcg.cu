@@ -192,17 +192,24 @@ k_cheb_init(int64_t n, const double* __restrict__ r, const double* __restrict__ 
         res[l] = rl; d[l] = dl; z[l] = last ? dl : 0.0;
     }
 }
-// Ad = M A_L d, masked but not assembled: QQ^T is applied here in gather form (gs_gathered)
-__global__ void __launch_bounds__(VEC_BLOCK, 4)
+// One step of the recurrence.  Ad = M A_L d, masked but not assembled: QQ^T is applied here in gather form.
+//   FIRST: res_in is the PCG residual r itself and z is 0 (neither res nor z was initialised: the first d was
+//          formed inside the axhelm launch, semb_axhelm_scaled_launch);
+//   LAST:  z += d + d_new is final, res and d are dead and not written; with rpcg != NULL the same pass
+//          accumulates rho = <rpcg, z> and its last block sets beta (what k_dot_rz did in a pass of its own).
+template <bool FIRST, bool LAST>
+__global__ void __launch_bounds__(VEC_BLOCK, 3)
 k_cheb_step(int64_t n, const double* __restrict__ Ad, gs_lists L, const double* __restrict__ dinv, double c1, double c2,
-            double* __restrict__ res, double* __restrict__ d, double* __restrict__ z, int last,
-            const semb_scalars* __restrict__ scal)
+            const double* res_in, double* res, double* __restrict__ d, double* __restrict__ z,
+            const double* rpcg, semb_scalars* __restrict__ scal, double* __restrict__ partials)
 {
+    __shared__ double red[32];
     if (scal && STOPPED(scal)) return;
     int32_t cn[GS_U];
+    double rz = 0.0;
     gs_codes(L, blockIdx.x * (int64_t)(GS_U * VEC_BLOCK) + threadIdx.x, n, cn);
     GS_CHUNKS(l0, n) {
-        double qa[GS_U], wgt[GS_U], dl[GS_U], zl[GS_U], rl[GS_U], dv[GS_U], own[GS_U], pv[GS_U];
+        double qa[GS_U], wgt[GS_U], dl[GS_U], zl[GS_U], rl[GS_U], dv[GS_U], own[GS_U], pv[GS_U], rp[GS_U];
         int32_t c[GS_U];
 #pragma unroll
         for (int u = 0; u < GS_U; ++u) c[u] = cn[u];
@@ -211,8 +218,12 @@ k_cheb_step(int64_t n, const double* __restrict__ Ad, gs_lists L, const double* 
 #pragma unroll
         for (int u = 0; u < GS_U; ++u) {
             const int64_t l = l0 + u * VEC_BLOCK;
-            own[u] = 0.0;
-            if (l < n) { own[u] = Ad[l]; dl[u] = d[l]; zl[u] = z[l]; rl[u] = res[l]; dv[u] = dinv[l]; }
+            own[u] = 0.0; zl[u] = 0.0; rp[u] = 0.0;
+            if (l < n) {
+                own[u] = Ad[l]; dl[u] = d[l]; rl[u] = res_in[l]; dv[u] = dinv[l];
+                if (!FIRST) zl[u] = z[l];
+                if (LAST && !FIRST && rpcg) rp[u] = rpcg[l];
+            }
         }
         gs_gathered(c, own, pv, qa, wgt);
 #pragma unroll
@@ -222,10 +233,20 @@ k_cheb_step(int64_t n, const double* __restrict__ Ad, gs_lists L, const double* 
                 double zn = zl[u] + dl[u];
                 const double rn = rl[u] - qa[u];
                 const double dn = c1 * dl[u] + c2 * (dv[u] * rn);
-                res[l] = rn; d[l] = dn;
-                if (last) zn += dn;
+                if (!LAST) { res[l] = rn; d[l] = dn; }
+                else {
+                    zn += dn;
+                    if (rpcg) rz += (FIRST ? rl[u] : rp[u]) * zn * wgt[u];
+                }
                 z[l] = zn;
             }
+        }
+    }
+    if (LAST && rpcg) {
+        double v[1] = { block_sum(rz, red) }, tot[1];
+        if (grid_sum<1>(v, partials, &scal->ticket[3], tot, red) && threadIdx.x == 0) {
+            scal->rho_new = tot[0]; scal->rz = tot[0];
+            scal->beta = (scal->iter == 0) ? 0.0 : tot[0] / scal->rho_old;
         }
     }
 }
@@ -291,18 +312,36 @@ static cheb_coef cheb_coefficients(int k, double lmax)
     return c;
 }
 
-// z = Cheb_k(r);  res, d, Ad: work vectors
+// z = Cheb_k(r);  res, d, Ad: work vectors.  in_pcg: also leave rho = <r,z> and beta in scal (PCG loop).
+// Per application (k >= 1): axhelm with the first d formed in its prologue (80 B/node), then per step k_mask,
+// k_gs_hi, k_cheb_step (first 60, middle 68, last 60 B/node) and, between steps, a plain axhelm (64).
 static int cheb_apply(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* dinv, int k, const cheb_coef& c,
-                      const double* r, double* z, double* res, double* d, double* Ad, semb_scalars* scal, cudaStream_t s)
+                      const double* r, double* z, double* res, double* d, double* Ad, semb_scalars* scal, bool in_pcg, cudaStream_t s)
 {
-    const int64_t n = h->n;
-    k_cheb_init<<<vec_grid(n), VEC_BLOCK, 0, s>>>(n, r, dinv, c.itheta, res, d, z, k == 0, scal);
-    h->launches += 1 + k;
+    const int64_t n = h->n; const unsigned G = vec_grid(n);
+    if (k == 0) {
+        k_cheb_init<<<G, VEC_BLOCK, 0, s>>>(n, r, dinv, c.itheta, res, d, z, 1, scal);
+        h->launches += 1;
+        if (in_pcg) { k_dot_rz<<<G, VEC_BLOCK, 0, s>>>(n, r, z, h->invmult, scal, h->partials); h->launches += 1; }
+        SEMB_CUDA(h, cudaGetLastError());
+        return SEMB_OK;
+    }
+    const gs_lists L{h->gs_code};
+    const double* rp = in_pcg ? r : nullptr;
+    int rc = semb_axhelm_scaled_launch(h, lambda, r, dinv, c.itheta, d, Ad, scal, s); if (rc) return rc;
     for (int it = 0; it < k; ++it) {
-        int rc = semb_axhelm_launch(h, lambda, nullptr, nullptr, d, Ad, 1, nullptr, s); if (rc) return rc;
+        if (it > 0) { rc = semb_axhelm_launch(h, lambda, nullptr, nullptr, d, Ad, 1, nullptr, s); if (rc) return rc; }
         rc = semb_mask_launch(h, m, Ad, 1, s); if (rc) return rc;       // every copy of a Dirichlet node is masked => sum 0
         rc = semb_gs_hi_launch(h, Ad, scal, s); if (rc) return rc;      // edges and corners; faces in k_cheb_step
-        k_cheb_step<<<vec_grid(n), VEC_BLOCK, 0, s>>>(n, Ad, gs_lists{h->gs_code}, dinv, c.c1[it], c.c2[it], res, d, z, it == k - 1, scal);
+        const bool first = (it == 0), last = (it == k - 1);
+        const double* rin = first ? r : res;
+#define SEMB_CHEB_STEP(F, La) k_cheb_step<F, La><<<G, VEC_BLOCK, 0, s>>>(n, Ad, L, dinv, c.c1[it], c.c2[it], rin, res, d, z, rp, scal, h->partials)
+        if (first && last) SEMB_CHEB_STEP(true, true);
+        else if (first)    SEMB_CHEB_STEP(true, false);
+        else if (last)     SEMB_CHEB_STEP(false, true);
+        else               SEMB_CHEB_STEP(false, false);
+#undef SEMB_CHEB_STEP
+        h->launches += 1;
     }
     SEMB_CUDA(h, cudaGetLastError());
     return SEMB_OK;
@@ -316,7 +355,7 @@ int semb_cheb_run(semb_mesh* h, double lambda, uint32_t tags, int k, double lmax
     rc = semb_get_dinv(h, lambda, tags, &dinv, s); if (rc) return rc;
     rc = semb_ensure_work(h, 3); if (rc) return rc;
     const int64_t n = h->n;
-    return cheb_apply(h, lambda, m, dinv, k, cheb_coefficients(k, lmax), r, z, h->work, h->work + n, h->work + 2 * n, nullptr, s);
+    return cheb_apply(h, lambda, m, dinv, k, cheb_coefficients(k, lmax), r, z, h->work, h->work + n, h->work + 2 * n, nullptr, false, s);
 }
 
 // largest eigenvalue of the symmetric tridiagonal (a[0..m), b[0..m-1)) by bisection on the Sturm count
@@ -446,9 +485,7 @@ int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* 
         for (int i = 0; i < mbatch; ++i) {
             const double* zsrc = r;
             if (o->precond == 2) {
-                rc = cheb_apply(h, o->lambda, m, dinv, o->cheb_degree, cc, r, z, res, d, q, h->scal, s); if (rc) return rc;
-                k_dot_rz<<<G, VEC_BLOCK, 0, s>>>(n, r, z, h->invmult, h->scal, h->partials);
-                h->launches += 1;
+                rc = cheb_apply(h, o->lambda, m, dinv, o->cheb_degree, cc, r, z, res, d, q, h->scal, true, s); if (rc) return rc;
                 zsrc = z;
             }
             const int itn = it0 + i;

@@ -104,6 +104,9 @@ int semb_axhelm_launch(semb_mesh* h, double lambda, const double* lam0, const do
 int semb_axhelm_pcg_launch(semb_mesh* h, double lambda, const double* zsrc, const double* dinv, double* p, double* x,
                            double* q, semb_scalars* scal, cudaStream_t s);
 
+int semb_axhelm_scaled_launch(semb_mesh* h, double lambda, const double* r, const double* dinv, double scale, double* d,
+                              double* Ad, semb_scalars* scal, cudaStream_t s);
+
 // ---- gs.cu
 int semb_gs_launch(semb_mesh* h, double* w, int nfields, cudaStream_t s);
 // QQ^T restricted to the classes with >= 3 members (the rest is done in gather form by the consumer, pcg.cu)
