@@ -162,6 +162,21 @@ typedef struct {
 SEMB_API int semb_pcg_solve(semb_handle h, const semb_pcg_opts* opts, const double* b, double* x,
                    semb_pcg_stats* stats, void* stream);
 
+/* One time step's worth of solves (BASELINE.json configs[4]: per step one pressure Poisson solve and the three
+ * velocity and one temperature Helmholtz solves implied by the diffusion terms of PAPER.md:L194-196 Eq. 1-2), run
+ * back to back on `stream` in the order given.  Each item is an independent semb_pcg_solve with its own
+ * lambda, Dirichlet tag set, preconditioner and tolerances; masks and Jacobi diagonals are cached in the handle
+ * per (tags, lambda), so repeated steps pay no setup.  items HOST [nsolves]; b, x device [n] each, caller-owned;
+ * stats HOST [nsolves] or NULL.  Returns the first error (< 0; later items are not run), else SEMB_MAXIT if any
+ * solve stopped at maxit, else SEMB_OK. */
+typedef struct {
+    semb_pcg_opts opts;
+    const double* b;          /* device [n] assembled, masked right-hand side            */
+    double*       x;          /* device [n] in: initial guess (see opts.x0_is_zero), out */
+} semb_solve_item;
+SEMB_API int semb_step_solve(semb_handle h, int nsolves, const semb_solve_item* items, semb_pcg_stats* stats,
+                    void* stream);
+
 /* 1.1 x the largest Ritz value of D^-1/2 A D^-1/2 after `steps` Lanczos steps from the continuous,
  * masked start vector v0 (device [n]). */
 SEMB_API int semb_estimate_lmax(semb_handle h, double lambda, uint32_t dirichlet_tags, const double* v0,

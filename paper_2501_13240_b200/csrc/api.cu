@@ -189,6 +189,19 @@ int semb_pcg_solve(semb_handle h, const semb_pcg_opts* o, const double* b, doubl
     return rc;
 }
 
+int semb_step_solve(semb_handle h, int nsolves, const semb_solve_item* items, semb_pcg_stats* stats, void* stream)
+{
+    if (!h) return SEMB_EINVAL;
+    if (nsolves < 0 || (nsolves > 0 && !items)) return semb_fail(h, SEMB_EINVAL, "step_solve: bad argument");
+    int worst = SEMB_OK;
+    for (int i = 0; i < nsolves; ++i) {
+        const int rc = semb_pcg_solve(h, &items[i].opts, items[i].b, items[i].x, stats ? &stats[i] : nullptr, stream);
+        if (rc < 0) return rc;
+        if (rc > worst) worst = rc;
+    }
+    return worst;
+}
+
 int semb_estimate_lmax(semb_handle h, double lambda, uint32_t tags, const double* v0, int steps, double* lmax_out, void* stream)
 {
     if (!h) return SEMB_EINVAL;

@@ -20,7 +20,7 @@ ERRORS = {-1: "SEMB_EINVAL", -2: "SEMB_ENOMEM", -3: "SEMB_ECUDA", -4: "SEMB_EGEO
 # every symbol include/semb200.h declares (tests check that the library exports all of them)
 SYMBOLS = ["semb_gll", "semb_setup", "semb_destroy", "semb_last_error", "semb_mesh_info", "semb_apply_axhelm",
            "semb_gather_scatter", "semb_apply_mask", "semb_assemble_rhs", "semb_apply_operator", "semb_jacobi_diag",
-           "semb_pcg_solve", "semb_estimate_lmax", "semb_cheb_jacobi", "semb_publish_field", "semb_publish_state",
+           "semb_pcg_solve", "semb_step_solve", "semb_estimate_lmax", "semb_cheb_jacobi", "semb_publish_field", "semb_publish_state",
            "semb_export_field", "semb_field_minmax_hist", "semb_apply_axhelm_host", "semb_pcg_solve_host", "semb_read_device", "semb_version"]
 
 
@@ -47,6 +47,10 @@ class PcgStats(C.Structure):
     _fields_ = [("iters", C.c_int32), ("status", C.c_int32), ("b_norm", C.c_double), ("r0_norm", C.c_double),
                 ("r_norm", C.c_double), ("lmax_used", C.c_double), ("hist", C.c_void_p), ("hist_len", C.c_int32),
                 ("profiled", C.c_int32), ("axhelm_ms", C.c_double), ("launches", C.c_int64)]
+
+
+class SolveItem(C.Structure):
+    _fields_ = [("opts", PcgOpts), ("b", C.c_void_p), ("x", C.c_void_p)]
 
 
 class FieldDesc(C.Structure):
@@ -193,6 +197,25 @@ class Mesh:
         return dict(iters=int(st.iters), status=int(rc), b_norm=st.b_norm, r0_norm=st.r0_norm, r_norm=st.r_norm,
                     lmax_used=st.lmax_used, hist=hist[:min(hist_len, st.iters + 1)], axhelm_ms=st.axhelm_ms,
                     profiled=int(st.profiled), launches=int(st.launches))
+
+    def step_solve(self, solves):
+        """One time step's solves back to back (semb_step_solve).  solves: list of dicts with keys b, x (device
+        tensors) and the pcg_solve keyword options.  Returns (status, [dict(iters, status, r_norm, b_norm)])."""
+        k = len(solves)
+        items = (SolveItem * max(k, 1))()
+        stats = (PcgStats * max(k, 1))()
+        for i, sv in enumerate(solves):
+            o = PcgOpts(sv.get("lam", 0.0), sv.get("tags", 0), sv.get("precond", 1), sv.get("cheb_degree", 2),
+                        sv.get("cheb_lmax", 0.0), sv.get("rtol", 1e-10), sv.get("atol", 0.0), sv.get("maxit", 10000),
+                        1 if sv.get("x0_is_zero", True) else 0, sv.get("check_every", 0), 0)
+            items[i].opts = o
+            items[i].b = _dp(sv["b"]).value
+            items[i].x = _dp(sv["x"]).value
+            stats[i].hist = None
+            stats[i].hist_len = 0
+        rc = self._check(lib().semb_step_solve(self._h, C.c_int(k), items, stats, _stream()))
+        return int(rc), [dict(iters=int(st.iters), status=int(st.status), r_norm=st.r_norm, b_norm=st.b_norm,
+                              launches=int(st.launches)) for st in stats[:k]]
 
     def pcg_solve_host(self, b_host, x_host, lam=0.0, tags=0, precond=1, cheb_degree=2, cheb_lmax=0.0, rtol=1e-10,
                        atol=0.0, maxit=10000, check_every=0):

@@ -259,6 +259,42 @@ def test_pcg_initial_guess_and_maxit(torch_cuda, cases, orc):
     assert r["status"] == 0 and r["iters"] == 0 and float(x.abs().max()) == 0.0
 
 
+def test_step_driver_cfg4_recipe(torch_cuda, cases, orc):
+    """configs[4] on the reduced N = 9 O-grid (R12): per step one pressure Poisson solve (Dirichlet {1}) and
+    three velocity ({1,2}) plus one temperature ({1}) Helmholtz solves with lambda = 1.5/dt = 3000, through ONE
+    semb_step_solve call; right-hand sides b(s) = M QQ^T B(f + 0.1 rms(f) eta(s)); steps >= 2 start from the previous
+    step's solution.  Every solve is compared with the oracle run on the same inputs (its own warm starts)."""
+    torch = torch_cuda
+    m, _, G = cases("ogrid9")
+    lam_h = 3000.0
+    kinds = [(0.0, 0b10), (lam_h, 0b110), (lam_h, 0b110), (lam_h, 0b110), (lam_h, 0b10)]
+    probs = [oracle_problem(orc, m, lam=l, tags=t) for l, t in kinds]
+    f0 = [I.divergence_source(m, I.seed_for(4, 30 + i)) for i in range(5)]
+    xg = [torch.zeros(m.n, dtype=torch.float64, device="cuda") for _ in range(5)]
+    xo = [None] * 5
+    for step in range(3):
+        bs = []
+        for i, P in enumerate(probs):
+            eta = I.uniform(I.seed_for(4, 100 * (step + 1) + i), m.n)
+            f = f0[i] + 0.1 * np.sqrt(np.mean(f0[i] ** 2)) * eta
+            bs.append(P.assemble_rhs(f))
+        solves = [dict(b=dev(torch, bs[i]), x=xg[i], lam=kinds[i][0], tags=kinds[i][1], precond=1, rtol=1e-10,
+                       x0_is_zero=(step == 0), check_every=7) for i in range(5)]
+        rc, stats = G.step_solve(solves)
+        assert rc == 0 and len(stats) == 5
+        for i, P in enumerate(probs):
+            ro = P.pcg(bs[i], x0=xo[i], precond=1, rtol=1e-10)
+            xo[i] = ro["x"]
+            assert ro["status"] == 0 and stats[i]["status"] == 0
+            assert abs(stats[i]["iters"] - ro["iters"]) <= 1, (step, i, stats[i]["iters"], ro["iters"])
+            assert normwise(xg[i].cpu().numpy(), ro["x"]) <= 1e-8
+            assert stats[i]["r_norm"] <= 1e-10 * stats[i]["b_norm"]
+    # an invalid item stops the sequence with its error
+    bad = [dict(b=dev(torch, bs[0]), x=xg[0], precond=7)]
+    with pytest.raises(Exception):
+        G.step_solve(bad)
+
+
 def test_cheb_jacobi_and_lmax(torch_cuda, cases, orc):
     m, _, G = cases("ogrid7")
     P = oracle_problem(orc, m, lam=0.0, tags=0b10)
