@@ -9,6 +9,25 @@
 // Algorithmic bytes per node: 8 (u) + 8 (w) + 48 (G) = 64, + 8 (B) when lambda != 0.
 #include "axhelm_kernels.cuh"
 
+template <int n1> static void perm_of(unsigned char perm[2][SEMB_MAXN1 * SEMB_MAXN1 + 7])
+{
+    using T = ax_tile<n1>;
+    ax_perm_build(n1, T::P1, T::P2, T::P2B, T::permuted, perm);
+}
+static int upload_perm(semb_mesh* h)
+{
+    unsigned char perm[2][SEMB_MAXN1 * SEMB_MAXN1 + 7] = {{0}};
+    switch (h->n1) {
+        case 2: perm_of<2>(perm); break;   case 3: perm_of<3>(perm); break;   case 4: perm_of<4>(perm); break;
+        case 5: perm_of<5>(perm); break;   case 6: perm_of<6>(perm); break;   case 7: perm_of<7>(perm); break;
+        case 8: perm_of<8>(perm); break;   case 9: perm_of<9>(perm); break;   case 10: perm_of<10>(perm); break;
+        case 11: perm_of<11>(perm); break;
+        default: return semb_fail(h, SEMB_EINVAL, "unsupported order N=%d", h->N);
+    }
+    SEMB_CUDA(h, cudaMemcpyToSymbol(c_perm, perm, sizeof(perm), sizeof(perm) * (size_t)h->N));
+    return SEMB_OK;
+}
+
 int semb_axhelm_upload_basis(semb_mesh* h)
 {
     SEMB_CUDA(h, cudaMemcpyToSymbol(c_D, h->D, sizeof(double) * h->n1 * h->n1,
@@ -16,7 +35,7 @@ int semb_axhelm_upload_basis(semb_mesh* h)
     ax_eo_tab tab[2];
     ax_eo_build(h->n1, h->D, tab);
     SEMB_CUDA(h, cudaMemcpyToSymbol(c_EO, tab, sizeof(tab), sizeof(ax_eo_tab) * 2 * (size_t)h->N));
-    return SEMB_OK;
+    return upload_perm(h);
 }
 
 int semb_axhelm_prepare_geo(semb_mesh* h, cudaStream_t) { h->geoK = h->geo; return SEMB_OK; }

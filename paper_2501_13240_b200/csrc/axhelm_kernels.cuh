@@ -26,22 +26,78 @@ __constant__ double c_D[SEMB_MAX_N + 1][SEMB_MAXN1 * SEMB_MAXN1];
 // ---- shared-memory layout of one element tile, index (k,j,i) -> double slot -------------------------------
 // All three line orientations read/write it with 64-bit accesses; a half-warp (16 lanes) is conflict-free iff
 // its 16 slots are distinct mod 16.
+// Generic n1: plain strides, row stride n1 (so the t-line pattern, slot = const + thread index, is always
+// conflict-free), plane strides P2A (tiles Su, Sr) and P2B (tile Ss) chosen per n1 together with the assignment of
+// r- and s-lines to threads (ax_perm_build) so that the 16 lines of each half-warp start in 16 different banks
+// wherever the residues of the line starts allow it (exhaustive search over P2A, P2B in [n1^2, n1^2 + 16)).
 template <int n1> struct ax_tile {
-    // padded strides found by exhaustive search (fewest wavefronts over the three orientations)
-    static constexpr int P1 = (n1 == 10) ? 10 : n1;
-    static constexpr int P2 = (n1 == 4) ? 19 : (n1 == 10) ? 101 : n1 * n1;
-    static constexpr int size = n1 * P2;
+    static constexpr int P1 = n1;
+    static constexpr int P2 = (n1 == 4) ? 19 : (n1 == 10) ? 103 : n1 * n1;                        // Su, Sr
+    static constexpr int P2B = (n1 == 4) ? 19 : (n1 == 7) ? 57 : (n1 == 10) ? 101 : n1 * n1;       // Ss
+    static constexpr int size = n1 * (P2 > P2B ? P2 : P2B);
+    // measured on B200 (A/B in one session): N = 6 +5 %, N = 9 +3 % (Poisson) / +10 % (Helmholtz), N = 10 +7 %;
+    // n1 = 9 was 3 % slower with its best permuted layout and n1 <= 6 within noise: those keep thread = line.
+    static constexpr bool permuted = (n1 == 7) || (n1 >= 10);
     __device__ static __forceinline__ int idx(int k, int j, int i) { return k * P2 + j * P1 + i; }
+    __device__ static __forceinline__ int idxB(int k, int j, int i) { return k * P2B + j * P1 + i; }
 };
 // n1 = 8: XOR swizzle, conflict-free in all three orientations without padding:
 //   slot mod 16 = ((j^k)&1)*8 + (i ^ (((j>>1)&3) | ((k&1)<<2)))
 template <> struct ax_tile<8> {
     static constexpr int size = 512;
+    static constexpr int P1 = 8, P2 = 64, P2B = 64;
+    static constexpr bool permuted = false;
     __device__ static __forceinline__ int idx(int k, int j, int i)
     {
         return k * 64 + ((j ^ (k & 1)) << 3) + (i ^ (((j >> 1) & 3) | ((k & 1) << 2)));
     }
+    __device__ static __forceinline__ int idxB(int k, int j, int i) { return idx(k, j, i); }
 };
+
+// Which r-line (j = q % n1, k = q / n1) and which s-line (i = q % n1, k = q / n1) a thread contracts:
+// c_perm[N][0][thread] and c_perm[N][1][thread], filled at setup (axhelm.cu: ax_perm_build).
+__constant__ unsigned char c_perm[SEMB_MAX_N + 1][2][SEMB_MAXN1 * SEMB_MAXN1 + 7];
+
+// host: greedy balanced grouping.  start_bank[q] = bank (64-bit, mod 16) of the first slot of line q.  Lines are
+// dealt to the half-warps (aligned groups of 16 threads) so that a group holds as few lines of equal bank as
+// possible; perm[thread] = line.
+static inline void ax_perm_group(int nt, const int* start_bank, unsigned char* perm)
+{
+    const int ng = (nt + 15) / 16;
+    int fill[16] = {0}, cnt[16][16] = {{0}}, members[16][16];
+    int order[16], size[16] = {0};
+    for (int q = 0; q < nt; ++q) size[start_bank[q]]++;
+    for (int v = 0; v < 16; ++v) order[v] = v;
+    for (int x = 0; x < 16; ++x) for (int y = x + 1; y < 16; ++y)
+        if (size[order[y]] > size[order[x]] || (size[order[y]] == size[order[x]] && order[y] < order[x])) { int t = order[x]; order[x] = order[y]; order[y] = t; }
+    for (int oi = 0; oi < 16; ++oi) {
+        const int v = order[oi];
+        for (int q = 0; q < nt; ++q) {
+            if (start_bank[q] != v) continue;
+            int best = -1;
+            for (int g = 0; g < ng; ++g) {
+                const int cap = (nt - 16 * g < 16) ? nt - 16 * g : 16;
+                if (fill[g] >= cap) continue;
+                if (best < 0) { best = g; continue; }
+                const int capb = (nt - 16 * best < 16) ? nt - 16 * best : 16;
+                if (cnt[g][v] < cnt[best][v] || (cnt[g][v] == cnt[best][v] && cap - fill[g] > capb - fill[best])) best = g;
+            }
+            members[best][fill[best]++] = q; cnt[best][v]++;
+        }
+    }
+    int t = 0;
+    for (int g = 0; g < ng; ++g) for (int x = 0; x < fill[g]; ++x) perm[t++] = (unsigned char)members[g][x];
+}
+static inline void ax_perm_build(int n1, int P1, int P2A, int P2B, bool permuted, unsigned char perm[2][SEMB_MAXN1 * SEMB_MAXN1 + 7])
+{
+    const int nt = n1 * n1;
+    int bank[SEMB_MAXN1 * SEMB_MAXN1];
+    if (!permuted) { for (int q = 0; q < nt; ++q) perm[0][q] = perm[1][q] = (unsigned char)q; return; }
+    for (int q = 0; q < nt; ++q) bank[q] = ((q / n1) * P2A + (q % n1) * P1) % 16;     // r-line (j, k) in Su, Sr
+    ax_perm_group(nt, bank, perm[0]);
+    for (int q = 0; q < nt; ++q) bank[q] = ((q / n1) * P2B + (q % n1)) % 16;          // s-line (i, k) in Ss
+    ax_perm_group(nt, bank, perm[1]);
+}
 
 // PCG epilogue shared by the kernels: grid-wide sum of u.w (= p.Ap before assembly, valid because p is
 // continuous and zero at masked nodes: SURVEY.md §8 a-6), then alpha = rho / p.Ap in the last block.
@@ -147,6 +203,11 @@ k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambd
     __shared__ double Su[T::size], Sr[T::size], Ss[T::size];
     if (scal && *(volatile const int32_t*)&scal->done) return;
     const int a = threadIdx.x % n1, b = threadIdx.x / n1;
+    int ra = a, rb = b, sa = a, sb = b;                                     // r-line (j=ra, k=rb), s-line (i=sa, k=sb)
+    if (T::permuted) {
+        const int rq = c_perm[n1 - 1][0][threadIdx.x], sq = c_perm[n1 - 1][1][threadIdx.x];
+        ra = rq % n1; rb = rq / n1; sa = sq % n1; sb = sq / n1;
+    }
     const int64_t e = blockIdx.x % E, f = blockIdx.x / E;
     // The element that a block pf_dist launches later will work on is pulled into L2 now: DRAM stays busy while
     // the resident blocks are in their compute phase, and that block's loads hit L2.
@@ -211,15 +272,15 @@ k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambd
     {
         double ln[n1], out[n1];
 #pragma unroll
-        for (int i = 0; i < n1; ++i) ln[i] = Su[T::idx(b, a, i)];
+        for (int i = 0; i < n1; ++i) ln[i] = Su[T::idx(rb, ra, i)];
         ax_line<n1, 0>(ln, out);
 #pragma unroll
-        for (int i = 0; i < n1; ++i) Sr[T::idx(b, a, i)] = out[i];
+        for (int i = 0; i < n1; ++i) Sr[T::idx(rb, ra, i)] = out[i];
 #pragma unroll
-        for (int j = 0; j < n1; ++j) ln[j] = Su[T::idx(b, j, a)];
+        for (int j = 0; j < n1; ++j) ln[j] = Su[T::idx(sb, j, sa)];
         ax_line<n1, 0>(ln, out);
 #pragma unroll
-        for (int j = 0; j < n1; ++j) Ss[T::idx(b, j, a)] = out[j];
+        for (int j = 0; j < n1; ++j) Ss[T::idxB(sb, j, sa)] = out[j];
     }
     double ut[n1];
     ax_line<n1, 0>(ru, ut);
@@ -228,12 +289,12 @@ k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambd
     double gt[n1];
 #pragma unroll
     for (int k = 0; k < n1; ++k) {
-        const int s = T::idx(k, b, a);
-        const double ur = Sr[s], us = Ss[s];
+        const int s = T::idx(k, b, a), sB = T::idxB(k, b, a);
+        const double ur = Sr[s], us = Ss[sB];
         double Grr = G[0][k], Grs = G[1][k], Grt = G[2][k], Gss = G[3][k], Gst = G[4][k], Gtt = G[5][k];
         if (VAR && lam0) { const double c = lam0[e * Np + k * n2 + threadIdx.x]; Grr *= c; Grs *= c; Grt *= c; Gss *= c; Gst *= c; Gtt *= c; }
         Sr[s] = Grr * ur + Grs * us + Grt * ut[k];
-        Ss[s] = Grs * ur + Gss * us + Gst * ut[k];
+        Ss[sB] = Grs * ur + Gss * us + Gst * ut[k];
         gt[k] = Grt * ur + Gst * us + Gtt * ut[k];
     }
     __syncthreads();
@@ -241,15 +302,15 @@ k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambd
     {
         double ln[n1], out[n1];
 #pragma unroll
-        for (int i = 0; i < n1; ++i) ln[i] = Sr[T::idx(b, a, i)];
+        for (int i = 0; i < n1; ++i) ln[i] = Sr[T::idx(rb, ra, i)];
         ax_line<n1, 1>(ln, out);
 #pragma unroll
-        for (int i = 0; i < n1; ++i) Sr[T::idx(b, a, i)] = out[i];
+        for (int i = 0; i < n1; ++i) Sr[T::idx(rb, ra, i)] = out[i];
 #pragma unroll
-        for (int j = 0; j < n1; ++j) ln[j] = Ss[T::idx(b, j, a)];
+        for (int j = 0; j < n1; ++j) ln[j] = Ss[T::idxB(sb, j, sa)];
         ax_line<n1, 1>(ln, out);
 #pragma unroll
-        for (int j = 0; j < n1; ++j) Ss[T::idx(b, j, a)] = out[j];
+        for (int j = 0; j < n1; ++j) Ss[T::idxB(sb, j, sa)] = out[j];
     }
     double wt[n1];
     ax_line<n1, 1>(gt, wt);
@@ -264,8 +325,7 @@ k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambd
     double dot = 0.0;
 #pragma unroll
     for (int k = 0; k < n1; ++k) {
-        const int s = T::idx(k, b, a);
-        const double wv = wt[k] + Sr[s] + Ss[s];
+        const double wv = wt[k] + Sr[T::idx(k, b, a)] + Ss[T::idxB(k, b, a)];
         we[k * n2] = wv;
         dot += ru[k] * wv;
     }
