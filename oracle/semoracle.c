@@ -430,20 +430,130 @@ void orc_cheb_jacobi(const orc_op* op, int k, double lmax, const double* dinv, c
     for (int64_t l = 0; l < n; ++l) z[l] += d[l];
 }
 
-/* z = M^-1 r : precond 0 = identity, 1 = Jacobi, 2 = Chebyshev-Jacobi(cheb_k) */
-static void precond_apply(const orc_op* op, int precond, int cheb_k, double lmax, const double* dinv,
+/* ------------------------------------------------------------------------------------ */
+/* f-1  p-multigrid V-cycle preconditioner (§2.2: "p-multigrid ... Chebyshev-accelerated
+ * ... smoothers" is NekRS's pressure preconditioner; the paper gives no formulas, reading R19
+ * fixes them).  Levels l = 0 (order N, the problem) .. L-1 (coarsest), each a re-discretisation of the
+ * same elements at order N_l: its own geometric factors, numbering, mask and Jacobi diagonal (orc_op).
+ *   prolongation   P_l : level l+1 -> l,  per element  v_f(i,j,k) = sum_abc J_ia J_jb J_kc v_c(a,b,c),
+ *                  J_ia = l^(l+1)_a(xi^(l)_i)  (coarse Lagrange basis at the fine GLL nodes);
+ *   restriction    R_l = M_c QQ^T_c (J^T x J^T x J^T)(invmult_f o r)   (the transpose of P_l on unique nodes);
+ *   smoother       S_l = Chebyshev-Jacobi(k) of c-10 on level l;
+ *   V(l, r):  coarsest: z = S(r) with degree k_coarse;  else
+ *             z = S r;  res = r - A z;  z += P V(l+1, R res);  res = r - A z;  z += S res.          */
+typedef struct {
+    orc_op op;
+    const double* dinv;
+    double lmax;
+    const double* J;         /* [n1_l][n1_{l+1}] row-major; NULL on the coarsest level */
+} orc_mg_level;
+typedef struct {
+    int32_t nlevels, k_smooth, k_coarse, pad_;
+    orc_mg_level lev[8];
+} orc_mg;
+
+/* J[(Nto+1) x (Nfrom+1)], J_ia = a-th Lagrange polynomial on the GLL nodes of order Nfrom at the
+ * i-th GLL node of order Nto (product formula: rows at coinciding nodes are exact unit vectors) */
+int orc_interp_matrix(int Nfrom, int Nto, double* J)
+{
+    double xf[ORC_MAXN1], xt[ORC_MAXN1], w[ORC_MAXN1];
+    if (orc_gll(Nfrom, xf, w) || orc_gll(Nto, xt, w)) return -1;
+    for (int i = 0; i <= Nto; ++i)
+        for (int a = 0; a <= Nfrom; ++a) {
+            double v = 1.0;
+            for (int m = 0; m <= Nfrom; ++m) if (m != a) v *= (xt[i] - xf[m]) / (xf[a] - xf[m]);
+            J[i * (Nfrom + 1) + a] = v;
+        }
+    return 0;
+}
+
+/* per element: transpose == 0: out(i,j,k) = sum_abc J_ia J_jb J_kc in(a,b,c)   (in: nc1^3, out: nf1^3)
+ *              transpose != 0: out(a,b,c) = sum_ijk J_ia J_jb J_kc in(i,j,k)   (in: nf1^3, out: nc1^3)
+ * J is [nf1][nc1].  The definition written out, no sum factorisation. */
+void orc_interp3(int64_t E, int nf1, int nc1, const double* J, int transpose, const double* in, double* out)
+{
+    const int Nf = nf1 * nf1 * nf1, Nc = nc1 * nc1 * nc1;
+#pragma omp parallel for schedule(static)
+    for (int64_t e = 0; e < E; ++e) {
+        const double* vi = in + e * (transpose ? Nf : Nc);
+        double* vo = out + e * (transpose ? Nc : Nf);
+        if (!transpose) {
+            for (int k = 0; k < nf1; ++k) for (int j = 0; j < nf1; ++j) for (int i = 0; i < nf1; ++i) {
+                double s = 0;
+                for (int c = 0; c < nc1; ++c) for (int b = 0; b < nc1; ++b) for (int a = 0; a < nc1; ++a)
+                    s += J[i * nc1 + a] * J[j * nc1 + b] * J[k * nc1 + c] * vi[(c * nc1 + b) * nc1 + a];
+                vo[(k * nf1 + j) * nf1 + i] = s;
+            }
+        } else {
+            for (int c = 0; c < nc1; ++c) for (int b = 0; b < nc1; ++b) for (int a = 0; a < nc1; ++a) {
+                double s = 0;
+                for (int k = 0; k < nf1; ++k) for (int j = 0; j < nf1; ++j) for (int i = 0; i < nf1; ++i)
+                    s += J[i * nc1 + a] * J[j * nc1 + b] * J[k * nc1 + c] * vi[(k * nf1 + j) * nf1 + i];
+                vo[(c * nc1 + b) * nc1 + a] = s;
+            }
+        }
+    }
+}
+
+/* v_f = M_f P v_c */
+void orc_mg_prolong(const orc_mg* mg, int l, const double* vc, double* vf)
+{
+    const orc_op* f = &mg->lev[l].op; const orc_op* c = &mg->lev[l + 1].op;
+    orc_interp3(f->E, f->N + 1, c->N + 1, mg->lev[l].J, 0, vc, vf);
+    for (int64_t q = 0; q < f->n; ++q) vf[q] *= f->mask[q];
+}
+/* r_c = M_c QQ^T_c J^T (invmult_f o r_f);  tmp: [n_f] */
+void orc_mg_restrict(const orc_mg* mg, int l, const double* rf, double* rc, double* tmp)
+{
+    const orc_op* f = &mg->lev[l].op; const orc_op* c = &mg->lev[l + 1].op;
+    for (int64_t q = 0; q < f->n; ++q) tmp[q] = f->invmult[q] * rf[q];
+    orc_interp3(f->E, f->N + 1, c->N + 1, mg->lev[l].J, 1, tmp, rc);
+    orc_gs(c->n, c->gid, c->n_unique, rc);
+    for (int64_t q = 0; q < c->n; ++q) rc[q] *= c->mask[q];
+}
+
+void orc_mg_vcycle(const orc_mg* mg, int l, const double* r, double* z)
+{
+    const orc_mg_level* L = &mg->lev[l];
+    const int64_t n = L->op.n;
+    double* work = (double*)malloc(sizeof(double) * (size_t)n * 7);
+    if (l == mg->nlevels - 1) {
+        orc_cheb_jacobi(&L->op, mg->k_coarse, L->lmax, L->dinv, r, z, work);
+        free(work);
+        return;
+    }
+    double* res = work + 4 * n; double* Az = work + 5 * n; double* tmp = work + 6 * n;
+    const int64_t nc = mg->lev[l + 1].op.n;
+    double* rc = (double*)malloc(sizeof(double) * (size_t)nc * 2); double* ec = rc + nc;
+    orc_cheb_jacobi(&L->op, mg->k_smooth, L->lmax, L->dinv, r, z, work);          /* z = S r            */
+    orc_apply_A(&L->op, z, Az, tmp);
+    for (int64_t q = 0; q < n; ++q) res[q] = r[q] - Az[q];                          /* res = r - A z      */
+    orc_mg_restrict(mg, l, res, rc, tmp);
+    orc_mg_vcycle(mg, l + 1, rc, ec);
+    orc_mg_prolong(mg, l, ec, tmp);
+    for (int64_t q = 0; q < n; ++q) z[q] += tmp[q];                                 /* z += P e           */
+    orc_apply_A(&L->op, z, Az, tmp);
+    for (int64_t q = 0; q < n; ++q) res[q] = r[q] - Az[q];                          /* res = r - A z      */
+    orc_cheb_jacobi(&L->op, mg->k_smooth, L->lmax, L->dinv, res, Az, work);        /* Az = S res         */
+    for (int64_t q = 0; q < n; ++q) z[q] += Az[q];
+    free(rc); free(work);
+}
+
+/* z = M^-1 r : precond 0 = identity, 1 = Jacobi, 2 = Chebyshev-Jacobi(cheb_k), 3 = p-multigrid V-cycle */
+static void precond_apply(const orc_op* op, int precond, int cheb_k, double lmax, const double* dinv, const orc_mg* mg,
                           const double* r, double* z, double* work)
 {
     if (precond == 0)      for (int64_t l = 0; l < op->n; ++l) z[l] = r[l];
     else if (precond == 1) for (int64_t l = 0; l < op->n; ++l) z[l] = dinv[l] * r[l];
-    else                   orc_cheb_jacobi(op, cheb_k, lmax, dinv, r, z, work);
+    else if (precond == 2) orc_cheb_jacobi(op, cheb_k, lmax, dinv, r, z, work);
+    else                   orc_mg_vcycle(mg, 0, r, z);
 }
 
 /* c-9  preconditioned conjugate gradients, step by step (the pressure Poisson solve).
  * b: assembled, masked rhs; x: initial guess in, solution out (continuous, zero at masked nodes).
  * hist[0..hist_len): ||r_it|| for it = 0,1,...  Returns 0 converged, 1 maxit reached,
  * -5 breakdown (gamma <= 0 or not finite).  out3 = { iterations, ||r0||, ||r_final|| }.   */
-int orc_pcg(const orc_op* op, int precond, int cheb_k, double lmax, const double* dinv,
+static int pcg_core(const orc_op* op, int precond, int cheb_k, double lmax, const double* dinv, const orc_mg* mg,
             const double* b, double* x, double rtol, double atol, int maxit, int x0_is_zero,
             double* hist, int hist_len, double* out3)
 {
@@ -462,7 +572,7 @@ int orc_pcg(const orc_op* op, int precond, int cheb_k, double lmax, const double
     for (int64_t l = 0; l < n; ++l) p[l] = 0.0;
     if (rnorm <= target) status = 0;
     else for (it = 1; it <= maxit; ++it) {
-        precond_apply(op, precond, cheb_k, lmax, dinv, r, z, work);
+        precond_apply(op, precond, cheb_k, lmax, dinv, mg, r, z, work);
         double rho_new = orc_dot(op, r, z);
         double beta = (it == 1) ? 0.0 : rho_new / rho_old;
         for (int64_t l = 0; l < n; ++l) p[l] = z[l] + beta * p[l];
@@ -480,6 +590,20 @@ int orc_pcg(const orc_op* op, int precond, int cheb_k, double lmax, const double
     out3[0] = (double)it; out3[2] = rnorm;
     free(r);
     return status;
+}
+
+int orc_pcg(const orc_op* op, int precond, int cheb_k, double lmax, const double* dinv,
+            const double* b, double* x, double rtol, double atol, int maxit, int x0_is_zero,
+            double* hist, int hist_len, double* out3)
+{
+    if (precond < 0 || precond > 2) return -1;
+    return pcg_core(op, precond, cheb_k, lmax, dinv, NULL, b, x, rtol, atol, maxit, x0_is_zero, hist, hist_len, out3);
+}
+/* PCG on level 0 of mg with the V-cycle as preconditioner (f-1) */
+int orc_pcg_mg(const orc_mg* mg, const double* b, double* x, double rtol, double atol, int maxit, int x0_is_zero,
+               double* hist, int hist_len, double* out3)
+{
+    return pcg_core(&mg->lev[0].op, 3, 0, 0.0, mg->lev[0].dinv, mg, b, x, rtol, atol, maxit, x0_is_zero, hist, hist_len, out3);
 }
 
 /* c-10  Lanczos on D^-1/2 A D^-1/2 from the start vector v0 (continuous, masked; normalised here).

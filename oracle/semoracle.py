@@ -208,3 +208,90 @@ class Problem:
                            C.c_int(1 if x0 is None else 0), _p(hist), C.c_int(hist_len), _p(out3))
         it = int(out3[0])
         return dict(x=x, iters=it, status=int(st), r0=out3[1], rn=out3[2], hist=hist[:min(hist_len, it + 1)])
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# f-1  p-multigrid V-cycle preconditioner (semoracle.c: orc_mg_*; reading R19)
+class _MgLevel(C.Structure):
+    _fields_ = [("op", _Op), ("dinv", C.c_void_p), ("lmax", C.c_double), ("J", C.c_void_p)]
+
+
+class _Mg(C.Structure):
+    _fields_ = [("nlevels", C.c_int32), ("k_smooth", C.c_int32), ("k_coarse", C.c_int32), ("pad_", C.c_int32),
+                ("lev", _MgLevel * 8)]
+
+
+def interp_matrix(Nfrom, Nto):
+    """J[(Nto+1), (Nfrom+1)]: Lagrange basis of the order-Nfrom GLL nodes evaluated at the order-Nto GLL nodes."""
+    J = np.zeros((Nto + 1, Nfrom + 1))
+    if lib().orc_interp_matrix(C.c_int(Nfrom), C.c_int(Nto), _p(J)):
+        raise ValueError("interp_matrix")
+    return J
+
+
+def interp3(E, J, v, transpose=False):
+    """per element J x J x J (or its transpose) applied to v; J is [nf1, nc1]."""
+    nf1, nc1 = J.shape
+    out = np.zeros(E * (nc1 if transpose else nf1) ** 3)
+    lib().orc_interp3(C.c_int64(E), C.c_int(nf1), C.c_int(nc1), _p(np.ascontiguousarray(J)), C.c_int(1 if transpose else 0),
+                      _p(_f64(v)), _p(out))
+    return out
+
+
+class Multigrid:
+    """Levels of the p-multigrid preconditioner for the operator (lam, tags) on a mesh: level 0 is order N, level l
+    the same elements at order orders[l] with coordinates interpolated from level 0.  lmax[l] = 1.1 x the largest
+    Ritz value of a 10-step Lanczos from the seeded start vector v0_of(level problem) (or given)."""
+
+    def __init__(self, E, N, x, y, z, face_tag, period, lam, tags, orders, k_smooth=2, k_coarse=2, lmax=None, v0_of=None):
+        assert orders[0] == N and all(a > b for a, b in zip(orders, orders[1:])) and len(orders) <= 8
+        self.orders = list(orders)
+        self.k_smooth, self.k_coarse = int(k_smooth), int(k_coarse)
+        self.levels, self.J, self.coords = [], [], []
+        for l, Nl in enumerate(orders):
+            if l == 0:
+                xl, yl, zl = _f64(x), _f64(y), _f64(z)
+            else:
+                Jc = interp_matrix(N, Nl)                       # fine Lagrange basis at the coarse nodes
+                xl, yl, zl = (interp3(E, Jc, a) for a in (x, y, z))
+            self.coords.append((xl, yl, zl))
+            self.levels.append(Problem(E, Nl, xl, yl, zl, face_tag, period, lam=lam, dirichlet_tags=tags))
+        for l in range(len(orders) - 1):
+            self.J.append(interp_matrix(orders[l + 1], orders[l]))      # [n1_l, n1_{l+1}]
+        if lmax is None:
+            lmax = []
+            for P in self.levels:
+                v0 = v0_of(P) if v0_of is not None else P.assemble_rhs(np.ones(P.n))
+                lmax.append(P.lanczos_lmax(v0, 10))
+        self.lmax = [float(v) for v in lmax]
+        self._mg = _Mg()
+        self._mg.nlevels, self._mg.k_smooth, self._mg.k_coarse = len(orders), self.k_smooth, self.k_coarse
+        for l, P in enumerate(self.levels):
+            self._mg.lev[l].op = P._op
+            self._mg.lev[l].dinv = P.dinv.ctypes.data
+            self._mg.lev[l].lmax = self.lmax[l]
+            self._mg.lev[l].J = self.J[l].ctypes.data if l < len(self.J) else None
+
+    def prolong(self, l, vc):
+        vf = np.zeros(self.levels[l].n)
+        lib().orc_mg_prolong(C.byref(self._mg), C.c_int(l), _p(_f64(vc)), _p(vf))
+        return vf
+
+    def restrict(self, l, rf):
+        rc = np.zeros(self.levels[l + 1].n); tmp = np.zeros(self.levels[l].n)
+        lib().orc_mg_restrict(C.byref(self._mg), C.c_int(l), _p(_f64(rf)), _p(rc), _p(tmp))
+        return rc
+
+    def vcycle(self, r, level=0):
+        z = np.zeros(self.levels[level].n)
+        lib().orc_mg_vcycle(C.byref(self._mg), C.c_int(level), _p(_f64(r)), _p(z))
+        return z
+
+    def pcg(self, b, x0=None, rtol=1e-10, atol=0.0, maxit=10000, hist_len=0):
+        P = self.levels[0]
+        x = np.zeros(P.n) if x0 is None else _f64(x0).copy()
+        hist = np.zeros(max(hist_len, 1)); out3 = np.zeros(3)
+        st = lib().orc_pcg_mg(C.byref(self._mg), _p(_f64(b)), _p(x), C.c_double(rtol), C.c_double(atol), C.c_int(maxit),
+                              C.c_int(1 if x0 is None else 0), _p(hist), C.c_int(hist_len), _p(out3))
+        it = int(out3[0])
+        return dict(x=x, iters=it, status=int(st), r0=out3[1], rn=out3[2], hist=hist[:min(hist_len, it + 1)])

@@ -1,0 +1,166 @@
+"""Pins of the p-multigrid V-cycle preconditioner of the oracle (reading R19).
+
+Expected values never come from the oracle's own multigrid code: interpolation matrices are rebuilt from monomial
+Vandermonde systems, the 3-D transfer from numpy.kron, the global prolongation from the numbering, the smoother
+from the closed-form Chebyshev residual polynomial through a dense eigendecomposition, and the V-cycle from the
+textbook error-propagation product  I - B A = (I - S A)(I - P B_c P^T A)(I - S A)  in dense algebra.
+"""
+import numpy as np
+import pytest
+from numpy.polynomial import chebyshev as Ch
+
+from paper_2501_13240_b200 import inputs as I
+from test_oracle_operator import dense_matrix, make, to_global, to_local
+
+
+def vandermonde_interp(x_from, x_to):
+    """Lagrange interpolation matrix through monomials: J = V(x_to) V(x_from)^-1 (independent of the product formula)."""
+    n = len(x_from)
+    return np.vander(x_to, n, increasing=True) @ np.linalg.inv(np.vander(x_from, n, increasing=True))
+
+
+def test_interp_matrix_closed_forms(orc):
+    J = orc.interp_matrix(1, 2)                                    # linear basis at -1, 0, 1
+    assert np.array_equal(J, np.array([[1.0, 0.0], [0.5, 0.5], [0.0, 1.0]]))
+    for Nc, Nf in [(1, 3), (3, 7), (1, 7), (5, 9), (2, 4), (7, 3), (9, 5)]:      # both directions (coordinates go fine -> coarse)
+        xc, xf = orc.gll(Nc)[0], orc.gll(Nf)[0]
+        J = orc.interp_matrix(Nc, Nf)
+        assert J.shape == (Nf + 1, Nc + 1)
+        assert np.allclose(J, vandermonde_interp(xc, xf), rtol=0, atol=1e-12)
+        assert np.allclose(J.sum(axis=1), 1.0, rtol=0, atol=1e-14)                 # partition of unity
+        for p in range(Nc + 1):                                                    # exact for degree <= N_from
+            assert np.allclose(J @ xc ** p, xf ** p, rtol=0, atol=1e-13)
+        assert np.array_equal(J[0], np.eye(Nc + 1)[0]) and np.array_equal(J[-1], np.eye(Nc + 1)[-1])   # end nodes coincide
+
+
+def test_interp3_is_the_kronecker_product(orc):
+    J = orc.interp_matrix(2, 4)
+    E = 3
+    v = I.uniform(3, E * 27)
+    K = np.kron(J, np.kron(J, J))                                   # (k,j,i) ordering, i fastest
+    out = orc.interp3(E, J, v)
+    assert np.allclose(out.reshape(E, -1), v.reshape(E, -1) @ K.T, rtol=0, atol=1e-14)
+    w = I.uniform(4, E * 125)
+    outT = orc.interp3(E, J, w, transpose=True)
+    assert np.allclose(outT.reshape(E, -1), w.reshape(E, -1) @ K, rtol=0, atol=1e-13)
+
+
+def _mg(orc, m, lam, tags, orders, k=2, kc=2, lmax=None):
+    return orc.Multigrid(m.E, m.N, m.x, m.y, m.z, m.face_tag, m.period, lam, tags, orders, k_smooth=k, k_coarse=kc, lmax=lmax)
+
+
+def _cont(orc, P, seed):
+    """continuous, masked random vector on the level problem P"""
+    return P.mask * orc.gs(P.gid, P.n_unique, P.invmult * I.uniform(seed, P.n))
+
+
+@pytest.mark.parametrize("kind", ["box", "ogrid"])
+def test_transfer_continuity_mask_and_adjointness(orc, xi_of, kind):
+    N = 4
+    m = I.box_mesh(3, 2, 2, N, xi_of(N), deform=0.05, periodic=(True, False, False)) if kind == "box" \
+        else I.ogrid_mesh(2, 2, 2, N, xi_of(N))
+    mg = _mg(orc, m, 0.0, 0b10, [4, 2, 1], lmax=[1.0, 1.0, 1.0])
+    for l in range(2):
+        Pf, Pc = mg.levels[l], mg.levels[l + 1]
+        # coarse coordinates are the fine interpolant at the coarse nodes: the coarse mesh has the same volume
+        vc = _cont(orc, Pc, 11 + l)
+        vf = mg.prolong(l, vc)
+        assert np.allclose(orc.gs(Pf.gid, Pf.n_unique, vf * Pf.invmult), vf, rtol=0, atol=1e-14)    # continuous
+        assert np.all(vf[Pf.mask == 0] == 0)
+        rf = _cont(orc, Pf, 21 + l)
+        rc = mg.restrict(l, rf)
+        assert np.allclose(orc.gs(Pc.gid, Pc.n_unique, rc * Pc.invmult), rc, rtol=0, atol=1e-13)
+        assert np.all(rc[Pc.mask == 0] == 0)
+        lhs, rhs = Pf.dot(vf, rf), Pc.dot(vc, rc)                   # <P v, r>_f = <v, R r>_c on unique nodes
+        assert abs(lhs - rhs) <= 1e-13 * max(abs(lhs), 1.0)
+    # prolongation reproduces a field of degree <= N_c exactly: the coordinate x of an affine mesh (degree 1)
+    if kind == "box":
+        ma = I.box_mesh(3, 2, 2, N, xi_of(N))
+        mga = _mg(orc, ma, 0.0, 0, [4, 2, 1], lmax=[1.0, 1.0, 1.0])
+        for l in range(2):
+            for c in range(3):
+                assert np.allclose(orc.interp3(ma.E, mga.J[l], mga.coords[l + 1][c]), mga.coords[l][c], rtol=0, atol=1e-13)
+
+
+def _global_prolongation(orc, Pf, Pc, Nf, Nc):
+    """dense [n_unique_f, n_unique_c] from numpy's own interpolation matrix and the two numberings"""
+    J = vandermonde_interp(orc.gll(Nc)[0], orc.gll(Nf)[0])
+    K = np.kron(J, np.kron(J, J))
+    Pg = np.zeros((Pf.n_unique, Pc.n_unique))
+    gf = Pf.gid.reshape(Pf.E, -1); gc = Pc.gid.reshape(Pc.E, -1)
+    for e in range(Pf.E):
+        Pg[gf[e][:, None], gc[e][None, :]] = K                      # every copy of a fine node gives the same row
+    return Pg
+
+
+def _cheb_dense(Af, k, lmax):
+    Dm = np.diag(Af)
+    ev, V = np.linalg.eigh(Af / np.sqrt(np.outer(Dm, Dm)))
+    lmin = 0.1 * lmax; theta = 0.5 * (lmax + lmin); delta = 0.5 * (lmax - lmin); sigma = theta / delta
+    Tk1 = Ch.Chebyshev.basis(k + 1)
+    pk = (1.0 - Tk1((theta - ev) / delta) / Tk1(sigma)) / ev
+    return ((V * pk) @ V.T) / np.sqrt(np.outer(Dm, Dm))
+
+
+@pytest.mark.parametrize("lam,tags", [(0.0, 0b10), (50.0, 0)])
+def test_vcycle_equals_dense_composition_and_is_spd(orc, xi_of, lam, tags):
+    N = 4
+    m = I.box_mesh(2, 2, 2, N, xi_of(N), deform=0.05)
+    orders = [4, 2, 1]
+    mg0 = _mg(orc, m, lam, tags, orders, lmax=[1.0, 1.0, 1.0])
+    A, free, lmax = [], [], []
+    for P in mg0.levels:
+        Ad = dense_matrix(P); fr = to_global(P, P.mask) > 0
+        A.append(Ad[np.ix_(fr, fr)]); free.append(fr)
+        Dm = np.diag(A[-1])
+        lmax.append(1.1 * np.linalg.eigvalsh(A[-1] / np.sqrt(np.outer(Dm, Dm)))[-1])
+    k, kc = 2, 3
+    mg = _mg(orc, m, lam, tags, orders, k=k, kc=kc, lmax=lmax)
+    B = _cheb_dense(A[2], kc, lmax[2])
+    for l in (1, 0):
+        Pg = _global_prolongation(orc, mg.levels[l], mg.levels[l + 1], orders[l], orders[l + 1])[np.ix_(free[l], free[l + 1])]
+        S = _cheb_dense(A[l], k, lmax[l]); Id = np.eye(A[l].shape[0])
+        B = S + (Id - S @ A[l]) @ (S + Pg @ B @ Pg.T @ (Id - A[l] @ S))
+    P0 = mg.levels[0]
+    nf = int(free[0].sum())
+    Bo = np.zeros((nf, nf))
+    idx = np.flatnonzero(free[0])
+    for c, g in enumerate(idx):
+        e = np.zeros(P0.n_unique); e[g] = 1.0
+        z = mg.vcycle(to_local(P0, e))
+        assert np.all(z[P0.mask == 0] == 0)
+        Bo[:, c] = to_global(P0, z)[free[0]]
+    scale = np.abs(B).max()
+    assert np.abs(Bo - B).max() <= 1e-11 * scale
+    assert np.abs(Bo - Bo.T).max() <= 1e-12 * scale                 # symmetric
+    assert np.linalg.eigvalsh(0.5 * (Bo + Bo.T))[0] > 0             # positive definite
+    ev = np.linalg.eigvals(Bo @ A[0]).real
+    # spectrum of M^-1 A: clustered below 1; it may exceed 1 slightly because the coarse operators are
+    # re-discretisations, not Galerkin products (measured here: [0.85, 1.004])
+    assert ev.min() > 0.3 and ev.max() < 1.2
+    # the restriction alone: R = P^T on the free unique nodes
+    rf = _cont(orc, P0, 9)
+    rc = mg.restrict(0, rf)
+    Pg = _global_prolongation(orc, mg.levels[0], mg.levels[1], orders[0], orders[1])[np.ix_(free[0], free[1])]
+    assert np.allclose(to_global(mg.levels[1], rc)[free[1]], Pg.T @ to_global(P0, rf)[free[0]], rtol=0, atol=1e-13)
+
+
+def test_pmg_pcg_solves_and_beats_chebyshev_jacobi(orc, xi_of):
+    m, _ = I.config_mesh(2, xi_of, small=True)                      # reduced O-grid, N = 7
+    mg = _mg(orc, m, 0.0, 0b10, [7, 3, 1], k=2, kc=4)
+    P = mg.levels[0]
+    b = P.assemble_rhs(I.divergence_source(m, 5))
+    rm = mg.pcg(b, rtol=1e-10, hist_len=200)
+    rj = P.pcg(b, precond=1)
+    rc = P.pcg(b, precond=2, cheb_k=2, lmax=mg.lmax[0])
+    assert rm["status"] == 0 and rj["status"] == 0
+    assert rm["iters"] < 0.5 * rc["iters"] < 0.5 * rj["iters"]
+    assert np.abs(rm["x"] - rj["x"]).max() <= 1e-8 * np.abs(rj["x"]).max()
+    res = b - P.apply_A(rm["x"])
+    assert np.sqrt(P.dot(res, res)) <= 2e-10 * np.sqrt(P.dot(b, b))
+    assert np.all(np.diff(rm["hist"]) < 0) or rm["iters"] < 40     # residuals fall fast
+    # Helmholtz with a large shift: the V-cycle must still be SPD (PCG converges) and cheap in iterations
+    mgh = _mg(orc, m, 3000.0, 0b110, [7, 3, 1], k=2, kc=4)
+    bh = mgh.levels[0].assemble_rhs(I.divergence_source(m, 6))
+    rh = mgh.pcg(bh)
+    assert rh["status"] == 0 and rh["iters"] <= mgh.levels[0].pcg(bh, precond=1)["iters"]
