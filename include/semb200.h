@@ -133,7 +133,7 @@ SEMB_API int semb_jacobi_diag(semb_handle h, double lambda, uint32_t dirichlet_t
 typedef struct {
     double   lambda;          /* operator D^T G D + lambda B                                     */
     uint32_t dirichlet_tags;  /* bit t set => faces tagged t are Dirichlet (homogeneous)         */
-    int32_t  precond;         /* 0 none, 1 Jacobi, 2 Chebyshev-Jacobi                            */
+    int32_t  precond;         /* 3 = p-multigrid V-cycle (mg_* fields); 0 none, 1 Jacobi, 2 Chebyshev-Jacobi                            */
     int32_t  cheb_degree;     /* k operator applications per preconditioner application          */
     double   cheb_lmax;       /* upper bound of spec(D^-1 A); <= 0 => 10-step Lanczos x 1.1      */
     double   rtol, atol;      /* stop when ||r|| <= max(rtol ||b||, atol) (unique-node 2-norm)   */
@@ -143,6 +143,16 @@ typedef struct {
                                  The iteration count returned is exact regardless.               */
     int32_t  profile;         /* 1: bracket every axhelm launch of the loop with CUDA events on the stream
                                  (no synchronisation added) and report their mean in stats.axhelm_ms     */
+    /* precond == 3: p-multigrid V-cycle (§2.2 "p-multigrid ... Chebyshev-accelerated ... smoothers";
+     * DESIGN.md reading R19).  Level l re-discretises the same elements at order mg_orders[l] (mg_orders[0] = N,
+     * strictly decreasing, >= 1), coordinates interpolated from level 0; transfer = Lagrange interpolation of the
+     * coarse basis at the fine GLL nodes and its transpose on unique nodes; smoother = Chebyshev-Jacobi of degree
+     * mg_smooth_degree before and after the coarse correction, of degree mg_coarse_degree alone on the last level;
+     * mg_lmax[l] <= 0 => estimated (10-step Lanczos x 1.1 from the level's M QQ^T B 1) and cached in the handle. */
+    int32_t  mg_nlevels;      /* 2..8; 0 with precond == 3 => orders N, 3, 1 (N > 3) or N, 1           */
+    int32_t  mg_orders[8];
+    int32_t  mg_smooth_degree, mg_coarse_degree;     /* <= 0 => 2 and 4                                 */
+    double   mg_lmax[8];
 } semb_pcg_opts;
 
 typedef struct {
@@ -181,6 +191,19 @@ SEMB_API int semb_step_solve(semb_handle h, int nsolves, const semb_solve_item* 
  * masked start vector v0 (device [n]). */
 SEMB_API int semb_estimate_lmax(semb_handle h, double lambda, uint32_t dirichlet_tags, const double* v0,
                        int steps, double* lmax_out, void* stream);
+
+/* z = one p-multigrid V-cycle applied to r (device [n] each, z != r; r continuous and masked) for the operator
+ * (opts->lambda, opts->dirichlet_tags) with the levels opts->mg_* describe.  lmax_used_or_null HOST [nlevels]:
+ * the bounds the smoothers used.  The coarse levels are built on first use and owned by the handle. */
+SEMB_API int semb_mg_vcycle(semb_handle h, const semb_pcg_opts* opts, const double* r, double* z,
+                   double* lmax_used_or_null, void* stream);
+/* Transfer between levels `level` and `level + 1` of the same hierarchy: restrict_ == 0: out (level, [n_level]) =
+ * M P in (level + 1); restrict_ != 0: out (level + 1) = M QQ^T J^T (invmult o in) (level).  Device pointers;
+ * sizes: semb_mg_level_size. */
+SEMB_API int semb_mg_transfer(semb_handle h, const semb_pcg_opts* opts, int level, int restrict_, const double* in,
+                     double* out, void* stream);
+/* local nodes of level `level` (E * (mg_orders[level] + 1)^3), or < 0 on error */
+SEMB_API int64_t semb_mg_level_size(semb_handle h, const semb_pcg_opts* opts, int level);
 
 /* z = Chebyshev-Jacobi(k) preconditioner applied to r (device [n] each, z != r). */
 SEMB_API int semb_cheb_jacobi(semb_handle h, double lambda, uint32_t dirichlet_tags, int k, double lmax,

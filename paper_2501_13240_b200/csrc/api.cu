@@ -53,6 +53,8 @@ int semb_destroy(semb_handle h)
 {
     if (!h) return SEMB_OK;
     cudaDeviceSynchronize();
+    semb_mg_destroy_all(h);
+    semb_dev_free(h, h->xyz);
     semb_dev_free(h, h->geo); semb_dev_free(h, h->gid); semb_dev_free(h, h->invmult); semb_dev_free(h, h->gs_code); semb_dev_free(h, h->gs_hi);
     if (h->geoK && h->geoK != h->geo) semb_dev_free(h, h->geoK);
     semb_dev_free(h, h->gs_off); semb_dev_free(h, h->gs_ids); semb_dev_free(h, h->face_tag_dev);
@@ -93,6 +95,16 @@ int semb_setup(int64_t E, int N, const double* x, const double* y, const double*
         if (!h->face_tag_dev) { rc = semb_fail(h, SEMB_ENOMEM, "face tags"); break; }
         if (cudaMemcpyAsync(h->face_tag_dev, face_tag, sizeof(int32_t) * (size_t)E * 6, cudaMemcpyHostToDevice, s) != cudaSuccess) {
             rc = semb_fail(h, SEMB_ECUDA, "face tag upload: %s", cudaGetErrorString(cudaGetLastError())); break;
+        }
+        h->xyz = (double*)semb_dev_alloc(h, sizeof(double) * 3 * (size_t)h->n);
+        if (!h->xyz) { rc = semb_fail(h, SEMB_ENOMEM, "coordinates"); break; }
+        {
+            const double* src[3] = { x, y, z };
+            bool ok = true;
+            for (int c = 0; c < 3; ++c)
+                ok = ok && cudaMemcpyAsync(h->xyz + c * h->n, src[c], sizeof(double) * (size_t)h->n, cudaMemcpyDeviceToDevice, s) == cudaSuccess;
+            if (!ok) { rc = semb_fail(h, SEMB_ECUDA, "coordinate copy: %s", cudaGetErrorString(cudaGetLastError())); break; }
+            for (int c = 0; c < 3; ++c) h->period[c] = period[c];
         }
         if ((rc = semb_axhelm_upload_basis(h))) break;
         if ((rc = semb_setup_geo(h, x, y, z, s))) break;
@@ -208,6 +220,33 @@ int semb_estimate_lmax(semb_handle h, double lambda, uint32_t tags, const double
     if (!v0 || !lmax_out) return semb_fail(h, SEMB_EINVAL, "estimate_lmax: bad argument");
     int rc = semb_ensure_work(h, 4); if (rc) return rc;
     return semb_lanczos_run(h, lambda, tags, v0, steps, lmax_out, (cudaStream_t)stream);
+}
+
+int semb_mg_vcycle(semb_handle h, const semb_pcg_opts* o, const double* r, double* z, double* lmax_used, void* stream)
+{
+    if (!h) return SEMB_EINVAL;
+    if (!o || !r || !z || r == z) return semb_fail(h, SEMB_EINVAL, "mg_vcycle: bad argument");
+    semb_mg_ctx ctx;
+    int rc = semb_mg_prepare(h, o, &ctx, (cudaStream_t)stream); if (rc) return rc;
+    if (lmax_used) for (int l = 0; semb_mg_level_n(ctx, l) >= 0 && l < 8; ++l) lmax_used[l] = ctx.lmax[l];
+    return semb_mg_vcycle_run(h, ctx, 0, r, z, nullptr, (cudaStream_t)stream);
+}
+
+int semb_mg_transfer(semb_handle h, const semb_pcg_opts* o, int level, int restrict_, const double* in, double* out, void* stream)
+{
+    if (!h) return SEMB_EINVAL;
+    if (!o || !in || !out || in == out) return semb_fail(h, SEMB_EINVAL, "mg_transfer: bad argument");
+    semb_mg_ctx ctx;
+    int rc = semb_mg_prepare(h, o, &ctx, (cudaStream_t)stream); if (rc) return rc;
+    return semb_mg_transfer_run(h, ctx, level, restrict_, in, out, (cudaStream_t)stream);
+}
+
+int64_t semb_mg_level_size(semb_handle h, const semb_pcg_opts* o, int level)
+{
+    if (!h || !o) return SEMB_EINVAL;
+    semb_mg_ctx ctx;
+    int rc = semb_mg_prepare(h, o, &ctx, nullptr); if (rc) return rc;
+    return semb_mg_level_n(ctx, level);
 }
 
 int semb_cheb_jacobi(semb_handle h, double lambda, uint32_t tags, int k, double lmax, const double* r, double* z, void* stream)

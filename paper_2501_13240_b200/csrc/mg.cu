@@ -1,0 +1,300 @@
+// p-multigrid V-cycle preconditioner (§2.2: NekRS preconditions the pressure
+// Poisson solve with "p-multigrid ... Chebyshev-accelerated ... smoothers"; the paper gives no formulas, DESIGN.md
+// reading R19 fixes them).
+//
+// Level l re-discretises the SAME elements at order N_l (N_0 = N > N_1 > ...): its coordinates are the level-0
+// coordinates interpolated to the order-N_l GLL nodes, and everything else -- geometric factors, numbering,
+// gather lists, masks, Jacobi diagonal, axhelm kernels -- is an ordinary semb_mesh built from them, so every
+// level runs the same hand-written kernels as the fine problem.
+//   prolongation  level l+1 -> l : v_f(i,j,k) = sum_abc J_ia J_jb J_kc v_c(a,b,c),  J_ia = l^(l+1)_a(xi^(l)_i)
+//   restriction   level l -> l+1 : r_c = M_c QQ^T_c (J^T x J^T x J^T)(invmult_f o r_f)
+//   V(l, r):  last level: z = Cheb_{k_coarse}(r);   else
+//             z = Cheb_k(r);  res = r - A z;  z += P V(l+1, R res);  res = r - A z;  z += Cheb_k(res)
+// which is symmetric positive definite (same symmetric smoother before and after; oracle pin: dense composition).
+#include <math.h>
+
+#include <array>
+#include <map>
+
+#include "semb_internal.h"
+
+struct semb_mg {
+    int nlevels = 0;
+    int orders[8] = {0};
+    semb_mesh* lev[8] = {nullptr};       // lev[0] = the owner (not owned), lev[l >= 1] owned
+    double* J[8] = {nullptr};            // device [n1_l][n1_{l+1}] row-major, transfer between l+1 and l
+    double* W[8][6] = {{nullptr}};       // per level: Chebyshev work (res, d, Ad), residual, A z / second smooth, spare
+    double* rc[8] = {nullptr};           // level l >= 1: restricted residual
+    double* ec[8] = {nullptr};           // level l >= 1: coarse correction
+    std::map<std::pair<uint32_t, double>, std::array<double, 8>> lmax_cache;
+};
+
+// J[(Nto+1) x (Nfrom+1)]: Lagrange basis of the order-Nfrom GLL nodes at the order-Nto GLL nodes (product formula;
+// rows at coinciding end nodes are exact unit vectors, so interpolation keeps exact zeros on Dirichlet faces).
+static void interp_matrix_host(int Nfrom, int Nto, double* J)
+{
+    double xf[SEMB_MAXN1], xt[SEMB_MAXN1], w[SEMB_MAXN1], D[SEMB_MAXN1 * SEMB_MAXN1];
+    semb_basis_host(Nfrom, xf, w, D);
+    semb_basis_host(Nto, xt, w, D);
+    for (int i = 0; i <= Nto; ++i)
+        for (int a = 0; a <= Nfrom; ++a) {
+            long double v = 1.0L;
+            for (int m = 0; m <= Nfrom; ++m)
+                if (m != a) v *= ((long double)xt[i] - (long double)xf[m]) / ((long double)xf[a] - (long double)xf[m]);
+            J[i * (Nfrom + 1) + a] = (double)v;
+        }
+}
+
+// One block per element: out = (J x J x J) in  (transpose == 0: J is [nout][nin]) or (J^T x J^T x J^T) in
+// (transpose != 0: J is [nin][nout]), by three one-dimensional passes through shared memory.
+// scale != NULL: the input is multiplied by scale (restriction: invmult);  accumulate: out += result.
+#define MG_MAXNP (SEMB_MAXN1 * SEMB_MAXN1 * SEMB_MAXN1)
+__global__ void __launch_bounds__(128)
+k_interp3(int nin, int nout, const double* __restrict__ J, int transpose, const double* __restrict__ in,
+          const double* __restrict__ scale, double* __restrict__ out, int accumulate, const semb_scalars* __restrict__ scal)
+{
+    __shared__ double A[MG_MAXNP], B[MG_MAXNP], Js[SEMB_MAXN1 * SEMB_MAXN1];
+    if (scal && *(volatile const int32_t*)&scal->done) return;
+    const int64_t e = blockIdx.x;
+    const int npi = nin * nin * nin, npo = nout * nout * nout;
+    for (int t = threadIdx.x; t < nin * nout; t += blockDim.x) {
+        const int o = t / nin, a = t % nin;                       // Js[o][a] = coefficient of input a in output o
+        Js[t] = transpose ? J[a * nout + o] : J[o * nin + a];
+    }
+    for (int t = threadIdx.x; t < npi; t += blockDim.x) {
+        const double v = in[e * npi + t];
+        A[t] = scale ? v * scale[e * npi + t] : v;
+    }
+    __syncthreads();
+    // pass 1 (i): B[c][b][i] = sum_a Js[i][a] A[c][b][a]
+    for (int t = threadIdx.x; t < nin * nin * nout; t += blockDim.x) {
+        const int i = t % nout, cb = t / nout;
+        double s = 0.0;
+        for (int a = 0; a < nin; ++a) s += Js[i * nin + a] * A[cb * nin + a];
+        B[t] = s;
+    }
+    __syncthreads();
+    // pass 2 (j): A[c][j][i] = sum_b Js[j][b] B[c][b][i]
+    for (int t = threadIdx.x; t < nin * nout * nout; t += blockDim.x) {
+        const int i = t % nout, j = (t / nout) % nout, c = t / (nout * nout);
+        double s = 0.0;
+        for (int b = 0; b < nin; ++b) s += Js[j * nin + b] * B[(c * nin + b) * nout + i];
+        A[t] = s;
+    }
+    __syncthreads();
+    // pass 3 (k): out[k][j][i] = sum_c Js[k][c] A[c][j][i]
+    for (int t = threadIdx.x; t < npo; t += blockDim.x) {
+        const int ji = t % (nout * nout), k = t / (nout * nout);
+        double s = 0.0;
+        for (int c = 0; c < nin; ++c) s += Js[k * nin + c] * A[c * nout * nout + ji];
+        if (accumulate) out[e * npo + t] += s; else out[e * npo + t] = s;
+    }
+}
+
+__global__ void k_mg_sub(int64_t n, const double* __restrict__ a, const double* __restrict__ b, double* __restrict__ out,
+                         const semb_scalars* __restrict__ scal)
+{
+    if (scal && *(volatile const int32_t*)&scal->done) return;
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) out[l] = a[l] - b[l];
+}
+__global__ void k_mg_add(int64_t n, const double* __restrict__ a, double* __restrict__ z, const semb_scalars* __restrict__ scal)
+{
+    if (scal && *(volatile const int32_t*)&scal->done) return;
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) z[l] += a[l];
+}
+__global__ void k_mg_fill(int64_t n, double* __restrict__ a, double v)
+{
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) a[l] = v;
+}
+static inline unsigned mg_grid(int64_t n) { int64_t b = (n + 1023) / 1024; return (unsigned)(b < 1 ? 1 : (b > 148 * 8 ? 148 * 8 : b)); }
+
+static void mg_free(semb_mesh* h, semb_mg* g)
+{
+    for (int l = 0; l < 8; ++l) {
+        semb_dev_free(h, g->J[l]); semb_dev_free(h, g->rc[l]); semb_dev_free(h, g->ec[l]);
+        for (int w = 0; w < 6; ++w) semb_dev_free(h, g->W[l][w]);
+        if (l >= 1 && g->lev[l]) semb_destroy(g->lev[l]);
+    }
+    delete g;
+}
+void semb_mg_destroy_all(semb_mesh* h)
+{
+    for (semb_mg* g : h->mgs) mg_free(h, g);
+    h->mgs.clear();
+}
+
+// ---- hierarchy ---------------------------------------------------------------------------------------------
+static int mg_build(semb_mesh* h, int nlevels, const int* orders, semb_mg** out, cudaStream_t s)
+{
+    semb_mg* g = new semb_mg();
+    g->nlevels = nlevels;
+    for (int l = 0; l < nlevels; ++l) g->orders[l] = orders[l];
+    g->lev[0] = h;
+    int rc = SEMB_OK;
+    do {
+        // the caller's x, y, z may be gone after setup: the hierarchy is built from the copy semb_setup kept
+        if (!h->xyz) { rc = semb_fail(h, SEMB_EINVAL, "multigrid: the handle holds no coordinates"); break; }
+        double Jh[SEMB_MAXN1 * SEMB_MAXN1];
+        for (int l = 1; l < nlevels && !rc; ++l) {
+            const int nc1 = orders[l] + 1; const int64_t npc = (int64_t)nc1 * nc1 * nc1, nl = h->E * npc;
+            double* xyz = (double*)semb_dev_alloc(h, sizeof(double) * 3 * (size_t)nl);
+            double* Jd = (double*)semb_dev_alloc(h, sizeof(double) * SEMB_MAXN1 * SEMB_MAXN1);
+            if (!xyz || !Jd) { semb_dev_free(h, xyz); semb_dev_free(h, Jd); rc = semb_fail(h, SEMB_ENOMEM, "multigrid: level %d coordinates", l); break; }
+            interp_matrix_host(h->N, orders[l], Jh);                                  // [nc1][n1]
+            if (cudaMemcpyAsync(Jd, Jh, sizeof(double) * nc1 * h->n1, cudaMemcpyHostToDevice, s) != cudaSuccess) rc = semb_fail(h, SEMB_ECUDA, "multigrid: upload");
+            for (int c = 0; c < 3 && !rc; ++c)
+                k_interp3<<<(unsigned)h->E, 128, 0, s>>>(h->n1, nc1, Jd, 0, h->xyz + c * h->n, nullptr, xyz + c * nl, 0, nullptr);
+            if (!rc && cudaStreamSynchronize(s) != cudaSuccess) rc = semb_fail(h, SEMB_ECUDA, "multigrid: coordinate interpolation: %s", cudaGetErrorString(cudaGetLastError()));
+            if (!rc) {
+                rc = semb_setup(h->E, orders[l], xyz, xyz + nl, xyz + 2 * nl, h->face_tag.data(), h->period,
+                                nullptr, h->has_alloc ? &h->alloc : nullptr, (void*)s, &g->lev[l]);
+                if (rc) semb_fail(h, rc, "multigrid: setup of level %d (order %d) failed: %s", l, orders[l], semb_last_error(nullptr));
+            }
+            semb_dev_free(h, xyz); semb_dev_free(h, Jd);
+        }
+        if (rc) break;
+        for (int l = 0; l < nlevels; ++l) {
+            semb_mesh* L = g->lev[l];
+            for (int w = 0; w < 6; ++w) {
+                g->W[l][w] = (double*)semb_dev_alloc(h, sizeof(double) * (size_t)L->n);
+                if (!g->W[l][w]) rc = semb_fail(h, SEMB_ENOMEM, "multigrid: work vectors of level %d", l);
+            }
+            if (l >= 1) {
+                g->rc[l] = (double*)semb_dev_alloc(h, sizeof(double) * (size_t)L->n);
+                g->ec[l] = (double*)semb_dev_alloc(h, sizeof(double) * (size_t)L->n);
+                if (!g->rc[l] || !g->ec[l]) rc = semb_fail(h, SEMB_ENOMEM, "multigrid: vectors of level %d", l);
+            }
+            if (l + 1 < nlevels) {
+                const int nf1 = orders[l] + 1, nc1 = orders[l + 1] + 1;
+                g->J[l] = (double*)semb_dev_alloc(h, sizeof(double) * nf1 * nc1);
+                if (!g->J[l]) { rc = semb_fail(h, SEMB_ENOMEM, "multigrid: transfer matrix"); break; }
+                interp_matrix_host(orders[l + 1], orders[l], Jh);                     // [nf1][nc1]
+                if (cudaMemcpy(g->J[l], Jh, sizeof(double) * nf1 * nc1, cudaMemcpyHostToDevice) != cudaSuccess) rc = semb_fail(h, SEMB_ECUDA, "multigrid: upload");
+            }
+            if (rc) break;
+        }
+    } while (0);
+    if (rc) { mg_free(h, g); return rc; }
+    h->mgs.push_back(g);
+    *out = g;
+    return SEMB_OK;
+}
+
+int semb_mg_prepare(semb_mesh* h, const semb_pcg_opts* o, semb_mg_ctx* ctx, cudaStream_t s)
+{
+    int nlev = o->mg_nlevels, orders[8];
+    if (nlev == 0) {
+        orders[0] = h->N; nlev = 1;
+        if (h->N > 3) orders[nlev++] = 3;
+        if (h->N > 1) orders[nlev++] = 1;
+    } else {
+        if (nlev < 1 || nlev > 8) return semb_fail(h, SEMB_EINVAL, "multigrid: mg_nlevels = %d", nlev);
+        for (int l = 0; l < nlev; ++l) orders[l] = o->mg_orders[l];
+    }
+    if (orders[0] != h->N) return semb_fail(h, SEMB_EINVAL, "multigrid: mg_orders[0] = %d must be the mesh order %d", orders[0], h->N);
+    for (int l = 1; l < nlev; ++l)
+        if (orders[l] < 1 || orders[l] >= orders[l - 1]) return semb_fail(h, SEMB_EINVAL, "multigrid: orders must decrease strictly and stay >= 1");
+    semb_mg* g = nullptr;
+    for (semb_mg* c : h->mgs) {
+        bool same = c->nlevels == nlev;
+        for (int l = 0; same && l < nlev; ++l) same = c->orders[l] == orders[l];
+        if (same) { g = c; break; }
+    }
+    if (!g) { int rc = mg_build(h, nlev, orders, &g, s); if (rc) return rc; }
+    ctx->mg = g; ctx->lambda = o->lambda; ctx->tags = o->dirichlet_tags;
+    ctx->k_smooth = o->mg_smooth_degree > 0 ? o->mg_smooth_degree : 2;
+    ctx->k_coarse = o->mg_coarse_degree > 0 ? o->mg_coarse_degree : 4;
+    if (ctx->k_smooth > 16 || ctx->k_coarse > 16) return semb_fail(h, SEMB_EINVAL, "multigrid: smoother degree > 16");
+    // Chebyshev bounds per level: given, cached, or estimated (10-step Lanczos x 1.1 from M QQ^T B 1)
+    const std::pair<uint32_t, double> key(o->dirichlet_tags, o->lambda);
+    auto it = g->lmax_cache.find(key);
+    std::array<double, 8> est{};
+    if (it != g->lmax_cache.end()) est = it->second;
+    bool changed = false;
+    for (int l = 0; l < nlev; ++l) {
+        if (o->mg_lmax[l] > 0.0) { ctx->lmax[l] = o->mg_lmax[l]; continue; }
+        if (!(est[l] > 0.0)) {
+            semb_mesh* L = g->lev[l];
+            double* ones = g->W[l][0]; double* v0 = g->W[l][1];
+            k_mg_fill<<<mg_grid(L->n), 256, 0, s>>>(L->n, ones, 1.0);
+            int rc = semb_assemble_rhs(L, o->dirichlet_tags, ones, v0, (void*)s);
+            if (!rc) rc = semb_estimate_lmax(L, o->lambda, o->dirichlet_tags, v0, 10, &est[l], (void*)s);
+            if (rc) return semb_fail(h, rc, "multigrid: lambda_max estimate on level %d: %s", l, semb_last_error(L));
+            changed = true;
+        }
+        ctx->lmax[l] = est[l];
+    }
+    if (changed) g->lmax_cache[key] = est;
+    // masks and diagonals of every level for this operator (cached in the level handles)
+    for (int l = 0; l < nlev; ++l) {
+        semb_mask_entry m; double* dinv;
+        int rc = semb_get_mask(g->lev[l], ctx->tags, &m, s);
+        if (!rc) rc = semb_get_dinv(g->lev[l], ctx->lambda, ctx->tags, &dinv, s);
+        if (rc) return semb_fail(h, rc, "multigrid: level %d: %s", l, semb_last_error(g->lev[l]));
+    }
+    return SEMB_OK;
+}
+
+int64_t semb_mg_level_n(const semb_mg_ctx& ctx, int level)
+{
+    return (level >= 0 && level < ctx.mg->nlevels) ? ctx.mg->lev[level]->n : -1;
+}
+
+int semb_mg_transfer_run(semb_mesh* h, const semb_mg_ctx& ctx, int l, int restrict_, const double* in, double* out, cudaStream_t s)
+{
+    semb_mg* g = ctx.mg;
+    if (l < 0 || l + 1 >= g->nlevels) return semb_fail(h, SEMB_EINVAL, "multigrid: transfer level %d", l);
+    semb_mesh* F = g->lev[l]; semb_mesh* C = g->lev[l + 1];
+    semb_mask_entry m;
+    if (!restrict_) {
+        k_interp3<<<(unsigned)F->E, 128, 0, s>>>(C->n1, F->n1, g->J[l], 0, in, nullptr, out, 0, nullptr);
+        int rc = semb_get_mask(F, ctx.tags, &m, s); if (rc) return rc;
+        h->launches += 1;
+        return semb_mask_launch(F, m, out, 1, s);
+    }
+    k_interp3<<<(unsigned)F->E, 128, 0, s>>>(F->n1, C->n1, g->J[l], 1, in, F->invmult, out, 0, nullptr);
+    h->launches += 1;
+    int rc = semb_gs_launch(C, out, 1, s); if (rc) return rc;
+    rc = semb_get_mask(C, ctx.tags, &m, s); if (rc) return rc;
+    return semb_mask_launch(C, m, out, 1, s);
+}
+
+// z = V(level, r).  scal (may be NULL): the PCG scalars of the fine handle, only read for the early exit.
+int semb_mg_vcycle_run(semb_mesh* h, const semb_mg_ctx& ctx, int l, const double* r, double* z, semb_scalars* scal, cudaStream_t s)
+{
+    semb_mg* g = ctx.mg;
+    semb_mesh* L = g->lev[l];
+    const int64_t n = L->n;
+    semb_mask_entry m; double* dinv;
+    int rc = semb_get_mask(L, ctx.tags, &m, s); if (rc) return rc;
+    rc = semb_get_dinv(L, ctx.lambda, ctx.tags, &dinv, s); if (rc) return rc;
+    double *cres = g->W[l][0], *cd = g->W[l][1], *cAd = g->W[l][2], *res = g->W[l][3], *t1 = g->W[l][4];
+    const int64_t l0 = L->launches;
+    if (l == g->nlevels - 1) {
+        rc = semb_cheb_apply(L, ctx.lambda, m, dinv, ctx.k_coarse, semb_cheb_coefficients(ctx.k_coarse, ctx.lmax[l]), r, z, cres, cd, cAd, scal, false, s);
+        if (L != h) { h->launches += L->launches - l0; }
+        return rc;
+    }
+    const semb_cheb_coef cc = semb_cheb_coefficients(ctx.k_smooth, ctx.lmax[l]);
+    semb_mesh* C = g->lev[l + 1];
+    semb_mask_entry mc;
+    rc = semb_get_mask(C, ctx.tags, &mc, s); if (rc) return rc;
+    rc = semb_cheb_apply(L, ctx.lambda, m, dinv, ctx.k_smooth, cc, r, z, cres, cd, cAd, scal, false, s); if (rc) return rc;   // z = S r
+    rc = semb_apply_A(L, ctx.lambda, m, z, t1, s); if (rc) return rc;
+    k_mg_sub<<<mg_grid(n), 256, 0, s>>>(n, r, t1, res, scal);                                                                 // res = r - A z
+    k_interp3<<<(unsigned)L->E, 128, 0, s>>>(L->n1, C->n1, g->J[l], 1, res, L->invmult, g->rc[l + 1], 0, scal);               // R res
+    rc = semb_gs_launch(C, g->rc[l + 1], 1, s); if (rc) return rc;
+    rc = semb_mask_launch(C, mc, g->rc[l + 1], 1, s); if (rc) return rc;
+    const int64_t lc0 = C->launches;
+    rc = semb_mg_vcycle_run(h, ctx, l + 1, g->rc[l + 1], g->ec[l + 1], scal, s); if (rc) return rc;
+    (void)lc0;
+    k_interp3<<<(unsigned)L->E, 128, 0, s>>>(C->n1, L->n1, g->J[l], 0, g->ec[l + 1], nullptr, z, 1, scal);                    // z += P e
+    rc = semb_apply_A(L, ctx.lambda, m, z, t1, s); if (rc) return rc;
+    k_mg_sub<<<mg_grid(n), 256, 0, s>>>(n, r, t1, res, scal);                                                                 // res = r - A z
+    rc = semb_cheb_apply(L, ctx.lambda, m, dinv, ctx.k_smooth, cc, res, t1, cres, cd, cAd, scal, false, s); if (rc) return rc; // t1 = S res
+    k_mg_add<<<mg_grid(n), 256, 0, s>>>(n, t1, z, scal);
+    L->launches += 5;
+    if (L != h) h->launches += L->launches - l0;
+    SEMB_CUDA(h, cudaGetLastError());
+    return SEMB_OK;
+}

@@ -288,6 +288,18 @@ static int apply_A(semb_mesh* h, double lambda, const semb_mask_entry& m, const 
     return semb_mask_launch(h, m, out, 1, s);
 }
 
+int semb_apply_A(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* v_masked, double* out, cudaStream_t s)
+{
+    return apply_A(h, lambda, m, v_masked, out, nullptr, s);
+}
+int semb_dot_rz_launch(semb_mesh* h, const double* r, const double* z, semb_scalars* scal, cudaStream_t s)
+{
+    k_dot_rz<<<vec_grid(h->n), VEC_BLOCK, 0, s>>>(h->n, r, z, h->invmult, scal, h->partials);
+    h->launches += 1;
+    SEMB_CUDA(h, cudaGetLastError());
+    return SEMB_OK;
+}
+
 int semb_operator_run(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* v, double* out, cudaStream_t s)
 {
     int rc = semb_ensure_work(h, 1); if (rc) return rc;
@@ -297,8 +309,8 @@ int semb_operator_run(semb_mesh* h, double lambda, const semb_mask_entry& m, con
     return apply_A(h, lambda, m, tmp, out, nullptr, s);
 }
 
-struct cheb_coef { double itheta; double c1[16], c2[16]; };
-static cheb_coef cheb_coefficients(int k, double lmax)
+typedef semb_cheb_coef cheb_coef;
+semb_cheb_coef semb_cheb_coefficients(int k, double lmax)
 {
     cheb_coef c;
     const double lmin = 0.1 * lmax, theta = 0.5 * (lmax + lmin), delta = 0.5 * (lmax - lmin), sigma = theta / delta;
@@ -315,7 +327,7 @@ static cheb_coef cheb_coefficients(int k, double lmax)
 // z = Cheb_k(r);  res, d, Ad: work vectors.  in_pcg: also leave rho = <r,z> and beta in scal (PCG loop).
 // Per application (k >= 1): axhelm with the first d formed in its prologue (80 B/node), then per step k_mask,
 // k_gs_hi, k_cheb_step (first 60, middle 68, last 60 B/node) and, between steps, a plain axhelm (64).
-static int cheb_apply(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* dinv, int k, const cheb_coef& c,
+int semb_cheb_apply(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* dinv, int k, const cheb_coef& c,
                       const double* r, double* z, double* res, double* d, double* Ad, semb_scalars* scal, bool in_pcg, cudaStream_t s)
 {
     const int64_t n = h->n; const unsigned G = vec_grid(n);
@@ -355,7 +367,7 @@ int semb_cheb_run(semb_mesh* h, double lambda, uint32_t tags, int k, double lmax
     rc = semb_get_dinv(h, lambda, tags, &dinv, s); if (rc) return rc;
     rc = semb_ensure_work(h, 3); if (rc) return rc;
     const int64_t n = h->n;
-    return cheb_apply(h, lambda, m, dinv, k, cheb_coefficients(k, lmax), r, z, h->work, h->work + n, h->work + 2 * n, nullptr, false, s);
+    return semb_cheb_apply(h, lambda, m, dinv, k, semb_cheb_coefficients(k, lmax), r, z, h->work, h->work + n, h->work + 2 * n, nullptr, false, s);
 }
 
 // largest eigenvalue of the symmetric tridiagonal (a[0..m), b[0..m-1)) by bisection on the Sturm count
@@ -429,15 +441,18 @@ int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* 
 {
     const int64_t n = h->n; const unsigned G = vec_grid(n);
     const int64_t launches0 = h->launches;
-    if (o->precond < 0 || o->precond > 2 || o->maxit < 0 || (o->precond == 2 && (o->cheb_degree < 0 || o->cheb_degree > 16)))
+    if (o->precond < 0 || o->precond > 3 || o->maxit < 0 || (o->precond == 2 && (o->cheb_degree < 0 || o->cheb_degree > 16)))
         return semb_fail(h, SEMB_EINVAL, "pcg: precond=%d cheb_degree=%d maxit=%d", o->precond, o->cheb_degree, o->maxit);
     semb_mask_entry m; double* dinv = nullptr;
     int rc = semb_get_mask(h, o->dirichlet_tags, &m, s); if (rc) return rc;
     if (o->precond >= 1) { rc = semb_get_dinv(h, o->lambda, o->dirichlet_tags, &dinv, s); if (rc) return rc; }
-    rc = semb_ensure_work(h, o->precond == 2 ? 6 : 3); if (rc) return rc;
+    semb_mg_ctx mgctx{};
+    if (o->precond == 3) { rc = semb_mg_prepare(h, o, &mgctx, s); if (rc) return rc; }   // may use h->work (lambda_max estimate)
+    rc = semb_ensure_work(h, o->precond == 2 ? 6 : (o->precond == 3 ? 4 : 3)); if (rc) return rc;
     double *r = h->work, *p = r + n, *q = r + 2 * n;
     double *z = nullptr, *res = nullptr, *d = nullptr;
     if (o->precond == 2) { z = r + 3 * n; res = r + 4 * n; d = r + 5 * n; }
+    if (o->precond == 3) z = r + 3 * n;
 
     double lmax = o->cheb_lmax;
     cheb_coef cc{};
@@ -447,7 +462,7 @@ int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* 
             rc = semb_lanczos_run(h, o->lambda, o->dirichlet_tags, b, 10, &lmax, s); if (rc) return rc;
             r = h->work; p = r + n; q = r + 2 * n; z = r + 3 * n; res = r + 4 * n; d = r + 5 * n;
         }
-        cc = cheb_coefficients(o->cheb_degree, lmax);
+        cc = semb_cheb_coefficients(o->cheb_degree, lmax);
     }
     // history buffer
     const int want_hist = (st && st->hist_host_or_null && st->hist_len > 0) ? st->hist_len : 0;
@@ -485,7 +500,11 @@ int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* 
         for (int i = 0; i < mbatch; ++i) {
             const double* zsrc = r;
             if (o->precond == 2) {
-                rc = cheb_apply(h, o->lambda, m, dinv, o->cheb_degree, cc, r, z, res, d, q, h->scal, true, s); if (rc) return rc;
+                rc = semb_cheb_apply(h, o->lambda, m, dinv, o->cheb_degree, cc, r, z, res, d, q, h->scal, true, s); if (rc) return rc;
+                zsrc = z;
+            } else if (o->precond == 3) {
+                rc = semb_mg_vcycle_run(h, mgctx, 0, r, z, h->scal, s); if (rc) return rc;
+                rc = semb_dot_rz_launch(h, r, z, h->scal, s); if (rc) return rc;
                 zsrc = z;
             }
             const int itn = it0 + i;
@@ -495,7 +514,7 @@ int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* 
             rc = semb_mask_launch(h, m, q, 1, s); if (rc) return rc;     // every copy of a Dirichlet node is masked => sum 0
             rc = semb_gs_hi_launch(h, q, h->scal, s); if (rc) return rc; // edges and corners; faces in k_update_r
             const gs_lists L{h->gs_code};
-            if (o->precond == 2) k_update_r<false><<<G, VEC_BLOCK, 0, s>>>(n, q, r, L, nullptr, h->scal, h->partials, hist, want_hist);
+            if (o->precond >= 2) k_update_r<false><<<G, VEC_BLOCK, 0, s>>>(n, q, r, L, nullptr, h->scal, h->partials, hist, want_hist);
             else                 k_update_r<true><<<G, VEC_BLOCK, 0, s>>>(n, q, r, L, dz, h->scal, h->partials, hist, want_hist);
             h->launches += 1;
         }
@@ -513,7 +532,7 @@ int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* 
     int status = S.status;
     if (st) {
         st->iters = S.iter; st->status = status; st->b_norm = S.bnorm; st->r0_norm = S.r0norm; st->r_norm = S.rnorm;
-        st->lmax_used = lmax;
+        st->lmax_used = (o->precond == 3) ? mgctx.lmax[0] : lmax;
         st->launches = h->launches - launches0;
         st->profiled = 0; st->axhelm_ms = 0.0;
         const int np_ = S.iter < nprof ? S.iter : nprof;

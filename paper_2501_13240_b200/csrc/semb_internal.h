@@ -32,6 +32,8 @@ struct semb_field_entry {
     bool derived = false;
 };
 
+struct semb_mg;
+
 struct semb_mesh {
     int64_t E = 0; int N = 0, n1 = 0; int64_t Np = 0, n = 0;
     int64_t n_unique = 0, n_shared = 0, n_gs = 0;
@@ -39,6 +41,8 @@ struct semb_mesh {
     bool has_alloc = false; semb_allocator alloc{};
     double xi[SEMB_MAXN1], rho[SEMB_MAXN1], D[SEMB_MAXN1 * SEMB_MAXN1];   // host copies
     // handle-owned device arrays
+    double*  xyz = nullptr;        // [3][n] copy of the node coordinates (coarse multigrid levels are built from it)
+    double   period[3] = {0.0, 0.0, 0.0};
     double*  geo = nullptr;        // [E][7][Np]  canonical layout (semb_info.geo)
     double*  geoK = nullptr;       // kernel-native layout of the same data (axhelm.cu), may alias geo
     int32_t* gid = nullptr;        // [n]
@@ -62,6 +66,7 @@ struct semb_mesh {
     double* stage = nullptr;            // device staging of the *_host entry points [2][n]
     int64_t launches = 0;               // kernels launched through this handle (bench.py reports it)
     std::vector<cudaEvent_t> prof_ev;   // event pairs around axhelm launches (opts.profile)
+    std::vector<semb_mg*> mgs;          // p-multigrid hierarchies built so far (mg.cu), owned
     // export
     std::vector<semb_field_entry> fields;
     int64_t cycle = 0; double time = 0.0;
@@ -123,6 +128,22 @@ int semb_cheb_run(semb_mesh* h, double lambda, uint32_t tags, int k, double lmax
 int semb_operator_run(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* v, double* out,
                       cudaStream_t s);
 int semb_ensure_work(semb_mesh* h, int64_t vecs);
+struct semb_cheb_coef { double itheta; double c1[16], c2[16]; };
+semb_cheb_coef semb_cheb_coefficients(int k, double lmax);
+// z = Cheb_k(r) on h;  res, d, Ad: work vectors [n].  in_pcg: also leave rho = <r,z> and beta in scal.
+int semb_cheb_apply(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* dinv, int k, const semb_cheb_coef& c,
+                    const double* r, double* z, double* res, double* d, double* Ad, semb_scalars* scal, bool in_pcg, cudaStream_t s);
+// out = M QQ^T A_L v  (v continuous and masked)
+int semb_apply_A(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* v_masked, double* out, cudaStream_t s);
+int semb_dot_rz_launch(semb_mesh* h, const double* r, const double* z, semb_scalars* scal, cudaStream_t s);
+
+// ---- mg.cu: p-multigrid V-cycle
+struct semb_mg_ctx { semb_mg* mg; double lambda; uint32_t tags; int k_smooth, k_coarse; double lmax[8]; };
+int semb_mg_prepare(semb_mesh* h, const semb_pcg_opts* o, semb_mg_ctx* ctx, cudaStream_t s);
+int semb_mg_vcycle_run(semb_mesh* h, const semb_mg_ctx& ctx, int level, const double* r, double* z, semb_scalars* scal, cudaStream_t s);
+int semb_mg_transfer_run(semb_mesh* h, const semb_mg_ctx& ctx, int level, int restrict_, const double* in, double* out, cudaStream_t s);
+int64_t semb_mg_level_n(const semb_mg_ctx& ctx, int level);
+void semb_mg_destroy_all(semb_mesh* h);
 
 // ---- export.cu
 int semb_vmag_launch(const double* vx, const double* vy, const double* vz, double* out, int64_t n, cudaStream_t s);

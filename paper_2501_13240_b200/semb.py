@@ -20,7 +20,7 @@ ERRORS = {-1: "SEMB_EINVAL", -2: "SEMB_ENOMEM", -3: "SEMB_ECUDA", -4: "SEMB_EGEO
 # every symbol include/semb200.h declares (tests check that the library exports all of them)
 SYMBOLS = ["semb_gll", "semb_setup", "semb_destroy", "semb_last_error", "semb_mesh_info", "semb_apply_axhelm",
            "semb_gather_scatter", "semb_apply_mask", "semb_assemble_rhs", "semb_apply_operator", "semb_jacobi_diag",
-           "semb_pcg_solve", "semb_step_solve", "semb_estimate_lmax", "semb_cheb_jacobi", "semb_publish_field", "semb_publish_state",
+           "semb_pcg_solve", "semb_step_solve", "semb_mg_vcycle", "semb_mg_transfer", "semb_mg_level_size", "semb_estimate_lmax", "semb_cheb_jacobi", "semb_publish_field", "semb_publish_state",
            "semb_export_field", "semb_field_minmax_hist", "semb_apply_axhelm_host", "semb_pcg_solve_host", "semb_read_device", "semb_version"]
 
 
@@ -40,7 +40,21 @@ class Info(C.Structure):
 class PcgOpts(C.Structure):
     _fields_ = [("lam", C.c_double), ("dirichlet_tags", C.c_uint32), ("precond", C.c_int32),
                 ("cheb_degree", C.c_int32), ("cheb_lmax", C.c_double), ("rtol", C.c_double), ("atol", C.c_double),
-                ("maxit", C.c_int32), ("x0_is_zero", C.c_int32), ("check_every", C.c_int32), ("profile", C.c_int32)]
+                ("maxit", C.c_int32), ("x0_is_zero", C.c_int32), ("check_every", C.c_int32), ("profile", C.c_int32),
+                ("mg_nlevels", C.c_int32), ("mg_orders", C.c_int32 * 8), ("mg_smooth_degree", C.c_int32),
+                ("mg_coarse_degree", C.c_int32), ("mg_lmax", C.c_double * 8)]
+
+
+def _mg_fill(o, mg_orders=None, mg_smooth=0, mg_coarse=0, mg_lmax=None):
+    """p-multigrid fields of a PcgOpts (precond == 3)."""
+    orders = list(mg_orders) if mg_orders is not None else []
+    o.mg_nlevels = len(orders)
+    for i, v in enumerate(orders):
+        o.mg_orders[i] = int(v)
+    o.mg_smooth_degree, o.mg_coarse_degree = int(mg_smooth), int(mg_coarse)
+    for i, v in enumerate(mg_lmax or []):
+        o.mg_lmax[i] = float(v)
+    return o
 
 
 class PcgStats(C.Structure):
@@ -186,9 +200,12 @@ class Mesh:
         return dinv_out
 
     def pcg_solve(self, b, x, lam=0.0, tags=0, precond=1, cheb_degree=2, cheb_lmax=0.0, rtol=1e-10, atol=0.0,
-                  maxit=10000, x0_is_zero=True, check_every=0, hist_len=0, profile=False):
-        """Returns dict(iters, status, b_norm, r0_norm, r_norm, lmax_used, hist)."""
+                  maxit=10000, x0_is_zero=True, check_every=0, hist_len=0, profile=False, mg_orders=None, mg_smooth=0,
+                  mg_coarse=0, mg_lmax=None):
+        """Returns dict(iters, status, b_norm, r0_norm, r_norm, lmax_used, hist).  precond: 0 none, 1 Jacobi,
+        2 Chebyshev-Jacobi, 3 p-multigrid V-cycle (mg_orders e.g. [7, 3, 1]; None = default)."""
         o = PcgOpts(lam, tags, precond, cheb_degree, cheb_lmax, rtol, atol, maxit, 1 if x0_is_zero else 0, check_every, 1 if profile else 0)
+        _mg_fill(o, mg_orders, mg_smooth, mg_coarse, mg_lmax)
         hist = np.zeros(max(hist_len, 1))
         st = PcgStats()
         st.hist = hist.ctypes.data_as(C.c_void_p).value if hist_len > 0 else None
@@ -216,6 +233,28 @@ class Mesh:
         rc = self._check(lib().semb_step_solve(self._h, C.c_int(k), items, stats, _stream()))
         return int(rc), [dict(iters=int(st.iters), status=int(st.status), r_norm=st.r_norm, b_norm=st.b_norm,
                               launches=int(st.launches)) for st in stats[:k]]
+
+    def _mg_opts(self, lam, tags, mg_orders, mg_smooth, mg_coarse, mg_lmax):
+        o = PcgOpts(lam, tags, 3, 0, 0.0, 0.0, 0.0, 0, 1, 0, 0)
+        return _mg_fill(o, mg_orders, mg_smooth, mg_coarse, mg_lmax)
+
+    def mg_vcycle(self, r, z, lam=0.0, tags=0, mg_orders=None, mg_smooth=0, mg_coarse=0, mg_lmax=None):
+        """z = one p-multigrid V-cycle applied to r; returns the Chebyshev bounds used per level."""
+        o = self._mg_opts(lam, tags, mg_orders, mg_smooth, mg_coarse, mg_lmax)
+        used = (C.c_double * 8)()
+        self._check(lib().semb_mg_vcycle(self._h, C.byref(o), _dp(r), _dp(z), used, _stream()))
+        nl = len(mg_orders) if mg_orders is not None else 8
+        return [used[i] for i in range(nl) if used[i] > 0.0]
+
+    def mg_level_size(self, level, lam=0.0, tags=0, mg_orders=None):
+        o = self._mg_opts(lam, tags, mg_orders, 0, 0, None)
+        lib().semb_mg_level_size.restype = C.c_int64
+        return int(lib().semb_mg_level_size(self._h, C.byref(o), C.c_int(level)))
+
+    def mg_transfer(self, level, restrict, vin, vout, lam=0.0, tags=0, mg_orders=None):
+        o = self._mg_opts(lam, tags, mg_orders, 0, 0, [1.0] * 8)
+        self._check(lib().semb_mg_transfer(self._h, C.byref(o), C.c_int(level), C.c_int(1 if restrict else 0), _dp(vin),
+                                           _dp(vout), _stream()))
 
     def pcg_solve_host(self, b_host, x_host, lam=0.0, tags=0, precond=1, cheb_degree=2, cheb_lmax=0.0, rtol=1e-10,
                        atol=0.0, maxit=10000, check_every=0):

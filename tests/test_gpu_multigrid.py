@@ -1,0 +1,140 @@
+"""GPU parity of the p-multigrid V-cycle preconditioner (reading R19) against the oracle:
+level sizes and numbering, transfer operators, one V-cycle, and full PCG solves, on the reduced members of the
+box and O-grid families.  The Chebyshev bounds of every level are the oracle's (the estimator is compared
+separately), so both sides apply the same polynomial."""
+import numpy as np
+import pytest
+
+from paper_2501_13240_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("CUDA device required for -m gpu tests (there is no CPU fallback)")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def semb():
+    from paper_2501_13240_b200 import semb as S
+    S.lib()
+    return S
+
+
+def dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def normwise(a, ref):
+    return np.abs(a - ref).max() / max(np.abs(ref).max(), 1e-300)
+
+
+CASES = {
+    "box5":   (lambda xi: I.box_mesh(3, 3, 4, 5, xi(5), deform=0.05, periodic=(True, False, False)), [5, 3, 1], 0.0, 0b10),
+    "ogrid7": (lambda xi: I.config_mesh(2, xi, small=True)[0], [7, 3, 1], 0.0, 0b10),
+    "ogrid9": (lambda xi: I.config_mesh(4, xi, small=True)[0], [9, 5, 3, 1], 0.0, 0b10),
+    "box4_2": (lambda xi: I.box_mesh(2, 3, 2, 4, xi(4), deform=0.05), [4, 1], 10.0, 0),
+}
+
+
+@pytest.fixture(scope="module")
+def cases(torch_cuda, semb, orc, xi_of):
+    cache = {}
+
+    def get(name):
+        if name not in cache:
+            mk, orders, lam, tags = CASES[name]
+            m = mk(xi_of)
+            mg = orc.Multigrid(m.E, m.N, m.x, m.y, m.z, m.face_tag, m.period, lam, tags, orders, k_smooth=2, k_coarse=4)
+            G = semb.Mesh(m.E, m.N, dev(torch_cuda, m.x), dev(torch_cuda, m.y), dev(torch_cuda, m.z), m.face_tag, m.period)
+            cache[name] = (m, mg, G, orders, lam, tags)
+        return cache[name]
+    yield get
+    for c in cache.values():
+        c[2].close()
+
+
+def cont(orc, P, seed):
+    return P.mask * orc.gs(P.gid, P.n_unique, P.invmult * I.uniform(seed, P.n))
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_levels_and_transfer(torch_cuda, cases, orc, name):
+    torch = torch_cuda
+    m, mg, G, orders, lam, tags = cases(name)
+    for l, P in enumerate(mg.levels):
+        assert G.mg_level_size(l, lam, tags, orders) == P.n
+    for l in range(len(orders) - 1):
+        Pf, Pc = mg.levels[l], mg.levels[l + 1]
+        vc = cont(orc, Pc, 40 + l)
+        out = torch.empty(Pf.n, dtype=torch.float64, device="cuda")
+        G.mg_transfer(l, False, dev(torch, vc), out, lam, tags, orders)
+        assert normwise(out.cpu().numpy(), mg.prolong(l, vc)) <= 1e-13
+        rf = cont(orc, Pf, 50 + l)
+        outc = torch.empty(Pc.n, dtype=torch.float64, device="cuda")
+        G.mg_transfer(l, True, dev(torch, rf), outc, lam, tags, orders)
+        assert normwise(outc.cpu().numpy(), mg.restrict(l, rf)) <= 1e-13
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_vcycle(torch_cuda, cases, orc, name):
+    torch = torch_cuda
+    m, mg, G, orders, lam, tags = cases(name)
+    P = mg.levels[0]
+    r = cont(orc, P, 60)
+    z = torch.empty(P.n, dtype=torch.float64, device="cuda")
+    used = G.mg_vcycle(dev(torch, r), z, lam, tags, orders, 2, 4, mg.lmax)
+    assert np.allclose(used, mg.lmax, rtol=0, atol=0)
+    ref = mg.vcycle(r)
+    assert normwise(z.cpu().numpy(), ref) <= 1e-11
+    assert np.all(z.cpu().numpy()[P.mask == 0] == 0)
+    # the library's own estimate of the bounds: same estimator, same start vector.  On a level with a few dozen
+    # unknowns the 10-step Krylov space is nearly exhausted and the last Ritz value is rounding-sensitive (1e-4).
+    used2 = G.mg_vcycle(dev(torch, r), z, lam, tags, orders, 2, 4, None)
+    assert np.allclose(used2, mg.lmax, rtol=1e-3, atol=0)
+    assert np.allclose(used2[0], mg.lmax[0], rtol=1e-6, atol=0)
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_pmg_pcg(torch_cuda, cases, orc, name):
+    torch = torch_cuda
+    m, mg, G, orders, lam, tags = cases(name)
+    P = mg.levels[0]
+    b = P.assemble_rhs(I.divergence_source(m, I.seed_for(2, 70)))
+    ro = mg.pcg(b, rtol=1e-10, hist_len=300)
+    x = torch.zeros(P.n, dtype=torch.float64, device="cuda")
+    rg = G.pcg_solve(dev(torch, b), x, lam=lam, tags=tags, precond=3, rtol=1e-10, hist_len=300, check_every=3,
+                     mg_orders=orders, mg_smooth=2, mg_coarse=4, mg_lmax=mg.lmax)
+    assert ro["status"] == 0 and rg["status"] == 0
+    assert abs(rg["iters"] - ro["iters"]) <= 1, (rg["iters"], ro["iters"])
+    xg = x.cpu().numpy()
+    assert normwise(xg, ro["x"]) <= 1e-8
+    res = b - P.apply_A(xg)
+    assert np.sqrt(P.dot(res, res)) <= 2e-10 * np.sqrt(P.dot(b, b))
+    k = min(10, len(ro["hist"]), len(rg["hist"]))
+    assert np.allclose(rg["hist"][:k], ro["hist"][:k], rtol=1e-8, atol=0)
+    # far fewer iterations than Jacobi on the same system
+    xj = torch.zeros_like(x)
+    rj = G.pcg_solve(dev(torch, b), xj, lam=lam, tags=tags, precond=1, rtol=1e-10)
+    assert rg["iters"] < rj["iters"]
+    assert normwise(xg, xj.cpu().numpy()) <= 1e-7
+
+
+def test_default_hierarchy_and_bad_orders(torch_cuda, cases, orc):
+    torch = torch_cuda
+    m, mg, G, orders, lam, tags = cases("ogrid7")
+    P = mg.levels[0]
+    b = P.assemble_rhs(I.divergence_source(m, 3))
+    x = torch.zeros(P.n, dtype=torch.float64, device="cuda")
+    rg = G.pcg_solve(dev(torch, b), x, lam=lam, tags=tags, precond=3)           # defaults: 7, 3, 1; degrees 2 and 4; estimated bounds
+    assert rg["status"] == 0
+    res = b - P.apply_A(x.cpu().numpy())
+    assert np.sqrt(P.dot(res, res)) <= 2e-10 * np.sqrt(P.dot(b, b))
+    with pytest.raises(Exception):
+        G.pcg_solve(dev(torch, b), x, lam=lam, tags=tags, precond=3, mg_orders=[7, 7, 1])
+    with pytest.raises(Exception):
+        G.pcg_solve(dev(torch, b), x, lam=lam, tags=tags, precond=3, mg_orders=[5, 3, 1])
