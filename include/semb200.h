@@ -148,7 +148,8 @@ typedef struct {
      * strictly decreasing, >= 1), coordinates interpolated from level 0; transfer = Lagrange interpolation of the
      * coarse basis at the fine GLL nodes and its transpose on unique nodes; smoother = Chebyshev-Jacobi of degree
      * mg_smooth_degree before and after the coarse correction, of degree mg_coarse_degree alone on the last level;
-     * mg_lmax[l] <= 0 => estimated (10-step Lanczos x 1.1 from the level's M QQ^T B 1) and cached in the handle. */
+     * mg_lmax[l] <= 0 => estimated (10-step Lanczos x 1.1 from the level's M QQ^T u, u ~ U[-1,1) seeded per level)
+     * and cached in the handle. */
     int32_t  mg_nlevels;      /* 2..8; 0 with precond == 3 => orders N, 3, 1 (N > 3) or N, 1           */
     int32_t  mg_orders[8];
     int32_t  mg_smooth_degree, mg_coarse_degree;     /* <= 0 => 2 and 4                                 */

@@ -238,10 +238,25 @@ def interp3(E, J, v, transpose=False):
     return out
 
 
+MG_LMAX_SEED = 250113240 + 900      # + level: start vector of the per-level lambda_max estimate (R19)
+
+
+def _splitmix_uniform(seed, n):
+    """U[-1,1) per index from the counter-based splitmix64 of the input recipe, restated here."""
+    with np.errstate(over="ignore"):
+        z = np.uint64(seed) + (np.arange(n, dtype=np.uint64) + np.uint64(1)) * np.uint64(0x9E3779B97F4A7C15)
+        z = (z ^ (z >> np.uint64(30))) * np.uint64(0xBF58476D1CE4E5B9)
+        z = (z ^ (z >> np.uint64(27))) * np.uint64(0x94D049BB133111EB)
+        z = z ^ (z >> np.uint64(31))
+    return (z >> np.uint64(11)).astype(np.float64) * (2.0 ** -53) * 2.0 - 1.0
+
+
 class Multigrid:
     """Levels of the p-multigrid preconditioner for the operator (lam, tags) on a mesh: level 0 is order N, level l
     the same elements at order orders[l] with coordinates interpolated from level 0.  lmax[l] = 1.1 x the largest
-    Ritz value of a 10-step Lanczos from the seeded start vector v0_of(level problem) (or given)."""
+    Ritz value of a 10-step Lanczos from the start vector M QQ^T u, u ~ U[-1,1) per local node from splitmix64 with
+    seed MG_LMAX_SEED + l (a ROUGH vector: a smooth one, e.g. M QQ^T B 1, underestimates lambda_max by 20 % on
+    meshes of some thousand elements and the V-cycle loses definiteness), or given."""
 
     def __init__(self, E, N, x, y, z, face_tag, period, lam, tags, orders, k_smooth=2, k_coarse=2, lmax=None, v0_of=None):
         assert orders[0] == N and all(a > b for a, b in zip(orders, orders[1:])) and len(orders) <= 8
@@ -260,8 +275,8 @@ class Multigrid:
             self.J.append(interp_matrix(orders[l + 1], orders[l]))      # [n1_l, n1_{l+1}]
         if lmax is None:
             lmax = []
-            for P in self.levels:
-                v0 = v0_of(P) if v0_of is not None else P.assemble_rhs(np.ones(P.n))
+            for l, P in enumerate(self.levels):
+                v0 = v0_of(P) if v0_of is not None else P.mask * gs(P.gid, P.n_unique, _splitmix_uniform(MG_LMAX_SEED + l, P.n))
                 lmax.append(P.lanczos_lmax(v0, 10))
         self.lmax = [float(v) for v in lmax]
         self._mg = _Mg()

@@ -106,6 +106,18 @@ __global__ void k_mg_fill(int64_t n, double* __restrict__ a, double v)
 {
     for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) a[l] = v;
 }
+// u ~ U[-1,1) per local node from the counter-based splitmix64 of the input recipe (R19)
+__global__ void k_mg_random(int64_t n, unsigned long long seed, double* __restrict__ a)
+{
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
+        unsigned long long z = seed + ((unsigned long long)l + 1ull) * 0x9E3779B97F4A7C15ull;
+        z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+        z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+        z ^= z >> 31;
+        a[l] = (double)(z >> 11) * 0x1.0p-53 * 2.0 - 1.0;
+    }
+}
+#define MG_LMAX_SEED (250113240ull + 900ull)
 static inline unsigned mg_grid(int64_t n) { int64_t b = (n + 1023) / 1024; return (unsigned)(b < 1 ? 1 : (b > 148 * 8 ? 148 * 8 : b)); }
 
 static void mg_free(semb_mesh* h, semb_mg* g)
@@ -215,9 +227,13 @@ int semb_mg_prepare(semb_mesh* h, const semb_pcg_opts* o, semb_mg_ctx* ctx, cuda
         if (o->mg_lmax[l] > 0.0) { ctx->lmax[l] = o->mg_lmax[l]; continue; }
         if (!(est[l] > 0.0)) {
             semb_mesh* L = g->lev[l];
-            double* ones = g->W[l][0]; double* v0 = g->W[l][1];
-            k_mg_fill<<<mg_grid(L->n), 256, 0, s>>>(L->n, ones, 1.0);
-            int rc = semb_assemble_rhs(L, o->dirichlet_tags, ones, v0, (void*)s);
+            // start vector M QQ^T u, u rough (a smooth start vector underestimates lambda_max badly: R19)
+            double* v0 = g->W[l][1];
+            semb_mask_entry ml;
+            k_mg_random<<<mg_grid(L->n), 256, 0, s>>>(L->n, MG_LMAX_SEED + (unsigned long long)l, v0);
+            int rc = semb_gs_launch(L, v0, 1, s);
+            if (!rc) rc = semb_get_mask(L, o->dirichlet_tags, &ml, s);
+            if (!rc) rc = semb_mask_launch(L, ml, v0, 1, s);
             if (!rc) rc = semb_estimate_lmax(L, o->lambda, o->dirichlet_tags, v0, 10, &est[l], (void*)s);
             if (rc) return semb_fail(h, rc, "multigrid: lambda_max estimate on level %d: %s", l, semb_last_error(L));
             changed = true;

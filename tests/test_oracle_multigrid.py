@@ -164,3 +164,18 @@ def test_pmg_pcg_solves_and_beats_chebyshev_jacobi(orc, xi_of):
     bh = mgh.levels[0].assemble_rhs(I.divergence_source(m, 6))
     rh = mgh.pcg(bh)
     assert rh["status"] == 0 and rh["iters"] <= mgh.levels[0].pcg(bh, precond=1)["iters"]
+
+
+def test_estimated_bounds_cover_the_spectrum(orc, xi_of):
+    """The per-level Chebyshev bound (1.1 x Lanczos-10 from the seeded rough vector) must lie above the true
+    lambda_max(D^-1 A) of its level -- below it the smoother amplifies the top modes and the V-cycle is indefinite."""
+    N = 4
+    m = I.box_mesh(3, 3, 3, N, xi_of(N), deform=0.05)
+    mg = _mg(orc, m, 0.0, 0b10, [4, 2, 1])
+    for P, lm in zip(mg.levels, mg.lmax):
+        Ad = dense_matrix(P); fr = to_global(P, P.mask) > 0
+        Af = Ad[np.ix_(fr, fr)]; Dm = np.diag(Af)
+        true = np.linalg.eigvalsh(Af / np.sqrt(np.outer(Dm, Dm)))[-1]
+        assert true <= lm <= 1.35 * true, (true, lm)
+    # the generator restated in the oracle is the recipe's (paper_2501_13240_b200/inputs.py)
+    assert np.array_equal(orc._splitmix_uniform(orc.MG_LMAX_SEED, 1000), I.uniform(orc.MG_LMAX_SEED, 1000))
