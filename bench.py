@@ -165,6 +165,7 @@ def main():
     ap.add_argument("--workload", default="cfg3_box64_deformed_N7", choices=list(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-solve", action="store_true", help="skip the time-to-solution section (full pressure solves)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -237,6 +238,26 @@ def main():
                        "frac_of_8TBs": nbytes * n / (t * 1e-3) / 8e12}
     del u, w
 
+    # ---- time to solution of the pressure solve on the same mesh and right-hand side, rtol 1e-10: Jacobi-PCG (the
+    #      north_star path) and the p-multigrid V-cycle preconditioner of PAPER.md:L102.  Context for
+    #      the per-iteration headline above, not part of it.
+    solve_tts = None
+    if not args.no_solve and world == 1:
+        solve_tts = {}
+        for name, kw in (("pmg_pcg", dict(precond=3, mg_smooth=1, mg_coarse=4)), ("jacobi_pcg", dict(precond=1))):
+            xs = torch.zeros_like(b)
+            if name == "pmg_pcg":
+                G.pcg_solve(b, xs, lam=0.0, tags=0b10, rtol=1e-10, maxit=2, **kw)        # builds the levels, estimates the bounds
+                xs.zero_()
+            s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize(); s0.record()
+            sst = G.pcg_solve(b, xs, lam=0.0, tags=0b10, rtol=1e-10, maxit=20000, **kw)
+            s1.record(); torch.cuda.synchronize()
+            solve_tts[name] = {"iters": sst["iters"], "status": sst["status"], "seconds": s0.elapsed_time(s1) * 1e-3,
+                               "rel_residual": sst["r_norm"] / sst["b_norm"]}
+            del xs
+        solve_tts["speedup"] = solve_tts["jacobi_pcg"]["seconds"] / solve_tts["pmg_pcg"]["seconds"]
+
     # ---- end to end through the C ABI with HOST buffers (pinned): b H2D, K iterations, x D2H
     e2e = None
     if not args.no_e2e:
@@ -267,6 +288,7 @@ def main():
                      "frac_of_measured_peak": B_ITER * n / (ms_step * 1e-3) / 1e9 / peak,
                      "frac_of_8TBs": B_ITER * n / (ms_step * 1e-3) / 8e12},
         "axhelm_sweep": sweep,
+        "time_to_solution": solve_tts,
         "e2e": e2e, "gpu_launches": st["launches"], "clocks": clocks,
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
