@@ -165,6 +165,7 @@ def main():
     ap.add_argument("--workload", default="cfg3_box64_deformed_N7", choices=list(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-export", action="store_true")
     ap.add_argument("--no-solve", action="store_true", help="skip the time-to-solution section (full pressure solves)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -258,6 +259,41 @@ def main():
             del xs
         solve_tts["speedup"] = solve_tts["jacobi_pcg"]["seconds"] / solve_tts["pmg_pcg"]["seconds"]
 
+    # ---- configs[3]: zero-copy export of temperature and velocity magnitude to the in-device min/max/256-bin histogram
+    #      consumer (PAPER.md:L138-159 hand-off; overhead formula of PAPER.md:L375 against the PCG iteration time)
+    export = None
+    if not args.no_export and world == 1:
+        T = torch.from_numpy((1.0 - m.z) + 0.05 * I.uniform(I.seed_for(3, 31), n)).cuda()
+        vel = [torch.from_numpy(3.0 * I.uniform(I.seed_for(3, 32 + c), n)).cuda() for c in range(3)]
+        G.publish_field("temperature", T)
+        for nm, t in zip(("velocity_x", "velocity_y", "velocity_z"), vel):
+            G.publish_field(nm, t)
+        mm = torch.zeros(2, dtype=torch.float64, device="cuda"); hist = torch.zeros(256, dtype=torch.int64, device="cuda")
+
+        def analysis_step(cycle):
+            G.publish_state(cycle, 1e-3 * cycle)                     # refreshes |v| (one kernel: 24 B read + 8 B written per node)
+            dT = G.export_field("temperature"); dV = G.export_field("velocity_magnitude")
+            semb.field_minmax_hist(dT, 256, 0.0, 1.0, mm, hist)      # one pass: 8 B/node
+            semb.field_minmax_hist(dV, 256, 0.0, 0.0, mm, hist)      # range found on the device: two passes, 16 B/node
+            return dT
+        dT = analysis_step(0)
+        torch.cuda.synchronize()
+        free0 = torch.cuda.mem_get_info()[0]
+        x0, x1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 10
+        x0.record()
+        for c in range(reps):
+            analysis_step(c + 1)
+        x1.record(); torch.cuda.synchronize()
+        t_an = x0.elapsed_time(x1) / reps
+        nbytes = (24 + 8 + 8 + 16) * n
+        export = {"ms_per_analysis_step": t_an, "bytes_per_node": 56, "gbs": nbytes / (t_an * 1e-3) / 1e9,
+                  "pointer_identity": bool(dT.ptr == T.data_ptr()), "bytes_allocated": int(free0 - torch.cuda.mem_get_info()[0]),
+                  "overhead_vs_pcg_iteration_pct": {str(nv): 100.0 * ((t_an + nv * ms_step) / (nv * ms_step) - 1.0) for nv in (1, 10, 100)},
+                  "note": "overhead = (t_vis + (n_vis - 1) t_novis) / (n_vis t_novis) - 1 with t_vis = t_novis + analysis step, "
+                          "t_novis = one PCG iteration (PAPER.md:L375)"}
+        del T, vel
+
     # ---- end to end through the C ABI with HOST buffers (pinned): b H2D, K iterations, x D2H
     e2e = None
     if not args.no_e2e:
@@ -289,6 +325,7 @@ def main():
                      "frac_of_8TBs": B_ITER * n / (ms_step * 1e-3) / 8e12},
         "axhelm_sweep": sweep,
         "time_to_solution": solve_tts,
+        "export": export,
         "e2e": e2e, "gpu_launches": st["launches"], "clocks": clocks,
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
