@@ -154,6 +154,9 @@ typedef struct {
     int32_t  mg_orders[8];
     int32_t  mg_smooth_degree, mg_coarse_degree;     /* <= 0 => 2 and 4                                 */
     double   mg_lmax[8];
+    int32_t  mg_smoother_kind; /* 4: Chebyshev polynomial of the FOURTH kind (needs only lmax); else the
+                                  first-kind recurrence on [0.1, 1] lmax of reading R9                          */
+    int32_t  pad_;
 } semb_pcg_opts;
 
 typedef struct {

@@ -448,7 +448,7 @@ typedef struct {
     const double* J;         /* [n1_l][n1_{l+1}] row-major; NULL on the coarsest level */
 } orc_mg_level;
 typedef struct {
-    int32_t nlevels, k_smooth, k_coarse, pad_;
+    int32_t nlevels, k_smooth, k_coarse, kind;      /* kind: 4 = fourth-kind Chebyshev smoother, else first kind (c-10) */
     orc_mg_level lev[8];
 } orc_mg;
 
@@ -512,20 +512,48 @@ void orc_mg_restrict(const orc_mg* mg, int l, const double* rf, double* rc, doub
     for (int64_t q = 0; q < c->n; ++q) rc[q] *= c->mask[q];
 }
 
+/* f-1  Chebyshev-Jacobi smoother of the FOURTH kind ("fourth-kind Chebyshev-accelerated"
+ * smoothers; the recurrence is the published one for polynomial smoothers that need only the upper bound lmax
+ * of spec(D^-1 A), restated):
+ *   z = 0; res = r; d = (4/3)(1/lmax) dinv o res;
+ *   for i = 1..k { z += d; res -= A d; d = ((2i-1)/(2i+3)) d + ((8i+4)/(2i+3)) (1/lmax) dinv o res };  z += d
+ * so that 1 - lam p_k(lam) = W_{k+1}(1 - 2 lam/lmax) / (2k+3), W_n the Chebyshev polynomial of the 4th kind
+ * (pin: tests/test_oracle_multigrid.py).  work: 4 vectors [n].                                        */
+void orc_cheb4_jacobi(const orc_op* op, int k, double lmax, const double* dinv, const double* r,
+                      double* z, double* work)
+{
+    const int64_t n = op->n;
+    double* res = work; double* d = work + n; double* Ad = work + 2 * n; double* tmp = work + 3 * n;
+    for (int64_t l = 0; l < n; ++l) { z[l] = 0.0; res[l] = r[l]; d[l] = dinv[l] * res[l] * (4.0 / (3.0 * lmax)); }
+    for (int i = 1; i <= k; ++i) {
+        for (int64_t l = 0; l < n; ++l) z[l] += d[l];
+        orc_apply_A(op, d, Ad, tmp);
+        for (int64_t l = 0; l < n; ++l) res[l] -= Ad[l];
+        const double c1 = (2.0 * i - 1.0) / (2.0 * i + 3.0), c2 = (8.0 * i + 4.0) / ((2.0 * i + 3.0) * lmax);
+        for (int64_t l = 0; l < n; ++l) d[l] = c1 * d[l] + c2 * (dinv[l] * res[l]);
+    }
+    for (int64_t l = 0; l < n; ++l) z[l] += d[l];
+}
+static void mg_smooth(const orc_mg* mg, const orc_mg_level* L, int k, const double* r, double* z, double* work)
+{
+    if (mg->kind == 4) orc_cheb4_jacobi(&L->op, k, L->lmax, L->dinv, r, z, work);
+    else               orc_cheb_jacobi(&L->op, k, L->lmax, L->dinv, r, z, work);
+}
+
 void orc_mg_vcycle(const orc_mg* mg, int l, const double* r, double* z)
 {
     const orc_mg_level* L = &mg->lev[l];
     const int64_t n = L->op.n;
     double* work = (double*)malloc(sizeof(double) * (size_t)n * 7);
     if (l == mg->nlevels - 1) {
-        orc_cheb_jacobi(&L->op, mg->k_coarse, L->lmax, L->dinv, r, z, work);
+        mg_smooth(mg, L, mg->k_coarse, r, z, work);
         free(work);
         return;
     }
     double* res = work + 4 * n; double* Az = work + 5 * n; double* tmp = work + 6 * n;
     const int64_t nc = mg->lev[l + 1].op.n;
     double* rc = (double*)malloc(sizeof(double) * (size_t)nc * 2); double* ec = rc + nc;
-    orc_cheb_jacobi(&L->op, mg->k_smooth, L->lmax, L->dinv, r, z, work);          /* z = S r            */
+    mg_smooth(mg, L, mg->k_smooth, r, z, work);                                     /* z = S r            */
     orc_apply_A(&L->op, z, Az, tmp);
     for (int64_t q = 0; q < n; ++q) res[q] = r[q] - Az[q];                          /* res = r - A z      */
     orc_mg_restrict(mg, l, res, rc, tmp);
@@ -534,7 +562,7 @@ void orc_mg_vcycle(const orc_mg* mg, int l, const double* r, double* z)
     for (int64_t q = 0; q < n; ++q) z[q] += tmp[q];                                 /* z += P e           */
     orc_apply_A(&L->op, z, Az, tmp);
     for (int64_t q = 0; q < n; ++q) res[q] = r[q] - Az[q];                          /* res = r - A z      */
-    orc_cheb_jacobi(&L->op, mg->k_smooth, L->lmax, L->dinv, res, Az, work);        /* Az = S res         */
+    mg_smooth(mg, L, mg->k_smooth, res, Az, work);                                  /* Az = S res         */
     for (int64_t q = 0; q < n; ++q) z[q] += Az[q];
     free(rc); free(work);
 }

@@ -192,6 +192,12 @@ class Problem:
         lib().orc_cheb_jacobi(C.byref(self._op), C.c_int(k), C.c_double(lmax), _p(self.dinv), _p(_f64(r)), _p(z), _p(work))
         return z
 
+    def cheb4_jacobi(self, k, lmax, r):
+        """fourth-kind Chebyshev-Jacobi smoother (f-1)"""
+        z = np.zeros(self.n); work = np.zeros(4 * self.n)
+        lib().orc_cheb4_jacobi(C.byref(self._op), C.c_int(k), C.c_double(lmax), _p(self.dinv), _p(_f64(r)), _p(z), _p(work))
+        return z
+
     def lanczos_lmax(self, v0, steps=10):
         """largest Ritz value of D^-1/2 A D^-1/2 after `steps` Lanczos steps, times 1.1 (c-10)."""
         a = np.zeros(steps); b = np.zeros(steps)
@@ -217,7 +223,7 @@ class _MgLevel(C.Structure):
 
 
 class _Mg(C.Structure):
-    _fields_ = [("nlevels", C.c_int32), ("k_smooth", C.c_int32), ("k_coarse", C.c_int32), ("pad_", C.c_int32),
+    _fields_ = [("nlevels", C.c_int32), ("k_smooth", C.c_int32), ("k_coarse", C.c_int32), ("kind", C.c_int32),
                 ("lev", _MgLevel * 8)]
 
 
@@ -258,7 +264,8 @@ class Multigrid:
     seed MG_LMAX_SEED + l (a ROUGH vector: a smooth one, e.g. M QQ^T B 1, underestimates lambda_max by 20 % on
     meshes of some thousand elements and the V-cycle loses definiteness), or given."""
 
-    def __init__(self, E, N, x, y, z, face_tag, period, lam, tags, orders, k_smooth=2, k_coarse=2, lmax=None, v0_of=None):
+    def __init__(self, E, N, x, y, z, face_tag, period, lam, tags, orders, k_smooth=2, k_coarse=2, lmax=None, v0_of=None,
+                 kind=1):
         assert orders[0] == N and all(a > b for a, b in zip(orders, orders[1:])) and len(orders) <= 8
         self.orders = list(orders)
         self.k_smooth, self.k_coarse = int(k_smooth), int(k_coarse)
@@ -281,6 +288,7 @@ class Multigrid:
         self.lmax = [float(v) for v in lmax]
         self._mg = _Mg()
         self._mg.nlevels, self._mg.k_smooth, self._mg.k_coarse = len(orders), self.k_smooth, self.k_coarse
+        self.kind = self._mg.kind = int(kind)          # 4 = fourth-kind Chebyshev smoother (orc_cheb4_jacobi), else first kind
         for l, P in enumerate(self.levels):
             self._mg.lev[l].op = P._op
             self._mg.lev[l].dinv = P.dinv.ctypes.data

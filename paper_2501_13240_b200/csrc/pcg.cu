@@ -310,9 +310,19 @@ int semb_operator_run(semb_mesh* h, double lambda, const semb_mask_entry& m, con
 }
 
 typedef semb_cheb_coef cheb_coef;
-semb_cheb_coef semb_cheb_coefficients(int k, double lmax)
+semb_cheb_coef semb_cheb_coefficients(int k, double lmax, int kind)
 {
     cheb_coef c;
+    if (kind == 4) {
+        // fourth-kind Chebyshev smoother: d_0 = (4/3)(1/lmax) dinv o r,
+        // d_i = ((2i-1)/(2i+3)) d_{i-1} + ((8i+4)/(2i+3)) (1/lmax) dinv o res_i
+        c.itheta = 4.0 / (3.0 * lmax);
+        for (int i = 1; i <= k && i <= 16; ++i) {
+            c.c1[i - 1] = (2.0 * i - 1.0) / (2.0 * i + 3.0);
+            c.c2[i - 1] = (8.0 * i + 4.0) / ((2.0 * i + 3.0) * lmax);
+        }
+        return c;
+    }
     const double lmin = 0.1 * lmax, theta = 0.5 * (lmax + lmin), delta = 0.5 * (lmax - lmin), sigma = theta / delta;
     double rho = 1.0 / sigma;
     c.itheta = 1.0 / theta;

@@ -138,3 +138,24 @@ def test_default_hierarchy_and_bad_orders(torch_cuda, cases, orc):
         G.pcg_solve(dev(torch, b), x, lam=lam, tags=tags, precond=3, mg_orders=[7, 7, 1])
     with pytest.raises(Exception):
         G.pcg_solve(dev(torch, b), x, lam=lam, tags=tags, precond=3, mg_orders=[5, 3, 1])
+
+
+def test_fourth_kind_smoother(torch_cuda, cases, orc):
+    """mg_smoother_kind = 4: the fourth-kind Chebyshev polynomial of PAPER.md:L102 in every smoother of the cycle."""
+    torch = torch_cuda
+    m, mg1, G, orders, lam, tags = cases("ogrid7")
+    mg = orc.Multigrid(m.E, m.N, m.x, m.y, m.z, m.face_tag, m.period, lam, tags, orders, k_smooth=2, k_coarse=4,
+                       lmax=mg1.lmax, kind=4)
+    P = mg.levels[0]
+    r = cont(orc, P, 61)
+    z = torch.empty(P.n, dtype=torch.float64, device="cuda")
+    G.mg_vcycle(dev(torch, r), z, lam, tags, orders, 2, 4, mg.lmax, mg_kind=4)
+    assert normwise(z.cpu().numpy(), mg.vcycle(r)) <= 1e-11
+    assert normwise(z.cpu().numpy(), mg1.vcycle(r)) > 1e-3           # and it is a different polynomial than the first kind
+    b = P.assemble_rhs(I.divergence_source(m, I.seed_for(2, 71)))
+    ro = mg.pcg(b, rtol=1e-10)
+    x = torch.zeros(P.n, dtype=torch.float64, device="cuda")
+    rg = G.pcg_solve(dev(torch, b), x, lam=lam, tags=tags, precond=3, rtol=1e-10, mg_orders=orders, mg_smooth=2, mg_coarse=4,
+                     mg_lmax=mg.lmax, mg_kind=4)
+    assert ro["status"] == 0 and rg["status"] == 0 and abs(rg["iters"] - ro["iters"]) <= 1
+    assert normwise(x.cpu().numpy(), ro["x"]) <= 1e-8

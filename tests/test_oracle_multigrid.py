@@ -45,8 +45,9 @@ def test_interp3_is_the_kronecker_product(orc):
     assert np.allclose(outT.reshape(E, -1), w.reshape(E, -1) @ K, rtol=0, atol=1e-13)
 
 
-def _mg(orc, m, lam, tags, orders, k=2, kc=2, lmax=None):
-    return orc.Multigrid(m.E, m.N, m.x, m.y, m.z, m.face_tag, m.period, lam, tags, orders, k_smooth=k, k_coarse=kc, lmax=lmax)
+def _mg(orc, m, lam, tags, orders, k=2, kc=2, lmax=None, kind=1):
+    return orc.Multigrid(m.E, m.N, m.x, m.y, m.z, m.face_tag, m.period, lam, tags, orders, k_smooth=k, k_coarse=kc, lmax=lmax,
+                         kind=kind)
 
 
 def _cont(orc, P, seed):
@@ -179,3 +180,42 @@ def test_estimated_bounds_cover_the_spectrum(orc, xi_of):
         assert true <= lm <= 1.35 * true, (true, lm)
     # the generator restated in the oracle is the recipe's (paper_2501_13240_b200/inputs.py)
     assert np.array_equal(orc._splitmix_uniform(orc.MG_LMAX_SEED, 1000), I.uniform(orc.MG_LMAX_SEED, 1000))
+
+
+@pytest.mark.parametrize("k", [0, 1, 2, 4])
+def test_fourth_kind_chebyshev_closed_form(orc, xi_of, k):
+    """z = p_k(D^-1 A) D^-1 r with 1 - lam p_k(lam) = W_{k+1}(1 - 2 lam/lmax) / (2k + 3), W_n(cos t) = sin((n + 1/2) t) / sin(t/2)
+    the Chebyshev polynomial of the fourth kind -- evaluated here through its trigonometric form on a dense spectrum."""
+    N = 3
+    m = I.ogrid_mesh(2, 2, 2, N, xi_of(N))
+    P = make(orc, m, tags=0b10)
+    A = dense_matrix(P); free = to_global(P, P.mask) > 0
+    Af = A[np.ix_(free, free)]; Dm = np.diag(Af)
+    ev, V = np.linalg.eigh(Af / np.sqrt(np.outer(Dm, Dm)))
+    lmax = 1.07 * ev[-1]
+    t = np.arccos(1.0 - 2.0 * ev / lmax)
+    n = k + 1
+    Wn = np.sin((n + 0.5) * t) / np.sin(0.5 * t)
+    pk = (1.0 - Wn / (2 * n + 1)) / ev
+    rg = np.zeros(P.n_unique); rg[free] = np.random.default_rng(8).standard_normal(free.sum())
+    z = P.cheb4_jacobi(k, lmax, to_local(P, rg))
+    expect = (V * pk) @ (V.T @ (rg[free] / np.sqrt(Dm))) / np.sqrt(Dm)
+    assert np.allclose(to_global(P, z)[free], expect, rtol=0, atol=1e-12 * np.abs(expect).max())
+    assert np.all(pk > 0)                                             # SPD smoother on (0, lmax]
+    assert np.all(np.abs(Wn) <= 2 * n + 1 + 1e-9)
+
+
+def test_fourth_kind_vcycle_converges_comparably(orc, xi_of):
+    m, _ = I.config_mesh(2, xi_of, small=True)
+    b = None; its = {}
+    for kind in (1, 4):
+        mg = _mg(orc, m, 0.0, 0b10, [7, 3, 1], k=2, kc=4, kind=kind)
+        P = mg.levels[0]
+        b = P.assemble_rhs(I.divergence_source(m, 5))
+        r = mg.pcg(b)
+        assert r["status"] == 0
+        res = b - P.apply_A(r["x"])
+        assert np.sqrt(P.dot(res, res)) <= 2e-10 * np.sqrt(P.dot(b, b))
+        its[kind] = r["iters"]
+    # measured: 37 (first kind on [0.1, 1] lmax) vs 40 (fourth kind, which needs no lower bound)
+    assert its[4] <= 1.25 * its[1] and its[1] <= 1.25 * its[4], its
