@@ -166,6 +166,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-export", action="store_true")
+    ap.add_argument("--solve-maxit", type=int, default=20000, help="iteration cap of the time-to-solution solves (profiling runs)")
     ap.add_argument("--no-solve", action="store_true", help="skip the time-to-solution section (full pressure solves)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -252,7 +253,7 @@ def main():
                 xs.zero_()
             s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             torch.cuda.synchronize(); s0.record()
-            sst = G.pcg_solve(b, xs, lam=0.0, tags=0b10, rtol=1e-10, maxit=20000, **kw)
+            sst = G.pcg_solve(b, xs, lam=0.0, tags=0b10, rtol=1e-10, maxit=args.solve_maxit, **kw)
             s1.record(); torch.cuda.synchronize()
             solve_tts[name] = {"iters": sst["iters"], "status": sst["status"], "seconds": s0.elapsed_time(s1) * 1e-3,
                                "rel_residual": sst["r_norm"] / sst["b_norm"]}

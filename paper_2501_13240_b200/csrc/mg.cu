@@ -49,12 +49,18 @@ static void interp_matrix_host(int Nfrom, int Nto, double* J)
 // (transpose != 0: J is [nin][nout]), by three one-dimensional passes through shared memory.
 // scale != NULL: the input is multiplied by scale (restriction: invmult);  accumulate: out += result.
 #define MG_MAXNP (SEMB_MAXN1 * SEMB_MAXN1 * SEMB_MAXN1)
+// NIN, NOUT > 0: compile-time sizes (the pairs the default hierarchies use; index arithmetic and the inner loops
+// unroll); NIN = NOUT = 0: run-time sizes nin, nout.
+template <int NIN, int NOUT>
 __global__ void __launch_bounds__(128)
-k_interp3(int nin, int nout, const double* __restrict__ J, int transpose, const double* __restrict__ in,
+k_interp3(int nin_rt, int nout_rt, const double* __restrict__ J, int transpose, const double* __restrict__ in,
           const double* __restrict__ scale, double* __restrict__ out, int accumulate, const semb_scalars* __restrict__ scal)
 {
-    __shared__ double A[MG_MAXNP], B[MG_MAXNP], Js[SEMB_MAXN1 * SEMB_MAXN1];
+    constexpr int SZ = (NIN > 0) ? ((NIN > NOUT ? NIN : NOUT) * (NIN > NOUT ? NIN : NOUT) * (NIN > NOUT ? NIN : NOUT)) : MG_MAXNP;
+    constexpr int SJ = (NIN > 0) ? NIN * NOUT : SEMB_MAXN1 * SEMB_MAXN1;
+    __shared__ double A[SZ], B[SZ], Js[SJ];
     if (scal && *(volatile const int32_t*)&scal->done) return;
+    const int nin = (NIN > 0) ? NIN : nin_rt, nout = (NOUT > 0) ? NOUT : nout_rt;
     const int64_t e = blockIdx.x;
     const int npi = nin * nin * nin, npo = nout * nout * nout;
     for (int t = threadIdx.x; t < nin * nout; t += blockDim.x) {
@@ -70,6 +76,7 @@ k_interp3(int nin, int nout, const double* __restrict__ J, int transpose, const 
     for (int t = threadIdx.x; t < nin * nin * nout; t += blockDim.x) {
         const int i = t % nout, cb = t / nout;
         double s = 0.0;
+#pragma unroll
         for (int a = 0; a < nin; ++a) s += Js[i * nin + a] * A[cb * nin + a];
         B[t] = s;
     }
@@ -78,6 +85,7 @@ k_interp3(int nin, int nout, const double* __restrict__ J, int transpose, const 
     for (int t = threadIdx.x; t < nin * nout * nout; t += blockDim.x) {
         const int i = t % nout, j = (t / nout) % nout, c = t / (nout * nout);
         double s = 0.0;
+#pragma unroll
         for (int b = 0; b < nin; ++b) s += Js[j * nin + b] * B[(c * nin + b) * nout + i];
         A[t] = s;
     }
@@ -86,22 +94,22 @@ k_interp3(int nin, int nout, const double* __restrict__ J, int transpose, const 
     for (int t = threadIdx.x; t < npo; t += blockDim.x) {
         const int ji = t % (nout * nout), k = t / (nout * nout);
         double s = 0.0;
+#pragma unroll
         for (int c = 0; c < nin; ++c) s += Js[k * nin + c] * A[c * nout * nout + ji];
         if (accumulate) out[e * npo + t] += s; else out[e * npo + t] = s;
     }
 }
 
-__global__ void k_mg_sub(int64_t n, const double* __restrict__ a, const double* __restrict__ b, double* __restrict__ out,
-                         const semb_scalars* __restrict__ scal)
+static void interp3_launch(int64_t E, int nin, int nout, const double* J, int transpose, const double* in, const double* scale,
+                           double* out, int accumulate, const semb_scalars* scal, cudaStream_t s)
 {
-    if (scal && *(volatile const int32_t*)&scal->done) return;
-    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) out[l] = a[l] - b[l];
+#define MG_CASE(A_, B_) if (nin == A_ && nout == B_) { k_interp3<A_, B_><<<(unsigned)E, 128, 0, s>>>(nin, nout, J, transpose, in, scale, out, accumulate, scal); return; }
+    MG_CASE(8, 4) MG_CASE(4, 8) MG_CASE(4, 2) MG_CASE(2, 4) MG_CASE(10, 6) MG_CASE(6, 10) MG_CASE(6, 4) MG_CASE(4, 6)
+    MG_CASE(8, 2) MG_CASE(10, 4) MG_CASE(10, 2) MG_CASE(6, 2) MG_CASE(2, 6) MG_CASE(8, 6) MG_CASE(6, 8)
+#undef MG_CASE
+    k_interp3<0, 0><<<(unsigned)E, 128, 0, s>>>(nin, nout, J, transpose, in, scale, out, accumulate, scal);
 }
-__global__ void k_mg_add(int64_t n, const double* __restrict__ a, double* __restrict__ z, const semb_scalars* __restrict__ scal)
-{
-    if (scal && *(volatile const int32_t*)&scal->done) return;
-    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) z[l] += a[l];
-}
+
 __global__ void k_mg_fill(int64_t n, double* __restrict__ a, double v)
 {
     for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) a[l] = v;
@@ -155,7 +163,7 @@ static int mg_build(semb_mesh* h, int nlevels, const int* orders, semb_mg** out,
             interp_matrix_host(h->N, orders[l], Jh);                                  // [nc1][n1]
             if (cudaMemcpyAsync(Jd, Jh, sizeof(double) * nc1 * h->n1, cudaMemcpyHostToDevice, s) != cudaSuccess) rc = semb_fail(h, SEMB_ECUDA, "multigrid: upload");
             for (int c = 0; c < 3 && !rc; ++c)
-                k_interp3<<<(unsigned)h->E, 128, 0, s>>>(h->n1, nc1, Jd, 0, h->xyz + c * h->n, nullptr, xyz + c * nl, 0, nullptr);
+                interp3_launch(h->E, h->n1, nc1, Jd, 0, h->xyz + c * h->n, nullptr, xyz + c * nl, 0, nullptr, s);
             if (!rc && cudaStreamSynchronize(s) != cudaSuccess) rc = semb_fail(h, SEMB_ECUDA, "multigrid: coordinate interpolation: %s", cudaGetErrorString(cudaGetLastError()));
             if (!rc) {
                 rc = semb_setup(h->E, orders[l], xyz, xyz + nl, xyz + 2 * nl, h->face_tag.data(), h->period,
@@ -264,12 +272,12 @@ int semb_mg_transfer_run(semb_mesh* h, const semb_mg_ctx& ctx, int l, int restri
     semb_mesh* F = g->lev[l]; semb_mesh* C = g->lev[l + 1];
     semb_mask_entry m;
     if (!restrict_) {
-        k_interp3<<<(unsigned)F->E, 128, 0, s>>>(C->n1, F->n1, g->J[l], 0, in, nullptr, out, 0, nullptr);
+        interp3_launch(F->E, C->n1, F->n1, g->J[l], 0, in, nullptr, out, 0, nullptr, s);
         int rc = semb_get_mask(F, ctx.tags, &m, s); if (rc) return rc;
         h->launches += 1;
         return semb_mask_launch(F, m, out, 1, s);
     }
-    k_interp3<<<(unsigned)F->E, 128, 0, s>>>(F->n1, C->n1, g->J[l], 1, in, F->invmult, out, 0, nullptr);
+    interp3_launch(F->E, F->n1, C->n1, g->J[l], 1, in, F->invmult, out, 0, nullptr, s);
     h->launches += 1;
     int rc = semb_gs_launch(C, out, 1, s); if (rc) return rc;
     rc = semb_get_mask(C, ctx.tags, &m, s); if (rc) return rc;
@@ -297,20 +305,17 @@ int semb_mg_vcycle_run(semb_mesh* h, const semb_mg_ctx& ctx, int l, const double
     semb_mask_entry mc;
     rc = semb_get_mask(C, ctx.tags, &mc, s); if (rc) return rc;
     rc = semb_cheb_apply(L, ctx.lambda, m, dinv, ctx.k_smooth, cc, r, z, cres, cd, cAd, scal, false, s); if (rc) return rc;   // z = S r
-    rc = semb_apply_A(L, ctx.lambda, m, z, t1, s); if (rc) return rc;
-    k_mg_sub<<<mg_grid(n), 256, 0, s>>>(n, r, t1, res, scal);                                                                 // res = r - A z
-    k_interp3<<<(unsigned)L->E, 128, 0, s>>>(L->n1, C->n1, g->J[l], 1, res, L->invmult, g->rc[l + 1], 0, scal);               // R res
+    rc = semb_residual_launch(L, ctx.lambda, m, z, r, res, t1, scal, s); if (rc) return rc;                                  // res = r - A z
+    interp3_launch(L->E, L->n1, C->n1, g->J[l], 1, res, L->invmult, g->rc[l + 1], 0, scal, s);               // R res
     rc = semb_gs_launch(C, g->rc[l + 1], 1, s); if (rc) return rc;
     rc = semb_mask_launch(C, mc, g->rc[l + 1], 1, s); if (rc) return rc;
     const int64_t lc0 = C->launches;
     rc = semb_mg_vcycle_run(h, ctx, l + 1, g->rc[l + 1], g->ec[l + 1], scal, s); if (rc) return rc;
     (void)lc0;
-    k_interp3<<<(unsigned)L->E, 128, 0, s>>>(C->n1, L->n1, g->J[l], 0, g->ec[l + 1], nullptr, z, 1, scal);                    // z += P e
-    rc = semb_apply_A(L, ctx.lambda, m, z, t1, s); if (rc) return rc;
-    k_mg_sub<<<mg_grid(n), 256, 0, s>>>(n, r, t1, res, scal);                                                                 // res = r - A z
-    rc = semb_cheb_apply(L, ctx.lambda, m, dinv, ctx.k_smooth, cc, res, t1, cres, cd, cAd, scal, false, s); if (rc) return rc; // t1 = S res
-    k_mg_add<<<mg_grid(n), 256, 0, s>>>(n, t1, z, scal);
-    L->launches += 5;
+    interp3_launch(L->E, C->n1, L->n1, g->J[l], 0, g->ec[l + 1], nullptr, z, 1, scal, s);                    // z += P e
+    rc = semb_residual_launch(L, ctx.lambda, m, z, r, res, t1, scal, s); if (rc) return rc;                                  // res = r - A z
+    rc = semb_cheb_apply(L, ctx.lambda, m, dinv, ctx.k_smooth, cc, res, z, cres, cd, cAd, scal, false, s, true); if (rc) return rc; // z += S res
+    L->launches += 2;
     if (L != h) h->launches += L->launches - l0;
     SEMB_CUDA(h, cudaGetLastError());
     return SEMB_OK;

@@ -201,7 +201,7 @@ template <bool FIRST, bool LAST>
 __global__ void __launch_bounds__(VEC_BLOCK, 3)
 k_cheb_step(int64_t n, const double* __restrict__ Ad, gs_lists L, const double* __restrict__ dinv, double c1, double c2,
             const double* res_in, double* res, double* __restrict__ d, double* __restrict__ z,
-            const double* rpcg, semb_scalars* __restrict__ scal, double* __restrict__ partials)
+            const double* rpcg, semb_scalars* __restrict__ scal, double* __restrict__ partials, int zacc)
 {
     __shared__ double red[32];
     if (scal && STOPPED(scal)) return;
@@ -221,7 +221,7 @@ k_cheb_step(int64_t n, const double* __restrict__ Ad, gs_lists L, const double* 
             own[u] = 0.0; zl[u] = 0.0; rp[u] = 0.0;
             if (l < n) {
                 own[u] = Ad[l]; dl[u] = d[l]; rl[u] = res_in[l]; dv[u] = dinv[l];
-                if (!FIRST) zl[u] = z[l];
+                if (!FIRST || zacc) zl[u] = z[l];          // zacc: the smoother's result is ADDED to the z passed in
                 if (LAST && !FIRST && rpcg) rp[u] = rpcg[l];
             }
         }
@@ -292,6 +292,47 @@ int semb_apply_A(semb_mesh* h, double lambda, const semb_mask_entry& m, const do
 {
     return apply_A(h, lambda, m, v_masked, out, nullptr, s);
 }
+// res = r - M QQ^T A_L z  (z continuous and masked; tmp: scratch [n]): the gather-scatter in gather form as in k_update_r
+__global__ void __launch_bounds__(VEC_BLOCK, 4)
+k_residual(int64_t n, const double* __restrict__ q, gs_lists L, const double* __restrict__ r, double* __restrict__ res,
+           const semb_scalars* __restrict__ scal)
+{
+    if (scal && STOPPED(scal)) return;
+    int32_t cn[GS_U];
+    gs_codes(L, blockIdx.x * (int64_t)(GS_U * VEC_BLOCK) + threadIdx.x, n, cn);
+    GS_CHUNKS(l0, n) {
+        double qa[GS_U], wgt[GS_U], rv[GS_U], own[GS_U], pv[GS_U];
+        int32_t c[GS_U];
+#pragma unroll
+        for (int u = 0; u < GS_U; ++u) c[u] = cn[u];
+        gs_partners(q, c, pv);
+        gs_codes(L, l0 + GS_STEP, n, cn);
+#pragma unroll
+        for (int u = 0; u < GS_U; ++u) {
+            const int64_t l = l0 + u * VEC_BLOCK;
+            own[u] = (l < n) ? q[l] : 0.0;
+            rv[u] = (l < n) ? r[l] : 0.0;
+        }
+        gs_gathered(c, own, pv, qa, wgt);
+#pragma unroll
+        for (int u = 0; u < GS_U; ++u) {
+            const int64_t l = l0 + u * VEC_BLOCK;
+            if (l < n) res[l] = rv[u] - qa[u];
+        }
+    }
+}
+int semb_residual_launch(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* z, const double* r, double* res,
+                         double* tmp, semb_scalars* scal, cudaStream_t s)
+{
+    int rc = semb_axhelm_launch(h, lambda, nullptr, nullptr, z, tmp, 1, nullptr, s); if (rc) return rc;
+    rc = semb_mask_launch(h, m, tmp, 1, s); if (rc) return rc;
+    rc = semb_gs_hi_launch(h, tmp, scal, s); if (rc) return rc;
+    k_residual<<<vec_grid(h->n), VEC_BLOCK, 0, s>>>(h->n, tmp, gs_lists{h->gs_code}, r, res, scal);
+    h->launches += 1;
+    SEMB_CUDA(h, cudaGetLastError());
+    return SEMB_OK;
+}
+
 int semb_dot_rz_launch(semb_mesh* h, const double* r, const double* z, semb_scalars* scal, cudaStream_t s)
 {
     k_dot_rz<<<vec_grid(h->n), VEC_BLOCK, 0, s>>>(h->n, r, z, h->invmult, scal, h->partials);
@@ -338,9 +379,11 @@ semb_cheb_coef semb_cheb_coefficients(int k, double lmax, int kind)
 // Per application (k >= 1): axhelm with the first d formed in its prologue (80 B/node), then per step k_mask,
 // k_gs_hi, k_cheb_step (first 60, middle 68, last 60 B/node) and, between steps, a plain axhelm (64).
 int semb_cheb_apply(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* dinv, int k, const cheb_coef& c,
-                      const double* r, double* z, double* res, double* d, double* Ad, semb_scalars* scal, bool in_pcg, cudaStream_t s)
+                      const double* r, double* z, double* res, double* d, double* Ad, semb_scalars* scal, bool in_pcg, cudaStream_t s,
+                      bool zacc)
 {
     const int64_t n = h->n; const unsigned G = vec_grid(n);
+    if (zacc && k == 0) return semb_fail(h, SEMB_EINVAL, "cheb_apply: accumulation needs k >= 1");
     if (k == 0) {
         k_cheb_init<<<G, VEC_BLOCK, 0, s>>>(n, r, dinv, c.itheta, res, d, z, 1, scal);
         h->launches += 1;
@@ -357,7 +400,7 @@ int semb_cheb_apply(semb_mesh* h, double lambda, const semb_mask_entry& m, const
         rc = semb_gs_hi_launch(h, Ad, scal, s); if (rc) return rc;      // edges and corners; faces in k_cheb_step
         const bool first = (it == 0), last = (it == k - 1);
         const double* rin = first ? r : res;
-#define SEMB_CHEB_STEP(F, La) k_cheb_step<F, La><<<G, VEC_BLOCK, 0, s>>>(n, Ad, L, dinv, c.c1[it], c.c2[it], rin, res, d, z, rp, scal, h->partials)
+#define SEMB_CHEB_STEP(F, La) k_cheb_step<F, La><<<G, VEC_BLOCK, 0, s>>>(n, Ad, L, dinv, c.c1[it], c.c2[it], rin, res, d, z, rp, scal, h->partials, zacc ? 1 : 0)
         if (first && last) SEMB_CHEB_STEP(true, true);
         else if (first)    SEMB_CHEB_STEP(true, false);
         else if (last)     SEMB_CHEB_STEP(false, true);

@@ -132,7 +132,11 @@ struct semb_cheb_coef { double itheta; double c1[16], c2[16]; };
 semb_cheb_coef semb_cheb_coefficients(int k, double lmax, int kind = 1);   // kind 4: fourth-kind polynomial (lmax only)
 // z = Cheb_k(r) on h;  res, d, Ad: work vectors [n].  in_pcg: also leave rho = <r,z> and beta in scal.
 int semb_cheb_apply(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* dinv, int k, const semb_cheb_coef& c,
-                    const double* r, double* z, double* res, double* d, double* Ad, semb_scalars* scal, bool in_pcg, cudaStream_t s);
+                    const double* r, double* z, double* res, double* d, double* Ad, semb_scalars* scal, bool in_pcg, cudaStream_t s,
+                    bool zacc = false);       // zacc: z += Cheb_k(r) instead of z = Cheb_k(r) (k >= 1)
+// res = r - M QQ^T A_L z  (z continuous and masked; tmp: scratch [n])
+int semb_residual_launch(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* z, const double* r, double* res,
+                         double* tmp, semb_scalars* scal, cudaStream_t s);
 // out = M QQ^T A_L v  (v continuous and masked)
 int semb_apply_A(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* v_masked, double* out, cudaStream_t s);
 int semb_dot_rz_launch(semb_mesh* h, const double* r, const double* z, semb_scalars* scal, cudaStream_t s);
