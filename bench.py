@@ -246,7 +246,7 @@ def main():
     solve_tts = None
     if not args.no_solve and world == 1:
         solve_tts = {}
-        for name, kw in (("pmg_pcg", dict(precond=3, mg_smooth=1, mg_coarse=4)), ("jacobi_pcg", dict(precond=1))):
+        for name, kw in (("pmg_pcg", dict(precond=3, mg_smooth=1, mg_coarse=64, mg_coarse_frac=0.003)), ("jacobi_pcg", dict(precond=1))):
             xs = torch.zeros_like(b)
             if name == "pmg_pcg":
                 G.pcg_solve(b, xs, lam=0.0, tags=0b10, rtol=1e-10, maxit=2, **kw)        # builds the levels, estimates the bounds

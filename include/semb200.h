@@ -157,6 +157,8 @@ typedef struct {
     int32_t  mg_smoother_kind; /* 4: Chebyshev polynomial of the FOURTH kind (needs only lmax); else the
                                   first-kind recurrence on [0.1, 1] lmax of reading R9                          */
     int32_t  pad_;
+    double   mg_coarse_lmin_frac; /* first-kind smoother of the LAST level runs on [frac, 1] lmax; <= 0 => 0.1.  A smaller
+                                     fraction with a higher mg_coarse_degree (<= 64) makes it act as a coarse solver      */
 } semb_pcg_opts;
 
 typedef struct {

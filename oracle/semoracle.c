@@ -410,12 +410,21 @@ void orc_assemble_rhs(const orc_op* op, const double* f, double* b)
 /* c-10  Chebyshev-Jacobi(k) preconditioner, 1st-kind recurrence on [0.1 lmax, lmax]
  * (PAPER.md:L102 names Chebyshev acceleration; bounds and kind: DESIGN.md reading R9).
  * work: 4 vectors [n].                                                                    */
+void orc_cheb_jacobi_frac(const orc_op* op, int k, double lmax, double lmin_frac, const double* dinv, const double* r,
+                          double* z, double* work);
 void orc_cheb_jacobi(const orc_op* op, int k, double lmax, const double* dinv, const double* r,
                      double* z, double* work)
 {
+    orc_cheb_jacobi_frac(op, k, lmax, 0.1, dinv, r, z, work);
+}
+/* the same recurrence on [lmin_frac, 1] lmax (f-1: the last multigrid level may use a smaller fraction and a higher
+ * degree, which turns the smoother into an approximate coarse solver) */
+void orc_cheb_jacobi_frac(const orc_op* op, int k, double lmax, double lmin_frac, const double* dinv, const double* r,
+                          double* z, double* work)
+{
     const int64_t n = op->n;
     double* res = work; double* d = work + n; double* Ad = work + 2 * n; double* tmp = work + 3 * n;
-    const double lmin = 0.1 * lmax, theta = 0.5 * (lmax + lmin), delta = 0.5 * (lmax - lmin);
+    const double lmin = lmin_frac * lmax, theta = 0.5 * (lmax + lmin), delta = 0.5 * (lmax - lmin);
     const double sigma = theta / delta;
     double rho = 1.0 / sigma;
     for (int64_t l = 0; l < n; ++l) { z[l] = 0.0; res[l] = r[l]; d[l] = dinv[l] * res[l] / theta; }
@@ -449,6 +458,7 @@ typedef struct {
 } orc_mg_level;
 typedef struct {
     int32_t nlevels, k_smooth, k_coarse, kind;      /* kind: 4 = fourth-kind Chebyshev smoother, else first kind (c-10) */
+    double coarse_frac;                             /* first kind, last level: interval [coarse_frac, 1] lmax (0.1 = c-10) */
     orc_mg_level lev[8];
 } orc_mg;
 
@@ -536,8 +546,9 @@ void orc_cheb4_jacobi(const orc_op* op, int k, double lmax, const double* dinv, 
 }
 static void mg_smooth(const orc_mg* mg, const orc_mg_level* L, int k, const double* r, double* z, double* work)
 {
+    const int last = (L == &mg->lev[mg->nlevels - 1]);
     if (mg->kind == 4) orc_cheb4_jacobi(&L->op, k, L->lmax, L->dinv, r, z, work);
-    else               orc_cheb_jacobi(&L->op, k, L->lmax, L->dinv, r, z, work);
+    else               orc_cheb_jacobi_frac(&L->op, k, L->lmax, last ? mg->coarse_frac : 0.1, L->dinv, r, z, work);
 }
 
 void orc_mg_vcycle(const orc_mg* mg, int l, const double* r, double* z)

@@ -223,7 +223,7 @@ class _MgLevel(C.Structure):
 
 
 class _Mg(C.Structure):
-    _fields_ = [("nlevels", C.c_int32), ("k_smooth", C.c_int32), ("k_coarse", C.c_int32), ("kind", C.c_int32),
+    _fields_ = [("nlevels", C.c_int32), ("k_smooth", C.c_int32), ("k_coarse", C.c_int32), ("kind", C.c_int32), ("coarse_frac", C.c_double),
                 ("lev", _MgLevel * 8)]
 
 
@@ -265,7 +265,7 @@ class Multigrid:
     meshes of some thousand elements and the V-cycle loses definiteness), or given."""
 
     def __init__(self, E, N, x, y, z, face_tag, period, lam, tags, orders, k_smooth=2, k_coarse=2, lmax=None, v0_of=None,
-                 kind=1):
+                 kind=1, coarse_frac=0.1):
         assert orders[0] == N and all(a > b for a, b in zip(orders, orders[1:])) and len(orders) <= 8
         self.orders = list(orders)
         self.k_smooth, self.k_coarse = int(k_smooth), int(k_coarse)
@@ -288,6 +288,7 @@ class Multigrid:
         self.lmax = [float(v) for v in lmax]
         self._mg = _Mg()
         self._mg.nlevels, self._mg.k_smooth, self._mg.k_coarse = len(orders), self.k_smooth, self.k_coarse
+        self.coarse_frac = self._mg.coarse_frac = float(coarse_frac)   # last level: first-kind interval [coarse_frac, 1] lmax
         self.kind = self._mg.kind = int(kind)          # 4 = fourth-kind Chebyshev smoother (orc_cheb4_jacobi), else first kind
         for l, P in enumerate(self.levels):
             self._mg.lev[l].op = P._op

@@ -225,7 +225,8 @@ int semb_mg_prepare(semb_mesh* h, const semb_pcg_opts* o, semb_mg_ctx* ctx, cuda
     ctx->k_smooth = o->mg_smooth_degree > 0 ? o->mg_smooth_degree : 2;
     ctx->k_coarse = o->mg_coarse_degree > 0 ? o->mg_coarse_degree : 4;
     ctx->kind = (o->mg_smoother_kind == 4) ? 4 : 1;
-    if (ctx->k_smooth > 16 || ctx->k_coarse > 16) return semb_fail(h, SEMB_EINVAL, "multigrid: smoother degree > 16");
+    if (ctx->k_smooth > SEMB_MAX_CHEB || ctx->k_coarse > SEMB_MAX_CHEB) return semb_fail(h, SEMB_EINVAL, "multigrid: smoother degree > %d", SEMB_MAX_CHEB);
+    ctx->coarse_frac = (o->mg_coarse_lmin_frac > 0.0 && o->mg_coarse_lmin_frac < 1.0) ? o->mg_coarse_lmin_frac : 0.1;
     // Chebyshev bounds per level: given, cached, or estimated (10-step Lanczos x 1.1 from M QQ^T B 1)
     const std::pair<uint32_t, double> key(o->dirichlet_tags, o->lambda);
     auto it = g->lmax_cache.find(key);
@@ -296,7 +297,7 @@ int semb_mg_vcycle_run(semb_mesh* h, const semb_mg_ctx& ctx, int l, const double
     double *cres = g->W[l][0], *cd = g->W[l][1], *cAd = g->W[l][2], *res = g->W[l][3], *t1 = g->W[l][4];
     const int64_t l0 = L->launches;
     if (l == g->nlevels - 1) {
-        rc = semb_cheb_apply(L, ctx.lambda, m, dinv, ctx.k_coarse, semb_cheb_coefficients(ctx.k_coarse, ctx.lmax[l], ctx.kind), r, z, cres, cd, cAd, scal, false, s);
+        rc = semb_cheb_apply(L, ctx.lambda, m, dinv, ctx.k_coarse, semb_cheb_coefficients(ctx.k_coarse, ctx.lmax[l], ctx.kind, ctx.coarse_frac), r, z, cres, cd, cAd, scal, false, s);
         if (L != h) { h->launches += L->launches - l0; }
         return rc;
     }

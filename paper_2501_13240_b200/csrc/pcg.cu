@@ -351,23 +351,23 @@ int semb_operator_run(semb_mesh* h, double lambda, const semb_mask_entry& m, con
 }
 
 typedef semb_cheb_coef cheb_coef;
-semb_cheb_coef semb_cheb_coefficients(int k, double lmax, int kind)
+semb_cheb_coef semb_cheb_coefficients(int k, double lmax, int kind, double lmin_frac)
 {
     cheb_coef c;
     if (kind == 4) {
         // fourth-kind Chebyshev smoother: d_0 = (4/3)(1/lmax) dinv o r,
         // d_i = ((2i-1)/(2i+3)) d_{i-1} + ((8i+4)/(2i+3)) (1/lmax) dinv o res_i
         c.itheta = 4.0 / (3.0 * lmax);
-        for (int i = 1; i <= k && i <= 16; ++i) {
+        for (int i = 1; i <= k && i <= SEMB_MAX_CHEB; ++i) {
             c.c1[i - 1] = (2.0 * i - 1.0) / (2.0 * i + 3.0);
             c.c2[i - 1] = (8.0 * i + 4.0) / ((2.0 * i + 3.0) * lmax);
         }
         return c;
     }
-    const double lmin = 0.1 * lmax, theta = 0.5 * (lmax + lmin), delta = 0.5 * (lmax - lmin), sigma = theta / delta;
+    const double lmin = ((lmin_frac > 0.0 && lmin_frac < 1.0) ? lmin_frac : 0.1) * lmax, theta = 0.5 * (lmax + lmin), delta = 0.5 * (lmax - lmin), sigma = theta / delta;
     double rho = 1.0 / sigma;
     c.itheta = 1.0 / theta;
-    for (int it = 0; it < k && it < 16; ++it) {
+    for (int it = 0; it < k && it < SEMB_MAX_CHEB; ++it) {
         const double rho1 = 1.0 / (2.0 * sigma - rho);
         c.c1[it] = rho1 * rho; c.c2[it] = 2.0 * rho1 / delta;
         rho = rho1;
@@ -414,7 +414,7 @@ int semb_cheb_apply(semb_mesh* h, double lambda, const semb_mask_entry& m, const
 
 int semb_cheb_run(semb_mesh* h, double lambda, uint32_t tags, int k, double lmax, const double* r, double* z, cudaStream_t s)
 {
-    if (k < 0 || k > 16 || !(lmax > 0.0)) return semb_fail(h, SEMB_EINVAL, "cheb_jacobi: k=%d lmax=%g", k, lmax);
+    if (k < 0 || k > SEMB_MAX_CHEB || !(lmax > 0.0)) return semb_fail(h, SEMB_EINVAL, "cheb_jacobi: k=%d lmax=%g", k, lmax);
     semb_mask_entry m; double* dinv;
     int rc = semb_get_mask(h, tags, &m, s); if (rc) return rc;
     rc = semb_get_dinv(h, lambda, tags, &dinv, s); if (rc) return rc;
@@ -494,7 +494,7 @@ int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* 
 {
     const int64_t n = h->n; const unsigned G = vec_grid(n);
     const int64_t launches0 = h->launches;
-    if (o->precond < 0 || o->precond > 3 || o->maxit < 0 || (o->precond == 2 && (o->cheb_degree < 0 || o->cheb_degree > 16)))
+    if (o->precond < 0 || o->precond > 3 || o->maxit < 0 || (o->precond == 2 && (o->cheb_degree < 0 || o->cheb_degree > SEMB_MAX_CHEB)))
         return semb_fail(h, SEMB_EINVAL, "pcg: precond=%d cheb_degree=%d maxit=%d", o->precond, o->cheb_degree, o->maxit);
     semb_mask_entry m; double* dinv = nullptr;
     int rc = semb_get_mask(h, o->dirichlet_tags, &m, s); if (rc) return rc;

@@ -128,8 +128,10 @@ int semb_cheb_run(semb_mesh* h, double lambda, uint32_t tags, int k, double lmax
 int semb_operator_run(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* v, double* out,
                       cudaStream_t s);
 int semb_ensure_work(semb_mesh* h, int64_t vecs);
-struct semb_cheb_coef { double itheta; double c1[16], c2[16]; };
-semb_cheb_coef semb_cheb_coefficients(int k, double lmax, int kind = 1);   // kind 4: fourth-kind polynomial (lmax only)
+#define SEMB_MAX_CHEB 64
+struct semb_cheb_coef { double itheta; double c1[SEMB_MAX_CHEB], c2[SEMB_MAX_CHEB]; };
+// kind 4: fourth-kind polynomial (lmax only); else first kind on [lmin_frac, 1] lmax (lmin_frac <= 0 => 0.1, reading R9)
+semb_cheb_coef semb_cheb_coefficients(int k, double lmax, int kind = 1, double lmin_frac = 0.1);
 // z = Cheb_k(r) on h;  res, d, Ad: work vectors [n].  in_pcg: also leave rho = <r,z> and beta in scal.
 int semb_cheb_apply(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* dinv, int k, const semb_cheb_coef& c,
                     const double* r, double* z, double* res, double* d, double* Ad, semb_scalars* scal, bool in_pcg, cudaStream_t s,
@@ -142,7 +144,7 @@ int semb_apply_A(semb_mesh* h, double lambda, const semb_mask_entry& m, const do
 int semb_dot_rz_launch(semb_mesh* h, const double* r, const double* z, semb_scalars* scal, cudaStream_t s);
 
 // ---- mg.cu: p-multigrid V-cycle
-struct semb_mg_ctx { semb_mg* mg; double lambda; uint32_t tags; int k_smooth, k_coarse, kind; double lmax[8]; };
+struct semb_mg_ctx { semb_mg* mg; double lambda; uint32_t tags; int k_smooth, k_coarse, kind; double coarse_frac; double lmax[8]; };
 int semb_mg_prepare(semb_mesh* h, const semb_pcg_opts* o, semb_mg_ctx* ctx, cudaStream_t s);
 int semb_mg_vcycle_run(semb_mesh* h, const semb_mg_ctx& ctx, int level, const double* r, double* z, semb_scalars* scal, cudaStream_t s);
 int semb_mg_transfer_run(semb_mesh* h, const semb_mg_ctx& ctx, int level, int restrict_, const double* in, double* out, cudaStream_t s);

@@ -159,3 +159,25 @@ def test_fourth_kind_smoother(torch_cuda, cases, orc):
                      mg_lmax=mg.lmax, mg_kind=4)
     assert ro["status"] == 0 and rg["status"] == 0 and abs(rg["iters"] - ro["iters"]) <= 1
     assert normwise(x.cpu().numpy(), ro["x"]) <= 1e-8
+
+
+def test_coarse_level_as_chebyshev_solver(torch_cuda, cases, orc):
+    """mg_coarse_lmin_frac / a high mg_coarse_degree: the last level's first-kind polynomial on [frac, 1] lmax."""
+    torch = torch_cuda
+    m, mg1, G, orders, lam, tags = cases("box5")
+    mg = orc.Multigrid(m.E, m.N, m.x, m.y, m.z, m.face_tag, m.period, lam, tags, orders, k_smooth=1, k_coarse=24,
+                       lmax=mg1.lmax, coarse_frac=0.01)
+    P = mg.levels[0]
+    r = cont(orc, P, 62)
+    z = torch.empty(P.n, dtype=torch.float64, device="cuda")
+    G.mg_vcycle(dev(torch, r), z, lam, tags, orders, 1, 24, mg.lmax, mg_coarse_frac=0.01)
+    assert normwise(z.cpu().numpy(), mg.vcycle(r)) <= 1e-11
+    b = P.assemble_rhs(I.divergence_source(m, I.seed_for(2, 72)))
+    ro = mg.pcg(b, rtol=1e-10)
+    x = torch.zeros(P.n, dtype=torch.float64, device="cuda")
+    rg = G.pcg_solve(dev(torch, b), x, lam=lam, tags=tags, precond=3, rtol=1e-10, mg_orders=orders, mg_smooth=1, mg_coarse=24,
+                     mg_lmax=mg.lmax, mg_coarse_frac=0.01)
+    assert ro["status"] == 0 and rg["status"] == 0 and abs(rg["iters"] - ro["iters"]) <= 1
+    assert normwise(x.cpu().numpy(), ro["x"]) <= 1e-8
+    with pytest.raises(Exception):
+        G.pcg_solve(dev(torch, b), x, lam=lam, tags=tags, precond=3, mg_orders=orders, mg_coarse=65)

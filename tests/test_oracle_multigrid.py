@@ -45,9 +45,9 @@ def test_interp3_is_the_kronecker_product(orc):
     assert np.allclose(outT.reshape(E, -1), w.reshape(E, -1) @ K, rtol=0, atol=1e-13)
 
 
-def _mg(orc, m, lam, tags, orders, k=2, kc=2, lmax=None, kind=1):
+def _mg(orc, m, lam, tags, orders, k=2, kc=2, lmax=None, kind=1, frac=0.1):
     return orc.Multigrid(m.E, m.N, m.x, m.y, m.z, m.face_tag, m.period, lam, tags, orders, k_smooth=k, k_coarse=kc, lmax=lmax,
-                         kind=kind)
+                         kind=kind, coarse_frac=frac)
 
 
 def _cont(orc, P, seed):
@@ -94,17 +94,17 @@ def _global_prolongation(orc, Pf, Pc, Nf, Nc):
     return Pg
 
 
-def _cheb_dense(Af, k, lmax):
+def _cheb_dense(Af, k, lmax, frac=0.1):
     Dm = np.diag(Af)
     ev, V = np.linalg.eigh(Af / np.sqrt(np.outer(Dm, Dm)))
-    lmin = 0.1 * lmax; theta = 0.5 * (lmax + lmin); delta = 0.5 * (lmax - lmin); sigma = theta / delta
+    lmin = frac * lmax; theta = 0.5 * (lmax + lmin); delta = 0.5 * (lmax - lmin); sigma = theta / delta
     Tk1 = Ch.Chebyshev.basis(k + 1)
     pk = (1.0 - Tk1((theta - ev) / delta) / Tk1(sigma)) / ev
     return ((V * pk) @ V.T) / np.sqrt(np.outer(Dm, Dm))
 
 
-@pytest.mark.parametrize("lam,tags", [(0.0, 0b10), (50.0, 0)])
-def test_vcycle_equals_dense_composition_and_is_spd(orc, xi_of, lam, tags):
+@pytest.mark.parametrize("lam,tags,kc,frac", [(0.0, 0b10, 3, 0.1), (50.0, 0, 3, 0.1), (0.0, 0b10, 7, 0.02)])
+def test_vcycle_equals_dense_composition_and_is_spd(orc, xi_of, lam, tags, kc, frac):
     N = 4
     m = I.box_mesh(2, 2, 2, N, xi_of(N), deform=0.05)
     orders = [4, 2, 1]
@@ -115,9 +115,9 @@ def test_vcycle_equals_dense_composition_and_is_spd(orc, xi_of, lam, tags):
         A.append(Ad[np.ix_(fr, fr)]); free.append(fr)
         Dm = np.diag(A[-1])
         lmax.append(1.1 * np.linalg.eigvalsh(A[-1] / np.sqrt(np.outer(Dm, Dm)))[-1])
-    k, kc = 2, 3
-    mg = _mg(orc, m, lam, tags, orders, k=k, kc=kc, lmax=lmax)
-    B = _cheb_dense(A[2], kc, lmax[2])
+    k = 2
+    mg = _mg(orc, m, lam, tags, orders, k=k, kc=kc, lmax=lmax, frac=frac)
+    B = _cheb_dense(A[2], kc, lmax[2], frac)                       # last level: interval [frac, 1] lmax
     for l in (1, 0):
         Pg = _global_prolongation(orc, mg.levels[l], mg.levels[l + 1], orders[l], orders[l + 1])[np.ix_(free[l], free[l + 1])]
         S = _cheb_dense(A[l], k, lmax[l]); Id = np.eye(A[l].shape[0])
