@@ -152,12 +152,12 @@ typedef struct {
      * and cached in the handle. */
     int32_t  mg_nlevels;      /* 2..8; 0 with precond == 3 => orders N, 3, 1 (N > 3) or N, 1           */
     int32_t  mg_orders[8];
-    int32_t  mg_smooth_degree, mg_coarse_degree;     /* <= 0 => 2 and 4                                 */
+    int32_t  mg_smooth_degree, mg_coarse_degree;     /* <= 0 => 1 and 32 (measured best compromise) */
     double   mg_lmax[8];
     int32_t  mg_smoother_kind; /* 4: Chebyshev polynomial of the FOURTH kind (needs only lmax); else the
                                   first-kind recurrence on [0.1, 1] lmax of reading R9                          */
     int32_t  pad_;
-    double   mg_coarse_lmin_frac; /* first-kind smoother of the LAST level runs on [frac, 1] lmax; <= 0 => 0.1.  A smaller
+    double   mg_coarse_lmin_frac; /* first-kind smoother of the LAST level runs on [frac, 1] lmax; <= 0 => 0.01.  A smaller
                                      fraction with a higher mg_coarse_degree (<= 64) makes it act as a coarse solver      */
 } semb_pcg_opts;
 

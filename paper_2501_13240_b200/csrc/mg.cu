@@ -222,11 +222,11 @@ int semb_mg_prepare(semb_mesh* h, const semb_pcg_opts* o, semb_mg_ctx* ctx, cuda
     }
     if (!g) { int rc = mg_build(h, nlev, orders, &g, s); if (rc) return rc; }
     ctx->mg = g; ctx->lambda = o->lambda; ctx->tags = o->dirichlet_tags;
-    ctx->k_smooth = o->mg_smooth_degree > 0 ? o->mg_smooth_degree : 2;
-    ctx->k_coarse = o->mg_coarse_degree > 0 ? o->mg_coarse_degree : 4;
+    ctx->k_smooth = o->mg_smooth_degree > 0 ? o->mg_smooth_degree : 1;
+    ctx->k_coarse = o->mg_coarse_degree > 0 ? o->mg_coarse_degree : 32;
     ctx->kind = (o->mg_smoother_kind == 4) ? 4 : 1;
     if (ctx->k_smooth > SEMB_MAX_CHEB || ctx->k_coarse > SEMB_MAX_CHEB) return semb_fail(h, SEMB_EINVAL, "multigrid: smoother degree > %d", SEMB_MAX_CHEB);
-    ctx->coarse_frac = (o->mg_coarse_lmin_frac > 0.0 && o->mg_coarse_lmin_frac < 1.0) ? o->mg_coarse_lmin_frac : 0.1;
+    ctx->coarse_frac = (o->mg_coarse_lmin_frac > 0.0 && o->mg_coarse_lmin_frac < 1.0) ? o->mg_coarse_lmin_frac : 0.01;
     // Chebyshev bounds per level: given, cached, or estimated (10-step Lanczos x 1.1 from M QQ^T B 1)
     const std::pair<uint32_t, double> key(o->dirichlet_tags, o->lambda);
     auto it = g->lmax_cache.find(key);

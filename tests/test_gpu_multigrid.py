@@ -87,14 +87,14 @@ def test_vcycle(torch_cuda, cases, orc, name):
     P = mg.levels[0]
     r = cont(orc, P, 60)
     z = torch.empty(P.n, dtype=torch.float64, device="cuda")
-    used = G.mg_vcycle(dev(torch, r), z, lam, tags, orders, 2, 4, mg.lmax)
+    used = G.mg_vcycle(dev(torch, r), z, lam, tags, orders, 2, 4, mg.lmax, mg_coarse_frac=0.1)
     assert np.allclose(used, mg.lmax, rtol=0, atol=0)
     ref = mg.vcycle(r)
     assert normwise(z.cpu().numpy(), ref) <= 1e-11
     assert np.all(z.cpu().numpy()[P.mask == 0] == 0)
     # the library's own estimate of the bounds: same estimator, same start vector.  On a level with a few dozen
     # unknowns the 10-step Krylov space is nearly exhausted and the last Ritz value is rounding-sensitive (1e-4).
-    used2 = G.mg_vcycle(dev(torch, r), z, lam, tags, orders, 2, 4, None)
+    used2 = G.mg_vcycle(dev(torch, r), z, lam, tags, orders, 2, 4, None, mg_coarse_frac=0.1)
     assert np.allclose(used2, mg.lmax, rtol=1e-3, atol=0)
     assert np.allclose(used2[0], mg.lmax[0], rtol=1e-6, atol=0)
 
@@ -108,7 +108,7 @@ def test_pmg_pcg(torch_cuda, cases, orc, name):
     ro = mg.pcg(b, rtol=1e-10, hist_len=300)
     x = torch.zeros(P.n, dtype=torch.float64, device="cuda")
     rg = G.pcg_solve(dev(torch, b), x, lam=lam, tags=tags, precond=3, rtol=1e-10, hist_len=300, check_every=3,
-                     mg_orders=orders, mg_smooth=2, mg_coarse=4, mg_lmax=mg.lmax)
+                     mg_orders=orders, mg_smooth=2, mg_coarse=4, mg_lmax=mg.lmax, mg_coarse_frac=0.1)
     assert ro["status"] == 0 and rg["status"] == 0
     assert abs(rg["iters"] - ro["iters"]) <= 1, (rg["iters"], ro["iters"])
     xg = x.cpu().numpy()
@@ -130,7 +130,7 @@ def test_default_hierarchy_and_bad_orders(torch_cuda, cases, orc):
     P = mg.levels[0]
     b = P.assemble_rhs(I.divergence_source(m, 3))
     x = torch.zeros(P.n, dtype=torch.float64, device="cuda")
-    rg = G.pcg_solve(dev(torch, b), x, lam=lam, tags=tags, precond=3)           # defaults: 7, 3, 1; degrees 2 and 4; estimated bounds
+    rg = G.pcg_solve(dev(torch, b), x, lam=lam, tags=tags, precond=3)           # defaults: 7, 3, 1; degrees 1 and 32 on [0.01, 1]; estimated bounds
     assert rg["status"] == 0
     res = b - P.apply_A(x.cpu().numpy())
     assert np.sqrt(P.dot(res, res)) <= 2e-10 * np.sqrt(P.dot(b, b))
@@ -149,14 +149,14 @@ def test_fourth_kind_smoother(torch_cuda, cases, orc):
     P = mg.levels[0]
     r = cont(orc, P, 61)
     z = torch.empty(P.n, dtype=torch.float64, device="cuda")
-    G.mg_vcycle(dev(torch, r), z, lam, tags, orders, 2, 4, mg.lmax, mg_kind=4)
+    G.mg_vcycle(dev(torch, r), z, lam, tags, orders, 2, 4, mg.lmax, mg_kind=4, mg_coarse_frac=0.1)
     assert normwise(z.cpu().numpy(), mg.vcycle(r)) <= 1e-11
     assert normwise(z.cpu().numpy(), mg1.vcycle(r)) > 1e-3           # and it is a different polynomial than the first kind
     b = P.assemble_rhs(I.divergence_source(m, I.seed_for(2, 71)))
     ro = mg.pcg(b, rtol=1e-10)
     x = torch.zeros(P.n, dtype=torch.float64, device="cuda")
     rg = G.pcg_solve(dev(torch, b), x, lam=lam, tags=tags, precond=3, rtol=1e-10, mg_orders=orders, mg_smooth=2, mg_coarse=4,
-                     mg_lmax=mg.lmax, mg_kind=4)
+                     mg_lmax=mg.lmax, mg_kind=4, mg_coarse_frac=0.1)
     assert ro["status"] == 0 and rg["status"] == 0 and abs(rg["iters"] - ro["iters"]) <= 1
     assert normwise(x.cpu().numpy(), ro["x"]) <= 1e-8
 
