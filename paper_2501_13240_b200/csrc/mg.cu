@@ -110,10 +110,6 @@ static void interp3_launch(int64_t E, int nin, int nout, const double* J, int tr
     k_interp3<0, 0><<<(unsigned)E, 128, 0, s>>>(nin, nout, J, transpose, in, scale, out, accumulate, scal);
 }
 
-__global__ void k_mg_fill(int64_t n, double* __restrict__ a, double v)
-{
-    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) a[l] = v;
-}
 // u ~ U[-1,1) per local node from the counter-based splitmix64 of the input recipe (R19)
 __global__ void k_mg_random(int64_t n, unsigned long long seed, double* __restrict__ a)
 {

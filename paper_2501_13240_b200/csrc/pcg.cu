@@ -288,10 +288,6 @@ static int apply_A(semb_mesh* h, double lambda, const semb_mask_entry& m, const 
     return semb_mask_launch(h, m, out, 1, s);
 }
 
-int semb_apply_A(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* v_masked, double* out, cudaStream_t s)
-{
-    return apply_A(h, lambda, m, v_masked, out, nullptr, s);
-}
 // res = r - M QQ^T A_L z  (z continuous and masked; tmp: scratch [n]): the gather-scatter in gather form as in k_update_r
 __global__ void __launch_bounds__(VEC_BLOCK, 4)
 k_residual(int64_t n, const double* __restrict__ q, gs_lists L, const double* __restrict__ r, double* __restrict__ res,

@@ -139,8 +139,6 @@ int semb_cheb_apply(semb_mesh* h, double lambda, const semb_mask_entry& m, const
 // res = r - M QQ^T A_L z  (z continuous and masked; tmp: scratch [n])
 int semb_residual_launch(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* z, const double* r, double* res,
                          double* tmp, semb_scalars* scal, cudaStream_t s);
-// out = M QQ^T A_L v  (v continuous and masked)
-int semb_apply_A(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* v_masked, double* out, cudaStream_t s);
 int semb_dot_rz_launch(semb_mesh* h, const double* r, const double* z, semb_scalars* scal, cudaStream_t s);
 
 // ---- mg.cu: p-multigrid V-cycle
