@@ -45,14 +45,16 @@ int semb_axhelm_prepare_geo(semb_mesh* h, cudaStream_t) { h->geoK = h->geo; retu
 #ifndef SEMB_MINB10
 #define SEMB_MINB10 3
 #endif
-template <int n1> struct ax_minb { static constexpr int v = (n1 <= 4) ? 16 : (n1 <= 6) ? 8 : (n1 <= 8) ? 4 : (n1 == 9) ? 4 : (n1 == 10) ? SEMB_MINB10 : 3; };
+// elements per block (axhelm_kernels.cuh): small orders pack several elements into one block of ~128 threads
+template <int n1> struct ax_epb { static constexpr int v = (n1 == 2) ? 32 : (n1 == 3) ? 14 : (n1 == 4) ? 8 : 1; };
+template <int n1> struct ax_minb { static constexpr int v = (n1 <= 4) ? 8 : (n1 <= 6) ? 8 : (n1 <= 8) ? 4 : (n1 == 9) ? 4 : (n1 == 10) ? SEMB_MINB10 : 3; };
 
 template <int n1>
 static int launch_line(semb_mesh* h, int mode, double lambda, const double* lam0, const double* lam1,
                        const double* u, double* w, int nfields, semb_scalars* scal, bool want_dot, const ax_pcg_args& pcg, cudaStream_t s)
 {
-    constexpr int MB = ax_minb<n1>::v;
-    const unsigned grid = (unsigned)(h->E * nfields);
+    constexpr int MB = ax_minb<n1>::v, EPB = ax_epb<n1>::v;
+    const unsigned grid = (unsigned)((h->E * nfields + EPB - 1) / EPB);
     double* dot = (scal && want_dot) ? h->ax_dot : nullptr;
     // L2 prefetch distance in elements: about 8 MB of this launch's traffic ahead of the block that issues it.
     // Measured on B200 (N = 3, 5, 7, 9, stand-alone and PCG-fused): 4-20 MB ahead is flat (N = 7 Poisson 6.2 -> 7.05 TB/s,
@@ -60,7 +62,7 @@ static int launch_line(semb_mesh* h, int mode, double lambda, const double* lam0
     // than without prefetch.
     const int64_t bytes_per_elem = (int64_t)n1 * n1 * n1 * ((mode & 4) ? (pcg.plain ? 80 : 104) : (mode & 2) ? 88 : (mode & 1) ? 72 : 64);
     const int pf = (int)(((int64_t)8 << 20) / bytes_per_elem);
-#define SEMB_AX_LAUNCH(M) k_axhelm_line<n1, M, MB><<<grid, n1 * n1, 0, s>>>(h->E, h->n, h->geoK, lambda, lam0, lam1, u, w, scal, dot, pcg, pf)
+#define SEMB_AX_LAUNCH(M) k_axhelm_line<n1, M, MB, EPB><<<grid, n1 * n1 * EPB, 0, s>>>(h->E, h->n, h->geoK, lambda, lam0, lam1, u, w, scal, dot, pcg, pf, nfields)
     switch (mode) {
         case 0: SEMB_AX_LAUNCH(0); break;
         case 1: SEMB_AX_LAUNCH(1); break;
@@ -73,9 +75,9 @@ static int launch_line(semb_mesh* h, int mode, double lambda, const double* lam0
     h->launches += 1;
     if (dot) {
         // p.Ap = sum of the per-element partials, alpha = rho / p.Ap (fixed order: bit-reproducible)
-        int64_t blocks = (h->E + 2047) / 2048;
+        int64_t blocks = ((int64_t)grid + 2047) / 2048;
         if (blocks > 128) blocks = 128;
-        k_ax_dot_finish<<<(unsigned)blocks, 256, 0, s>>>(h->E, dot, scal, h->partials);
+        k_ax_dot_finish<<<(unsigned)blocks, 256, 0, s>>>((int64_t)grid, dot, scal, h->partials);     // one partial per block
         h->launches += 1;
     }
     SEMB_CUDA(h, cudaGetLastError());

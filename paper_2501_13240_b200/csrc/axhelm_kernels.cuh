@@ -189,29 +189,38 @@ __device__ __forceinline__ void ax_prefetch_l2(const double* ptr, int count)
     if (b > a) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" :: "l"(a), "r"((unsigned)(b - a)) : "memory");
 }
 
-template <int n1, int MODE, int MINB>
-__global__ void __launch_bounds__(n1 * n1, MINB)
+// EPB elements per block (small orders: a block of n1^2 = 4, 9 or 16 threads per element cannot fill an SM -- the
+// N = 1 level of the multigrid ran at 1 TB/s): thread group el = tl / n1^2 works on element
+// blockIdx.x * EPB + el with its own shared-memory tiles; groups past the end recompute the last element and write nothing.
+template <int n1, int MODE, int MINB, int EPB>
+__global__ void __launch_bounds__(n1 * n1 * EPB, MINB)
 k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambda,
               const double* __restrict__ lam0, const double* __restrict__ lam1,
               const double* __restrict__ u, double* __restrict__ w,
-              const semb_scalars* __restrict__ scal, double* __restrict__ dot_out, ax_pcg_args pcg, int pf_dist)
+              const semb_scalars* __restrict__ scal, double* __restrict__ dot_out, ax_pcg_args pcg, int pf_dist, int nfields)
 {
     constexpr int n2 = n1 * n1, Np = n1 * n1 * n1;
     constexpr bool HELM = MODE & 1, VAR = MODE & 2, FUSE = MODE & 4;
     constexpr int NG = HELM ? 7 : 6;
     using T = ax_tile<n1>;
-    __shared__ double Su[T::size], Sr[T::size], Ss[T::size];
+    __shared__ double SuA[EPB * T::size], SrA[EPB * T::size], SsA[EPB * T::size];
     if (scal && *(volatile const int32_t*)&scal->done) return;
-    const int a = threadIdx.x % n1, b = threadIdx.x / n1;
+    const int el = (EPB > 1) ? threadIdx.x / n2 : 0, tl = (EPB > 1) ? threadIdx.x - el * n2 : threadIdx.x;
+    double* __restrict__ Su = SuA + el * T::size; double* __restrict__ Sr = SrA + el * T::size; double* __restrict__ Ss = SsA + el * T::size;
+    const int64_t nef = E * (int64_t)nfields;
+    int64_t ef = blockIdx.x * (int64_t)EPB + el;
+    const bool valid = ef < nef;
+    if (!valid) ef = nef - 1;
+    const int a = tl % n1, b = tl / n1;
     int ra = a, rb = b, sa = a, sb = b;                                     // r-line (j=ra, k=rb), s-line (i=sa, k=sb)
     if (T::permuted) {
-        const int rq = c_perm[n1 - 1][0][threadIdx.x], sq = c_perm[n1 - 1][1][threadIdx.x];
+        const int rq = c_perm[n1 - 1][0][tl], sq = c_perm[n1 - 1][1][tl];
         ra = rq % n1; rb = rq / n1; sa = sq % n1; sb = sq / n1;
     }
-    const int64_t e = blockIdx.x % E, f = blockIdx.x / E;
+    const int64_t e = ef % E, f = ef / E;
     // The element that a block pf_dist launches later will work on is pulled into L2 now: DRAM stays busy while
     // the resident blocks are in their compute phase, and that block's loads hit L2.
-    if (pf_dist > 0 && threadIdx.x == 0 && e + pf_dist < E) {
+    if (pf_dist > 0 && tl == 0 && valid && e + pf_dist < E) {
         const int64_t ep = e + pf_dist;
         ax_prefetch_l2(geo + ep * 7 * (int64_t)Np, NG * Np);
         if (FUSE) {
@@ -222,11 +231,11 @@ k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambd
         if (VAR && lam0) ax_prefetch_l2(lam0 + ep * Np, Np);
         if (VAR && lam1) ax_prefetch_l2(lam1 + ep * Np, Np);
     }
-    double* __restrict__ we = w + f * n + e * Np + threadIdx.x;
-    const double* __restrict__ g = geo + e * 7 * (int64_t)Np + threadIdx.x;
+    double* __restrict__ we = w + f * n + e * Np + tl;
+    const double* __restrict__ g = geo + e * 7 * (int64_t)Np + tl;
     double ru[n1], G[NG][n1];
     if (FUSE) {
-        const int64_t l0 = e * Np + threadIdx.x;
+        const int64_t l0 = e * Np + tl;
         const bool plain = pcg.plain != 0;
         const double beta = plain ? 0.0 : scal->beta, alpha = plain ? 0.0 : scal->alpha;
         const bool pend = !plain && scal->x_pending != 0, first = plain || (beta == 0.0);
@@ -247,15 +256,15 @@ k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambd
         }
         if (pend) {
 #pragma unroll
-            for (int k = 0; k < n1; ++k) pcg.x[l0 + k * n2] += alpha * po[k];
+            for (int k = 0; k < n1; ++k) if (valid) pcg.x[l0 + k * n2] += alpha * po[k];
         }
 #pragma unroll
         for (int k = 0; k < n1; ++k) {
             ru[k] = first ? z[k] : z[k] + beta * po[k];
-            pcg.p_io[l0 + k * n2] = ru[k];
+            if (valid) pcg.p_io[l0 + k * n2] = ru[k];
         }
     } else {
-        const double* __restrict__ ue = u + f * n + e * Np + threadIdx.x;
+        const double* __restrict__ ue = u + f * n + e * Np + tl;
 #pragma unroll
         for (int k = 0; k < n1; ++k) ru[k] = ue[k * n2];
     }
@@ -292,7 +301,7 @@ k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambd
         const int s = T::idx(k, b, a), sB = T::idxB(k, b, a);
         const double ur = Sr[s], us = Ss[sB];
         double Grr = G[0][k], Grs = G[1][k], Grt = G[2][k], Gss = G[3][k], Gst = G[4][k], Gtt = G[5][k];
-        if (VAR && lam0) { const double c = lam0[e * Np + k * n2 + threadIdx.x]; Grr *= c; Grs *= c; Grt *= c; Gss *= c; Gst *= c; Gtt *= c; }
+        if (VAR && lam0) { const double c = lam0[e * Np + k * n2 + tl]; Grr *= c; Grs *= c; Grt *= c; Gss *= c; Gst *= c; Gtt *= c; }
         Sr[s] = Grr * ur + Grs * us + Grt * ut[k];
         Ss[sB] = Grs * ur + Gss * us + Gst * ut[k];
         gt[k] = Grt * ur + Gst * us + Gtt * ut[k];
@@ -317,7 +326,7 @@ k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambd
     if (HELM) {
 #pragma unroll
         for (int k = 0; k < n1; ++k) {
-            const double lam = (VAR && lam1) ? lam1[e * Np + k * n2 + threadIdx.x] : lambda;
+            const double lam = (VAR && lam1) ? lam1[e * Np + k * n2 + tl] : lambda;
             wt[k] += lam * G[NG - 1][k] * ru[k];
         }
     }
@@ -326,8 +335,7 @@ k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambd
 #pragma unroll
     for (int k = 0; k < n1; ++k) {
         const double wv = wt[k] + Sr[T::idx(k, b, a)] + Ss[T::idxB(k, b, a)];
-        we[k * n2] = wv;
-        dot += ru[k] * wv;
+        if (valid) { we[k * n2] = wv; dot += ru[k] * wv; }
     }
     if (dot_out) {
         __shared__ double red[32];
