@@ -54,6 +54,10 @@ MESHES = {
     "one_elem":    lambda xi: I.box_mesh(1, 1, 1, 4, xi(4)),
     "N1":          lambda xi: I.box_mesh(3, 2, 2, 1, xi(1), deform=0.05),
     "N10":         lambda xi: I.box_mesh(2, 2, 2, 10, xi(10), deform=0.05),
+    # small orders pack several elements into one block (32 / 14 / 8): element counts that leave a ragged last block
+    "N1_ragged":   lambda xi: I.box_mesh(5, 3, 5, 1, xi(1), deform=0.05),
+    "N2_ragged":   lambda xi: I.box_mesh(3, 5, 3, 2, xi(2), deform=0.05),
+    "N3_ragged":   lambda xi: I.box_mesh(3, 3, 3, 3, xi(3), deform=0.05),
 }
 
 
@@ -136,8 +140,9 @@ def test_axhelm(torch_cuda, cases, orc, name, lam):
     assert per_elem.max() <= TOL
 
 
-def test_axhelm_batched_and_variable_coefficients(torch_cuda, cases, orc):
-    m, P, G = cases("box_def")
+@pytest.mark.parametrize("name", ["box_def", "N1_ragged", "N2_ragged", "N3_ragged"])
+def test_axhelm_batched_and_variable_coefficients(torch_cuda, cases, orc, name):
+    m, P, G = cases(name)
     U = np.stack([I.uniform(I.seed_for(1, 10 + f), m.n) for f in range(3)])
     W = torch_cuda.zeros((3, m.n), dtype=torch_cuda.float64, device="cuda")
     G.apply_axhelm(dev(torch_cuda, U), W, lam=1e4, nfields=3)
@@ -231,6 +236,7 @@ def test_pcg_cfg0(torch_cuda, cases, orc, precond):
 
 
 @pytest.mark.parametrize("name,lam,tags,precond", [
+    ("N1_ragged", 0.0, 0b10, 1), ("N2_ragged", 5.0, 0b10, 2), ("N3_ragged", 0.0, 0b110, 1),
     ("box_def", 0.0, 0b110, 1), ("box_def", 1e4, 0, 1), ("ogrid7", 0.0, 0b10, 2), ("ogrid7", 0.0, 0b10, 1),
     ("ogrid9", 3000.0, 0b110, 1), ("ogrid9", 0.0, 0b10, 1), ("box_per_str", 0.0, 0b10, 2)])
 def test_pcg_mesh_families(torch_cuda, cases, orc, name, lam, tags, precond):
