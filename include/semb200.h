@@ -159,6 +159,11 @@ typedef struct {
     int32_t  pad_;
     double   mg_coarse_lmin_frac; /* first-kind smoother of the LAST level runs on [frac, 1] lmax; <= 0 => 0.01.  A smaller
                                      fraction with a higher mg_coarse_degree (<= 64) makes it act as a coarse solver      */
+    int32_t  null_mean;       /* 1: the operator has the constants as null space (lambda = 0 and no Dirichlet node: the
+                                 all-Neumann pressure problem of a closed cell): solve A x = b - mean(b)
+                                 and return the solution of zero mean, mean(v) = <v,1> / n_unique over unique nodes
+                                 (reading R20).  SEMB_EINVAL if the tag set selects any Dirichlet node. */
+    int32_t  pad2_;
 } semb_pcg_opts;
 
 typedef struct {

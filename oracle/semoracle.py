@@ -205,8 +205,18 @@ class Problem:
         T = np.diag(a[:m]) + np.diag(b[:m - 1], 1) + np.diag(b[:m - 1], -1)
         return 1.1 * float(np.linalg.eigvalsh(T)[-1])
 
-    def pcg(self, b, x0=None, precond=1, cheb_k=2, lmax=0.0, rtol=1e-10, atol=0.0, maxit=10000, hist_len=0):
-        """c-9.  Returns dict(x, iters, status, r0, rn, hist)."""
+    def mean(self, v):
+        """mean over the unique nodes, <v,1> / n_unique (reading R20)"""
+        return float(np.sum(_f64(v) * self.invmult)) / self.n_unique
+
+    def pcg(self, b, x0=None, precond=1, cheb_k=2, lmax=0.0, rtol=1e-10, atol=0.0, maxit=10000, hist_len=0, null_mean=False):
+        """c-9.  Returns dict(x, iters, status, r0, rn, hist).  null_mean (R20, operators whose null space is the
+        constants): solve A x = b - mean(b) and return the solution of zero mean."""
+        if null_mean:
+            assert self.lam == 0.0 and np.all(self.mask == 1.0)
+            r = self.pcg(_f64(b) - self.mean(b), x0, precond, cheb_k, lmax, rtol, atol, maxit, hist_len)
+            r["x"] = r["x"] - self.mean(r["x"])
+            return r
         x = np.zeros(self.n) if x0 is None else _f64(x0).copy()
         hist = np.zeros(max(hist_len, 1)); out3 = np.zeros(3)
         st = lib().orc_pcg(C.byref(self._op), C.c_int(precond), C.c_int(cheb_k), C.c_double(lmax), _p(self.dinv),
@@ -311,8 +321,13 @@ class Multigrid:
         lib().orc_mg_vcycle(C.byref(self._mg), C.c_int(level), _p(_f64(r)), _p(z))
         return z
 
-    def pcg(self, b, x0=None, rtol=1e-10, atol=0.0, maxit=10000, hist_len=0):
+    def pcg(self, b, x0=None, rtol=1e-10, atol=0.0, maxit=10000, hist_len=0, null_mean=False):
         P = self.levels[0]
+        if null_mean:
+            assert P.lam == 0.0 and np.all(P.mask == 1.0)
+            r = self.pcg(_f64(b) - P.mean(b), x0, rtol, atol, maxit, hist_len)
+            r["x"] = r["x"] - P.mean(r["x"])
+            return r
         x = np.zeros(P.n) if x0 is None else _f64(x0).copy()
         hist = np.zeros(max(hist_len, 1)); out3 = np.zeros(3)
         st = lib().orc_pcg_mg(C.byref(self._mg), _p(_f64(b)), _p(x), C.c_double(rtol), C.c_double(atol), C.c_int(maxit),

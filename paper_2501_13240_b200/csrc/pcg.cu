@@ -59,16 +59,35 @@ __device__ __forceinline__ void gs_gathered(const int32_t (&c)[GS_U], const doub
 #define GS_STEP ((int64_t)gridDim.x * (GS_U * VEC_BLOCK))
 #define GS_CHUNKS(l0, n) for (int64_t l0 = blockIdx.x * (int64_t)(GS_U * VEC_BLOCK) + threadIdx.x; l0 - threadIdx.x < (n); l0 += GS_STEP)
 
-// r = b (x = 0) or r = b - q (q = A x0);  bb, rr, rz
+// scal->shift = mean of v over the unique nodes (null_mean: reading R20)
+__global__ void __launch_bounds__(VEC_BLOCK)
+k_mean(int64_t n, const double* __restrict__ v, const double* __restrict__ invmult, double inv_nu,
+       semb_scalars* __restrict__ scal, double* __restrict__ partials)
+{
+    __shared__ double red[32];
+    double s = 0.0;
+    GSTRIDE(l, n) s += v[l] * invmult[l];
+    double vv[1] = { block_sum(s, red) }, tot[1];
+    if (grid_sum<1>(vv, partials, &scal->ticket[4], tot, red) && threadIdx.x == 0) scal->shift = tot[0] * inv_nu;
+}
+__global__ void __launch_bounds__(VEC_BLOCK)
+k_shift(int64_t n, double* __restrict__ v, const semb_scalars* __restrict__ scal)
+{
+    const double sh = scal->shift;
+    GSTRIDE(l, n) v[l] -= sh;
+}
+
+// r = b (x = 0) or r = b - q (q = A x0);  bb, rr, rz.  use_shift: b is replaced by b - scal->shift (null_mean)
 __global__ void __launch_bounds__(VEC_BLOCK)
 k_pcg_init(int64_t n, const double* __restrict__ b, const double* __restrict__ q, double* __restrict__ x,
            double* __restrict__ r, const double* __restrict__ invmult, const double* __restrict__ dinv,
-           semb_scalars* __restrict__ scal, double* __restrict__ partials, double* __restrict__ hist)
+           semb_scalars* __restrict__ scal, double* __restrict__ partials, double* __restrict__ hist, int use_shift)
 {
     __shared__ double red[32];
     double bb = 0.0, rr = 0.0, rz = 0.0;
+    const double sh = use_shift ? scal->shift : 0.0;
     GSTRIDE(l, n) {
-        const double bl = b[l], w = invmult[l];
+        const double bl = b[l] - sh, w = invmult[l];
         double rl = bl;
         if (q) rl -= q[l]; else x[l] = 0.0;
         r[l] = rl;
@@ -528,11 +547,18 @@ int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* 
     SEMB_CUDA(h, cudaMemcpyAsync(h->scal, &init, sizeof(init), cudaMemcpyHostToDevice, s));
 
     const double* dz = (o->precond == 1) ? dinv : nullptr;      // fused z = dinv o r
+    const int nm = o->null_mean ? 1 : 0;
+    if (nm) {
+        if (m.count != 0 || o->lambda != 0.0)
+            return semb_fail(h, SEMB_EINVAL, "pcg: null_mean needs lambda = 0 and a tag set without Dirichlet nodes");
+        k_mean<<<G, VEC_BLOCK, 0, s>>>(n, b, h->invmult, 1.0 / (double)h->n_unique, h->scal, h->partials);
+        h->launches += 1;
+    }
     if (!o->x0_is_zero) {
         rc = apply_A(h, o->lambda, m, x, q, nullptr, s); if (rc) return rc;
-        k_pcg_init<<<G, VEC_BLOCK, 0, s>>>(n, b, q, x, r, h->invmult, dz, h->scal, h->partials, hist);
+        k_pcg_init<<<G, VEC_BLOCK, 0, s>>>(n, b, q, x, r, h->invmult, dz, h->scal, h->partials, hist, nm);
     } else {
-        k_pcg_init<<<G, VEC_BLOCK, 0, s>>>(n, b, nullptr, x, r, h->invmult, dz, h->scal, h->partials, hist);
+        k_pcg_init<<<G, VEC_BLOCK, 0, s>>>(n, b, nullptr, x, r, h->invmult, dz, h->scal, h->partials, hist, nm);
     }
     SEMB_CUDA(h, cudaGetLastError());
 
@@ -573,6 +599,12 @@ int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* 
         finished = h->scal_host->done != 0;
     }
     if (o->maxit > 0) { k_final_x<<<G, VEC_BLOCK, 0, s>>>(n, p, x, h->scal); h->launches += 1; SEMB_CUDA(h, cudaGetLastError()); }
+    if (nm) {                                                   // the solution of zero mean
+        k_mean<<<G, VEC_BLOCK, 0, s>>>(n, x, h->invmult, 1.0 / (double)h->n_unique, h->scal, h->partials);
+        k_shift<<<G, VEC_BLOCK, 0, s>>>(n, x, h->scal);
+        h->launches += 2;
+        SEMB_CUDA(h, cudaGetLastError());
+    }
     if (o->maxit == 0 || !finished) {
         SEMB_CUDA(h, cudaMemcpyAsync(h->scal_host, h->scal, sizeof(semb_scalars), cudaMemcpyDeviceToHost, s));
         SEMB_CUDA(h, cudaStreamSynchronize(s));

@@ -15,7 +15,7 @@
 // "fused PCG vector updates and dot-product reductions").  One copy lives in device memory, a pinned host
 // mirror receives it when the host polls the stop flag.
 struct semb_scalars {
-    double rho_old, rho_new, pAp, alpha, beta, rr, rz, rnorm, bnorm, r0norm, target, rtol, atol, aux;
+    double rho_old, rho_new, pAp, alpha, beta, rr, rz, rnorm, bnorm, r0norm, target, rtol, atol, aux, shift;
     int32_t iter, done, status, maxit, x_pending, pad_;
     uint32_t ticket[8];
 };

@@ -181,3 +181,36 @@ def test_coarse_level_as_chebyshev_solver(torch_cuda, cases, orc):
     assert normwise(x.cpu().numpy(), ro["x"]) <= 1e-8
     with pytest.raises(Exception):
         G.pcg_solve(dev(torch, b), x, lam=lam, tags=tags, precond=3, mg_orders=orders, mg_coarse=65)
+
+
+@pytest.mark.parametrize("precond", [1, 3])
+def test_all_neumann_pressure_zero_mean(torch_cuda, semb, orc, xi_of, precond):
+    """null_mean (R20): lambda = 0, no Dirichlet node -- the closed-cell pressure problem (PAPER.md:L238, L266:
+    no-slip walls all around).  Inconsistent right-hand side in, zero-mean solution of A x = b - mean(b) out."""
+    torch = torch_cuda
+    m = I.box_mesh(4, 3, 3, 5, xi_of(5), deform=0.05, zstretch=2.0)
+    orders = [5, 3, 1]
+    mg = orc.Multigrid(m.E, m.N, m.x, m.y, m.z, m.face_tag, m.period, 0.0, 0, orders, k_smooth=1, k_coarse=8, coarse_frac=0.05)
+    P = mg.levels[0]
+    b = P.assemble_rhs(I.divergence_source(m, 9) + 0.3)
+    assert abs(P.mean(b)) > 1e-6
+    G = semb.Mesh(m.E, m.N, dev(torch, m.x), dev(torch, m.y), dev(torch, m.z), m.face_tag, m.period)
+    try:
+        x = torch.zeros(P.n, dtype=torch.float64, device="cuda")
+        if precond == 1:
+            ro = P.pcg(b, precond=1, rtol=1e-10, null_mean=True)
+            rg = G.pcg_solve(dev(torch, b), x, lam=0.0, tags=0, precond=1, rtol=1e-10, null_mean=True)
+        else:
+            ro = mg.pcg(b, rtol=1e-10, null_mean=True)
+            rg = G.pcg_solve(dev(torch, b), x, lam=0.0, tags=0, precond=3, rtol=1e-10, null_mean=True, mg_orders=orders,
+                             mg_smooth=1, mg_coarse=8, mg_coarse_frac=0.05, mg_lmax=mg.lmax)
+        assert ro["status"] == 0 and rg["status"] == 0 and abs(rg["iters"] - ro["iters"]) <= 1, (rg["iters"], ro["iters"])
+        xg = x.cpu().numpy()
+        assert normwise(xg, ro["x"]) <= 1e-8
+        assert abs(P.mean(xg)) <= 1e-13 * np.abs(xg).max()
+        res = (b - P.mean(b)) - P.apply_A(xg)
+        assert np.sqrt(P.dot(res, res)) <= 2e-10 * np.sqrt(P.dot(b - P.mean(b), b - P.mean(b)))
+        with pytest.raises(Exception):                      # Dirichlet nodes and null_mean exclude each other
+            G.pcg_solve(dev(torch, b), x, lam=0.0, tags=0b10, precond=1, null_mean=True)
+    finally:
+        G.close()

@@ -167,3 +167,28 @@ def test_minmax_hist_and_vmag(orc):
     x, y, z = rng.standard_normal((3, 1000))
     ref = np.sqrt(x.astype(np.longdouble) ** 2 + y.astype(np.longdouble) ** 2 + z.astype(np.longdouble) ** 2)
     assert np.all(np.abs(orc.vmag(x, y, z) - ref.astype(np.float64)) <= 2 * np.spacing(ref.astype(np.float64)))
+
+
+# ---------------------------------------------------------------- R20: all-Neumann problem, zero-mean solution
+@pytest.mark.parametrize("precond", [1, 2])
+def test_null_mean_solution_is_the_pseudo_inverse_solution(orc, xi_of, precond):
+    """lambda = 0 without Dirichlet nodes: A is singular with the constants as null space.  The solve of b - mean(b)
+    returned with zero mean must equal numpy's pseudo-inverse (minimum-norm) solution on the unique nodes."""
+    N = 3
+    m = I.box_mesh(2, 3, 2, N, xi_of(N), deform=0.05)
+    P = make(orc, m, lam=0.0, tags=0)
+    A = dense_matrix(P)
+    assert abs(np.linalg.eigvalsh(A)[0]) <= 1e-12 * np.linalg.eigvalsh(A)[-1]          # singular
+    b = P.assemble_rhs(orc.gs(P.gid, P.n_unique, I.uniform(33, m.n) * P.invmult))       # NOT consistent: mean(b) != 0
+    assert abs(P.mean(b)) > 1e-6
+    lmax = 0.0
+    if precond == 2:
+        Dm = np.diag(A)
+        lmax = 1.05 * np.linalg.eigvalsh(A / np.sqrt(np.outer(Dm, Dm)))[-1]
+    r = P.pcg(b, precond=precond, cheb_k=2, lmax=lmax, rtol=1e-12, null_mean=True)
+    assert r["status"] == 0
+    xg = to_global(P, r["x"])
+    bg = to_global(P, b)
+    expect = np.linalg.pinv(A, hermitian=True) @ (bg - bg.mean())
+    assert abs(xg.mean()) <= 1e-13 * np.abs(xg).max()
+    assert np.allclose(xg, expect, rtol=0, atol=1e-9 * np.abs(expect).max())
