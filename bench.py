@@ -39,11 +39,18 @@ B_AXHELM_HELM = 72.0
 B_AXHELM_PCG = 104.0     # the PCG-fused launch: reads r, dinv, p, x (32) + G (48), writes p, x, q (24)
 NCU_TRAFFIC_AXHELM_PCG = 13.943e9   # dram read + write bytes of one launch on cfg3, ncu --set full (profiles/r1_v4_axhelm_full.md)
 B_ITER = 171.6           # algorithmic bytes per node per Jacobi-PCG iteration, N = 7, Poisson
-WORKLOADS = {            # name -> elements per direction of the deformed box (BASELINE.json configs[3] / configs[1])
-    "cfg3_box64_deformed_N7": 64,
+WORKLOADS = {            # name -> elements per direction of the deformed box (BASELINE.json configs[3] / configs[1]),
+    "cfg3_box64_deformed_N7": 64,     # or ("ogrid", cfg): the cylinder O-grids of configs[2] / configs[4]
     "cfg1_box16_deformed_N7": 16,
     "box32_deformed_N7": 32,
+    "cfg2_ogrid_N7": ("ogrid", 2),
+    "cfg4_ogrid_N9": ("ogrid", 4),
 }
+
+
+def model_bytes_per_iteration(N):
+    """64 (axhelm) + 20 * n_shared/n (gather-scatter) + 64 + 32, n_shared/n = 1 - ((N-1)/(N+1))^3."""
+    return 64.0 + 20.0 * (1.0 - ((N - 1.0) / (N + 1.0)) ** 3) + 64.0 + 32.0
 
 
 def measured_peak():
@@ -111,9 +118,12 @@ def aggregate(ms_local, nodes_local, steps, dist=None, device=None):
 
 
 def build_problem(torch, semb, ne):
-    """64^3 (or ne^3) deformed box, N = 7: mesh on the host, coordinates to the device, setup, rhs."""
-    xi = semb.gll(7)[0]
-    m = I.box_mesh(ne, ne, ne, 7, xi, deform=0.05, name=f"box{ne}_deformed")
+    """64^3 (or ne^3) deformed box, N = 7, or an O-grid of configs[2] / [4]: mesh on the host, coordinates to the device, setup."""
+    if isinstance(ne, tuple):
+        m, _ = I.config_mesh(ne[1], lambda N: semb.gll(N)[0])
+    else:
+        xi = semb.gll(7)[0]
+        m = I.box_mesh(ne, ne, ne, 7, xi, deform=0.05, name=f"box{ne}_deformed")
     x, y, z = (torch.from_numpy(a).cuda() for a in (m.x, m.y, m.z))
     G = semb.Mesh(m.E, m.N, x, y, z, m.face_tag, m.period)
     del x, y, z
@@ -190,6 +200,7 @@ def main():
     ne = WORKLOADS[args.workload]
     m, G = build_problem(torch, semb, ne)
     n = m.n
+    b_iter = B_ITER if m.N == 7 else model_bytes_per_iteration(m.N)
     f = torch.from_numpy(I.uniform(I.seed_for(3, 2), n)).cuda()
     b = torch.empty_like(f)
     G.assemble_rhs(f, b, 0b10)
@@ -314,16 +325,16 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": args.workload, "E": m.E, "N": 7, "local_nodes": n, "lambda": 0.0,
+        "config": {"workload": args.workload, "E": m.E, "N": m.N, "local_nodes": n, "lambda": 0.0,
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": "inputs larger than L2 (every vector is %.2f GB)" % (8 * n / 1e9)},
-        "roofline": {"bound": "hbm", "kernel": "k_axhelm_line<8,4,4>: axhelm (Poisson) with the fused PCG prologue (x += alpha p, p = dinv r + beta p) and p.Ap epilogue", "achieved": ax_gbs, "peak": peak,
+        "roofline": {"bound": "hbm", "kernel": f"k_axhelm_line<{m.N + 1},4,*>: axhelm (Poisson) with the fused PCG prologue (x += alpha p, p = dinv r + beta p) and p.Ap epilogue", "achieved": ax_gbs, "peak": peak,
                      "unit": "GB/s", "frac": ax_gbs / peak, "traffic": NCU_TRAFFIC_AXHELM_PCG if args.workload.startswith("cfg3") else None, "peak_source": peak_src,
                      "bytes_per_node": B_AXHELM_PCG, "ms": ax_ms, "timed_launches": st["profiled"],
                      "frac_of_8TBs": ax_gbs / 8000.0, "gdofs": n / (ax_ms * 1e-3) / 1e9},
-        "pcg_iter": {"ms": ms_step, "model_bytes_per_node": B_ITER, "gbs": B_ITER * n / (ms_step * 1e-3) / 1e9,
-                     "frac_of_measured_peak": B_ITER * n / (ms_step * 1e-3) / 1e9 / peak,
-                     "frac_of_8TBs": B_ITER * n / (ms_step * 1e-3) / 8e12},
+        "pcg_iter": {"ms": ms_step, "model_bytes_per_node": b_iter, "gbs": b_iter * n / (ms_step * 1e-3) / 1e9,
+                     "frac_of_measured_peak": b_iter * n / (ms_step * 1e-3) / 1e9 / peak,
+                     "frac_of_8TBs": b_iter * n / (ms_step * 1e-3) / 8e12},
         "axhelm_sweep": sweep,
         "time_to_solution": solve_tts,
         "export": export,

@@ -150,7 +150,7 @@ typedef struct {
      * mg_smooth_degree before and after the coarse correction, of degree mg_coarse_degree alone on the last level;
      * mg_lmax[l] <= 0 => estimated (10-step Lanczos x 1.1 from the level's M QQ^T u, u ~ U[-1,1) seeded per level)
      * and cached in the handle. */
-    int32_t  mg_nlevels;      /* 2..8; 0 with precond == 3 => orders N, 3, 1 (N > 3) or N, 1           */
+    int32_t  mg_nlevels;      /* 2..8; 0 with precond == 3 => orders N, 5, 3, 1 (N > 7), N, 3, 1 (N > 3) or N, 1 */
     int32_t  mg_orders[8];
     int32_t  mg_smooth_degree, mg_coarse_degree;     /* <= 0 => 1 and 32 (measured best compromise) */
     double   mg_lmax[8];

@@ -201,6 +201,7 @@ int semb_mg_prepare(semb_mesh* h, const semb_pcg_opts* o, semb_mg_ctx* ctx, cuda
     int nlev = o->mg_nlevels, orders[8];
     if (nlev == 0) {
         orders[0] = h->N; nlev = 1;
+        if (h->N > 7) orders[nlev++] = 5;          // cfg4 (N = 9): 9, 5, 3, 1 needs 64 iterations, 9, 3, 1 needs 94
         if (h->N > 3) orders[nlev++] = 3;
         if (h->N > 1) orders[nlev++] = 1;
     } else {
