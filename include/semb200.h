@@ -163,7 +163,9 @@ typedef struct {
                                  all-Neumann pressure problem of a closed cell): solve A x = b - mean(b)
                                  and return the solution of zero mean, mean(v) = <v,1> / n_unique over unique nodes
                                  (reading R20).  SEMB_EINVAL if the tag set selects any Dirichlet node. */
-    int32_t  pad2_;
+    int32_t  mg_fp32;         /* 1: the V-cycle keeps its vectors and geometric factors in FP32 (the
+                                 preconditioner runs in FP32 "to save on memory bandwidth"); every kernel still computes
+                                 in fp64 registers and rounds at its stores; the PCG around it stays fp64 (reading R21) */
 } semb_pcg_opts;
 
 typedef struct {

@@ -364,13 +364,25 @@ typedef struct {
     double lambda;
 } orc_op;
 
+/* f-1, reading R21: FP32 STORAGE of the multigrid levels.  While g_r32 is set (only inside
+ * orc_mg_vcycle with mg->fp32), every vector an operation of the V-cycle produces is rounded to float where it would
+ * be stored; the arithmetic stays fp64.  Off everywhere else, so nothing outside the fp32 V-cycle changes. */
+static int g_r32 = 0;
+static void rnd32(double* v, int64_t n)
+{
+    if (!g_r32) return;
+    for (int64_t l = 0; l < n; ++l) v[l] = (double)(float)v[l];
+}
+
 /* out = M QQ^T ( A_L ( M v ) );  tmp is scratch [n] */
 void orc_apply_A(const orc_op* op, const double* v, double* out, double* tmp)
 {
     for (int64_t l = 0; l < op->n; ++l) tmp[l] = op->mask[l] * v[l];
     orc_axhelm(op->E, op->N, op->geo, op->D, op->lambda, NULL, NULL, tmp, out);
+    rnd32(out, op->n);
     orc_gs(op->n, op->gid, op->n_unique, out);
     for (int64_t l = 0; l < op->n; ++l) out[l] *= op->mask[l];
+    rnd32(out, op->n);
 }
 
 /* <a,b> = sum_l a_l b_l / mult_l  (= dot product over unique nodes for continuous a,b) */
@@ -428,15 +440,20 @@ void orc_cheb_jacobi_frac(const orc_op* op, int k, double lmax, double lmin_frac
     const double sigma = theta / delta;
     double rho = 1.0 / sigma;
     for (int64_t l = 0; l < n; ++l) { z[l] = 0.0; res[l] = r[l]; d[l] = dinv[l] * res[l] / theta; }
+    rnd32(d, n);
     for (int it = 0; it < k; ++it) {
         for (int64_t l = 0; l < n; ++l) z[l] += d[l];
+        rnd32(z, n);
         orc_apply_A(op, d, Ad, tmp);
         for (int64_t l = 0; l < n; ++l) res[l] -= Ad[l];
+        rnd32(res, n);
         double rho1 = 1.0 / (2.0 * sigma - rho);
         for (int64_t l = 0; l < n; ++l) d[l] = rho1 * rho * d[l] + (2.0 * rho1 / delta) * (dinv[l] * res[l]);
+        rnd32(d, n);
         rho = rho1;
     }
     for (int64_t l = 0; l < n; ++l) z[l] += d[l];
+    rnd32(z, n);
 }
 
 /* ------------------------------------------------------------------------------------ */
@@ -511,6 +528,7 @@ void orc_mg_prolong(const orc_mg* mg, int l, const double* vc, double* vf)
     const orc_op* f = &mg->lev[l].op; const orc_op* c = &mg->lev[l + 1].op;
     orc_interp3(f->E, f->N + 1, c->N + 1, mg->lev[l].J, 0, vc, vf);
     for (int64_t q = 0; q < f->n; ++q) vf[q] *= f->mask[q];
+    rnd32(vf, f->n);
 }
 /* r_c = M_c QQ^T_c J^T (invmult_f o r_f);  tmp: [n_f] */
 void orc_mg_restrict(const orc_mg* mg, int l, const double* rf, double* rc, double* tmp)
@@ -518,8 +536,10 @@ void orc_mg_restrict(const orc_mg* mg, int l, const double* rf, double* rc, doub
     const orc_op* f = &mg->lev[l].op; const orc_op* c = &mg->lev[l + 1].op;
     for (int64_t q = 0; q < f->n; ++q) tmp[q] = f->invmult[q] * rf[q];
     orc_interp3(f->E, f->N + 1, c->N + 1, mg->lev[l].J, 1, tmp, rc);
+    rnd32(rc, c->n);
     orc_gs(c->n, c->gid, c->n_unique, rc);
     for (int64_t q = 0; q < c->n; ++q) rc[q] *= c->mask[q];
+    rnd32(rc, c->n);
 }
 
 /* f-1  Chebyshev-Jacobi smoother of the FOURTH kind ("fourth-kind Chebyshev-accelerated"
@@ -535,14 +555,19 @@ void orc_cheb4_jacobi(const orc_op* op, int k, double lmax, const double* dinv, 
     const int64_t n = op->n;
     double* res = work; double* d = work + n; double* Ad = work + 2 * n; double* tmp = work + 3 * n;
     for (int64_t l = 0; l < n; ++l) { z[l] = 0.0; res[l] = r[l]; d[l] = dinv[l] * res[l] * (4.0 / (3.0 * lmax)); }
+    rnd32(d, n);
     for (int i = 1; i <= k; ++i) {
         for (int64_t l = 0; l < n; ++l) z[l] += d[l];
+        rnd32(z, n);
         orc_apply_A(op, d, Ad, tmp);
         for (int64_t l = 0; l < n; ++l) res[l] -= Ad[l];
+        rnd32(res, n);
         const double c1 = (2.0 * i - 1.0) / (2.0 * i + 3.0), c2 = (8.0 * i + 4.0) / ((2.0 * i + 3.0) * lmax);
         for (int64_t l = 0; l < n; ++l) d[l] = c1 * d[l] + c2 * (dinv[l] * res[l]);
+        rnd32(d, n);
     }
     for (int64_t l = 0; l < n; ++l) z[l] += d[l];
+    rnd32(z, n);
 }
 static void mg_smooth(const orc_mg* mg, const orc_mg_level* L, int k, const double* r, double* z, double* work)
 {
@@ -567,15 +592,32 @@ void orc_mg_vcycle(const orc_mg* mg, int l, const double* r, double* z)
     mg_smooth(mg, L, mg->k_smooth, r, z, work);                                     /* z = S r            */
     orc_apply_A(&L->op, z, Az, tmp);
     for (int64_t q = 0; q < n; ++q) res[q] = r[q] - Az[q];                          /* res = r - A z      */
+    rnd32(res, n);
     orc_mg_restrict(mg, l, res, rc, tmp);
     orc_mg_vcycle(mg, l + 1, rc, ec);
     orc_mg_prolong(mg, l, ec, tmp);
     for (int64_t q = 0; q < n; ++q) z[q] += tmp[q];                                 /* z += P e           */
+    rnd32(z, n);
     orc_apply_A(&L->op, z, Az, tmp);
     for (int64_t q = 0; q < n; ++q) res[q] = r[q] - Az[q];                          /* res = r - A z      */
+    rnd32(res, n);
     mg_smooth(mg, L, mg->k_smooth, res, Az, work);                                  /* Az = S res         */
     for (int64_t q = 0; q < n; ++q) z[q] += Az[q];
+    rnd32(z, n);
     free(rc); free(work);
+}
+
+/* z = V(0, r) with FP32 storage (R21): r is rounded on entry, every stored vector inside the cycle is rounded, the
+ * level operators mg32 must have been built from float-rounded geometric factors, diagonals and multiplicities. */
+void orc_mg_vcycle_fp32(const orc_mg* mg32, const double* r, double* z)
+{
+    const int64_t n = mg32->lev[0].op.n;
+    double* r32 = (double*)malloc(sizeof(double) * (size_t)n);
+    for (int64_t l = 0; l < n; ++l) r32[l] = (double)(float)r[l];
+    g_r32 = 1;
+    orc_mg_vcycle(mg32, 0, r32, z);
+    g_r32 = 0;
+    free(r32);
 }
 
 /* z = M^-1 r : precond 0 = identity, 1 = Jacobi, 2 = Chebyshev-Jacobi(cheb_k), 3 = p-multigrid V-cycle */
@@ -585,7 +627,8 @@ static void precond_apply(const orc_op* op, int precond, int cheb_k, double lmax
     if (precond == 0)      for (int64_t l = 0; l < op->n; ++l) z[l] = r[l];
     else if (precond == 1) for (int64_t l = 0; l < op->n; ++l) z[l] = dinv[l] * r[l];
     else if (precond == 2) orc_cheb_jacobi(op, cheb_k, lmax, dinv, r, z, work);
-    else                   orc_mg_vcycle(mg, 0, r, z);
+    else if (precond == 3) orc_mg_vcycle(mg, 0, r, z);
+    else                   orc_mg_vcycle_fp32(mg, r, z);          /* precond 4: mg holds the float-rounded levels */
 }
 
 /* c-9  preconditioned conjugate gradients, step by step (the pressure Poisson solve).
@@ -643,6 +686,12 @@ int orc_pcg_mg(const orc_mg* mg, const double* b, double* x, double rtol, double
                double* hist, int hist_len, double* out3)
 {
     return pcg_core(&mg->lev[0].op, 3, 0, 0.0, mg->lev[0].dinv, mg, b, x, rtol, atol, maxit, x0_is_zero, hist, hist_len, out3);
+}
+/* the same with the FP32-storage V-cycle (R21): the outer PCG runs on op64 (fp64 operator), the preconditioner on mg32 */
+int orc_pcg_mg_fp32(const orc_op* op64, const orc_mg* mg32, const double* b, double* x, double rtol, double atol, int maxit,
+                    int x0_is_zero, double* hist, int hist_len, double* out3)
+{
+    return pcg_core(op64, 4, 0, 0.0, NULL, mg32, b, x, rtol, atol, maxit, x0_is_zero, hist, hist_len, out3);
 }
 
 /* c-10  Lanczos on D^-1/2 A D^-1/2 from the start vector v0 (continuous, masked; normalised here).

@@ -275,7 +275,7 @@ class Multigrid:
     meshes of some thousand elements and the V-cycle loses definiteness), or given."""
 
     def __init__(self, E, N, x, y, z, face_tag, period, lam, tags, orders, k_smooth=2, k_coarse=2, lmax=None, v0_of=None,
-                 kind=1, coarse_frac=0.1):
+                 kind=1, coarse_frac=0.1, fp32=False):
         assert orders[0] == N and all(a > b for a, b in zip(orders, orders[1:])) and len(orders) <= 8
         self.orders = list(orders)
         self.k_smooth, self.k_coarse = int(k_smooth), int(k_coarse)
@@ -300,9 +300,18 @@ class Multigrid:
         self._mg.nlevels, self._mg.k_smooth, self._mg.k_coarse = len(orders), self.k_smooth, self.k_coarse
         self.coarse_frac = self._mg.coarse_frac = float(coarse_frac)   # last level: first-kind interval [coarse_frac, 1] lmax
         self.kind = self._mg.kind = int(kind)          # 4 = fourth-kind Chebyshev smoother (orc_cheb4_jacobi), else first kind
+        self.fp32 = bool(fp32)
+        self._r32 = []          # float-rounded level data (R21), kept alive here
         for l, P in enumerate(self.levels):
-            self._mg.lev[l].op = P._op
-            self._mg.lev[l].dinv = P.dinv.ctypes.data
+            if self.fp32:       # FP32 storage: the level operators see the factors, diagonal and multiplicities as stored
+                r32 = lambda a: np.ascontiguousarray(a, dtype=np.float32).astype(np.float64)
+                geo32, dinv32, inv32 = r32(P.geo), r32(P.dinv), r32(P.invmult)
+                self._r32.append((geo32, dinv32, inv32))
+                self._mg.lev[l].op = _Op(P.E, P.N, 0, P.n, P.n_unique, _p(geo32), _p(P.D), _p(P.gid), _p(P.mask), _p(inv32), P.lam)
+                self._mg.lev[l].dinv = dinv32.ctypes.data
+            else:
+                self._mg.lev[l].op = P._op
+                self._mg.lev[l].dinv = P.dinv.ctypes.data
             self._mg.lev[l].lmax = self.lmax[l]
             self._mg.lev[l].J = self.J[l].ctypes.data if l < len(self.J) else None
 
@@ -318,7 +327,11 @@ class Multigrid:
 
     def vcycle(self, r, level=0):
         z = np.zeros(self.levels[level].n)
-        lib().orc_mg_vcycle(C.byref(self._mg), C.c_int(level), _p(_f64(r)), _p(z))
+        if self.fp32:
+            assert level == 0
+            lib().orc_mg_vcycle_fp32(C.byref(self._mg), _p(_f64(r)), _p(z))
+        else:
+            lib().orc_mg_vcycle(C.byref(self._mg), C.c_int(level), _p(_f64(r)), _p(z))
         return z
 
     def pcg(self, b, x0=None, rtol=1e-10, atol=0.0, maxit=10000, hist_len=0, null_mean=False):
@@ -330,7 +343,11 @@ class Multigrid:
             return r
         x = np.zeros(P.n) if x0 is None else _f64(x0).copy()
         hist = np.zeros(max(hist_len, 1)); out3 = np.zeros(3)
-        st = lib().orc_pcg_mg(C.byref(self._mg), _p(_f64(b)), _p(x), C.c_double(rtol), C.c_double(atol), C.c_int(maxit),
-                              C.c_int(1 if x0 is None else 0), _p(hist), C.c_int(hist_len), _p(out3))
+        if self.fp32:
+            st = lib().orc_pcg_mg_fp32(C.byref(P._op), C.byref(self._mg), _p(_f64(b)), _p(x), C.c_double(rtol), C.c_double(atol),
+                                       C.c_int(maxit), C.c_int(1 if x0 is None else 0), _p(hist), C.c_int(hist_len), _p(out3))
+        else:
+            st = lib().orc_pcg_mg(C.byref(self._mg), _p(_f64(b)), _p(x), C.c_double(rtol), C.c_double(atol), C.c_int(maxit),
+                                  C.c_int(1 if x0 is None else 0), _p(hist), C.c_int(hist_len), _p(out3))
         it = int(out3[0])
         return dict(x=x, iters=it, status=int(st), r0=out3[1], rn=out3[2], hist=hist[:min(hist_len, it + 1)])

@@ -49,9 +49,9 @@ int semb_axhelm_prepare_geo(semb_mesh* h, cudaStream_t) { h->geoK = h->geo; retu
 template <int n1> struct ax_epb { static constexpr int v = (n1 == 2) ? 32 : (n1 == 3) ? 14 : (n1 == 4) ? 8 : 1; };
 template <int n1> struct ax_minb { static constexpr int v = (n1 <= 4) ? 8 : (n1 <= 6) ? 8 : (n1 <= 8) ? 4 : (n1 == 9) ? 4 : (n1 == 10) ? SEMB_MINB10 : 3; };
 
-template <int n1>
-static int launch_line(semb_mesh* h, int mode, double lambda, const double* lam0, const double* lam1,
-                       const double* u, double* w, int nfields, semb_scalars* scal, bool want_dot, const ax_pcg_args& pcg, cudaStream_t s)
+template <int n1, typename ST>
+static int launch_line(semb_mesh* h, const ST* geo, int mode, double lambda, const double* lam0, const double* lam1,
+                       const ST* u, ST* w, int nfields, semb_scalars* scal, bool want_dot, const ax_pcg_args_t<ST>& pcg, cudaStream_t s)
 {
     constexpr int MB = ax_minb<n1>::v, EPB = ax_epb<n1>::v;
     const unsigned grid = (unsigned)((h->E * nfields + EPB - 1) / EPB);
@@ -60,9 +60,10 @@ static int launch_line(semb_mesh* h, int mode, double lambda, const double* lam0
     // Measured on B200 (N = 3, 5, 7, 9, stand-alone and PCG-fused): 4-20 MB ahead is flat (N = 7 Poisson 6.2 -> 7.05 TB/s,
     // N = 9 4.5 -> 5.7 TB/s), beyond ~30 MB the prefetched lines are evicted before use and the launch gets SLOWER
     // than without prefetch.
-    const int64_t bytes_per_elem = (int64_t)n1 * n1 * n1 * ((mode & 4) ? (pcg.plain ? 80 : 104) : (mode & 2) ? 88 : (mode & 1) ? 72 : 64);
+    const int64_t bytes_per_elem = (int64_t)n1 * n1 * n1 * ((mode & 4) ? (pcg.plain ? 80 : 104) : (mode & 2) ? 88 : (mode & 1) ? 72 : 64)
+                                   * (int64_t)sizeof(ST) / 8;
     const int pf = (int)(((int64_t)8 << 20) / bytes_per_elem);
-#define SEMB_AX_LAUNCH(M) k_axhelm_line<n1, M, MB, EPB><<<grid, n1 * n1 * EPB, 0, s>>>(h->E, h->n, h->geoK, lambda, lam0, lam1, u, w, scal, dot, pcg, pf, nfields)
+#define SEMB_AX_LAUNCH(M) k_axhelm_line<n1, M, MB, EPB, ST><<<grid, n1 * n1 * EPB, 0, s>>>(h->E, h->n, geo, lambda, lam0, lam1, u, w, scal, dot, pcg, pf, nfields)
     switch (mode) {
         case 0: SEMB_AX_LAUNCH(0); break;
         case 1: SEMB_AX_LAUNCH(1); break;
@@ -84,25 +85,27 @@ static int launch_line(semb_mesh* h, int mode, double lambda, const double* lam0
     return SEMB_OK;
 }
 
-static int axhelm_dispatch(semb_mesh* h, int mode, double lambda, const double* lam0, const double* lam1,
-                           const double* u, double* w, int nfields, semb_scalars* scal, bool want_dot, const ax_pcg_args& pcg, cudaStream_t s)
+template <typename ST>
+static int axhelm_dispatch(semb_mesh* h, const ST* geo, int mode, double lambda, const double* lam0, const double* lam1,
+                           const ST* u, ST* w, int nfields, semb_scalars* scal, bool want_dot, const ax_pcg_args_t<ST>& pcg, cudaStream_t s)
 {
+    if (sizeof(ST) < 8 && (mode & 2)) return semb_fail(h, SEMB_EINVAL, "axhelm: coefficient fields need fp64 storage");
     if (scal && nfields != 1) return semb_fail(h, SEMB_EINVAL, "axhelm: fused p.Ap needs nfields == 1");
     if (scal && want_dot && !h->ax_dot) {
         h->ax_dot = (double*)semb_dev_alloc(h, sizeof(double) * (size_t)h->E);
         if (!h->ax_dot) return semb_fail(h, SEMB_ENOMEM, "axhelm: p.Ap partials");
     }
     switch (h->n1) {
-        case 2:  return launch_line<2>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
-        case 3:  return launch_line<3>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
-        case 4:  return launch_line<4>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
-        case 5:  return launch_line<5>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
-        case 6:  return launch_line<6>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
-        case 7:  return launch_line<7>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
-        case 8:  return launch_line<8>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
-        case 9:  return launch_line<9>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
-        case 10: return launch_line<10>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
-        case 11: return launch_line<11>(h, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
+        case 2:  return launch_line<2, ST>(h, geo, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
+        case 3:  return launch_line<3, ST>(h, geo, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
+        case 4:  return launch_line<4, ST>(h, geo, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
+        case 5:  return launch_line<5, ST>(h, geo, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
+        case 6:  return launch_line<6, ST>(h, geo, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
+        case 7:  return launch_line<7, ST>(h, geo, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
+        case 8:  return launch_line<8, ST>(h, geo, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
+        case 9:  return launch_line<9, ST>(h, geo, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
+        case 10: return launch_line<10, ST>(h, geo, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
+        case 11: return launch_line<11, ST>(h, geo, mode, lambda, lam0, lam1, u, w, nfields, scal, want_dot, pcg, s);
     }
     return semb_fail(h, SEMB_EINVAL, "unsupported order N=%d", h->N);
 }
@@ -111,7 +114,7 @@ int semb_axhelm_launch(semb_mesh* h, double lambda, const double* lam0, const do
                        const double* u, double* w, int nfields, semb_scalars* scal, cudaStream_t s)
 {
     const int mode = (lam0 || lam1) ? 3 : (lambda != 0.0) ? 1 : 0;
-    return axhelm_dispatch(h, mode, lambda, lam0, lam1, u, w, nfields, scal, scal != nullptr, ax_pcg_args{nullptr, nullptr, nullptr, nullptr, 1.0, 0}, s);
+    return axhelm_dispatch<double>(h, h->geoK, mode, lambda, lam0, lam1, u, w, nfields, scal, scal != nullptr, ax_pcg_args{nullptr, nullptr, nullptr, nullptr, 1.0, 0}, s);
 }
 
 // PCG-fused form (pcg.cu): x += alpha p_old (if pending), p = dinv o zsrc + beta p_old, q = A_L p, partial p.q;
@@ -120,7 +123,7 @@ int semb_axhelm_pcg_launch(semb_mesh* h, double lambda, const double* zsrc, cons
                            double* q, semb_scalars* scal, cudaStream_t s)
 {
     const int mode = 4 | ((lambda != 0.0) ? 1 : 0);
-    return axhelm_dispatch(h, mode, lambda, nullptr, nullptr, nullptr, q, 1, scal, true, ax_pcg_args{zsrc, dinv, p, x, 1.0, 0}, s);
+    return axhelm_dispatch<double>(h, h->geoK, mode, lambda, nullptr, nullptr, nullptr, q, 1, scal, true, ax_pcg_args{zsrc, dinv, p, x, 1.0, 0}, s);
 }
 
 // First Chebyshev step fused into the operator (pcg.cu: cheb_apply): d = (dinv o r) * scale, written to d, Ad = A_L d.
@@ -129,5 +132,18 @@ int semb_axhelm_scaled_launch(semb_mesh* h, double lambda, const double* r, cons
                               double* Ad, semb_scalars* scal, cudaStream_t s)
 {
     const int mode = 4 | ((lambda != 0.0) ? 1 : 0);
-    return axhelm_dispatch(h, mode, lambda, nullptr, nullptr, nullptr, Ad, 1, scal, false, ax_pcg_args{r, dinv, d, nullptr, scale, 1}, s);
+    return axhelm_dispatch<double>(h, h->geoK, mode, lambda, nullptr, nullptr, nullptr, Ad, 1, scal, false, ax_pcg_args{r, dinv, d, nullptr, scale, 1}, s);
+}
+
+// ---- fp32-storage variants for the multigrid levels (geo: float copy of the level's factors, [E][7][Np])
+int semb_axhelm_launch_f(semb_mesh* h, double lambda, const float* geo, const float* u, float* w, semb_scalars* scal, cudaStream_t s)
+{
+    const int mode = (lambda != 0.0) ? 1 : 0;
+    return axhelm_dispatch<float>(h, geo, mode, lambda, nullptr, nullptr, u, w, 1, scal, false, ax_pcg_args_t<float>{nullptr, nullptr, nullptr, nullptr, 1.0, 0}, s);
+}
+int semb_axhelm_scaled_launch_f(semb_mesh* h, double lambda, const float* geo, const float* r, const float* dinv, double scale, float* d,
+                                float* Ad, semb_scalars* scal, cudaStream_t s)
+{
+    const int mode = 4 | ((lambda != 0.0) ? 1 : 0);
+    return axhelm_dispatch<float>(h, geo, mode, lambda, nullptr, nullptr, nullptr, Ad, 1, scal, false, ax_pcg_args_t<float>{r, dinv, d, nullptr, scale, 1}, s);
 }

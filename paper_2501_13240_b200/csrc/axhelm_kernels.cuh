@@ -177,14 +177,16 @@ __device__ __forceinline__ void ax_line(const double (&x)[n1], double (&y)[n1])
 // u.w to dot_out[b] (fixed summation order; reduced by k_ax_dot_finish).
 // plain != 0 (first Chebyshev step): no recurrence, p = (dinv o zsrc) * scale is written to p_io and the operator is
 // applied to it; x, alpha, beta are not touched.
-struct ax_pcg_args { const double* zsrc; const double* dinv; double* p_io; double* x; double scale; int plain; };
+template <typename ST> struct ax_pcg_args_t { const ST* zsrc; const ST* dinv; ST* p_io; ST* x; double scale; int plain; };
+typedef ax_pcg_args_t<double> ax_pcg_args;
 
 // L2 prefetch of one contiguous run of doubles (TMA unit, no destination in the SM):
 // cp.async.bulk.prefetch.L2 needs a 16-byte aligned address and size; runs that are only 8-byte aligned (odd n1)
 // are widened inward to the aligned part.  Issued by ONE thread.
-__device__ __forceinline__ void ax_prefetch_l2(const double* ptr, int count)
+template <typename ST>
+__device__ __forceinline__ void ax_prefetch_l2(const ST* ptr, int count)
 {
-    uintptr_t a = (uintptr_t)ptr, b = a + (size_t)count * 8;
+    uintptr_t a = (uintptr_t)ptr, b = a + (size_t)count * sizeof(ST);
     a = (a + 15) & ~(uintptr_t)15; b &= ~(uintptr_t)15;
     if (b > a) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" :: "l"(a), "r"((unsigned)(b - a)) : "memory");
 }
@@ -192,12 +194,14 @@ __device__ __forceinline__ void ax_prefetch_l2(const double* ptr, int count)
 // EPB elements per block (small orders: a block of n1^2 = 4, 9 or 16 threads per element cannot fill an SM -- the
 // N = 1 level of the multigrid ran at 1 TB/s): thread group el = tl / n1^2 works on element
 // blockIdx.x * EPB + el with its own shared-memory tiles; groups past the end recompute the last element and write nothing.
-template <int n1, int MODE, int MINB, int EPB>
+// ST: STORAGE type of the vectors and geometric factors in global memory (double, or float for the multigrid levels:
+// PAPER.md:L102 runs the preconditioner in FP32 "to save on memory bandwidth"); the arithmetic is fp64 either way.
+template <int n1, int MODE, int MINB, int EPB, typename ST>
 __global__ void __launch_bounds__(n1 * n1 * EPB, MINB)
-k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambda,
+k_axhelm_line(int64_t E, int64_t n, const ST* __restrict__ geo, double lambda,
               const double* __restrict__ lam0, const double* __restrict__ lam1,
-              const double* __restrict__ u, double* __restrict__ w,
-              const semb_scalars* __restrict__ scal, double* __restrict__ dot_out, ax_pcg_args pcg, int pf_dist, int nfields)
+              const ST* __restrict__ u, ST* __restrict__ w,
+              const semb_scalars* __restrict__ scal, double* __restrict__ dot_out, ax_pcg_args_t<ST> pcg, int pf_dist, int nfields)
 {
     constexpr int n2 = n1 * n1, Np = n1 * n1 * n1;
     constexpr bool HELM = MODE & 1, VAR = MODE & 2, FUSE = MODE & 4;
@@ -231,8 +235,8 @@ k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambd
         if (VAR && lam0) ax_prefetch_l2(lam0 + ep * Np, Np);
         if (VAR && lam1) ax_prefetch_l2(lam1 + ep * Np, Np);
     }
-    double* __restrict__ we = w + f * n + e * Np + tl;
-    const double* __restrict__ g = geo + e * 7 * (int64_t)Np + tl;
+    ST* __restrict__ we = w + f * n + e * Np + tl;
+    const ST* __restrict__ g = geo + e * 7 * (int64_t)Np + tl;
     double ru[n1], G[NG][n1];
     if (FUSE) {
         const int64_t l0 = e * Np + tl;
@@ -241,10 +245,10 @@ k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambd
         const bool pend = !plain && scal->x_pending != 0, first = plain || (beta == 0.0);
         double z[n1], po[n1];
 #pragma unroll
-        for (int k = 0; k < n1; ++k) z[k] = pcg.zsrc[l0 + k * n2];
+        for (int k = 0; k < n1; ++k) z[k] = semb_wide(pcg.zsrc[l0 + k * n2]);
         if (pcg.dinv) {
 #pragma unroll
-            for (int k = 0; k < n1; ++k) z[k] *= pcg.dinv[l0 + k * n2];
+            for (int k = 0; k < n1; ++k) z[k] *= semb_wide(pcg.dinv[l0 + k * n2]);
         }
         if (plain) {
 #pragma unroll
@@ -252,27 +256,28 @@ k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambd
         }
         if (pend || !first) {
 #pragma unroll
-            for (int k = 0; k < n1; ++k) po[k] = pcg.p_io[l0 + k * n2];
+            for (int k = 0; k < n1; ++k) po[k] = semb_wide(pcg.p_io[l0 + k * n2]);
         }
         if (pend) {
 #pragma unroll
-            for (int k = 0; k < n1; ++k) if (valid) pcg.x[l0 + k * n2] += alpha * po[k];
+            for (int k = 0; k < n1; ++k) if (valid) pcg.x[l0 + k * n2] = (ST)(semb_wide(pcg.x[l0 + k * n2]) + alpha * po[k]);
         }
 #pragma unroll
         for (int k = 0; k < n1; ++k) {
             ru[k] = first ? z[k] : z[k] + beta * po[k];
-            if (valid) pcg.p_io[l0 + k * n2] = ru[k];
+            if (sizeof(ST) < 8) ru[k] = (double)(ST)ru[k];      // the operator is applied to the STORED (rounded) vector
+            if (valid) pcg.p_io[l0 + k * n2] = (ST)ru[k];
         }
     } else {
-        const double* __restrict__ ue = u + f * n + e * Np + tl;
+        const ST* __restrict__ ue = u + f * n + e * Np + tl;
 #pragma unroll
-        for (int k = 0; k < n1; ++k) ru[k] = ue[k * n2];
+        for (int k = 0; k < n1; ++k) ru[k] = semb_wide(ue[k * n2]);
     }
     // ---- global loads, t-line layout: lane -> consecutive nodes of plane k (coalesced 64-bit)
 #pragma unroll
     for (int k = 0; k < n1; ++k) {
 #pragma unroll
-        for (int c = 0; c < NG; ++c) G[c][k] = __ldg(g + c * Np + k * n2);
+        for (int c = 0; c < NG; ++c) G[c][k] = semb_wide(__ldg(g + c * Np + k * n2));
     }
 #pragma unroll
     for (int k = 0; k < n1; ++k) Su[T::idx(k, b, a)] = ru[k];
@@ -335,7 +340,7 @@ k_axhelm_line(int64_t E, int64_t n, const double* __restrict__ geo, double lambd
 #pragma unroll
     for (int k = 0; k < n1; ++k) {
         const double wv = wt[k] + Sr[T::idx(k, b, a)] + Ss[T::idxB(k, b, a)];
-        if (valid) { we[k * n2] = wv; dot += ru[k] * wv; }
+        if (valid) { we[k * n2] = (ST)wv; dot += ru[k] * wv; }
     }
     if (dot_out) {
         __shared__ double red[32];

@@ -4,23 +4,33 @@
 // index and writes the sum back to every copy, so the result is deterministic.
 #include "semb_internal.h"
 
+// ST: storage type of the vector (double; float on the fp32 multigrid levels); sums in fp64
+template <typename ST>
 __global__ void k_gs(int64_t n_gs, int64_t n, const int32_t* __restrict__ off, const int32_t* __restrict__ ids,
-                     double* __restrict__ w)
+                     ST* __restrict__ w)
 {
     const int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (g >= n_gs) return;
-    double* __restrict__ wf = w + blockIdx.y * n;
+    ST* __restrict__ wf = w + blockIdx.y * n;
     const int32_t a = off[g], b = off[g + 1];
     double s = 0.0;
-    for (int32_t t = a; t < b; ++t) s += wf[ids[t]];
-    for (int32_t t = a; t < b; ++t) wf[ids[t]] = s;
+    for (int32_t t = a; t < b; ++t) s += semb_wide(wf[ids[t]]);
+    for (int32_t t = a; t < b; ++t) wf[ids[t]] = (ST)s;
 }
 
 int semb_gs_launch(semb_mesh* h, double* w, int nfields, cudaStream_t s)
 {
     if (h->n_gs == 0) return SEMB_OK;
     dim3 grid((unsigned)((h->n_gs + 255) / 256), (unsigned)nfields);
-    k_gs<<<grid, 256, 0, s>>>(h->n_gs, h->n, h->gs_off, h->gs_ids, w);
+    k_gs<double><<<grid, 256, 0, s>>>(h->n_gs, h->n, h->gs_off, h->gs_ids, w);
+    h->launches += 1;
+    SEMB_CUDA(h, cudaGetLastError());
+    return SEMB_OK;
+}
+int semb_gs_launch_f(semb_mesh* h, float* w, cudaStream_t s)
+{
+    if (h->n_gs == 0) return SEMB_OK;
+    k_gs<float><<<(unsigned)((h->n_gs + 255) / 256), 256, 0, s>>>(h->n_gs, h->n, h->gs_off, h->gs_ids, w);
     h->launches += 1;
     SEMB_CUDA(h, cudaGetLastError());
     return SEMB_OK;
@@ -28,8 +38,9 @@ int semb_gs_launch(semb_mesh* h, double* w, int nfields, cudaStream_t s)
 
 // The same sum for the listed classes only (those with >= 3 members: element edges and corners).  The fused PCG /
 // Chebyshev updates (pcg.cu) do the remaining classes -- one partner each -- in gather form.
+template <typename ST>
 __global__ void k_gs_hi(int64_t n_hi, const int32_t* __restrict__ hi, const int32_t* __restrict__ off,
-                        const int32_t* __restrict__ ids, double* __restrict__ w, const semb_scalars* __restrict__ scal)
+                        const int32_t* __restrict__ ids, ST* __restrict__ w, const semb_scalars* __restrict__ scal)
 {
     if (scal && *(volatile const int32_t*)&scal->done) return;
     const int64_t q = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
@@ -37,30 +48,47 @@ __global__ void k_gs_hi(int64_t n_hi, const int32_t* __restrict__ hi, const int3
     const int32_t g = hi[q];
     const int32_t a = off[g], b = off[g + 1];
     double s = 0.0;
-    for (int32_t t = a; t < b; ++t) s += w[ids[t]];
-    for (int32_t t = a; t < b; ++t) w[ids[t]] = s;
+    for (int32_t t = a; t < b; ++t) s += semb_wide(w[ids[t]]);
+    for (int32_t t = a; t < b; ++t) w[ids[t]] = (ST)s;
 }
 
 int semb_gs_hi_launch(semb_mesh* h, double* w, const semb_scalars* scal, cudaStream_t s)
 {
     if (h->n_gs_hi == 0) return SEMB_OK;
-    k_gs_hi<<<(unsigned)((h->n_gs_hi + 255) / 256), 256, 0, s>>>(h->n_gs_hi, h->gs_hi, h->gs_off, h->gs_ids, w, scal);
+    k_gs_hi<double><<<(unsigned)((h->n_gs_hi + 255) / 256), 256, 0, s>>>(h->n_gs_hi, h->gs_hi, h->gs_off, h->gs_ids, w, scal);
+    h->launches += 1;
+    SEMB_CUDA(h, cudaGetLastError());
+    return SEMB_OK;
+}
+int semb_gs_hi_launch_f(semb_mesh* h, float* w, const semb_scalars* scal, cudaStream_t s)
+{
+    if (h->n_gs_hi == 0) return SEMB_OK;
+    k_gs_hi<float><<<(unsigned)((h->n_gs_hi + 255) / 256), 256, 0, s>>>(h->n_gs_hi, h->gs_hi, h->gs_off, h->gs_ids, w, scal);
     h->launches += 1;
     SEMB_CUDA(h, cudaGetLastError());
     return SEMB_OK;
 }
 
-__global__ void k_mask(int64_t c, int64_t n, const int32_t* __restrict__ list, double* __restrict__ w)
+template <typename ST>
+__global__ void k_mask(int64_t c, int64_t n, const int32_t* __restrict__ list, ST* __restrict__ w)
 {
     const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (t < c) w[blockIdx.y * n + list[t]] = 0.0;
+    if (t < c) w[blockIdx.y * n + list[t]] = (ST)0;
 }
 
 int semb_mask_launch(semb_mesh* h, const semb_mask_entry& m, double* w, int nfields, cudaStream_t s)
 {
     if (m.count == 0) return SEMB_OK;
     dim3 grid((unsigned)((m.count + 255) / 256), (unsigned)nfields);
-    k_mask<<<grid, 256, 0, s>>>(m.count, h->n, m.list, w);
+    k_mask<double><<<grid, 256, 0, s>>>(m.count, h->n, m.list, w);
+    h->launches += 1;
+    SEMB_CUDA(h, cudaGetLastError());
+    return SEMB_OK;
+}
+int semb_mask_launch_f(semb_mesh* h, const semb_mask_entry& m, float* w, cudaStream_t s)
+{
+    if (m.count == 0) return SEMB_OK;
+    k_mask<float><<<(unsigned)((m.count + 255) / 256), 256, 0, s>>>(m.count, h->n, m.list, w);
     h->launches += 1;
     SEMB_CUDA(h, cudaGetLastError());
     return SEMB_OK;

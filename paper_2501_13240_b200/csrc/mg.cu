@@ -27,6 +27,14 @@ struct semb_mg {
     double* rc[8] = {nullptr};           // level l >= 1: restricted residual
     double* ec[8] = {nullptr};           // level l >= 1: coarse correction
     std::map<std::pair<uint32_t, double>, std::array<double, 8>> lmax_cache;
+    // fp32-storage levels (mg_fp32): float copies of the level data and float work vectors, built on first use
+    bool f32_ready = false;
+    float* geoF[8] = {nullptr};          // [E][7][Np]
+    float* invmultF[8] = {nullptr};
+    float* WF[8][5] = {{nullptr}};       // Chebyshev work (res, d, Ad), residual, scratch
+    float* rF[8] = {nullptr};            // level l: right-hand side (level 0: the converted PCG residual)
+    float* zF[8] = {nullptr};            // level l: result
+    std::map<std::pair<uint32_t, double>, std::array<float*, 8>> dinvF;   // per (tags, lambda), owned
 };
 
 // J[(Nto+1) x (Nfrom+1)]: Lagrange basis of the order-Nfrom GLL nodes at the order-Nto GLL nodes (product formula;
@@ -51,10 +59,10 @@ static void interp_matrix_host(int Nfrom, int Nto, double* J)
 #define MG_MAXNP (SEMB_MAXN1 * SEMB_MAXN1 * SEMB_MAXN1)
 // NIN, NOUT > 0: compile-time sizes (the pairs the default hierarchies use; index arithmetic and the inner loops
 // unroll); NIN = NOUT = 0: run-time sizes nin, nout.
-template <int NIN, int NOUT>
+template <int NIN, int NOUT, typename ST>
 __global__ void __launch_bounds__(128)
-k_interp3(int nin_rt, int nout_rt, const double* __restrict__ J, int transpose, const double* __restrict__ in,
-          const double* __restrict__ scale, double* __restrict__ out, int accumulate, const semb_scalars* __restrict__ scal)
+k_interp3(int nin_rt, int nout_rt, const double* __restrict__ J, int transpose, const ST* __restrict__ in,
+          const ST* __restrict__ scale, ST* __restrict__ out, int accumulate, const semb_scalars* __restrict__ scal)
 {
     constexpr int SZ = (NIN > 0) ? ((NIN > NOUT ? NIN : NOUT) * (NIN > NOUT ? NIN : NOUT) * (NIN > NOUT ? NIN : NOUT)) : MG_MAXNP;
     constexpr int SJ = (NIN > 0) ? NIN * NOUT : SEMB_MAXN1 * SEMB_MAXN1;
@@ -68,8 +76,8 @@ k_interp3(int nin_rt, int nout_rt, const double* __restrict__ J, int transpose, 
         Js[t] = transpose ? J[a * nout + o] : J[o * nin + a];
     }
     for (int t = threadIdx.x; t < npi; t += blockDim.x) {
-        const double v = in[e * npi + t];
-        A[t] = scale ? v * scale[e * npi + t] : v;
+        const double v = semb_wide(in[e * npi + t]);
+        A[t] = scale ? v * semb_wide(scale[e * npi + t]) : v;
     }
     __syncthreads();
     // pass 1 (i): B[c][b][i] = sum_a Js[i][a] A[c][b][a]
@@ -96,18 +104,19 @@ k_interp3(int nin_rt, int nout_rt, const double* __restrict__ J, int transpose, 
         double s = 0.0;
 #pragma unroll
         for (int c = 0; c < nin; ++c) s += Js[k * nin + c] * A[c * nout * nout + ji];
-        if (accumulate) out[e * npo + t] += s; else out[e * npo + t] = s;
+        if (accumulate) out[e * npo + t] = (ST)(semb_wide(out[e * npo + t]) + s); else out[e * npo + t] = (ST)s;
     }
 }
 
-static void interp3_launch(int64_t E, int nin, int nout, const double* J, int transpose, const double* in, const double* scale,
-                           double* out, int accumulate, const semb_scalars* scal, cudaStream_t s)
+template <typename ST>
+static void interp3_launch(int64_t E, int nin, int nout, const double* J, int transpose, const ST* in, const ST* scale,
+                           ST* out, int accumulate, const semb_scalars* scal, cudaStream_t s)
 {
-#define MG_CASE(A_, B_) if (nin == A_ && nout == B_) { k_interp3<A_, B_><<<(unsigned)E, 128, 0, s>>>(nin, nout, J, transpose, in, scale, out, accumulate, scal); return; }
+#define MG_CASE(A_, B_) if (nin == A_ && nout == B_) { k_interp3<A_, B_, ST><<<(unsigned)E, 128, 0, s>>>(nin, nout, J, transpose, in, scale, out, accumulate, scal); return; }
     MG_CASE(8, 4) MG_CASE(4, 8) MG_CASE(4, 2) MG_CASE(2, 4) MG_CASE(10, 6) MG_CASE(6, 10) MG_CASE(6, 4) MG_CASE(4, 6)
     MG_CASE(8, 2) MG_CASE(10, 4) MG_CASE(10, 2) MG_CASE(6, 2) MG_CASE(2, 6) MG_CASE(8, 6) MG_CASE(6, 8)
 #undef MG_CASE
-    k_interp3<0, 0><<<(unsigned)E, 128, 0, s>>>(nin, nout, J, transpose, in, scale, out, accumulate, scal);
+    k_interp3<0, 0, ST><<<(unsigned)E, 128, 0, s>>>(nin, nout, J, transpose, in, scale, out, accumulate, scal);
 }
 
 // u ~ U[-1,1) per local node from the counter-based splitmix64 of the input recipe (R19)
@@ -129,8 +138,11 @@ static void mg_free(semb_mesh* h, semb_mg* g)
     for (int l = 0; l < 8; ++l) {
         semb_dev_free(h, g->J[l]); semb_dev_free(h, g->rc[l]); semb_dev_free(h, g->ec[l]);
         for (int w = 0; w < 6; ++w) semb_dev_free(h, g->W[l][w]);
+        for (int w = 0; w < 5; ++w) semb_dev_free(h, g->WF[l][w]);
+        semb_dev_free(h, g->geoF[l]); semb_dev_free(h, g->invmultF[l]); semb_dev_free(h, g->rF[l]); semb_dev_free(h, g->zF[l]);
         if (l >= 1 && g->lev[l]) semb_destroy(g->lev[l]);
     }
+    for (auto& kv : g->dinvF) for (float* p : kv.second) semb_dev_free(h, p);
     delete g;
 }
 void semb_mg_destroy_all(semb_mesh* h)
@@ -159,7 +171,7 @@ static int mg_build(semb_mesh* h, int nlevels, const int* orders, semb_mg** out,
             interp_matrix_host(h->N, orders[l], Jh);                                  // [nc1][n1]
             if (cudaMemcpyAsync(Jd, Jh, sizeof(double) * nc1 * h->n1, cudaMemcpyHostToDevice, s) != cudaSuccess) rc = semb_fail(h, SEMB_ECUDA, "multigrid: upload");
             for (int c = 0; c < 3 && !rc; ++c)
-                interp3_launch(h->E, h->n1, nc1, Jd, 0, h->xyz + c * h->n, nullptr, xyz + c * nl, 0, nullptr, s);
+                interp3_launch<double>(h->E, h->n1, nc1, Jd, 0, h->xyz + c * h->n, nullptr, xyz + c * nl, 0, nullptr, s);
             if (!rc && cudaStreamSynchronize(s) != cudaSuccess) rc = semb_fail(h, SEMB_ECUDA, "multigrid: coordinate interpolation: %s", cudaGetErrorString(cudaGetLastError()));
             if (!rc) {
                 rc = semb_setup(h->E, orders[l], xyz, xyz + nl, xyz + 2 * nl, h->face_tag.data(), h->period,
@@ -222,6 +234,7 @@ int semb_mg_prepare(semb_mesh* h, const semb_pcg_opts* o, semb_mg_ctx* ctx, cuda
     ctx->k_smooth = o->mg_smooth_degree > 0 ? o->mg_smooth_degree : 1;
     ctx->k_coarse = o->mg_coarse_degree > 0 ? o->mg_coarse_degree : 32;
     ctx->kind = (o->mg_smoother_kind == 4) ? 4 : 1;
+    ctx->fp32 = o->mg_fp32 ? 1 : 0;
     if (ctx->k_smooth > SEMB_MAX_CHEB || ctx->k_coarse > SEMB_MAX_CHEB) return semb_fail(h, SEMB_EINVAL, "multigrid: smoother degree > %d", SEMB_MAX_CHEB);
     ctx->coarse_frac = (o->mg_coarse_lmin_frac > 0.0 && o->mg_coarse_lmin_frac < 1.0) ? o->mg_coarse_lmin_frac : 0.01;
     // Chebyshev bounds per level: given, cached, or estimated (10-step Lanczos x 1.1 from M QQ^T B 1)
@@ -270,12 +283,12 @@ int semb_mg_transfer_run(semb_mesh* h, const semb_mg_ctx& ctx, int l, int restri
     semb_mesh* F = g->lev[l]; semb_mesh* C = g->lev[l + 1];
     semb_mask_entry m;
     if (!restrict_) {
-        interp3_launch(F->E, C->n1, F->n1, g->J[l], 0, in, nullptr, out, 0, nullptr, s);
+        interp3_launch<double>(F->E, C->n1, F->n1, g->J[l], 0, in, nullptr, out, 0, nullptr, s);
         int rc = semb_get_mask(F, ctx.tags, &m, s); if (rc) return rc;
         h->launches += 1;
         return semb_mask_launch(F, m, out, 1, s);
     }
-    interp3_launch(F->E, F->n1, C->n1, g->J[l], 1, in, F->invmult, out, 0, nullptr, s);
+    interp3_launch<double>(F->E, F->n1, C->n1, g->J[l], 1, in, (const double*)F->invmult, out, 0, nullptr, s);
     h->launches += 1;
     int rc = semb_gs_launch(C, out, 1, s); if (rc) return rc;
     rc = semb_get_mask(C, ctx.tags, &m, s); if (rc) return rc;
@@ -283,8 +296,10 @@ int semb_mg_transfer_run(semb_mesh* h, const semb_mg_ctx& ctx, int l, int restri
 }
 
 // z = V(level, r).  scal (may be NULL): the PCG scalars of the fine handle, only read for the early exit.
+static int mg_vcycle_f32_top(semb_mesh* h, const semb_mg_ctx& ctx, const double* r, double* z, semb_scalars* scal, cudaStream_t s);
 int semb_mg_vcycle_run(semb_mesh* h, const semb_mg_ctx& ctx, int l, const double* r, double* z, semb_scalars* scal, cudaStream_t s)
 {
+    if (ctx.fp32 && l == 0) return mg_vcycle_f32_top(h, ctx, r, z, scal, s);
     semb_mg* g = ctx.mg;
     semb_mesh* L = g->lev[l];
     const int64_t n = L->n;
@@ -304,17 +319,113 @@ int semb_mg_vcycle_run(semb_mesh* h, const semb_mg_ctx& ctx, int l, const double
     rc = semb_get_mask(C, ctx.tags, &mc, s); if (rc) return rc;
     rc = semb_cheb_apply(L, ctx.lambda, m, dinv, ctx.k_smooth, cc, r, z, cres, cd, cAd, scal, false, s); if (rc) return rc;   // z = S r
     rc = semb_residual_launch(L, ctx.lambda, m, z, r, res, t1, scal, s); if (rc) return rc;                                  // res = r - A z
-    interp3_launch(L->E, L->n1, C->n1, g->J[l], 1, res, L->invmult, g->rc[l + 1], 0, scal, s);               // R res
+    interp3_launch<double>(L->E, L->n1, C->n1, g->J[l], 1, res, (const double*)L->invmult, g->rc[l + 1], 0, scal, s);               // R res
     rc = semb_gs_launch(C, g->rc[l + 1], 1, s); if (rc) return rc;
     rc = semb_mask_launch(C, mc, g->rc[l + 1], 1, s); if (rc) return rc;
     const int64_t lc0 = C->launches;
     rc = semb_mg_vcycle_run(h, ctx, l + 1, g->rc[l + 1], g->ec[l + 1], scal, s); if (rc) return rc;
     (void)lc0;
-    interp3_launch(L->E, C->n1, L->n1, g->J[l], 0, g->ec[l + 1], nullptr, z, 1, scal, s);                    // z += P e
+    interp3_launch<double>(L->E, C->n1, L->n1, g->J[l], 0, (const double*)g->ec[l + 1], (const double*)nullptr, z, 1, scal, s);                    // z += P e
     rc = semb_residual_launch(L, ctx.lambda, m, z, r, res, t1, scal, s); if (rc) return rc;                                  // res = r - A z
     rc = semb_cheb_apply(L, ctx.lambda, m, dinv, ctx.k_smooth, cc, res, z, cres, cd, cAd, scal, false, s, true); if (rc) return rc; // z += S res
     L->launches += 2;
     if (L != h) h->launches += L->launches - l0;
+    SEMB_CUDA(h, cudaGetLastError());
+    return SEMB_OK;
+}
+
+
+// ---- fp32-storage levels (the preconditioner runs in FP32 "to save on memory bandwidth").  Vectors and
+// geometric factors of every level live in float, every kernel computes in fp64 registers and rounds at its stores.
+template <typename TI, typename TO>
+__global__ void k_mg_convert(int64_t n, const TI* __restrict__ in, TO* __restrict__ out, const semb_scalars* __restrict__ scal)
+{
+    if (scal && *(volatile const int32_t*)&scal->done) return;
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) out[l] = (TO)in[l];
+}
+
+static int mg_f32_prepare(semb_mesh* h, const semb_mg_ctx& ctx, cudaStream_t s)
+{
+    semb_mg* g = ctx.mg;
+    if (!g->f32_ready) {
+        for (int l = 0; l < g->nlevels; ++l) {
+            semb_mesh* L = g->lev[l];
+            const int64_t n = L->n, ng = L->E * 7 * L->Np;
+            g->geoF[l] = (float*)semb_dev_alloc(h, sizeof(float) * (size_t)ng);
+            g->invmultF[l] = (float*)semb_dev_alloc(h, sizeof(float) * (size_t)n);
+            g->rF[l] = (float*)semb_dev_alloc(h, sizeof(float) * (size_t)n);
+            g->zF[l] = (float*)semb_dev_alloc(h, sizeof(float) * (size_t)n);
+            bool ok = g->geoF[l] && g->invmultF[l] && g->rF[l] && g->zF[l];
+            for (int w = 0; w < 5; ++w) { g->WF[l][w] = (float*)semb_dev_alloc(h, sizeof(float) * (size_t)n); ok = ok && g->WF[l][w]; }
+            if (!ok) return semb_fail(h, SEMB_ENOMEM, "multigrid: fp32 data of level %d", l);
+            k_mg_convert<double, float><<<mg_grid(ng), 256, 0, s>>>(ng, L->geo, g->geoF[l], nullptr);
+            k_mg_convert<double, float><<<mg_grid(n), 256, 0, s>>>(n, L->invmult, g->invmultF[l], nullptr);
+        }
+        SEMB_CUDA(h, cudaGetLastError());
+        g->f32_ready = true;
+    }
+    const std::pair<uint32_t, double> key(ctx.tags, ctx.lambda);
+    if (g->dinvF.find(key) == g->dinvF.end()) {
+        std::array<float*, 8> a{};
+        for (int l = 0; l < g->nlevels; ++l) {
+            semb_mesh* L = g->lev[l];
+            double* dinv;
+            int rc = semb_get_dinv(L, ctx.lambda, ctx.tags, &dinv, s); if (rc) return rc;
+            a[l] = (float*)semb_dev_alloc(h, sizeof(float) * (size_t)L->n);
+            if (!a[l]) return semb_fail(h, SEMB_ENOMEM, "multigrid: fp32 diagonal of level %d", l);
+            k_mg_convert<double, float><<<mg_grid(L->n), 256, 0, s>>>(L->n, dinv, a[l], nullptr);
+        }
+        SEMB_CUDA(h, cudaGetLastError());
+        g->dinvF[key] = a;
+    }
+    return SEMB_OK;
+}
+
+static int mg_vcycle_f32(semb_mesh* h, const semb_mg_ctx& ctx, int l, const float* r, float* z, semb_scalars* scal, cudaStream_t s)
+{
+    semb_mg* g = ctx.mg;
+    semb_mesh* L = g->lev[l];
+    semb_mask_entry m;
+    int rc = semb_get_mask(L, ctx.tags, &m, s); if (rc) return rc;
+    const float* dinv = g->dinvF[std::pair<uint32_t, double>(ctx.tags, ctx.lambda)][l];
+    const float* geo = g->geoF[l];
+    float *cres = g->WF[l][0], *cd = g->WF[l][1], *cAd = g->WF[l][2], *res = g->WF[l][3], *t1 = g->WF[l][4];
+    const int64_t l0 = L->launches;
+    if (l == g->nlevels - 1) {
+        rc = semb_cheb_apply_f(L, ctx.lambda, geo, m, dinv, ctx.k_coarse, semb_cheb_coefficients(ctx.k_coarse, ctx.lmax[l], ctx.kind, ctx.coarse_frac),
+                               r, z, cres, cd, cAd, scal, s, false);
+        if (L != h) h->launches += L->launches - l0;
+        return rc;
+    }
+    const semb_cheb_coef cc = semb_cheb_coefficients(ctx.k_smooth, ctx.lmax[l], ctx.kind);
+    semb_mesh* C = g->lev[l + 1];
+    semb_mask_entry mc;
+    rc = semb_get_mask(C, ctx.tags, &mc, s); if (rc) return rc;
+    rc = semb_cheb_apply_f(L, ctx.lambda, geo, m, dinv, ctx.k_smooth, cc, r, z, cres, cd, cAd, scal, s, false); if (rc) return rc;   // z = S r
+    rc = semb_residual_launch_f(L, ctx.lambda, geo, m, z, r, res, t1, scal, s); if (rc) return rc;                                  // res = r - A z
+    interp3_launch<float>(L->E, L->n1, C->n1, g->J[l], 1, res, g->invmultF[l], g->rF[l + 1], 0, scal, s);                           // R res
+    rc = semb_gs_launch_f(C, g->rF[l + 1], s); if (rc) return rc;
+    rc = semb_mask_launch_f(C, mc, g->rF[l + 1], s); if (rc) return rc;
+    rc = mg_vcycle_f32(h, ctx, l + 1, g->rF[l + 1], g->zF[l + 1], scal, s); if (rc) return rc;
+    interp3_launch<float>(L->E, C->n1, L->n1, g->J[l], 0, (const float*)g->zF[l + 1], (const float*)nullptr, z, 1, scal, s);        // z += P e
+    rc = semb_residual_launch_f(L, ctx.lambda, geo, m, z, r, res, t1, scal, s); if (rc) return rc;                                  // res = r - A z
+    rc = semb_cheb_apply_f(L, ctx.lambda, geo, m, dinv, ctx.k_smooth, cc, res, z, cres, cd, cAd, scal, s, true); if (rc) return rc; // z += S res
+    L->launches += 2;
+    if (L != h) h->launches += L->launches - l0;
+    SEMB_CUDA(h, cudaGetLastError());
+    return SEMB_OK;
+}
+
+// double in, double out, fp32 storage inside
+static int mg_vcycle_f32_top(semb_mesh* h, const semb_mg_ctx& ctx, const double* r, double* z, semb_scalars* scal, cudaStream_t s)
+{
+    semb_mg* g = ctx.mg;
+    int rc = mg_f32_prepare(h, ctx, s); if (rc) return rc;
+    const int64_t n = h->n;
+    k_mg_convert<double, float><<<mg_grid(n), 256, 0, s>>>(n, r, g->rF[0], scal);
+    rc = mg_vcycle_f32(h, ctx, 0, g->rF[0], g->zF[0], scal, s); if (rc) return rc;
+    k_mg_convert<float, double><<<mg_grid(n), 256, 0, s>>>(n, g->zF[0], z, scal);
+    h->launches += 2;
     SEMB_CUDA(h, cudaGetLastError());
     return SEMB_OK;
 }

@@ -41,10 +41,11 @@ __device__ __forceinline__ void gs_codes(const gs_lists& L, int64_t l0, int64_t 
     for (int u = 0; u < GS_U; ++u) { const int64_t l = l0 + u * VEC_BLOCK; c[u] = (l < n) ? __ldg(L.code + l) : -1; }
 }
 // own[u] = q at the node itself (already loaded by the caller, coalesced)
-__device__ __forceinline__ void gs_partners(const double* __restrict__ q, const int32_t (&c)[GS_U], double (&pv)[GS_U])
+template <typename ST>
+__device__ __forceinline__ void gs_partners(const ST* __restrict__ q, const int32_t (&c)[GS_U], double (&pv)[GS_U])
 {
 #pragma unroll
-    for (int u = 0; u < GS_U; ++u) pv[u] = (c[u] <= -2) ? q[-(c[u] + 2)] : 0.0;
+    for (int u = 0; u < GS_U; ++u) pv[u] = (c[u] <= -2) ? semb_wide(q[-(c[u] + 2)]) : 0.0;
 }
 __device__ __forceinline__ void gs_gathered(const int32_t (&c)[GS_U], const double (&own)[GS_U], const double (&pv)[GS_U],
                                             double (&qa)[GS_U], double (&wgt)[GS_U])
@@ -216,10 +217,10 @@ k_cheb_init(int64_t n, const double* __restrict__ r, const double* __restrict__ 
 //          formed inside the axhelm launch, semb_axhelm_scaled_launch);
 //   LAST:  z += d + d_new is final, res and d are dead and not written; with rpcg != NULL the same pass
 //          accumulates rho = <rpcg, z> and its last block sets beta (what k_dot_rz did in a pass of its own).
-template <bool FIRST, bool LAST>
+template <bool FIRST, bool LAST, typename ST>
 __global__ void __launch_bounds__(VEC_BLOCK, 3)
-k_cheb_step(int64_t n, const double* __restrict__ Ad, gs_lists L, const double* __restrict__ dinv, double c1, double c2,
-            const double* res_in, double* res, double* __restrict__ d, double* __restrict__ z,
+k_cheb_step(int64_t n, const ST* __restrict__ Ad, gs_lists L, const ST* __restrict__ dinv, double c1, double c2,
+            const ST* res_in, ST* res, ST* __restrict__ d, ST* __restrict__ z,
             const double* rpcg, semb_scalars* __restrict__ scal, double* __restrict__ partials, int zacc)
 {
     __shared__ double red[32];
@@ -239,8 +240,8 @@ k_cheb_step(int64_t n, const double* __restrict__ Ad, gs_lists L, const double* 
             const int64_t l = l0 + u * VEC_BLOCK;
             own[u] = 0.0; zl[u] = 0.0; rp[u] = 0.0;
             if (l < n) {
-                own[u] = Ad[l]; dl[u] = d[l]; rl[u] = res_in[l]; dv[u] = dinv[l];
-                if (!FIRST || zacc) zl[u] = z[l];          // zacc: the smoother's result is ADDED to the z passed in
+                own[u] = semb_wide(Ad[l]); dl[u] = semb_wide(d[l]); rl[u] = semb_wide(res_in[l]); dv[u] = semb_wide(dinv[l]);
+                if (!FIRST || zacc) zl[u] = semb_wide(z[l]);          // zacc: the smoother's result is ADDED to the z passed in
                 if (LAST && !FIRST && rpcg) rp[u] = rpcg[l];
             }
         }
@@ -252,12 +253,12 @@ k_cheb_step(int64_t n, const double* __restrict__ Ad, gs_lists L, const double* 
                 double zn = zl[u] + dl[u];
                 const double rn = rl[u] - qa[u];
                 const double dn = c1 * dl[u] + c2 * (dv[u] * rn);
-                if (!LAST) { res[l] = rn; d[l] = dn; }
+                if (!LAST) { res[l] = (ST)rn; d[l] = (ST)dn; }
                 else {
                     zn += dn;
                     if (rpcg) rz += (FIRST ? rl[u] : rp[u]) * zn * wgt[u];
                 }
-                z[l] = zn;
+                z[l] = (ST)zn;
             }
         }
     }
@@ -308,8 +309,9 @@ static int apply_A(semb_mesh* h, double lambda, const semb_mask_entry& m, const 
 }
 
 // res = r - M QQ^T A_L z  (z continuous and masked; tmp: scratch [n]): the gather-scatter in gather form as in k_update_r
+template <typename ST>
 __global__ void __launch_bounds__(VEC_BLOCK, 4)
-k_residual(int64_t n, const double* __restrict__ q, gs_lists L, const double* __restrict__ r, double* __restrict__ res,
+k_residual(int64_t n, const ST* __restrict__ q, gs_lists L, const ST* __restrict__ r, ST* __restrict__ res,
            const semb_scalars* __restrict__ scal)
 {
     if (scal && STOPPED(scal)) return;
@@ -325,14 +327,14 @@ k_residual(int64_t n, const double* __restrict__ q, gs_lists L, const double* __
 #pragma unroll
         for (int u = 0; u < GS_U; ++u) {
             const int64_t l = l0 + u * VEC_BLOCK;
-            own[u] = (l < n) ? q[l] : 0.0;
-            rv[u] = (l < n) ? r[l] : 0.0;
+            own[u] = (l < n) ? semb_wide(q[l]) : 0.0;
+            rv[u] = (l < n) ? semb_wide(r[l]) : 0.0;
         }
         gs_gathered(c, own, pv, qa, wgt);
 #pragma unroll
         for (int u = 0; u < GS_U; ++u) {
             const int64_t l = l0 + u * VEC_BLOCK;
-            if (l < n) res[l] = rv[u] - qa[u];
+            if (l < n) res[l] = (ST)(rv[u] - qa[u]);
         }
     }
 }
@@ -342,8 +344,47 @@ int semb_residual_launch(semb_mesh* h, double lambda, const semb_mask_entry& m, 
     int rc = semb_axhelm_launch(h, lambda, nullptr, nullptr, z, tmp, 1, nullptr, s); if (rc) return rc;
     rc = semb_mask_launch(h, m, tmp, 1, s); if (rc) return rc;
     rc = semb_gs_hi_launch(h, tmp, scal, s); if (rc) return rc;
-    k_residual<<<vec_grid(h->n), VEC_BLOCK, 0, s>>>(h->n, tmp, gs_lists{h->gs_code}, r, res, scal);
+    k_residual<double><<<vec_grid(h->n), VEC_BLOCK, 0, s>>>(h->n, tmp, gs_lists{h->gs_code}, r, res, scal);
     h->launches += 1;
+    SEMB_CUDA(h, cudaGetLastError());
+    return SEMB_OK;
+}
+
+// ---- fp32-storage variants for the multigrid levels (mg.cu): same kernels, float vectors, fp64 arithmetic
+int semb_residual_launch_f(semb_mesh* h, double lambda, const float* geo, const semb_mask_entry& m, const float* z, const float* r,
+                           float* res, float* tmp, semb_scalars* scal, cudaStream_t s)
+{
+    int rc = semb_axhelm_launch_f(h, lambda, geo, z, tmp, nullptr, s); if (rc) return rc;
+    rc = semb_mask_launch_f(h, m, tmp, s); if (rc) return rc;
+    rc = semb_gs_hi_launch_f(h, tmp, scal, s); if (rc) return rc;
+    k_residual<float><<<vec_grid(h->n), VEC_BLOCK, 0, s>>>(h->n, tmp, gs_lists{h->gs_code}, r, res, scal);
+    h->launches += 1;
+    SEMB_CUDA(h, cudaGetLastError());
+    return SEMB_OK;
+}
+// z (+)= Cheb_k(r), k >= 1
+int semb_cheb_apply_f(semb_mesh* h, double lambda, const float* geo, const semb_mask_entry& m, const float* dinv, int k,
+                      const semb_cheb_coef& c, const float* r, float* z, float* res, float* d, float* Ad, semb_scalars* scal,
+                      cudaStream_t s, bool zacc)
+{
+    const int64_t n = h->n; const unsigned G = vec_grid(n);
+    if (k < 1) return semb_fail(h, SEMB_EINVAL, "cheb_apply (fp32): k >= 1 required");
+    const gs_lists L{h->gs_code};
+    int rc = semb_axhelm_scaled_launch_f(h, lambda, geo, r, dinv, c.itheta, d, Ad, scal, s); if (rc) return rc;
+    for (int it = 0; it < k; ++it) {
+        if (it > 0) { rc = semb_axhelm_launch_f(h, lambda, geo, d, Ad, nullptr, s); if (rc) return rc; }
+        rc = semb_mask_launch_f(h, m, Ad, s); if (rc) return rc;
+        rc = semb_gs_hi_launch_f(h, Ad, scal, s); if (rc) return rc;
+        const bool first = (it == 0), last = (it == k - 1);
+        const float* rin = first ? r : res;
+#define SEMB_CHEB_STEP_F(F, La) k_cheb_step<F, La, float><<<G, VEC_BLOCK, 0, s>>>(n, Ad, L, dinv, c.c1[it], c.c2[it], rin, res, d, z, nullptr, scal, h->partials, zacc ? 1 : 0)
+        if (first && last) SEMB_CHEB_STEP_F(true, true);
+        else if (first)    SEMB_CHEB_STEP_F(true, false);
+        else if (last)     SEMB_CHEB_STEP_F(false, true);
+        else               SEMB_CHEB_STEP_F(false, false);
+#undef SEMB_CHEB_STEP_F
+        h->launches += 1;
+    }
     SEMB_CUDA(h, cudaGetLastError());
     return SEMB_OK;
 }
@@ -415,7 +456,7 @@ int semb_cheb_apply(semb_mesh* h, double lambda, const semb_mask_entry& m, const
         rc = semb_gs_hi_launch(h, Ad, scal, s); if (rc) return rc;      // edges and corners; faces in k_cheb_step
         const bool first = (it == 0), last = (it == k - 1);
         const double* rin = first ? r : res;
-#define SEMB_CHEB_STEP(F, La) k_cheb_step<F, La><<<G, VEC_BLOCK, 0, s>>>(n, Ad, L, dinv, c.c1[it], c.c2[it], rin, res, d, z, rp, scal, h->partials, zacc ? 1 : 0)
+#define SEMB_CHEB_STEP(F, La) k_cheb_step<F, La, double><<<G, VEC_BLOCK, 0, s>>>(n, Ad, L, dinv, c.c1[it], c.c2[it], rin, res, d, z, rp, scal, h->partials, zacc ? 1 : 0)
         if (first && last) SEMB_CHEB_STEP(true, true);
         else if (first)    SEMB_CHEB_STEP(true, false);
         else if (last)     SEMB_CHEB_STEP(false, true);

@@ -73,6 +73,14 @@ struct semb_mesh {
     std::string err;
 };
 
+// Widening of a stored value (double, or float on the fp32-storage multigrid levels) to the fp64 the kernels compute
+// in.  Measured and rejected: doing the float -> double widening with integer operations instead of F2F.F64.F32 made
+// the fp32 V-cycle 8 % SLOWER than the plain cast (cfg3: 23.2 vs 19.1 ms per iteration; fp64 storage: 21.7 ms).
+#ifdef __CUDACC__
+__device__ __forceinline__ double semb_wide(double v) { return v; }
+__device__ __forceinline__ double semb_wide(float f) { return (double)f; }
+#endif
+
 // ---- helpers -------------------------------------------------------------------------------
 int  semb_fail(semb_mesh* h, int code, const char* fmt, ...);
 void* semb_dev_alloc(semb_mesh* h, size_t bytes);
@@ -112,11 +120,18 @@ int semb_axhelm_pcg_launch(semb_mesh* h, double lambda, const double* zsrc, cons
 int semb_axhelm_scaled_launch(semb_mesh* h, double lambda, const double* r, const double* dinv, double scale, double* d,
                               double* Ad, semb_scalars* scal, cudaStream_t s);
 
+int semb_axhelm_launch_f(semb_mesh* h, double lambda, const float* geo, const float* u, float* w, semb_scalars* scal, cudaStream_t s);
+int semb_axhelm_scaled_launch_f(semb_mesh* h, double lambda, const float* geo, const float* r, const float* dinv, double scale, float* d,
+                                float* Ad, semb_scalars* scal, cudaStream_t s);
+
 // ---- gs.cu
 int semb_gs_launch(semb_mesh* h, double* w, int nfields, cudaStream_t s);
 // QQ^T restricted to the classes with >= 3 members (the rest is done in gather form by the consumer, pcg.cu)
 int semb_gs_hi_launch(semb_mesh* h, double* w, const semb_scalars* scal, cudaStream_t s);
 int semb_mask_launch(semb_mesh* h, const semb_mask_entry& m, double* w, int nfields, cudaStream_t s);
+int semb_gs_launch_f(semb_mesh* h, float* w, cudaStream_t s);
+int semb_gs_hi_launch_f(semb_mesh* h, float* w, const semb_scalars* scal, cudaStream_t s);
+int semb_mask_launch_f(semb_mesh* h, const semb_mask_entry& m, float* w, cudaStream_t s);
 
 // ---- pcg.cu
 int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* x, semb_pcg_stats* st,
@@ -139,10 +154,15 @@ int semb_cheb_apply(semb_mesh* h, double lambda, const semb_mask_entry& m, const
 // res = r - M QQ^T A_L z  (z continuous and masked; tmp: scratch [n])
 int semb_residual_launch(semb_mesh* h, double lambda, const semb_mask_entry& m, const double* z, const double* r, double* res,
                          double* tmp, semb_scalars* scal, cudaStream_t s);
+int semb_residual_launch_f(semb_mesh* h, double lambda, const float* geo, const semb_mask_entry& m, const float* z, const float* r,
+                           float* res, float* tmp, semb_scalars* scal, cudaStream_t s);
+int semb_cheb_apply_f(semb_mesh* h, double lambda, const float* geo, const semb_mask_entry& m, const float* dinv, int k,
+                      const semb_cheb_coef& c, const float* r, float* z, float* res, float* d, float* Ad, semb_scalars* scal,
+                      cudaStream_t s, bool zacc);
 int semb_dot_rz_launch(semb_mesh* h, const double* r, const double* z, semb_scalars* scal, cudaStream_t s);
 
 // ---- mg.cu: p-multigrid V-cycle
-struct semb_mg_ctx { semb_mg* mg; double lambda; uint32_t tags; int k_smooth, k_coarse, kind; double coarse_frac; double lmax[8]; };
+struct semb_mg_ctx { semb_mg* mg; double lambda; uint32_t tags; int k_smooth, k_coarse, kind, fp32; double coarse_frac; double lmax[8]; };
 int semb_mg_prepare(semb_mesh* h, const semb_pcg_opts* o, semb_mg_ctx* ctx, cudaStream_t s);
 int semb_mg_vcycle_run(semb_mesh* h, const semb_mg_ctx& ctx, int level, const double* r, double* z, semb_scalars* scal, cudaStream_t s);
 int semb_mg_transfer_run(semb_mesh* h, const semb_mg_ctx& ctx, int level, int restrict_, const double* in, double* out, cudaStream_t s);

@@ -43,7 +43,7 @@ class PcgOpts(C.Structure):
                 ("maxit", C.c_int32), ("x0_is_zero", C.c_int32), ("check_every", C.c_int32), ("profile", C.c_int32),
                 ("mg_nlevels", C.c_int32), ("mg_orders", C.c_int32 * 8), ("mg_smooth_degree", C.c_int32),
                 ("mg_coarse_degree", C.c_int32), ("mg_lmax", C.c_double * 8), ("mg_smoother_kind", C.c_int32), ("pad_", C.c_int32),
-                ("mg_coarse_lmin_frac", C.c_double), ("null_mean", C.c_int32), ("pad2_", C.c_int32)]
+                ("mg_coarse_lmin_frac", C.c_double), ("null_mean", C.c_int32), ("mg_fp32", C.c_int32)]
 
 
 def _mg_fill(o, mg_orders=None, mg_smooth=0, mg_coarse=0, mg_lmax=None, mg_kind=1, mg_coarse_frac=0.0):
@@ -204,12 +204,13 @@ class Mesh:
 
     def pcg_solve(self, b, x, lam=0.0, tags=0, precond=1, cheb_degree=2, cheb_lmax=0.0, rtol=1e-10, atol=0.0,
                   maxit=10000, x0_is_zero=True, check_every=0, hist_len=0, profile=False, mg_orders=None, mg_smooth=0,
-                  mg_coarse=0, mg_lmax=None, mg_kind=1, mg_coarse_frac=0.0, null_mean=False):
+                  mg_coarse=0, mg_lmax=None, mg_kind=1, mg_coarse_frac=0.0, null_mean=False, mg_fp32=False):
         """Returns dict(iters, status, b_norm, r0_norm, r_norm, lmax_used, hist).  precond: 0 none, 1 Jacobi,
         2 Chebyshev-Jacobi, 3 p-multigrid V-cycle (mg_orders e.g. [7, 3, 1]; None = default)."""
         o = PcgOpts(lam, tags, precond, cheb_degree, cheb_lmax, rtol, atol, maxit, 1 if x0_is_zero else 0, check_every, 1 if profile else 0)
         _mg_fill(o, mg_orders, mg_smooth, mg_coarse, mg_lmax, mg_kind, mg_coarse_frac)
         o.null_mean = 1 if null_mean else 0
+        o.mg_fp32 = 1 if mg_fp32 else 0
         hist = np.zeros(max(hist_len, 1))
         st = PcgStats()
         st.hist = hist.ctypes.data_as(C.c_void_p).value if hist_len > 0 else None
@@ -243,9 +244,10 @@ class Mesh:
         return _mg_fill(o, mg_orders, mg_smooth, mg_coarse, mg_lmax, mg_kind, mg_coarse_frac)
 
     def mg_vcycle(self, r, z, lam=0.0, tags=0, mg_orders=None, mg_smooth=0, mg_coarse=0, mg_lmax=None, mg_kind=1,
-                  mg_coarse_frac=0.0):
+                  mg_coarse_frac=0.0, mg_fp32=False):
         """z = one p-multigrid V-cycle applied to r; returns the Chebyshev bounds used per level."""
         o = self._mg_opts(lam, tags, mg_orders, mg_smooth, mg_coarse, mg_lmax, mg_kind, mg_coarse_frac)
+        o.mg_fp32 = 1 if mg_fp32 else 0
         used = (C.c_double * 8)()
         self._check(lib().semb_mg_vcycle(self._h, C.byref(o), _dp(r), _dp(z), used, _stream()))
         nl = len(mg_orders) if mg_orders is not None else 8

@@ -214,3 +214,36 @@ def test_all_neumann_pressure_zero_mean(torch_cuda, semb, orc, xi_of, precond):
             G.pcg_solve(dev(torch, b), x, lam=0.0, tags=0b10, precond=1, null_mean=True)
     finally:
         G.close()
+
+
+@pytest.mark.parametrize("name", ["ogrid7", "box5"])
+def test_fp32_storage_levels(torch_cuda, cases, orc, name):
+    """mg_fp32 (R21): vectors and geometric factors of the levels stored in float, arithmetic in fp64.  The
+    oracle rounds every vector of the cycle where it is stored; kernels that fuse two of the oracle's steps round once
+    where the oracle rounds twice, so the two cycles agree to a few float roundings (bar 2e-6 normwise, derived in
+    DESIGN.md), while the PCG around the cycle stays fp64: same iteration count +-1, same solution to 1e-8."""
+    torch = torch_cuda
+    m, mg64, G, orders, lam, tags = cases(name)
+    mg32 = orc.Multigrid(m.E, m.N, m.x, m.y, m.z, m.face_tag, m.period, lam, tags, orders, k_smooth=1, k_coarse=8,
+                         coarse_frac=0.05, lmax=mg64.lmax, fp32=True)
+    P = mg32.levels[0]
+    r = cont(orc, P, 63)
+    z = torch.empty(P.n, dtype=torch.float64, device="cuda")
+    G.mg_vcycle(dev(torch, r), z, lam, tags, orders, 1, 8, mg32.lmax, mg_coarse_frac=0.05, mg_fp32=True)
+    zg = z.cpu().numpy()
+    assert normwise(zg, mg32.vcycle(r)) <= 2e-6
+    assert np.array_equal(zg.astype(np.float32).astype(np.float64), zg)          # a stored float vector, widened
+    assert np.all(zg[P.mask == 0] == 0)
+    z64 = torch.empty_like(z)
+    G.mg_vcycle(dev(torch, r), z64, lam, tags, orders, 1, 8, mg32.lmax, mg_coarse_frac=0.05)
+    assert 1e-9 < normwise(zg, z64.cpu().numpy()) < 5e-6                          # it really ran in float storage
+    b = P.assemble_rhs(I.divergence_source(m, I.seed_for(2, 73)))
+    ro = mg32.pcg(b, rtol=1e-10)
+    x = torch.zeros(P.n, dtype=torch.float64, device="cuda")
+    rg = G.pcg_solve(dev(torch, b), x, lam=lam, tags=tags, precond=3, rtol=1e-10, mg_orders=orders, mg_smooth=1, mg_coarse=8,
+                     mg_lmax=mg32.lmax, mg_coarse_frac=0.05, mg_fp32=True)
+    assert ro["status"] == 0 and rg["status"] == 0 and abs(rg["iters"] - ro["iters"]) <= 1
+    xg = x.cpu().numpy()
+    assert normwise(xg, ro["x"]) <= 1e-8
+    res = b - P.apply_A(xg)
+    assert np.sqrt(P.dot(res, res)) <= 2e-10 * np.sqrt(P.dot(b, b))

@@ -219,3 +219,29 @@ def test_fourth_kind_vcycle_converges_comparably(orc, xi_of):
         its[kind] = r["iters"]
     # measured: 37 (first kind on [0.1, 1] lmax) vs 40 (fourth kind, which needs no lower bound)
     assert its[4] <= 1.25 * its[1] and its[1] <= 1.25 * its[4], its
+
+
+def test_fp32_storage_vcycle_is_a_small_perturbation(orc, xi_of):
+    """R21: with FP32 storage of the levels the V-cycle differs from the fp64 one by float rounding only (each stored
+    vector carries a relative error <= 2^-24, a few dozen stores per cycle), it leaves the fp64 V-cycle bit-for-bit
+    untouched, and PCG around it reaches the same fp64 solution in the same number of iterations (+-1)."""
+    m, _ = I.config_mesh(2, xi_of, small=True)
+    kw = dict(k=1, kc=8, frac=0.05)
+    mg64 = _mg(orc, m, 0.0, 0b10, [7, 3, 1], **kw)
+    mg32 = orc.Multigrid(m.E, m.N, m.x, m.y, m.z, m.face_tag, m.period, 0.0, 0b10, [7, 3, 1], k_smooth=1, k_coarse=8,
+                         coarse_frac=0.05, lmax=mg64.lmax, fp32=True)
+    P = mg64.levels[0]
+    r = _cont(orc, P, 77)
+    z64 = mg64.vcycle(r)
+    z32 = mg32.vcycle(r)
+    err = np.abs(z32 - z64).max() / np.abs(z64).max()
+    assert 1e-9 < err < 5e-6, err                                   # rounding did happen, and only rounding
+    assert np.array_equal(mg64.vcycle(r), z64)                      # the flag is off again outside the fp32 cycle
+    assert np.array_equal(z32.astype(np.float32).astype(np.float64), z32)   # the result is a stored (float) vector
+    assert np.all(z32[P.mask == 0] == 0)
+    b = P.assemble_rhs(I.divergence_source(m, 5))
+    r64, r32 = mg64.pcg(b), mg32.pcg(b)
+    assert r64["status"] == 0 and r32["status"] == 0 and abs(r64["iters"] - r32["iters"]) <= 1
+    assert np.abs(r32["x"] - r64["x"]).max() <= 1e-8 * np.abs(r64["x"]).max()
+    res = b - P.apply_A(r32["x"])                                   # fp64 operator, fp64 residual
+    assert np.sqrt(P.dot(res, res)) <= 2e-10 * np.sqrt(P.dot(b, b))
