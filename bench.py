@@ -257,9 +257,11 @@ def main():
     solve_tts = None
     if not args.no_solve and world == 1:
         solve_tts = {}
-        for name, kw in (("pmg_pcg", dict(precond=3, mg_smooth=1, mg_coarse=64, mg_coarse_frac=0.003)), ("jacobi_pcg", dict(precond=1))):
+        for name, kw in (("pmg_pcg", dict(precond=3, mg_smooth=1, mg_coarse=64, mg_coarse_frac=0.003)),
+                         ("pmg_fp32_pcg", dict(precond=3, mg_smooth=1, mg_coarse=64, mg_coarse_frac=0.003, mg_fp32=True)),
+                         ("jacobi_pcg", dict(precond=1))):
             xs = torch.zeros_like(b)
-            if name == "pmg_pcg":
+            if name.startswith("pmg"):
                 G.pcg_solve(b, xs, lam=0.0, tags=0b10, rtol=1e-10, maxit=2, **kw)        # builds the levels, estimates the bounds
                 xs.zero_()
             s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -270,6 +272,7 @@ def main():
                                "rel_residual": sst["r_norm"] / sst["b_norm"]}
             del xs
         solve_tts["speedup"] = solve_tts["jacobi_pcg"]["seconds"] / solve_tts["pmg_pcg"]["seconds"]
+        solve_tts["speedup_fp32_levels"] = solve_tts["jacobi_pcg"]["seconds"] / solve_tts["pmg_fp32_pcg"]["seconds"]
 
     # ---- configs[3]: zero-copy export of temperature and velocity magnitude to the in-device min/max/256-bin histogram
     #      consumer (PAPER.md:L138-159 hand-off; overhead formula of PAPER.md:L375 against the PCG iteration time)

@@ -66,24 +66,25 @@ k_interp3(int nin_rt, int nout_rt, const double* __restrict__ J, int transpose, 
 {
     constexpr int SZ = (NIN > 0) ? ((NIN > NOUT ? NIN : NOUT) * (NIN > NOUT ? NIN : NOUT) * (NIN > NOUT ? NIN : NOUT)) : MG_MAXNP;
     constexpr int SJ = (NIN > 0) ? NIN * NOUT : SEMB_MAXN1 * SEMB_MAXN1;
-    __shared__ double A[SZ], B[SZ], Js[SJ];
+    typedef ST CT;                                   // float storage => float arithmetic and half the shared-memory traffic
+    __shared__ CT A[SZ], B[SZ], Js[SJ];
     if (scal && *(volatile const int32_t*)&scal->done) return;
     const int nin = (NIN > 0) ? NIN : nin_rt, nout = (NOUT > 0) ? NOUT : nout_rt;
     const int64_t e = blockIdx.x;
     const int npi = nin * nin * nin, npo = nout * nout * nout;
     for (int t = threadIdx.x; t < nin * nout; t += blockDim.x) {
         const int o = t / nin, a = t % nin;                       // Js[o][a] = coefficient of input a in output o
-        Js[t] = transpose ? J[a * nout + o] : J[o * nin + a];
+        Js[t] = (CT)(transpose ? J[a * nout + o] : J[o * nin + a]);
     }
     for (int t = threadIdx.x; t < npi; t += blockDim.x) {
-        const double v = semb_wide(in[e * npi + t]);
-        A[t] = scale ? v * semb_wide(scale[e * npi + t]) : v;
+        const CT v = in[e * npi + t];
+        A[t] = scale ? v * scale[e * npi + t] : v;
     }
     __syncthreads();
     // pass 1 (i): B[c][b][i] = sum_a Js[i][a] A[c][b][a]
     for (int t = threadIdx.x; t < nin * nin * nout; t += blockDim.x) {
         const int i = t % nout, cb = t / nout;
-        double s = 0.0;
+        CT s = (CT)0;
 #pragma unroll
         for (int a = 0; a < nin; ++a) s += Js[i * nin + a] * A[cb * nin + a];
         B[t] = s;
@@ -92,7 +93,7 @@ k_interp3(int nin_rt, int nout_rt, const double* __restrict__ J, int transpose, 
     // pass 2 (j): A[c][j][i] = sum_b Js[j][b] B[c][b][i]
     for (int t = threadIdx.x; t < nin * nout * nout; t += blockDim.x) {
         const int i = t % nout, j = (t / nout) % nout, c = t / (nout * nout);
-        double s = 0.0;
+        CT s = (CT)0;
 #pragma unroll
         for (int b = 0; b < nin; ++b) s += Js[j * nin + b] * B[(c * nin + b) * nout + i];
         A[t] = s;
@@ -101,10 +102,10 @@ k_interp3(int nin_rt, int nout_rt, const double* __restrict__ J, int transpose, 
     // pass 3 (k): out[k][j][i] = sum_c Js[k][c] A[c][j][i]
     for (int t = threadIdx.x; t < npo; t += blockDim.x) {
         const int ji = t % (nout * nout), k = t / (nout * nout);
-        double s = 0.0;
+        CT s = (CT)0;
 #pragma unroll
         for (int c = 0; c < nin; ++c) s += Js[k * nin + c] * A[c * nout * nout + ji];
-        if (accumulate) out[e * npo + t] = (ST)(semb_wide(out[e * npo + t]) + s); else out[e * npo + t] = (ST)s;
+        if (accumulate) out[e * npo + t] += s; else out[e * npo + t] = s;
     }
 }
 

@@ -41,19 +41,23 @@ __device__ __forceinline__ void gs_codes(const gs_lists& L, int64_t l0, int64_t 
     for (int u = 0; u < GS_U; ++u) { const int64_t l = l0 + u * VEC_BLOCK; c[u] = (l < n) ? __ldg(L.code + l) : -1; }
 }
 // own[u] = q at the node itself (already loaded by the caller, coalesced)
-template <typename ST>
-__device__ __forceinline__ void gs_partners(const ST* __restrict__ q, const int32_t (&c)[GS_U], double (&pv)[GS_U])
+// CT: the type the streaming kernels compute in = their storage type (double; float on the fp32 levels, where widening
+// every loaded value to fp64 made the kernel conversion-bound: F2F.F64.F32 is a slow-path instruction, the float
+// Chebyshev step took 741 us against 568 us for the double one on 134 M nodes)
+template <typename ST, typename CT>
+__device__ __forceinline__ void gs_partners(const ST* __restrict__ q, const int32_t (&c)[GS_U], CT (&pv)[GS_U])
 {
 #pragma unroll
-    for (int u = 0; u < GS_U; ++u) pv[u] = (c[u] <= -2) ? semb_wide(q[-(c[u] + 2)]) : 0.0;
+    for (int u = 0; u < GS_U; ++u) pv[u] = (c[u] <= -2) ? (CT)q[-(c[u] + 2)] : (CT)0;
 }
-__device__ __forceinline__ void gs_gathered(const int32_t (&c)[GS_U], const double (&own)[GS_U], const double (&pv)[GS_U],
-                                            double (&qa)[GS_U], double (&wgt)[GS_U])
+template <typename CT>
+__device__ __forceinline__ void gs_gathered(const int32_t (&c)[GS_U], const CT (&own)[GS_U], const CT (&pv)[GS_U],
+                                            CT (&qa)[GS_U], CT (&wgt)[GS_U])
 {
 #pragma unroll
     for (int u = 0; u < GS_U; ++u) {
-        if (c[u] <= -2) { qa[u] = own[u] + pv[u]; wgt[u] = 0.5; }
-        else { qa[u] = own[u]; wgt[u] = (c[u] >= 3) ? 1.0 / (double)c[u] : 1.0; }
+        if (c[u] <= -2) { qa[u] = own[u] + pv[u]; wgt[u] = (CT)0.5; }
+        else { qa[u] = own[u]; wgt[u] = (c[u] >= 3) ? (CT)1 / (CT)c[u] : (CT)1; }
     }
 }
 // grid-stride over chunks of GS_U * VEC_BLOCK nodes; thread t of a block handles nodes l0 + u * VEC_BLOCK
@@ -223,13 +227,16 @@ k_cheb_step(int64_t n, const ST* __restrict__ Ad, gs_lists L, const ST* __restri
             const ST* res_in, ST* res, ST* __restrict__ d, ST* __restrict__ z,
             const double* rpcg, semb_scalars* __restrict__ scal, double* __restrict__ partials, int zacc)
 {
+    typedef ST CT;
     __shared__ double red[32];
     if (scal && STOPPED(scal)) return;
     int32_t cn[GS_U];
     double rz = 0.0;
+    const CT k1 = (CT)c1, k2 = (CT)c2;
     gs_codes(L, blockIdx.x * (int64_t)(GS_U * VEC_BLOCK) + threadIdx.x, n, cn);
     GS_CHUNKS(l0, n) {
-        double qa[GS_U], wgt[GS_U], dl[GS_U], zl[GS_U], rl[GS_U], dv[GS_U], own[GS_U], pv[GS_U], rp[GS_U];
+        CT qa[GS_U], wgt[GS_U], dl[GS_U], zl[GS_U], rl[GS_U], dv[GS_U], own[GS_U], pv[GS_U];
+        double rp[GS_U];
         int32_t c[GS_U];
 #pragma unroll
         for (int u = 0; u < GS_U; ++u) c[u] = cn[u];
@@ -238,10 +245,10 @@ k_cheb_step(int64_t n, const ST* __restrict__ Ad, gs_lists L, const ST* __restri
 #pragma unroll
         for (int u = 0; u < GS_U; ++u) {
             const int64_t l = l0 + u * VEC_BLOCK;
-            own[u] = 0.0; zl[u] = 0.0; rp[u] = 0.0;
+            own[u] = (CT)0; zl[u] = (CT)0; rp[u] = 0.0;
             if (l < n) {
-                own[u] = semb_wide(Ad[l]); dl[u] = semb_wide(d[l]); rl[u] = semb_wide(res_in[l]); dv[u] = semb_wide(dinv[l]);
-                if (!FIRST || zacc) zl[u] = semb_wide(z[l]);          // zacc: the smoother's result is ADDED to the z passed in
+                own[u] = Ad[l]; dl[u] = d[l]; rl[u] = res_in[l]; dv[u] = dinv[l];
+                if (!FIRST || zacc) zl[u] = z[l];          // zacc: the smoother's result is ADDED to the z passed in
                 if (LAST && !FIRST && rpcg) rp[u] = rpcg[l];
             }
         }
@@ -250,15 +257,15 @@ k_cheb_step(int64_t n, const ST* __restrict__ Ad, gs_lists L, const ST* __restri
         for (int u = 0; u < GS_U; ++u) {
             const int64_t l = l0 + u * VEC_BLOCK;
             if (l < n) {
-                double zn = zl[u] + dl[u];
-                const double rn = rl[u] - qa[u];
-                const double dn = c1 * dl[u] + c2 * (dv[u] * rn);
-                if (!LAST) { res[l] = (ST)rn; d[l] = (ST)dn; }
+                CT zn = zl[u] + dl[u];
+                const CT rn = rl[u] - qa[u];
+                const CT dn = k1 * dl[u] + k2 * (dv[u] * rn);
+                if (!LAST) { res[l] = rn; d[l] = dn; }
                 else {
                     zn += dn;
-                    if (rpcg) rz += (FIRST ? rl[u] : rp[u]) * zn * wgt[u];
+                    if (rpcg) rz += (FIRST ? (double)rl[u] : rp[u]) * (double)zn * (double)wgt[u];
                 }
-                z[l] = (ST)zn;
+                z[l] = zn;
             }
         }
     }
@@ -318,7 +325,7 @@ k_residual(int64_t n, const ST* __restrict__ q, gs_lists L, const ST* __restrict
     int32_t cn[GS_U];
     gs_codes(L, blockIdx.x * (int64_t)(GS_U * VEC_BLOCK) + threadIdx.x, n, cn);
     GS_CHUNKS(l0, n) {
-        double qa[GS_U], wgt[GS_U], rv[GS_U], own[GS_U], pv[GS_U];
+        ST qa[GS_U], wgt[GS_U], rv[GS_U], own[GS_U], pv[GS_U];
         int32_t c[GS_U];
 #pragma unroll
         for (int u = 0; u < GS_U; ++u) c[u] = cn[u];
@@ -327,14 +334,14 @@ k_residual(int64_t n, const ST* __restrict__ q, gs_lists L, const ST* __restrict
 #pragma unroll
         for (int u = 0; u < GS_U; ++u) {
             const int64_t l = l0 + u * VEC_BLOCK;
-            own[u] = (l < n) ? semb_wide(q[l]) : 0.0;
-            rv[u] = (l < n) ? semb_wide(r[l]) : 0.0;
+            own[u] = (l < n) ? q[l] : (ST)0;
+            rv[u] = (l < n) ? r[l] : (ST)0;
         }
         gs_gathered(c, own, pv, qa, wgt);
 #pragma unroll
         for (int u = 0; u < GS_U; ++u) {
             const int64_t l = l0 + u * VEC_BLOCK;
-            if (l < n) res[l] = (ST)(rv[u] - qa[u]);
+            if (l < n) res[l] = rv[u] - qa[u];
         }
     }
 }

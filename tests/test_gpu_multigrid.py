@@ -220,8 +220,10 @@ def test_all_neumann_pressure_zero_mean(torch_cuda, semb, orc, xi_of, precond):
 def test_fp32_storage_levels(torch_cuda, cases, orc, name):
     """mg_fp32 (R21): vectors and geometric factors of the levels stored in float, arithmetic in fp64.  The
     oracle rounds every vector of the cycle where it is stored; kernels that fuse two of the oracle's steps round once
-    where the oracle rounds twice, so the two cycles agree to a few float roundings (bar 2e-6 normwise, derived in
-    DESIGN.md), while the PCG around the cycle stays fp64: same iteration count +-1, same solution to 1e-8."""
+    where the oracle rounds twice and the streaming kernels add in float, so the two cycles agree to a few float roundings
+    (bar 2e-6 normwise, derived in DESIGN.md R21), while the PCG around the cycle stays fp64: same iteration count +-1, true
+    residual below 2e-10.  The two PRECONDITIONERS differ at 1e-7, so the iterates part ways and the converged solutions
+    agree only as well as two solves to rtol 1e-10 do: kappa(A) * 2 rtol ~ 1e-7 (bar 2e-7), not the 1e-8 of the fp64 path."""
     torch = torch_cuda
     m, mg64, G, orders, lam, tags = cases(name)
     mg32 = orc.Multigrid(m.E, m.N, m.x, m.y, m.z, m.face_tag, m.period, lam, tags, orders, k_smooth=1, k_coarse=8,
@@ -244,6 +246,6 @@ def test_fp32_storage_levels(torch_cuda, cases, orc, name):
                      mg_lmax=mg32.lmax, mg_coarse_frac=0.05, mg_fp32=True)
     assert ro["status"] == 0 and rg["status"] == 0 and abs(rg["iters"] - ro["iters"]) <= 1
     xg = x.cpu().numpy()
-    assert normwise(xg, ro["x"]) <= 1e-8
+    assert normwise(xg, ro["x"]) <= 2e-7
     res = b - P.apply_A(xg)
     assert np.sqrt(P.dot(res, res)) <= 2e-10 * np.sqrt(P.dot(b, b))
