@@ -83,3 +83,13 @@ def test_setup_fails_loudly_without_a_device(semb):
     # bad arguments are rejected before anything else
     assert L.semb_setup(C.c_int64(0), C.c_int(1), p, p, p, None, None, None, None, None, C.byref(h)) == -1
     assert L.semb_export_field(None, b"temperature", None) < 0
+
+
+def test_bench_byte_model_matches_the_survey():
+    """bench.py's per-iteration byte model: 171.6 B/node at N = 7, 169.8 at N = 9."""
+    import importlib.util
+    import os
+    spec = importlib.util.spec_from_file_location("bench", os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "bench.py"))
+    bench = importlib.util.module_from_spec(spec); spec.loader.exec_module(bench)
+    assert abs(bench.model_bytes_per_iteration(7) - 171.6) < 0.05 and abs(bench.model_bytes_per_iteration(9) - 169.8) < 0.05
+    assert bench.B_ITER == 171.6 and bench.B_AXHELM == 64.0 and bench.B_AXHELM_HELM == 72.0 and bench.B_AXHELM_PCG == 104.0
