@@ -59,30 +59,36 @@ static void interp_matrix_host(int Nfrom, int Nto, double* J)
 #define MG_MAXNP (SEMB_MAXN1 * SEMB_MAXN1 * SEMB_MAXN1)
 // NIN, NOUT > 0: compile-time sizes (the pairs the default hierarchies use; index arithmetic and the inner loops
 // unroll); NIN = NOUT = 0: run-time sizes nin, nout.
-template <int NIN, int NOUT, typename ST>
+// EPB elements per block, 128 / EPB threads each (the transfers between the N = 3 and N = 1 levels move 8 <-> 64 nodes per
+// element: one block per element was 262 144 blocks of almost no work, 285 us per launch on the bench mesh).
+template <int NIN, int NOUT, typename ST, int EPB>
 __global__ void __launch_bounds__(128)
-k_interp3(int nin_rt, int nout_rt, const double* __restrict__ J, int transpose, const ST* __restrict__ in,
+k_interp3(int64_t E, int nin_rt, int nout_rt, const double* __restrict__ J, int transpose, const ST* __restrict__ in,
           const ST* __restrict__ scale, ST* __restrict__ out, int accumulate, const semb_scalars* __restrict__ scal)
 {
     constexpr int SZ = (NIN > 0) ? ((NIN > NOUT ? NIN : NOUT) * (NIN > NOUT ? NIN : NOUT) * (NIN > NOUT ? NIN : NOUT)) : MG_MAXNP;
     constexpr int SJ = (NIN > 0) ? NIN * NOUT : SEMB_MAXN1 * SEMB_MAXN1;
+    constexpr int TPE = 128 / EPB;
     typedef ST CT;                                   // float storage => float arithmetic and half the shared-memory traffic
-    __shared__ CT A[SZ], B[SZ], Js[SJ];
+    __shared__ CT As[EPB * SZ], Bs[EPB * SZ], Js[SJ];
     if (scal && *(volatile const int32_t*)&scal->done) return;
     const int nin = (NIN > 0) ? NIN : nin_rt, nout = (NOUT > 0) ? NOUT : nout_rt;
-    const int64_t e = blockIdx.x;
+    const int el = threadIdx.x / TPE, tl = threadIdx.x - el * TPE;
+    const int64_t e = blockIdx.x * (int64_t)EPB + el;
+    const bool valid = e < E;
+    CT* __restrict__ A = As + el * SZ; CT* __restrict__ B = Bs + el * SZ;
     const int npi = nin * nin * nin, npo = nout * nout * nout;
     for (int t = threadIdx.x; t < nin * nout; t += blockDim.x) {
         const int o = t / nin, a = t % nin;                       // Js[o][a] = coefficient of input a in output o
         Js[t] = (CT)(transpose ? J[a * nout + o] : J[o * nin + a]);
     }
-    for (int t = threadIdx.x; t < npi; t += blockDim.x) {
+    if (valid) for (int t = tl; t < npi; t += TPE) {
         const CT v = in[e * npi + t];
         A[t] = scale ? v * scale[e * npi + t] : v;
     }
     __syncthreads();
     // pass 1 (i): B[c][b][i] = sum_a Js[i][a] A[c][b][a]
-    for (int t = threadIdx.x; t < nin * nin * nout; t += blockDim.x) {
+    if (valid) for (int t = tl; t < nin * nin * nout; t += TPE) {
         const int i = t % nout, cb = t / nout;
         CT s = (CT)0;
 #pragma unroll
@@ -91,7 +97,7 @@ k_interp3(int nin_rt, int nout_rt, const double* __restrict__ J, int transpose, 
     }
     __syncthreads();
     // pass 2 (j): A[c][j][i] = sum_b Js[j][b] B[c][b][i]
-    for (int t = threadIdx.x; t < nin * nout * nout; t += blockDim.x) {
+    if (valid) for (int t = tl; t < nin * nout * nout; t += TPE) {
         const int i = t % nout, j = (t / nout) % nout, c = t / (nout * nout);
         CT s = (CT)0;
 #pragma unroll
@@ -100,7 +106,7 @@ k_interp3(int nin_rt, int nout_rt, const double* __restrict__ J, int transpose, 
     }
     __syncthreads();
     // pass 3 (k): out[k][j][i] = sum_c Js[k][c] A[c][j][i]
-    for (int t = threadIdx.x; t < npo; t += blockDim.x) {
+    if (valid) for (int t = tl; t < npo; t += TPE) {
         const int ji = t % (nout * nout), k = t / (nout * nout);
         CT s = (CT)0;
 #pragma unroll
@@ -113,11 +119,12 @@ template <typename ST>
 static void interp3_launch(int64_t E, int nin, int nout, const double* J, int transpose, const ST* in, const ST* scale,
                            ST* out, int accumulate, const semb_scalars* scal, cudaStream_t s)
 {
-#define MG_CASE(A_, B_) if (nin == A_ && nout == B_) { k_interp3<A_, B_, ST><<<(unsigned)E, 128, 0, s>>>(nin, nout, J, transpose, in, scale, out, accumulate, scal); return; }
+#define MG_CASE(A_, B_) if (nin == A_ && nout == B_) { constexpr int EPB = ((A_ > B_ ? A_ : B_) <= 4) ? 8 : 1; \
+        k_interp3<A_, B_, ST, EPB><<<(unsigned)((E + EPB - 1) / EPB), 128, 0, s>>>(E, nin, nout, J, transpose, in, scale, out, accumulate, scal); return; }
     MG_CASE(8, 4) MG_CASE(4, 8) MG_CASE(4, 2) MG_CASE(2, 4) MG_CASE(10, 6) MG_CASE(6, 10) MG_CASE(6, 4) MG_CASE(4, 6)
     MG_CASE(8, 2) MG_CASE(10, 4) MG_CASE(10, 2) MG_CASE(6, 2) MG_CASE(2, 6) MG_CASE(8, 6) MG_CASE(6, 8)
 #undef MG_CASE
-    k_interp3<0, 0, ST><<<(unsigned)E, 128, 0, s>>>(nin, nout, J, transpose, in, scale, out, accumulate, scal);
+    k_interp3<0, 0, ST, 1><<<(unsigned)E, 128, 0, s>>>(E, nin, nout, J, transpose, in, scale, out, accumulate, scal);
 }
 
 // u ~ U[-1,1) per local node from the counter-based splitmix64 of the input recipe (R19)
