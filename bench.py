@@ -176,6 +176,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-export", action="store_true")
+    ap.add_argument("--no-cfg1", action="store_true", help="skip the configs[1] batched axhelm + gather-scatter section")
     ap.add_argument("--solve-maxit", type=int, default=20000, help="iteration cap of the time-to-solution solves (profiling runs)")
     ap.add_argument("--no-solve", action="store_true", help="skip the time-to-solution section (full pressure solves)")
     args = ap.parse_args()
@@ -309,6 +310,26 @@ def main():
                           "t_novis = one PCG iteration (PAPER.md:L375)"}
         del T, vel
 
+    # ---- configs[1]: batched axhelm + gather-scatter on the 16^3 deformed box, Helmholtz lambda = 10/dt = 1e4, nfields = 3,
+    #      100 applications timed.  Its working set (~150 MB + 3 x 2 x 17 MB) is about the size of the L2: reported, but no
+    #      roofline claim is made from it.
+    cfg1 = None
+    if not args.no_cfg1 and world == 1:
+        m1, G1 = build_problem(torch, semb, 16)
+        U = torch.from_numpy(I.uniform(I.seed_for(1, 1), 3 * m1.n)).cuda()
+        Wv = torch.empty_like(U)
+        for _ in range(5):
+            G1.apply_axhelm(U, Wv, lam=1e4, nfields=3); G1.gather_scatter(Wv, nfields=3)
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(); c0.record()
+        for _ in range(100):
+            G1.apply_axhelm(U, Wv, lam=1e4, nfields=3); G1.gather_scatter(Wv, nfields=3)
+        c1.record(); torch.cuda.synchronize()
+        t1 = c0.elapsed_time(c1) / 100
+        cfg1 = {"ms_per_application": t1, "nfields": 3, "local_nodes": m1.n, "gdofs": 3 * m1.n / (t1 * 1e-3) / 1e9,
+                "note": "axhelm (72 B/node) + stand-alone gather-scatter on 3 fields; working set about the size of L2"}
+        G1.close(); del U, Wv
+
     # ---- end to end through the C ABI with HOST buffers (pinned): b H2D, K iterations, x D2H
     e2e = None
     if not args.no_e2e:
@@ -341,6 +362,7 @@ def main():
         "axhelm_sweep": sweep,
         "time_to_solution": solve_tts,
         "export": export,
+        "cfg1_batched_axhelm_gs": cfg1,
         "e2e": e2e, "gpu_launches": st["launches"], "clocks": clocks,
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
