@@ -330,6 +330,41 @@ def main():
                 "note": "axhelm (72 B/node) + stand-alone gather-scatter on 3 fields; working set about the size of L2"}
         G1.close(); del U, Wv
 
+    # ---- configs[4]: 10 synthetic time steps, each one pressure Poisson solve + 3 velocity + 1 temperature Helmholtz solves
+    #      (lambda = 1.5/dt = 3000) through ONE semb_step_solve call, right-hand sides perturbed per step, warm starts
+    #      (R12).  Only on the cfg4 workload; every solve with Jacobi-PCG (as configs[4] words it), then every solve
+    #      with the p-multigrid preconditioner on FP32-storage levels.
+    steps10 = None
+    if args.workload.startswith("cfg4") and not args.no_solve and world == 1:
+        lam_h = 1.5 / 5e-4
+        kinds = [(0.0, 0b10), (lam_h, 0b110), (lam_h, 0b110), (lam_h, 0b110), (lam_h, 0b10)]
+        f0 = [I.divergence_source(m, I.seed_for(4, 30 + i)) for i in range(5)]
+        rms = [float(np.sqrt(np.mean(v ** 2))) for v in f0]
+        f0d = [torch.from_numpy(v).cuda() for v in f0]
+        steps10 = {}
+        for pname, pkw in (("jacobi_pcg_all_solves", dict(precond=1)), ("pmg_fp32_pcg_all_solves", dict(precond=3, mg_fp32=True))):
+            xs = [torch.zeros(n, dtype=torch.float64, device="cuda") for _ in range(5)]
+            bs = [torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(5)]
+            secs, iters = [], []
+            for step in range(10):
+                for i in range(5):
+                    eta = torch.from_numpy(I.uniform(I.seed_for(4, 100 * (step + 1) + i), n)).cuda()
+                    eta.mul_(0.1 * rms[i]).add_(f0d[i])
+                    G.assemble_rhs(eta, bs[i], kinds[i][1])
+                    del eta
+                solves = [dict(b=bs[i], x=xs[i], lam=kinds[i][0], tags=kinds[i][1], rtol=1e-10, x0_is_zero=(step == 0),
+                               **pkw) for i in range(5)]
+                t0e, t1e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize(); t0e.record()
+                rcs, sts = G.step_solve(solves)
+                t1e.record(); torch.cuda.synchronize()
+                secs.append(t0e.elapsed_time(t1e) * 1e-3); iters.append([q["iters"] for q in sts])
+            steps10[pname] = {"seconds_per_step_mean": float(np.mean(secs)), "seconds_first_step": secs[0],
+                              "seconds_per_step_after_first": float(np.mean(secs[1:])),
+                              "iterations_last_step": iters[-1], "status": rcs}
+            del xs, bs
+        del f0d
+
     # ---- end to end through the C ABI with HOST buffers (pinned): b H2D, K iterations, x D2H
     e2e = None
     if not args.no_e2e:
@@ -363,6 +398,7 @@ def main():
         "time_to_solution": solve_tts,
         "export": export,
         "cfg1_batched_axhelm_gs": cfg1,
+        "cfg4_ten_steps": steps10,
         "e2e": e2e, "gpu_launches": st["launches"], "clocks": clocks,
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

@@ -230,6 +230,10 @@ class Mesh:
             o = PcgOpts(sv.get("lam", 0.0), sv.get("tags", 0), sv.get("precond", 1), sv.get("cheb_degree", 2),
                         sv.get("cheb_lmax", 0.0), sv.get("rtol", 1e-10), sv.get("atol", 0.0), sv.get("maxit", 10000),
                         1 if sv.get("x0_is_zero", True) else 0, sv.get("check_every", 0), 0)
+            _mg_fill(o, sv.get("mg_orders"), sv.get("mg_smooth", 0), sv.get("mg_coarse", 0), sv.get("mg_lmax"), sv.get("mg_kind", 1),
+                     sv.get("mg_coarse_frac", 0.0))
+            o.null_mean = 1 if sv.get("null_mean", False) else 0
+            o.mg_fp32 = 1 if sv.get("mg_fp32", False) else 0
             items[i].opts = o
             items[i].b = _dp(sv["b"]).value
             items[i].x = _dp(sv["x"]).value
