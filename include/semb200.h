@@ -164,9 +164,9 @@ typedef struct {
                                  and return the solution of zero mean, mean(v) = <v,1> / n_unique over unique nodes
                                  (reading R20).  SEMB_EINVAL if the tag set selects any Dirichlet node. */
     int32_t  mg_fp32;         /* 1: the V-cycle keeps its vectors and geometric factors in FP32 (the
-                                 preconditioner runs in FP32 "to save on memory bandwidth").  axhelm and gather-scatter
-                                 compute in fp64 registers and round at their stores, the vector updates and transfers
-                                 compute in float; the PCG around the cycle, its residual and its solution stay fp64
+                                 preconditioner runs in FP32 "to save on memory bandwidth") and computes in float (only
+                                 the class sums of the gather-scatter accumulate in fp64); the PCG around the cycle, its
+                                 residual and its solution stay fp64
                                  (reading R21: same iteration counts, fp64 true residual <= 2e-10)          */
 } semb_pcg_opts;
 

@@ -35,6 +35,12 @@ int semb_axhelm_upload_basis(semb_mesh* h)
     ax_eo_tab tab[2];
     ax_eo_build(h->n1, h->D, tab);
     SEMB_CUDA(h, cudaMemcpyToSymbol(c_EO, tab, sizeof(tab), sizeof(ax_eo_tab) * 2 * (size_t)h->N));
+    ax_eo_tab_f tabf[2];
+    for (int t = 0; t < 2; ++t) {
+        for (int q = 0; q < SEMB_EO_H2 * SEMB_EO_H; ++q) { tabf[t].P[q] = (float)tab[t].P[q]; tabf[t].M[q] = (float)tab[t].M[q]; }
+        for (int q = 0; q < SEMB_EO_H2; ++q) tabf[t].mid[q] = (float)tab[t].mid[q];
+    }
+    SEMB_CUDA(h, cudaMemcpyToSymbol(c_EOf, tabf, sizeof(tabf), sizeof(ax_eo_tab_f) * 2 * (size_t)h->N));
     return upload_perm(h);
 }
 

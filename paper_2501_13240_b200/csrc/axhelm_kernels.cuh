@@ -40,6 +40,7 @@ template <int n1> struct ax_tile {
     static constexpr bool permuted = (n1 == 7) || (n1 >= 10);
     __device__ static __forceinline__ int idx(int k, int j, int i) { return k * P2 + j * P1 + i; }
     __device__ static __forceinline__ int idxB(int k, int j, int i) { return k * P2B + j * P1 + i; }
+    __device__ static __forceinline__ int idx32(int k, int j, int i) { return idx(k, j, i); }       // no 32-bit layouts searched yet
 };
 // n1 = 8: XOR swizzle, conflict-free in all three orientations without padding:
 //   slot mod 16 = ((j^k)&1)*8 + (i ^ (((j>>1)&3) | ((k&1)<<2)))
@@ -52,6 +53,12 @@ template <> struct ax_tile<8> {
         return k * 64 + ((j ^ (k & 1)) << 3) + (i ^ (((j >> 1) & 3) | ((k & 1) << 2)));
     }
     __device__ static __forceinline__ int idxB(int k, int j, int i) { return idx(k, j, i); }
+    // 32-bit tiles (float arithmetic on the fp32 multigrid levels): a warp covers 8 x 4 lines; word within plane k =
+    // j[2]*32 + ((j[1:0] ^ k[1:0]) << 3) + (i ^ j[2:0]) puts the 32 lanes of all three orientations into 32 different banks
+    __device__ static __forceinline__ int idx32(int k, int j, int i)
+    {
+        return k * 64 + ((j >> 2) << 5) + (((j ^ k) & 3) << 3) + (i ^ (j & 7));
+    }
 };
 
 // Which r-line (j = q % n1, k = q / n1) and which s-line (i = q % n1, k = q / n1) a thread contracts:
@@ -143,24 +150,31 @@ static inline void ax_eo_build(int n1, const double* D, ax_eo_tab tab[2])
     }
 }
 
-template <int n1, int TR>
-__device__ __forceinline__ void ax_line(const double (&x)[n1], double (&y)[n1])
+// float copies of the tables for the fp32-storage multigrid levels, where the whole kernel computes in float
+struct ax_eo_tab_f { float P[SEMB_EO_H2 * SEMB_EO_H], M[SEMB_EO_H2 * SEMB_EO_H], mid[SEMB_EO_H2]; };
+__constant__ ax_eo_tab_f c_EOf[SEMB_MAX_N + 1][2];
+template <typename CT> struct ax_eo_sel;
+template <> struct ax_eo_sel<double> { typedef ax_eo_tab tab; __device__ static __forceinline__ const ax_eo_tab& get(int N, int tr) { return c_EO[N][tr]; } };
+template <> struct ax_eo_sel<float> { typedef ax_eo_tab_f tab; __device__ static __forceinline__ const ax_eo_tab_f& get(int N, int tr) { return c_EOf[N][tr]; } };
+
+template <int n1, int TR, typename CT>
+__device__ __forceinline__ void ax_line(const CT (&x)[n1], CT (&y)[n1])
 {
     constexpr int N = n1 - 1, h = n1 / 2;
     constexpr bool odd = n1 & 1;
-    const ax_eo_tab& T = c_EO[N][TR];
-    double e[h > 0 ? h : 1], o[h > 0 ? h : 1];
+    const typename ax_eo_sel<CT>::tab& T = ax_eo_sel<CT>::get(N, TR);
+    CT e[h > 0 ? h : 1], o[h > 0 ? h : 1];
 #pragma unroll
     for (int m = 0; m < h; ++m) { e[m] = x[m] + x[N - m]; o[m] = x[m] - x[N - m]; }
 #pragma unroll
     for (int i = 0; i < h; ++i) {
-        double a = odd ? T.mid[i] * x[h] : 0.0, s = 0.0;
+        CT a = odd ? T.mid[i] * x[h] : (CT)0, s = (CT)0;
 #pragma unroll
         for (int m = 0; m < h; ++m) { a += T.P[i * SEMB_EO_H + m] * e[m]; s += T.M[i * SEMB_EO_H + m] * o[m]; }
         y[i] = s + a; y[N - i] = s - a;
     }
     if (odd) {
-        double s = 0.0;
+        CT s = (CT)0;
 #pragma unroll
         for (int m = 0; m < h; ++m) s += T.M[h * SEMB_EO_H + m] * o[m];
         y[h] = s;
@@ -207,10 +221,15 @@ k_axhelm_line(int64_t E, int64_t n, const ST* __restrict__ geo, double lambda,
     constexpr bool HELM = MODE & 1, VAR = MODE & 2, FUSE = MODE & 4;
     constexpr int NG = HELM ? 7 : 6;
     using T = ax_tile<n1>;
-    __shared__ double SuA[EPB * T::size], SrA[EPB * T::size], SsA[EPB * T::size];
+    typedef ST CT;                    // float storage => float arithmetic and 32-bit tiles (the fp64-arithmetic float-storage
+                                      // kernel was bound by its 64-bit transposes at 138 GDOF/s: profiles/r1_v6_fp32_levels.md)
+    constexpr bool W32 = sizeof(CT) == 4;
+#define AX_I(k, j, i) (W32 ? T::idx32(k, j, i) : T::idx(k, j, i))
+#define AX_IB(k, j, i) (W32 ? T::idx32(k, j, i) : T::idxB(k, j, i))
+    __shared__ CT SuA[EPB * T::size], SrA[EPB * T::size], SsA[EPB * T::size];
     if (scal && *(volatile const int32_t*)&scal->done) return;
     const int el = (EPB > 1) ? threadIdx.x / n2 : 0, tl = (EPB > 1) ? threadIdx.x - el * n2 : threadIdx.x;
-    double* __restrict__ Su = SuA + el * T::size; double* __restrict__ Sr = SrA + el * T::size; double* __restrict__ Ss = SsA + el * T::size;
+    CT* __restrict__ Su = SuA + el * T::size; CT* __restrict__ Sr = SrA + el * T::size; CT* __restrict__ Ss = SsA + el * T::size;
     const int64_t nef = E * (int64_t)nfields;
     int64_t ef = blockIdx.x * (int64_t)EPB + el;
     const bool valid = ef < nef;
@@ -237,76 +256,76 @@ k_axhelm_line(int64_t E, int64_t n, const ST* __restrict__ geo, double lambda,
     }
     ST* __restrict__ we = w + f * n + e * Np + tl;
     const ST* __restrict__ g = geo + e * 7 * (int64_t)Np + tl;
-    double ru[n1], G[NG][n1];
+    CT ru[n1], G[NG][n1];
     if (FUSE) {
         const int64_t l0 = e * Np + tl;
         const bool plain = pcg.plain != 0;
-        const double beta = plain ? 0.0 : scal->beta, alpha = plain ? 0.0 : scal->alpha;
-        const bool pend = !plain && scal->x_pending != 0, first = plain || (beta == 0.0);
-        double z[n1], po[n1];
+        const CT beta = plain ? (CT)0 : (CT)scal->beta, alpha = plain ? (CT)0 : (CT)scal->alpha;
+        const bool pend = !plain && scal->x_pending != 0, first = plain || (beta == (CT)0);
+        const CT pscale = (CT)pcg.scale;
+        CT z[n1], po[n1];
 #pragma unroll
-        for (int k = 0; k < n1; ++k) z[k] = semb_wide(pcg.zsrc[l0 + k * n2]);
+        for (int k = 0; k < n1; ++k) z[k] = pcg.zsrc[l0 + k * n2];
         if (pcg.dinv) {
 #pragma unroll
-            for (int k = 0; k < n1; ++k) z[k] *= semb_wide(pcg.dinv[l0 + k * n2]);
+            for (int k = 0; k < n1; ++k) z[k] *= pcg.dinv[l0 + k * n2];
         }
         if (plain) {
 #pragma unroll
-            for (int k = 0; k < n1; ++k) z[k] *= pcg.scale;
+            for (int k = 0; k < n1; ++k) z[k] *= pscale;
         }
         if (pend || !first) {
 #pragma unroll
-            for (int k = 0; k < n1; ++k) po[k] = semb_wide(pcg.p_io[l0 + k * n2]);
+            for (int k = 0; k < n1; ++k) po[k] = pcg.p_io[l0 + k * n2];
         }
         if (pend) {
 #pragma unroll
-            for (int k = 0; k < n1; ++k) if (valid) pcg.x[l0 + k * n2] = (ST)(semb_wide(pcg.x[l0 + k * n2]) + alpha * po[k]);
+            for (int k = 0; k < n1; ++k) if (valid) pcg.x[l0 + k * n2] += alpha * po[k];
         }
 #pragma unroll
         for (int k = 0; k < n1; ++k) {
             ru[k] = first ? z[k] : z[k] + beta * po[k];
-            if (sizeof(ST) < 8) ru[k] = (double)(ST)ru[k];      // the operator is applied to the STORED (rounded) vector
-            if (valid) pcg.p_io[l0 + k * n2] = (ST)ru[k];
+            if (valid) pcg.p_io[l0 + k * n2] = ru[k];
         }
     } else {
         const ST* __restrict__ ue = u + f * n + e * Np + tl;
 #pragma unroll
-        for (int k = 0; k < n1; ++k) ru[k] = semb_wide(ue[k * n2]);
+        for (int k = 0; k < n1; ++k) ru[k] = ue[k * n2];
     }
     // ---- global loads, t-line layout: lane -> consecutive nodes of plane k (coalesced 64-bit)
 #pragma unroll
     for (int k = 0; k < n1; ++k) {
 #pragma unroll
-        for (int c = 0; c < NG; ++c) G[c][k] = semb_wide(__ldg(g + c * Np + k * n2));
+        for (int c = 0; c < NG; ++c) G[c][k] = __ldg(g + c * Np + k * n2);
     }
 #pragma unroll
-    for (int k = 0; k < n1; ++k) Su[T::idx(k, b, a)] = ru[k];
+    for (int k = 0; k < n1; ++k) Su[AX_I(k, b, a)] = ru[k];
     __syncthreads();
     // ---- forward contractions, one line per orientation
     {
-        double ln[n1], out[n1];
+        CT ln[n1], out[n1];
 #pragma unroll
-        for (int i = 0; i < n1; ++i) ln[i] = Su[T::idx(rb, ra, i)];
-        ax_line<n1, 0>(ln, out);
+        for (int i = 0; i < n1; ++i) ln[i] = Su[AX_I(rb, ra, i)];
+        ax_line<n1, 0, CT>(ln, out);
 #pragma unroll
-        for (int i = 0; i < n1; ++i) Sr[T::idx(rb, ra, i)] = out[i];
+        for (int i = 0; i < n1; ++i) Sr[AX_I(rb, ra, i)] = out[i];
 #pragma unroll
-        for (int j = 0; j < n1; ++j) ln[j] = Su[T::idx(sb, j, sa)];
-        ax_line<n1, 0>(ln, out);
+        for (int j = 0; j < n1; ++j) ln[j] = Su[AX_I(sb, j, sa)];
+        ax_line<n1, 0, CT>(ln, out);
 #pragma unroll
-        for (int j = 0; j < n1; ++j) Ss[T::idxB(sb, j, sa)] = out[j];
+        for (int j = 0; j < n1; ++j) Ss[AX_IB(sb, j, sa)] = out[j];
     }
-    double ut[n1];
-    ax_line<n1, 0>(ru, ut);
+    CT ut[n1];
+    ax_line<n1, 0, CT>(ru, ut);
     __syncthreads();
     // ---- geometric factors at the nodes of the t-line
-    double gt[n1];
+    CT gt[n1];
 #pragma unroll
     for (int k = 0; k < n1; ++k) {
-        const int s = T::idx(k, b, a), sB = T::idxB(k, b, a);
-        const double ur = Sr[s], us = Ss[sB];
-        double Grr = G[0][k], Grs = G[1][k], Grt = G[2][k], Gss = G[3][k], Gst = G[4][k], Gtt = G[5][k];
-        if (VAR && lam0) { const double c = lam0[e * Np + k * n2 + tl]; Grr *= c; Grs *= c; Grt *= c; Gss *= c; Gst *= c; Gtt *= c; }
+        const int s = AX_I(k, b, a), sB = AX_IB(k, b, a);
+        const CT ur = Sr[s], us = Ss[sB];
+        CT Grr = G[0][k], Grs = G[1][k], Grt = G[2][k], Gss = G[3][k], Gst = G[4][k], Gtt = G[5][k];
+        if (VAR && lam0) { const CT c = (CT)lam0[e * Np + k * n2 + tl]; Grr *= c; Grs *= c; Grt *= c; Gss *= c; Gst *= c; Gtt *= c; }
         Sr[s] = Grr * ur + Grs * us + Grt * ut[k];
         Ss[sB] = Grs * ur + Gss * us + Gst * ut[k];
         gt[k] = Grt * ur + Gst * us + Gtt * ut[k];
@@ -314,24 +333,24 @@ k_axhelm_line(int64_t E, int64_t n, const ST* __restrict__ geo, double lambda,
     __syncthreads();
     // ---- transposed contractions
     {
-        double ln[n1], out[n1];
+        CT ln[n1], out[n1];
 #pragma unroll
-        for (int i = 0; i < n1; ++i) ln[i] = Sr[T::idx(rb, ra, i)];
-        ax_line<n1, 1>(ln, out);
+        for (int i = 0; i < n1; ++i) ln[i] = Sr[AX_I(rb, ra, i)];
+        ax_line<n1, 1, CT>(ln, out);
 #pragma unroll
-        for (int i = 0; i < n1; ++i) Sr[T::idx(rb, ra, i)] = out[i];
+        for (int i = 0; i < n1; ++i) Sr[AX_I(rb, ra, i)] = out[i];
 #pragma unroll
-        for (int j = 0; j < n1; ++j) ln[j] = Ss[T::idxB(sb, j, sa)];
-        ax_line<n1, 1>(ln, out);
+        for (int j = 0; j < n1; ++j) ln[j] = Ss[AX_IB(sb, j, sa)];
+        ax_line<n1, 1, CT>(ln, out);
 #pragma unroll
-        for (int j = 0; j < n1; ++j) Ss[T::idxB(sb, j, sa)] = out[j];
+        for (int j = 0; j < n1; ++j) Ss[AX_IB(sb, j, sa)] = out[j];
     }
-    double wt[n1];
-    ax_line<n1, 1>(gt, wt);
+    CT wt[n1];
+    ax_line<n1, 1, CT>(gt, wt);
     if (HELM) {
 #pragma unroll
         for (int k = 0; k < n1; ++k) {
-            const double lam = (VAR && lam1) ? lam1[e * Np + k * n2 + tl] : lambda;
+            const CT lam = (VAR && lam1) ? (CT)lam1[e * Np + k * n2 + tl] : (CT)lambda;
             wt[k] += lam * G[NG - 1][k] * ru[k];
         }
     }
@@ -339,8 +358,8 @@ k_axhelm_line(int64_t E, int64_t n, const ST* __restrict__ geo, double lambda,
     double dot = 0.0;
 #pragma unroll
     for (int k = 0; k < n1; ++k) {
-        const double wv = wt[k] + Sr[T::idx(k, b, a)] + Ss[T::idxB(k, b, a)];
-        if (valid) { we[k * n2] = (ST)wv; dot += ru[k] * wv; }
+        const CT wv = wt[k] + Sr[AX_I(k, b, a)] + Ss[AX_IB(k, b, a)];
+        if (valid) { we[k * n2] = wv; dot += (double)ru[k] * (double)wv; }
     }
     if (dot_out) {
         __shared__ double red[32];
@@ -348,6 +367,8 @@ k_axhelm_line(int64_t E, int64_t n, const ST* __restrict__ geo, double lambda,
         if (threadIdx.x == 0) dot_out[blockIdx.x] = dot;
     }
 }
+#undef AX_I
+#undef AX_IB
 
 // Sum of the per-block partials dot_in[0..count) in a fixed order (two stages, last block by ticket), then
 // the PCG scalars: p.Ap, alpha = rho / p.Ap, breakdown detection.
