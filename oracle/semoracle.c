@@ -30,8 +30,12 @@
  * Layout: local node l = e*Np + k*n1*n1 + j*n1 + i, i fastest ("(ijk) ordering").
  * geo[e][g][Np], g = 0..6 : G_rr, G_rs, G_rt, G_ss, G_st, G_tt, B.
  *
- * Pins (tests/test_oracle_*.py, -m "not gpu"): P1-P16 of SURVEY.md §8(c).  Functions with
- * no independent pin: none ("parity unpinned" list is empty; see DESIGN.md §Oracle pins).
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): P1-P16 of SURVEY.md §8(c).  The "next" rows built so far follow the
+ * same rule: p-multigrid V-cycle (f-1, R19: orc_interp_matrix, orc_interp3, orc_mg_*; pins: Vandermonde
+ * interpolation, Kronecker transfer, adjointness, dense V-cycle composition, bounds covering the dense spectrum),
+ * fourth-kind Chebyshev smoother (closed-form residual polynomial), FP32-storage levels (R21: a float-rounding
+ * perturbation of the pinned fp64 cycle), all-Neumann solves (R20, in semoracle.py: pseudo-inverse solution).
+ * Functions with no independent pin: none ("parity unpinned" list is empty; see DESIGN.md §Oracle pins).
  */
 #include <math.h>
 #include <stdint.h>
