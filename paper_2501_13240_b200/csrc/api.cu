@@ -15,6 +15,17 @@ int semb_fail(semb_mesh* h, int code, const char* fmt, ...)
     return code;
 }
 
+int semb_sm_count()
+{
+    static int sms = 0;
+    if (sms <= 0) {
+        int dev = 0, v = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) sms = v;
+        else { cudaGetLastError(); return 148; }
+    }
+    return sms;
+}
+
 void* semb_dev_alloc(semb_mesh* h, size_t bytes)
 {
     if (bytes == 0) bytes = 8;
@@ -59,7 +70,8 @@ int semb_destroy(semb_handle h)
     if (h->geoK && h->geoK != h->geo) semb_dev_free(h, h->geoK);
     semb_dev_free(h, h->gs_off); semb_dev_free(h, h->gs_ids); semb_dev_free(h, h->face_tag_dev);
     for (auto& kv : h->masks) semb_dev_free(h, kv.second.list);
-    for (auto& kv : h->dinvs) semb_dev_free(h, kv.second);
+    for (auto& en : h->dinvs) semb_dev_free(h, en.d);
+    semb_dev_free(h, h->diagA); semb_dev_free(h, h->diagB);
     semb_dev_free(h, h->work); semb_dev_free(h, h->partials); semb_dev_free(h, h->ax_dot); semb_dev_free(h, h->scal); semb_dev_free(h, h->hist_dev); semb_dev_free(h, h->stage);
     if (h->scal_host) cudaFreeHost(h->scal_host);
     for (cudaEvent_t ev : h->prof_ev) cudaEventDestroy(ev);
@@ -166,7 +178,7 @@ int semb_assemble_rhs(semb_handle h, uint32_t tags, const double* f, double* b, 
     cudaStream_t s = (cudaStream_t)stream;
     semb_mask_entry m;
     int rc = semb_get_mask(h, tags, &m, s); if (rc) return rc;
-    int64_t blocks = (h->n + 1023) / 1024; if (blocks > 148 * 8) blocks = 148 * 8;
+    int64_t blocks = (h->n + 1023) / 1024; if (blocks > semb_sm_count() * 8) blocks = semb_sm_count() * 8;
     k_mass_times<<<(unsigned)blocks, 256, 0, s>>>(h->n, h->Np, h->geo, f, b);
     SEMB_CUDA(h, cudaGetLastError());
     rc = semb_gs_launch(h, b, 1, s); if (rc) return rc;
@@ -228,7 +240,7 @@ int semb_mg_vcycle(semb_handle h, const semb_pcg_opts* o, const double* r, doubl
     if (!o || !r || !z || r == z) return semb_fail(h, SEMB_EINVAL, "mg_vcycle: bad argument");
     semb_mg_ctx ctx;
     int rc = semb_mg_prepare(h, o, &ctx, (cudaStream_t)stream); if (rc) return rc;
-    if (lmax_used) for (int l = 0; semb_mg_level_n(ctx, l) >= 0 && l < 8; ++l) lmax_used[l] = ctx.lmax[l];
+    if (lmax_used) for (int l = 0; l < 8 && semb_mg_level_n(ctx, l) >= 0; ++l) lmax_used[l] = ctx.lmax[l];
     return semb_mg_vcycle_run(h, ctx, 0, r, z, nullptr, (cudaStream_t)stream);
 }
 
@@ -244,9 +256,11 @@ int semb_mg_transfer(semb_handle h, const semb_pcg_opts* o, int level, int restr
 int64_t semb_mg_level_size(semb_handle h, const semb_pcg_opts* o, int level)
 {
     if (!h || !o) return SEMB_EINVAL;
-    semb_mg_ctx ctx;
-    int rc = semb_mg_prepare(h, o, &ctx, nullptr); if (rc) return rc;
-    return semb_mg_level_n(ctx, level);
+    int nlev = 0, orders[8];
+    const int rc = semb_mg_orders(h, o, &nlev, orders); if (rc) return rc;       // validates; builds nothing
+    if (level < 0 || level >= nlev) return semb_fail(h, SEMB_EINVAL, "mg_level_size: level %d of %d", level, nlev);
+    const int64_t n1 = orders[level] + 1;
+    return h->E * n1 * n1 * n1;
 }
 
 int semb_cheb_jacobi(semb_handle h, double lambda, uint32_t tags, int k, double lmax, const double* r, double* z, void* stream)

@@ -17,7 +17,7 @@ __global__ void k_vmag(int64_t n, const double* __restrict__ vx, const double* _
 
 int semb_vmag_launch(const double* vx, const double* vy, const double* vz, double* out, int64_t n, cudaStream_t s)
 {
-    int64_t b = (n + 1023) / 1024; if (b > 148 * 8) b = 148 * 8; if (b < 1) b = 1;
+    int64_t b = (n + 1023) / 1024; if (b > semb_sm_count() * 8) b = semb_sm_count() * 8; if (b < 1) b = 1;
     k_vmag<<<(unsigned)b, 256, 0, s>>>(n, vx, vy, vz, out);
     return cudaGetLastError() == cudaSuccess ? SEMB_OK : SEMB_ECUDA;
 }
@@ -89,7 +89,7 @@ int semb_minmax_hist_launch(const double* v, int64_t n, int64_t stride, int nbin
 {
     if (nbins < 1 || nbins > 8192 || n < 1 || stride < 1) return SEMB_EINVAL;
     // each block's shared counters are 32-bit: keep every block's share of the input below 2^32
-    int64_t blocks = (n + 2047) / 2048; if (blocks > 148 * 8) blocks = 148 * 8; if (blocks < 1) blocks = 1;
+    int64_t blocks = (n + 2047) / 2048; if (blocks > semb_sm_count() * 8) blocks = semb_sm_count() * 8; if (blocks < 1) blocks = 1;
     unsigned long long* mm = (unsigned long long*)minmax_dev;
     k_mm_init<<<1, 1, 0, s>>>(mm);
     k_minmax<<<(unsigned)blocks, 256, 0, s>>>(n, stride, v, mm);

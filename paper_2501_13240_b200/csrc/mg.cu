@@ -34,7 +34,10 @@ struct semb_mg {
     float* WF[8][5] = {{nullptr}};       // Chebyshev work (res, d, Ad), residual, scratch
     float* rF[8] = {nullptr};            // level l: right-hand side (level 0: the converted PCG residual)
     float* zF[8] = {nullptr};            // level l: result
-    std::map<std::pair<uint32_t, double>, std::array<float*, 8>> dinvF;   // per (tags, lambda), owned
+    // float copies of the level diagonals for the MG_DINVF_CACHE most recently used (tags, lambda) pairs, owned
+    struct dinvF_entry { uint32_t tags; double lambda; std::array<float*, 8> d; uint64_t stamp; };
+    std::vector<dinvF_entry> dinvF; uint64_t dinvF_clock = 0;
+    const float* const* dinvF_cur = nullptr;   // the entry mg_f32_prepare selected for the cycle being enqueued
 };
 
 // J[(Nto+1) x (Nfrom+1)]: Lagrange basis of the order-Nfrom GLL nodes at the order-Nto GLL nodes (product formula;
@@ -139,7 +142,9 @@ __global__ void k_mg_random(int64_t n, unsigned long long seed, double* __restri
     }
 }
 #define MG_LMAX_SEED (250113240ull + 900ull)
-static inline unsigned mg_grid(int64_t n) { int64_t b = (n + 1023) / 1024; return (unsigned)(b < 1 ? 1 : (b > 148 * 8 ? 148 * 8 : b)); }
+#define MG_DINVF_CACHE 4
+#define MG_LMAX_CACHE 256     // (tags, lambda) pairs whose estimated Chebyshev bounds are remembered (64 B each)
+static inline unsigned mg_grid(int64_t n) { int64_t b = (n + 1023) / 1024; const int64_t cap = semb_sm_count() * 8; return (unsigned)(b < 1 ? 1 : (b > cap ? cap : b)); }
 
 static void mg_free(semb_mesh* h, semb_mg* g)
 {
@@ -150,7 +155,7 @@ static void mg_free(semb_mesh* h, semb_mg* g)
         semb_dev_free(h, g->geoF[l]); semb_dev_free(h, g->invmultF[l]); semb_dev_free(h, g->rF[l]); semb_dev_free(h, g->zF[l]);
         if (l >= 1 && g->lev[l]) semb_destroy(g->lev[l]);
     }
-    for (auto& kv : g->dinvF) for (float* p : kv.second) semb_dev_free(h, p);
+    for (auto& en : g->dinvF) for (float* p : en.d) semb_dev_free(h, p);
     delete g;
 }
 void semb_mg_destroy_all(semb_mesh* h)
@@ -216,9 +221,10 @@ static int mg_build(semb_mesh* h, int nlevels, const int* orders, semb_mg** out,
     return SEMB_OK;
 }
 
-int semb_mg_prepare(semb_mesh* h, const semb_pcg_opts* o, semb_mg_ctx* ctx, cudaStream_t s)
+// orders of the hierarchy opts describe (defaults filled in), validated against the mesh order; builds nothing
+int semb_mg_orders(semb_mesh* h, const semb_pcg_opts* o, int* nlev_out, int* orders)
 {
-    int nlev = o->mg_nlevels, orders[8];
+    int nlev = o->mg_nlevels;
     if (nlev == 0) {
         orders[0] = h->N; nlev = 1;
         if (h->N > 7) orders[nlev++] = 5;          // cfg4 (N = 9): 9, 5, 3, 1 needs 64 iterations, 9, 3, 1 needs 94
@@ -231,6 +237,14 @@ int semb_mg_prepare(semb_mesh* h, const semb_pcg_opts* o, semb_mg_ctx* ctx, cuda
     if (orders[0] != h->N) return semb_fail(h, SEMB_EINVAL, "multigrid: mg_orders[0] = %d must be the mesh order %d", orders[0], h->N);
     for (int l = 1; l < nlev; ++l)
         if (orders[l] < 1 || orders[l] >= orders[l - 1]) return semb_fail(h, SEMB_EINVAL, "multigrid: orders must decrease strictly and stay >= 1");
+    *nlev_out = nlev;
+    return SEMB_OK;
+}
+
+int semb_mg_prepare(semb_mesh* h, const semb_pcg_opts* o, semb_mg_ctx* ctx, cudaStream_t s)
+{
+    int nlev = 0, orders[8];
+    { const int rc = semb_mg_orders(h, o, &nlev, orders); if (rc) return rc; }
     semb_mg* g = nullptr;
     for (semb_mg* c : h->mgs) {
         bool same = c->nlevels == nlev;
@@ -268,7 +282,10 @@ int semb_mg_prepare(semb_mesh* h, const semb_pcg_opts* o, semb_mg_ctx* ctx, cuda
         }
         ctx->lmax[l] = est[l];
     }
-    if (changed) g->lmax_cache[key] = est;
+    if (changed) {
+        if (g->lmax_cache.size() >= MG_LMAX_CACHE) g->lmax_cache.clear();
+        g->lmax_cache[key] = est;
+    }
     // masks and diagonals of every level for this operator (cached in the level handles)
     for (int l = 0; l < nlev; ++l) {
         semb_mask_entry m; double* dinv;
@@ -372,20 +389,32 @@ static int mg_f32_prepare(semb_mesh* h, const semb_mg_ctx& ctx, cudaStream_t s)
         SEMB_CUDA(h, cudaGetLastError());
         g->f32_ready = true;
     }
-    const std::pair<uint32_t, double> key(ctx.tags, ctx.lambda);
-    if (g->dinvF.find(key) == g->dinvF.end()) {
-        std::array<float*, 8> a{};
+    for (auto& en : g->dinvF)
+        if (en.tags == ctx.tags && en.lambda == ctx.lambda) { en.stamp = ++g->dinvF_clock; g->dinvF_cur = en.d.data(); return SEMB_OK; }
+    std::array<float*, 8> a{};
+    if (g->dinvF.size() >= MG_DINVF_CACHE) {       // reuse the buffers of the least recently used operator
+        size_t lru = 0;
+        for (size_t q = 1; q < g->dinvF.size(); ++q) if (g->dinvF[q].stamp < g->dinvF[lru].stamp) lru = q;
+        SEMB_CUDA(h, cudaStreamSynchronize(s));
+        a = g->dinvF[lru].d;
+        g->dinvF.erase(g->dinvF.begin() + (long)lru);
+    } else {
         for (int l = 0; l < g->nlevels; ++l) {
-            semb_mesh* L = g->lev[l];
-            double* dinv;
-            int rc = semb_get_dinv(L, ctx.lambda, ctx.tags, &dinv, s); if (rc) return rc;
-            a[l] = (float*)semb_dev_alloc(h, sizeof(float) * (size_t)L->n);
-            if (!a[l]) return semb_fail(h, SEMB_ENOMEM, "multigrid: fp32 diagonal of level %d", l);
-            k_mg_convert<double, float><<<mg_grid(L->n), 256, 0, s>>>(L->n, dinv, a[l], nullptr);
+            a[l] = (float*)semb_dev_alloc(h, sizeof(float) * (size_t)g->lev[l]->n);
+            if (!a[l]) { for (float* p : a) semb_dev_free(h, p); return semb_fail(h, SEMB_ENOMEM, "multigrid: fp32 diagonal of level %d", l); }
         }
-        SEMB_CUDA(h, cudaGetLastError());
-        g->dinvF[key] = a;
     }
+    int rc = SEMB_OK;
+    for (int l = 0; l < g->nlevels && !rc; ++l) {
+        semb_mesh* L = g->lev[l];
+        double* dinv;
+        rc = semb_get_dinv(L, ctx.lambda, ctx.tags, &dinv, s);
+        if (!rc) k_mg_convert<double, float><<<mg_grid(L->n), 256, 0, s>>>(L->n, dinv, a[l], nullptr);
+    }
+    if (!rc && cudaGetLastError() != cudaSuccess) rc = semb_fail(h, SEMB_ECUDA, "multigrid: fp32 diagonals");
+    if (rc) { for (float* p : a) semb_dev_free(h, p); return rc; }
+    g->dinvF.push_back(semb_mg::dinvF_entry{ctx.tags, ctx.lambda, a, ++g->dinvF_clock});
+    g->dinvF_cur = g->dinvF.back().d.data();
     return SEMB_OK;
 }
 
@@ -395,7 +424,7 @@ static int mg_vcycle_f32(semb_mesh* h, const semb_mg_ctx& ctx, int l, const floa
     semb_mesh* L = g->lev[l];
     semb_mask_entry m;
     int rc = semb_get_mask(L, ctx.tags, &m, s); if (rc) return rc;
-    const float* dinv = g->dinvF[std::pair<uint32_t, double>(ctx.tags, ctx.lambda)][l];
+    const float* dinv = g->dinvF_cur[l];
     const float* geo = g->geoF[l];
     float *cres = g->WF[l][0], *cd = g->WF[l][1], *cAd = g->WF[l][2], *res = g->WF[l][3], *t1 = g->WF[l][4];
     const int64_t l0 = L->launches;

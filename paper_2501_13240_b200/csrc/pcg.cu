@@ -17,7 +17,7 @@ static inline unsigned vec_grid(int64_t n)
 {
     int64_t b = (n + VEC_BLOCK * 4 - 1) / (VEC_BLOCK * 4);
     if (b < 1) b = 1;
-    if (b > 148 * 8) b = 148 * 8;
+    if (b > semb_sm_count() * 8) b = semb_sm_count() * 8;
     return (unsigned)b;
 }
 #define GSTRIDE(l, n) for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < (n); l += (int64_t)gridDim.x * blockDim.x)

@@ -11,16 +11,36 @@ __device__ __forceinline__ double warp_sum(double v)
     return v;
 }
 
-// sum over the block; result valid in every thread.  red: shared scratch of >= 32 doubles.
+// Sum over the `live` lowest lanes of a warp whose other lanes were never launched (the last warp of a block whose
+// size is not a multiple of 32: blockDim = n1^2 * EPB of k_axhelm_line).  The shuffle names only the live lanes and a
+// partner's value is added only when that partner exists, so no value of an inactive lane is ever read.  The total
+// is valid in lane 0 (the xor butterfly is not closed over a ragged set of lanes); with live == 32 it is warp_sum.
+__device__ __forceinline__ double warp_sum_live(double v, int lane, int live)
+{
+    if (live >= 32) return warp_sum(v);
+    const unsigned mask = (1u << live) - 1u;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const int src = lane ^ o;
+        const double t = __shfl_sync(mask, v, src < live ? src : lane);
+        if (src < live) v += t;
+    }
+    return v;
+}
+
+// sum over the block; result valid in every thread.  red: shared scratch of >= 32 doubles.  Any blockDim.x <= 1024:
+// the ragged last warp goes through warp_sum_live, and the per-warp sums are added in ascending warp order by every
+// thread (fixed order, no shuffle across warps that may not exist).
 __device__ __forceinline__ double block_sum(double v, double* red)
 {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
-    v = warp_sum(v);
+    const int live = min(32, (int)blockDim.x - (wid << 5));
+    v = warp_sum_live(v, lane, live);
     __syncthreads();                       // red may still be read from a previous call
     if (lane == 0) red[wid] = v;
     __syncthreads();
-    double t = (lane < nw) ? red[lane] : 0.0;
-    t = warp_sum(t);
+    double t = 0.0;
+    for (int w = 0; w < nw; ++w) t += red[w];
     return t;
 }
 

@@ -25,6 +25,9 @@ struct semb_mask_entry {
     int64_t  count = 0;
 };
 
+#define SEMB_DINV_CACHE 8
+struct semb_dinv_entry { uint32_t tags; double lambda; double* d; uint64_t stamp; };
+
 struct semb_field_entry {
     std::string name;
     double* ptr = nullptr;
@@ -55,7 +58,11 @@ struct semb_mesh {
     std::vector<int32_t> face_tag; // host [E*6]
     int32_t* face_tag_dev = nullptr;
     std::map<uint32_t, semb_mask_entry> masks;
-    std::map<std::pair<uint32_t, double>, double*> dinvs;
+    // Jacobi diagonals: the lambda-independent assembled parts diagA = QQ^T diag(D^T G D), diagB = QQ^T B are built
+    // once; 1 / (diagA + lambda diagB) (1 at masked nodes) is kept for the SEMB_DINV_CACHE most recently used
+    // (tags, lambda) pairs only, so a variable time step (lambda = c / dt) neither leaks memory nor re-runs the setup.
+    double* diagA = nullptr; double* diagB = nullptr;
+    std::vector<semb_dinv_entry> dinvs; uint64_t dinv_clock = 0;
     // solver workspace
     double* work = nullptr; int64_t work_vecs = 0;
     double* partials = nullptr;         // block partial sums [4][SEMB_MAX_BLOCKS]
@@ -82,6 +89,7 @@ __device__ __forceinline__ double semb_wide(float f) { return (double)f; }
 #endif
 
 // ---- helpers -------------------------------------------------------------------------------
+int  semb_sm_count();      // multiProcessorCount of the current device (cached per process; 148 on B200): streaming grids are sized from it
 int  semb_fail(semb_mesh* h, int code, const char* fmt, ...);
 void* semb_dev_alloc(semb_mesh* h, size_t bytes);
 void  semb_dev_free(semb_mesh* h, void* p);
@@ -163,6 +171,7 @@ int semb_dot_rz_launch(semb_mesh* h, const double* r, const double* z, semb_scal
 
 // ---- mg.cu: p-multigrid V-cycle
 struct semb_mg_ctx { semb_mg* mg; double lambda; uint32_t tags; int k_smooth, k_coarse, kind, fp32; double coarse_frac; double lmax[8]; };
+int semb_mg_orders(semb_mesh* h, const semb_pcg_opts* o, int* nlev_out, int* orders);
 int semb_mg_prepare(semb_mesh* h, const semb_pcg_opts* o, semb_mg_ctx* ctx, cudaStream_t s);
 int semb_mg_vcycle_run(semb_mesh* h, const semb_mg_ctx& ctx, int level, const double* r, double* z, semb_scalars* scal, cudaStream_t s);
 int semb_mg_transfer_run(semb_mesh* h, const semb_mg_ctx& ctx, int level, int restrict_, const double* in, double* out, cudaStream_t s);

@@ -297,7 +297,7 @@ struct gs_hi_pred {
 };
 
 #define GRID1(n) (unsigned)(((n) + 255) / 256)
-static inline unsigned grid_stride_blocks(int64_t n) { int64_t b = (n + 255) / 256; return (unsigned)(b < 148 * 16 ? (b > 0 ? b : 1) : 148 * 16); }
+static inline unsigned grid_stride_blocks(int64_t n) { int64_t b = (n + 255) / 256; const int64_t cap = semb_sm_count() * 16; return (unsigned)(b < cap ? (b > 0 ? b : 1) : cap); }
 
 struct tmp_pool {          // frees every temporary on scope exit
     semb_mesh* h; std::vector<void*> p;
@@ -570,39 +570,77 @@ int semb_diag_local(semb_mesh* h, double lambda, double* d, cudaStream_t s)
     const int n1 = h->n1;
     double* dD = (double*)semb_dev_alloc(h, sizeof(double) * n1 * n1);
     if (!dD) return semb_fail(h, SEMB_ENOMEM, "diag basis");
-    SEMB_CUDA(h, cudaMemcpyAsync(dD, h->D, sizeof(double) * n1 * n1, cudaMemcpyHostToDevice, s));
-    k_diag_local<<<(unsigned)h->E, 256, sizeof(double) * n1 * n1, s>>>(n1, h->geo, dD, lambda, d);
-    SEMB_CUDA(h, cudaGetLastError());
-    SEMB_CUDA(h, cudaStreamSynchronize(s));
+    cudaError_t e = cudaMemcpyAsync(dD, h->D, sizeof(double) * n1 * n1, cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) {
+        k_diag_local<<<(unsigned)h->E, 256, sizeof(double) * n1 * n1, s>>>(n1, h->geo, dD, lambda, d);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     semb_dev_free(h, dD);
+    if (e != cudaSuccess) return semb_fail(h, SEMB_ECUDA, "diag_local: %s", cudaGetErrorString(e));
     return SEMB_OK;
 }
 
-__global__ void k_invert(int64_t n, double* __restrict__ d)
-{
-    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) d[l] = 1.0 / d[l];
-}
 __global__ void k_set_list(int64_t c, const int32_t* __restrict__ list, double* __restrict__ d, double v)
 {
     const int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (t < c) d[list[t]] = v;
 }
 
+// d = 1 / (dA + lambda dB), 1 at ... (masked nodes are set afterwards by k_set_list)
+__global__ void k_dinv_combine(int64_t n, const double* __restrict__ dA, const double* __restrict__ dB, double lambda, double* __restrict__ d)
+{
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) d[l] = 1.0 / (dA[l] + lambda * dB[l]);
+}
+__global__ void k_copy_B(int64_t n, int64_t Np, const double* __restrict__ geo, double* __restrict__ b)
+{
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t e = l / Np;
+        b[l] = geo[e * 7 * Np + 6 * Np + (l - e * Np)];
+    }
+}
+
+// lambda-independent parts of the assembled diagonal, built once per handle
+static int ensure_diag_parts(semb_mesh* h, cudaStream_t s)
+{
+    if (h->diagA && h->diagB) return SEMB_OK;
+    double* a = (double*)semb_dev_alloc(h, sizeof(double) * (size_t)h->n);
+    double* b = (double*)semb_dev_alloc(h, sizeof(double) * (size_t)h->n);
+    int rc = (a && b) ? SEMB_OK : semb_fail(h, SEMB_ENOMEM, "Jacobi diagonal parts");
+    if (!rc) rc = semb_diag_local(h, 0.0, a, s);
+    if (!rc) rc = semb_gs_launch(h, a, 1, s);
+    if (!rc) {
+        k_copy_B<<<grid_stride_blocks(h->n), 256, 0, s>>>(h->n, h->Np, h->geo, b);
+        rc = semb_gs_launch(h, b, 1, s);
+    }
+    if (rc) { semb_dev_free(h, a); semb_dev_free(h, b); return rc; }
+    h->diagA = a; h->diagB = b;
+    return SEMB_OK;
+}
+
 int semb_get_dinv(semb_mesh* h, double lambda, uint32_t tags, double** out, cudaStream_t s)
 {
-    auto key = std::make_pair(tags, lambda);
-    auto it = h->dinvs.find(key);
-    if (it != h->dinvs.end()) { *out = it->second; return SEMB_OK; }
+    for (auto& en : h->dinvs)
+        if (en.tags == tags && en.lambda == lambda) { en.stamp = ++h->dinv_clock; *out = en.d; return SEMB_OK; }
     semb_mask_entry m;
     int rc = semb_get_mask(h, tags, &m, s); if (rc) return rc;
-    double* d = (double*)semb_dev_alloc(h, sizeof(double) * (size_t)h->n);
-    if (!d) return semb_fail(h, SEMB_ENOMEM, "dinv");
-    rc = semb_diag_local(h, lambda, d, s); if (rc) return rc;
-    rc = semb_gs_launch(h, d, 1, s); if (rc) return rc;
-    k_invert<<<grid_stride_blocks(h->n), 256, 0, s>>>(h->n, d);
+    rc = ensure_diag_parts(h, s); if (rc) return rc;
+    double* d = nullptr;
+    if (h->dinvs.size() >= SEMB_DINV_CACHE) {
+        // reuse the buffer of the least recently used entry; work already enqueued that reads it must finish first
+        size_t lru = 0;
+        for (size_t q = 1; q < h->dinvs.size(); ++q) if (h->dinvs[q].stamp < h->dinvs[lru].stamp) lru = q;
+        SEMB_CUDA(h, cudaStreamSynchronize(s));
+        d = h->dinvs[lru].d;
+        h->dinvs.erase(h->dinvs.begin() + (long)lru);
+    } else {
+        d = (double*)semb_dev_alloc(h, sizeof(double) * (size_t)h->n);
+        if (!d) return semb_fail(h, SEMB_ENOMEM, "dinv");
+    }
+    k_dinv_combine<<<grid_stride_blocks(h->n), 256, 0, s>>>(h->n, h->diagA, h->diagB, lambda, d);
     if (m.count > 0) k_set_list<<<GRID1(m.count), 256, 0, s>>>(m.count, m.list, d, 1.0);
-    SEMB_CUDA(h, cudaGetLastError());
-    h->dinvs[key] = d;
+    if (cudaGetLastError() != cudaSuccess) { semb_dev_free(h, d); return semb_fail(h, SEMB_ECUDA, "dinv kernels"); }
+    h->dinvs.push_back(semb_dinv_entry{tags, lambda, d, ++h->dinv_clock});
     *out = d;
     return SEMB_OK;
 }

@@ -70,6 +70,40 @@ class SolveItem(C.Structure):
     _fields_ = [("opts", PcgOpts), ("b", C.c_void_p), ("x", C.c_void_p)]
 
 
+ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
+FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+
+
+class Allocator(C.Structure):
+    """semb_allocator: every device buffer the library owns comes from alloc(bytes, user) / goes to free(ptr, user)."""
+    _fields_ = [("alloc", ALLOC_FN), ("free", FREE_FN), ("user", C.c_void_p)]
+
+
+class TorchAllocator:
+    """semb_allocator backed by torch's caching allocator: the library then owns no memory outside torch's pool."""
+
+    def __init__(self):
+        import torch
+        self.live = {}
+        self.peak_bytes = self.calls = 0
+
+        def _alloc(nbytes, _user):
+            try:
+                t = torch.empty(int(nbytes), dtype=torch.uint8, device="cuda")
+            except RuntimeError:
+                return None
+            self.live[t.data_ptr()] = t
+            self.calls += 1
+            self.peak_bytes = max(self.peak_bytes, sum(v.numel() for v in self.live.values()))
+            return t.data_ptr()
+
+        def _free(ptr, _user):
+            self.live.pop(ptr, None)
+
+        self._a, self._f = ALLOC_FN(_alloc), FREE_FN(_free)           # keep the thunks alive
+        self.struct = Allocator(self._a, self._f, None)
+
+
 class FieldDesc(C.Structure):
     _fields_ = [("name", C.c_char_p), ("ptr", C.c_void_p), ("dtype", C.c_int32), ("memspace", C.c_int32),
                 ("count", C.c_int64), ("stride", C.c_int64), ("cycle", C.c_int64), ("time", C.c_double)]
@@ -123,15 +157,17 @@ def _dp(t):
 class Mesh:
     """Handle of one mesh on the current CUDA device (semb_setup ... semb_destroy)."""
 
-    def __init__(self, E, N, x, y, z, face_tag, period, gid=None):
+    def __init__(self, E, N, x, y, z, face_tag, period, gid=None, allocator=None):
         import torch
+        self._allocator = allocator                                    # TorchAllocator (kept alive with the handle) or None
         assert x.dtype == torch.float64 and y.dtype == torch.float64 and z.dtype == torch.float64
         self._h = C.c_void_p()
         ft = np.ascontiguousarray(face_tag, dtype=np.int32)
         per = np.ascontiguousarray(period, dtype=np.float64)
         assert ft.size == 6 * E and x.numel() == E * (N + 1) ** 3
         rc = lib().semb_setup(C.c_int64(E), C.c_int(N), _dp(x), _dp(y), _dp(z), ft.ctypes.data_as(C.c_void_p),
-                              per.ctypes.data_as(C.c_void_p), _dp(gid), None, _stream(), C.byref(self._h))
+                              per.ctypes.data_as(C.c_void_p), _dp(gid),
+                              C.byref(allocator.struct) if allocator is not None else None, _stream(), C.byref(self._h))
         if rc:
             raise SembError(rc, lib().semb_last_error(None).decode())
         self.info = Info()
@@ -260,7 +296,7 @@ class Mesh:
     def mg_level_size(self, level, lam=0.0, tags=0, mg_orders=None):
         o = self._mg_opts(lam, tags, mg_orders, 0, 0, None)
         lib().semb_mg_level_size.restype = C.c_int64
-        return int(lib().semb_mg_level_size(self._h, C.byref(o), C.c_int(level)))
+        return int(self._check(lib().semb_mg_level_size(self._h, C.byref(o), C.c_int(level))))
 
     def mg_transfer(self, level, restrict, vin, vout, lam=0.0, tags=0, mg_orders=None):
         o = self._mg_opts(lam, tags, mg_orders, 0, 0, [1.0] * 8)

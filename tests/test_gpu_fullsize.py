@@ -7,8 +7,9 @@
     test_oracle_operator.py), (iii) gather-scatter is checked through a property that holds at any size: an
     integer-valued continuous field sums exactly, QQ^T v = mult * v bitwise, with mult from the lattice.
   * cfg1 (16^3 deformed box): everything element by element against the oracle.
-  * cfg2 (cylinder O-grid, 73 728 elements, N=7): numbering bit-exact, axhelm and gather-scatter element by element,
-    Chebyshev(2)-Jacobi and Jacobi PCG: first 20 residual-history entries and the ORACLE-VERIFIED true residual
+  * cfg2 (cylinder O-grid, 73 728 elements, N=7): numbering bit-exact; the geometric factors against the oracle's within
+    the conditioning bound of DESIGN.md R22; axhelm and gather-scatter element by element at 1e-12 on the library's
+    factors; Chebyshev(2)-Jacobi and Jacobi PCG: first 20 residual-history entries and the ORACLE-VERIFIED true residual
     ||b - A_oracle x_gpu|| / ||b|| <= 2e-10.
   * cfg4 (O-grid, 64 000 elements, N=9): numbering, axhelm, gather-scatter, one Helmholtz solve, same bars.
 """
@@ -44,17 +45,29 @@ def normwise(a, ref):
     return np.abs(a - ref).max() / max(np.abs(ref).max(), 1e-300)
 
 
-def geometry_tolerance(orc, m):
-    """Parity bar for outputs that depend on G when BOTH sides recompute G from the coordinates (R16):
-    differentiating coordinates of size c with D (||D||_inf = max row sum) has absolute error <= ~eps ||D||_inf c,
-    against a derivative of size (element half-width) = min node spacing / (xi_1 - xi_0); the ratio is the
-    conditioning of G, identical for the oracle and the GPU, so two correct fp64 evaluations may differ by
-    2 eps kappa.  1e-12 (north_star) wherever that bound is smaller."""
+def geometry_bound(orc, m):
+    """DESIGN.md reading R22: bar on |G_gpu - G_oracle| per factor, relative to the largest entry of the factor tensor,
+    when BOTH sides compute the factors from the coordinates.  A coordinate derivative sum_m D_im c_m carries an absolute
+    rounding error <= eps ||D||_inf max|c| against a true value of (element width)/2 >= min node spacing / (xi_1 - xi_0),
+    i.e. a relative error delta = eps kappa, kappa = ||D||_inf max|c| (xi_1 - xi_0) / min spacing; every factor is a
+    degree-2 rational function of the nine derivatives (adj J adj J^T / det J), so two correct evaluations can differ by
+    up to ~(2 + 2) delta each way, 8 eps kappa, if every rounding error aligned.  They do not: measured 0.01 eps kappa
+    (profiles/r2_fullsize_parity.md).  Bar = eps kappa: 8x below the worst case, 20-100x above what is measured.  Only the
+    factors are held to this; axhelm and gather-scatter are held to north_star's 1e-12 on the SAME factors (the library's)."""
     xi = orc.gll(m.N)[0]
     D = orc.dhat(m.N)
     cmax = max(np.abs(m.x).max(), np.abs(m.y).max(), np.abs(m.z).max())
     kappa = np.abs(D).sum(axis=1).max() * cmax * (xi[1] - xi[0]) / orc.min_spacing(m.E, m.N, m.x, m.y, m.z)
-    return max(TOL, 2.0 * np.finfo(np.float64).eps * kappa)
+    return np.finfo(np.float64).eps * kappa, kappa
+
+
+def record(line):
+    """measured errors, kept next to the run (gpurun_out/fullsize_parity.txt; summarised in profiles/ and DESIGN.md R22)"""
+    import os
+    os.makedirs("gpurun_out", exist_ok=True)
+    with open(os.path.join("gpurun_out", "fullsize_parity.txt"), "a") as f:
+        f.write(line + "\n")
+    print(line)
 
 
 def lattice_ids(ne, N):
@@ -187,18 +200,33 @@ def test_ogrid_fullsize(torch_cuda, semb, orc, xi_of, cfg):
     try:
         assert G.n_unique == P.n_unique == I.ogrid_unique_nodes(m.meta["n_c"], m.meta["n_r"], m.meta["n_z"], m.N)
         assert np.array_equal(G.gid_host(), P.gid)
-        tol = geometry_tolerance(orc, m)          # tanh-clustered layers: kappa ~ 4e4 (N=7), ~ 9e4 (N=9): tol ~ 8e-12 / 4e-11
-        assert tol <= 5e-11
+        # (a) the factors themselves: conditioning bound of reading R22, per factor against the tensor's largest entry
+        geo_gpu = G.geo_host()
+        bar, kappa = geometry_bound(orc, m)
+        assert bar <= 2.5e-11
+        scale = np.abs(P.geo[:, :6]).max(axis=(1, 2))[:, None]                    # per element
+        gerr = max(float((np.abs(geo_gpu[:, c] - P.geo[:, c]) / scale).max()) for c in range(6))
+        berr = float((np.abs(geo_gpu[:, 6] - P.geo[:, 6]) / np.abs(P.geo[:, 6]).max(axis=1)[:, None]).max())
+        record(f"cfg{cfg} geometric factors: kappa {kappa:.3e}, bar eps kappa {bar:.2e}, measured G {gerr:.2e}, B {berr:.2e}")
+        assert gerr <= bar and berr <= bar
+        # (b) axhelm and gather-scatter at north_star's 1e-12: the oracle applies ITS operator to the library's factors,
+        #     so a kernel defect of 1e-12 cannot hide behind the conditioning of G
         for lam in (0.0, prm["lam"] if prm["lam"] else 1e4):
             u = I.uniform(I.seed_for(cfg, 1), m.n)
             ud = dev(torch, u); wd = torch.empty_like(ud)
             G.apply_axhelm(ud, wd, lam=lam)
-            ref = orc.axhelm(m.E, m.N, P.geo, lam, u)
-            err = normwise(wd.cpu().numpy(), ref)
-            print(f"cfg{cfg} lam={lam}: axhelm normwise error {err:.2e} (bar {tol:.2e})")
-            assert err <= tol
+            ref = orc.axhelm(m.E, m.N, geo_gpu, lam, u)
+            w = wd.cpu().numpy()
+            err = normwise(w, ref)
+            err_el = float((np.abs(w - ref).reshape(m.E, -1).max(axis=1) / np.abs(ref).reshape(m.E, -1).max(axis=1)).max())
+            err_own = normwise(w, orc.axhelm(m.E, m.N, P.geo, lam, u))
             G.gather_scatter(wd)
-            assert normwise(wd.cpu().numpy(), orc.gs(P.gid, P.n_unique, ref)) <= tol
+            err_gs = normwise(wd.cpu().numpy(), orc.gs(P.gid, P.n_unique, ref))
+            record(f"cfg{cfg} lam={lam}: axhelm normwise {err:.2e} (per element {err_el:.2e}), gather-scatter {err_gs:.2e} "
+                   f"[bar 1e-12]; axhelm against the oracle's own factors {err_own:.2e} [context: bounded by R22, {bar:.1e}]")
+            assert err <= TOL and err_el <= TOL and err_gs <= TOL
+            assert err_own <= bar
+        del geo_gpu
         f = I.divergence_source(m, I.seed_for(cfg, 3))
         if cfg == 2:       # pressure Poisson, Chebyshev(2)-Jacobi with the oracle's lambda_max, then plain Jacobi
             b = P.assemble_rhs(f)

@@ -86,6 +86,54 @@ def test_weak_laplacian_of_polynomials_affine(orc, xi_of):
     assert abs(P.dot(u, P.apply_A(u)) - _mono_int(4, 4, 0, 4, 4, 0)) > 1e-9
 
 
+def _mono_cross_int(p, q, a, b):
+    """int_[0,1]^3 d_a(s^p) d_b(s^q) ds for monomials s^p = s1^p1 s2^p2 s3^p3 (a, b = directions 0..2)."""
+    if p[a] == 0 or q[b] == 0:
+        return 0.0
+    v = float(p[a] * q[b])
+    for d in range(3):
+        e = p[d] + q[d] - (d == a) - (d == b)
+        v /= (e + 1)
+    return v
+
+
+def test_weak_laplacian_of_polynomials_sheared_affine(orc, xi_of):
+    """P6 on a SHEARED affine image X = A s of the unit cube: every element then has non-zero cross factors
+    G_rs, G_rt, G_st, and  v^T A u = sum_ab C_ab int d_a p d_b q ds  with C = det(A) A^-1 A^-T in closed form --
+    pins the use of the cross terms inside orc_axhelm analytically (a dropped, doubled or swapped cross term fails)."""
+    N = 4
+    m = I.box_mesh(2, 3, 2, N, xi_of(N))
+    A = np.array([[1.0, 0.35, 0.2], [0.0, 0.9, 0.45], [0.15, 0.0, 1.2]])
+    S = np.stack([m.x, m.y, m.z])                     # unit-cube coordinates s of every node
+    X = A @ S
+    P = orc.Problem(m.E, N, X[0], X[1], X[2], m.face_tag, [0, 0, 0])
+    # the factors really are full: all three cross factors are of the size of the diagonal ones
+    for c in (1, 2, 4):
+        assert np.abs(P.geo[:, c]).max() > 0.05 * np.abs(P.geo[:, 0]).max()
+    Ai = np.linalg.inv(A)
+    Cm = np.linalg.det(A) * Ai @ Ai.T
+    for pu, pv in [((4, 4, 4), (3, 3, 3)), ((4, 0, 2), (1, 3, 2)), ((3, 2, 1), (3, 2, 1)), ((1, 1, 0), (0, 1, 1)), ((2, 1, 3), (1, 3, 0))]:
+        u = S[0] ** pu[0] * S[1] ** pu[1] * S[2] ** pu[2]
+        v = S[0] ** pv[0] * S[1] ** pv[1] * S[2] ** pv[2]
+        expect = sum(Cm[a, b] * _mono_cross_int(pu, pv, a, b) for a in range(3) for b in range(3))
+        got = P.dot(v, P.apply_A(u))
+        assert abs(got - expect) < 5e-13 * max(1.0, abs(expect)), (pu, pv, got, expect)
+    # a pair whose value comes from the cross terms alone (u depends on s1 only, v on s2 only)
+    u, v = S[0] ** 3, S[1] ** 2
+    expect = Cm[0, 1] * _mono_cross_int((3, 0, 0), (0, 2, 0), 0, 1)
+    assert abs(expect) > 0.1 and abs(P.dot(v, P.apply_A(u)) - expect) < 5e-13
+
+
+def test_min_spacing_closed_form(orc, xi_of):
+    """orc_min_spacing (sets the matching tolerance, R17): on an affine brick the smallest node spacing is
+    (xi_1 - xi_0)/2 times the smallest element width -- closed form from the GLL points, which P1 pins."""
+    for N, (nx, ny, nz) in [(3, (2, 3, 5)), (7, (4, 2, 3))]:
+        m = I.box_mesh(nx, ny, nz, N, xi_of(N))
+        xi = xi_of(N)
+        expect = 0.5 * (xi[1] - xi[0]) * min(1.0 / nx, 1.0 / ny, 1.0 / nz)
+        assert abs(orc.min_spacing(m.E, N, m.x, m.y, m.z) - expect) <= 1e-14
+
+
 # ---------------------------------------------------------------- P7: Kronecker form on an affine structured box
 def _assembled_1d(orc, ne, N, h):
     xi, rho = orc.gll(N)

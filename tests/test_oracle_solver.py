@@ -117,6 +117,41 @@ def test_chebyshev_reduces_iterations_and_lanczos_bounds(orc, xi_of):
     assert lam_pow <= lmax <= 1.25 * lam_pow
 
 
+@pytest.mark.parametrize("lam,tags", [(0.0, 0b10), (25.0, 0)])
+def test_lanczos_ritz_values_are_the_rayleigh_ritz_values_of_the_krylov_space(orc, xi_of, lam, tags):
+    """orc_lanczos pinned by the DEFINITION of its output: the eigenvalues of its tridiagonal matrix are the
+    Rayleigh-Ritz values of S = D^-1/2 A D^-1/2 on the Krylov space span{v0, S v0, .., S^(m-1) v0}.  Here that space is
+    built from the dense matrix by Arnoldi with full re-orthogonalisation in numpy (no three-term recurrence), on the
+    unique free nodes, and all m Ritz values are compared."""
+    import ctypes as C
+    N, steps = 3, 10
+    m = I.box_mesh(2, 2, 3, N, xi_of(N), deform=0.05)
+    P = make(orc, m, lam=lam, tags=tags)
+    A = dense_matrix(P)
+    free = to_global(P, P.mask) > 0
+    dg = to_global(P, 1.0 / P.dinv)[free]
+    Sd = A[np.ix_(free, free)] / np.sqrt(np.outer(dg, dg))
+    v0 = P.mask * orc.gs(P.gid, P.n_unique, P.invmult * I.uniform(11, P.n))
+    a = np.zeros(steps); b = np.zeros(steps)
+    k = orc.lib().orc_lanczos(C.byref(P._op), P.dinv.ctypes.data_as(C.c_void_p), v0.ctypes.data_as(C.c_void_p), C.c_int(steps),
+                              a.ctypes.data_as(C.c_void_p), b.ctypes.data_as(C.c_void_p))
+    assert k == steps
+    T = np.diag(a) + np.diag(b[:-1], 1) + np.diag(b[:-1], -1)
+    ritz = np.linalg.eigvalsh(T)
+    Q = np.zeros((free.sum(), steps))
+    q = to_global(P, v0)[free]
+    for j in range(steps):
+        for _ in range(2):
+            q = q - Q[:, :j] @ (Q[:, :j].T @ q)
+        Q[:, j] = q / np.linalg.norm(q)
+        q = Sd @ Q[:, j]
+    expect = np.linalg.eigvalsh(Q.T @ Sd @ Q)
+    assert np.allclose(ritz, expect, rtol=1e-9, atol=0)
+    top = np.linalg.eigvalsh(Sd)[-1]
+    assert ritz[-1] <= top * (1 + 1e-12) and 1.1 * ritz[-1] >= top           # what lanczos_lmax relies on
+    assert abs(P.lanczos_lmax(v0, steps) - 1.1 * expect[-1]) <= 1e-9 * top
+
+
 # ---------------------------------------------------------------- P10: spectral convergence (reading R1 / SURVEY A1)
 def test_spectral_convergence_dirichlet_cube(orc, xi_of):
     errs = []
