@@ -110,6 +110,27 @@ SEMB_API int semb_apply_axhelm(semb_handle h, double lambda, const double* lambd
                       const double* lambda1_or_null, const double* u, double* w, int nfields,
                       void* stream);
 
+/* ---- geometry representation read by semb_apply_axhelm and by every fp64 operator application of the solvers
+ * (SURVEY.md §8 f-3 "on-the-fly geometric factors ... mixed-precision geo storage"; PAPER.md:L100 fixes only the chain
+ * rule; the paper's box meshes are vertically stretched Cartesian element maps, i.e. affine bricks).
+ * The operator is unchanged (reading R23); what changes is what is streamed from memory per application:
+ *   SEMB_GEO_STORED     (default) G(6)+B per node in fp64                                  48 (56) B/node
+ *   SEMB_GEO_F32        the same factors rounded to float once, widened on load, fp64 arithmetic:
+ *                       w = D^T fl32(G) D u + lambda fl32(B) u exactly                     24 (28) B/node
+ *   SEMB_GEO_AFFINE     every element a parallelepiped: 7 constants per element            64 B/element
+ *   SEMB_GEO_TRILINEAR  every element the trilinear image of its 8 corner nodes: 24 coefficients per element, Jacobian,
+ *                       cofactors and J recomputed per node                                 192 B/element
+ * tol: largest admissible distance of any node from the affine / trilinear map of its element's corners, relative to the
+ * largest |coordinate| of the mesh; <= 0 => 16 eps (coordinates that ARE that map up to their own rounding).
+ * dev_out_or_null HOST [2]: the measured deviations (trilinear, affine).  Returns SEMB_EGEOM and leaves the mode
+ * unchanged when the mesh is not in the class.  Coefficient fields (lambda0 / lambda1) need SEMB_GEO_STORED.
+ * Synchronises the stream the first time a class is measured. */
+#define SEMB_GEO_STORED     0
+#define SEMB_GEO_F32        1
+#define SEMB_GEO_AFFINE     2
+#define SEMB_GEO_TRILINEAR  3
+SEMB_API int semb_set_geometry_mode(semb_handle h, int mode, double tol, double* dev_out_or_null, void* stream);
+
 /* ---- direct-stiffness summation QQ^T -------------------------------------
  * w device [nfields][n], in place: every copy of a global node receives the sum of all copies,
  * summed in ascending local index (deterministic, no atomics). */
@@ -263,6 +284,12 @@ SEMB_API int semb_pcg_solve_host(semb_handle h, const semb_pcg_opts* opts, const
 
 /* Blocking copy of `bytes` bytes from device memory (e.g. a semb_info view) to host memory. */
 SEMB_API int semb_read_device(const void* dev, void* host, size_t bytes);
+
+/* Measurement aid, not part of the method ("a measured read-heavy stream ceiling"): dst[l] = sum over
+ * c < nread of src[c*n + l], a pure stream with nread : 1 read : write mix (axhelm's is 7 : 1).  src device [nread*n],
+ * dst device [n], both 16-byte aligned, n even, 1 <= nread <= 8.  Asynchronous on stream.  bench.py times it to state
+ * what HBM delivers for that mix next to the 1 : 1 copy bandwidth. */
+SEMB_API int semb_stream_probe(const double* src, double* dst, int64_t n, int nread, void* stream);
 
 /* Library version and the compute capability it was built for ("sm_100a"). */
 SEMB_API const char* semb_version(void);

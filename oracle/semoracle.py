@@ -15,15 +15,16 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "semoracle.c")
+_SRCS = [_SRC, os.path.join(_HERE, "semimage.c")]
 _LIB = os.path.join(_HERE, "libsemoracle.so")
 _lib = None
 
 
 def build(force=False):
     """Compile semoracle.c -> libsemoracle.so (gcc -O2, OpenMP, no FP contraction)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(f) for f in _SRCS):
         cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-ffp-contract=off", "-fPIC", "-shared",
-               "-o", _LIB, _SRC, "-lm"]
+               "-o", _LIB] + _SRCS + ["-lm"]
         subprocess.run(cmd, check=True)
     return _LIB
 
@@ -351,3 +352,56 @@ class Multigrid:
                                   C.c_int(1 if x0 is None else 0), _p(hist), C.c_int(hist_len), _p(out3))
         it = int(out3[0])
         return dict(x=x, iters=it, status=int(st), r0=out3[1], rn=out3[2], hist=hist[:min(hist_len, it + 1)])
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# f-4  in-situ image consumer (semimage.c; reading R24)
+class ImgView(C.Structure):
+    _fields_ = [("width", C.c_int32), ("height", C.c_int32), ("origin", C.c_double * 3), ("u", C.c_double * 3),
+                ("v", C.c_double * 3), ("du", C.c_double), ("dv", C.c_double)]
+
+
+class ImgCmap(C.Structure):
+    _fields_ = [("lo", C.c_double), ("hi", C.c_double), ("ncolors", C.c_int32), ("rgb", (C.c_uint8 * 3) * 16),
+                ("background", C.c_uint32)]
+
+
+def make_view(width, height, origin, u, v, du, dv):
+    vw = ImgView(width, height)
+    for c in range(3):
+        vw.origin[c], vw.u[c], vw.v[c] = float(origin[c]), float(u[c]), float(v[c])
+    vw.du, vw.dv = float(du), float(dv)
+    return vw
+
+
+def make_cmap(lo, hi, colors, background=0xff000000):
+    cm = ImgCmap(float(lo), float(hi), len(colors))
+    for m, col in enumerate(colors):
+        for c in range(3):
+            cm.rgb[m][c] = int(col[c])
+    cm.background = int(background)
+    return cm
+
+
+def colormap(cm, val):
+    val = _f64(val); out = np.zeros(val.size, dtype=np.uint32)
+    lib().orc_colormap(C.byref(cm), C.c_int64(val.size), _p(val), _p(out))
+    return out
+
+
+def image_slice(E, N, x, y, z, field, vw, cm):
+    """(rgba uint32 [H, W], cell_of int64 [H, W])"""
+    rgba = np.zeros(vw.width * vw.height, dtype=np.uint32); cell = np.zeros(vw.width * vw.height, dtype=np.int64)
+    lib().orc_image_slice(C.c_int64(E), C.c_int(N), _p(_f64(x)), _p(_f64(y)), _p(_f64(z)), _p(_f64(field)), C.byref(vw), C.byref(cm),
+                          _p(rgba), _p(cell))
+    return rgba.reshape(vw.height, vw.width), cell.reshape(vw.height, vw.width)
+
+
+def image_isosurface(E, N, x, y, z, field, iso, cfield, vw, cm, light, dlo, dhi):
+    """(rgba uint32 [H, W], key uint64 [H, W]); key >> 32 = depth quantised to 2^-32 of [dlo, dhi]"""
+    rgba = np.zeros(vw.width * vw.height, dtype=np.uint32); key = np.zeros(vw.width * vw.height, dtype=np.uint64)
+    lt = _f64(light)
+    lib().orc_image_isosurface(C.c_int64(E), C.c_int(N), _p(_f64(x)), _p(_f64(y)), _p(_f64(z)), _p(_f64(field)), C.c_double(iso),
+                               _p(_f64(cfield)) if cfield is not None else None, C.byref(vw), C.byref(cm), _p(lt),
+                               C.c_double(dlo), C.c_double(dhi), _p(rgba), _p(key))
+    return rgba.reshape(vw.height, vw.width), key.reshape(vw.height, vw.width)

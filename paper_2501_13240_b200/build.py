@@ -9,10 +9,11 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-LIB = os.path.join(HERE, "libsemb200.so")
+LIB = os.environ.get("SEMB_LIB_OUT") or os.path.join(HERE, "libsemb200.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-         "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr"]
+         "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr"] + \
+    os.environ.get("SEMB_NVCC_FLAGS", "").split()          # tuning experiments: e.g. SEMB_NVCC_FLAGS=-DSEMB_MINB10=2
 
 
 def sources():

@@ -21,7 +21,29 @@
 #include "semb_internal.h"
 
 // D for every order 1..SEMB_MAX_N, row-major n1 x n1 at c_D[N]; filled at setup.
-__constant__ double c_D[SEMB_MAX_N + 1][SEMB_MAXN1 * SEMB_MAXN1];
+static __constant__ double c_D[SEMB_MAX_N + 1][SEMB_MAXN1 * SEMB_MAXN1];
+// GLL nodes and weights per order (the on-the-fly geometry modes rebuild W = rho_i rho_j rho_k and the trilinear map from them)
+static __constant__ double c_xi[SEMB_MAX_N + 1][SEMB_MAXN1], c_rho[SEMB_MAX_N + 1][SEMB_MAXN1];
+
+// ---- geometry representations (semb_set_geometry_mode) -----------------------------------
+//   GEO 0  stored factors, geo[E][7][Np] in the storage type ST                              48 (56) B/node
+//   GEO 1  the same layout in float, widened exactly on load, fp64 arithmetic                 24 (28) B/node
+//   GEO 2  affine elements (parallelepipeds): 7 constants per element, geoc[E][8] =
+//          (1/J) C_a.C_b for ab = rr, rs, rt, ss, st, tt, then J; G_ab = rho_i rho_j rho_k * that    64 B/element
+//   GEO 3  trilinear elements (straight edges): the 8 x 3 coefficients of x = c0 + c1 r + c2 s + c3 t + c4 rs + c5 rt
+//          + c6 st + c7 rst per coordinate, tri[E][3][8]; the Jacobian, its cofactors C_r = x_s x x_t, C_s = x_t x x_r,
+//          C_t = x_r x x_s and J = x_r . C_r are recomputed per node and G applied in factored form
+//          g_a = (W / J) C_a . (C_r u_r + C_s u_s + C_t u_t)                                        192 B/element
+
+// 1 / d for d > 0 in the normal range: hardware seed (2^-23) + two Newton steps (2^-46, 2^-92 -> rounding level)
+__device__ __forceinline__ double ax_rcp(double d)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
+    r = fma(r, fma(-d, r, 1.0), r);
+    r = fma(r, fma(-d, r, 1.0), r);
+    return r;
+}
 
 // ---- shared-memory layout of one element tile, index (k,j,i) -> double slot -------------------------------
 // All three line orientations read/write it with 64-bit accesses; a half-warp (16 lanes) is conflict-free iff
@@ -63,7 +85,7 @@ template <> struct ax_tile<8> {
 
 // Which r-line (j = q % n1, k = q / n1) and which s-line (i = q % n1, k = q / n1) a thread contracts:
 // c_perm[N][0][thread] and c_perm[N][1][thread], filled at setup (axhelm.cu: ax_perm_build).
-__constant__ unsigned char c_perm[SEMB_MAX_N + 1][2][SEMB_MAXN1 * SEMB_MAXN1 + 7];
+static __constant__ unsigned char c_perm[SEMB_MAX_N + 1][2][SEMB_MAXN1 * SEMB_MAXN1 + 7];
 
 // host: greedy balanced grouping.  start_bank[q] = bank (64-bit, mod 16) of the first slot of line q.  Lines are
 // dealt to the half-warps (aligned groups of 16 threads) so that a group holds as few lines of equal bank as
@@ -128,7 +150,7 @@ __device__ __forceinline__ void ax_finish_dot(double dot, semb_scalars* __restri
 #define SEMB_EO_H  ((SEMB_MAXN1) / 2)          // max h
 #define SEMB_EO_H2 ((SEMB_MAXN1 + 1) / 2)      // max number of rows i <= h
 struct ax_eo_tab { double P[SEMB_EO_H2 * SEMB_EO_H], M[SEMB_EO_H2 * SEMB_EO_H], mid[SEMB_EO_H2]; };
-__constant__ ax_eo_tab c_EO[SEMB_MAX_N + 1][2];      // [N][0] for D, [N][1] for D^T
+static __constant__ ax_eo_tab c_EO[SEMB_MAX_N + 1][2];      // [N][0] for D, [N][1] for D^T
 
 // host: fill the two tables of order N from D (row-major n1 x n1)
 static inline void ax_eo_build(int n1, const double* D, ax_eo_tab tab[2])
@@ -152,7 +174,7 @@ static inline void ax_eo_build(int n1, const double* D, ax_eo_tab tab[2])
 
 // float copies of the tables for the fp32-storage multigrid levels, where the whole kernel computes in float
 struct ax_eo_tab_f { float P[SEMB_EO_H2 * SEMB_EO_H], M[SEMB_EO_H2 * SEMB_EO_H], mid[SEMB_EO_H2]; };
-__constant__ ax_eo_tab_f c_EOf[SEMB_MAX_N + 1][2];
+static __constant__ ax_eo_tab_f c_EOf[SEMB_MAX_N + 1][2];
 template <typename CT> struct ax_eo_sel;
 template <> struct ax_eo_sel<double> { typedef ax_eo_tab tab; __device__ static __forceinline__ const ax_eo_tab& get(int N, int tr) { return c_EO[N][tr]; } };
 template <> struct ax_eo_sel<float> { typedef ax_eo_tab_f tab; __device__ static __forceinline__ const ax_eo_tab_f& get(int N, int tr) { return c_EOf[N][tr]; } };
@@ -191,6 +213,8 @@ __device__ __forceinline__ void ax_line(const CT (&x)[n1], CT (&y)[n1])
 // u.w to dot_out[b] (fixed summation order; reduced by k_ax_dot_finish).
 // plain != 0 (first Chebyshev step): no recurrence, p = (dinv o zsrc) * scale is written to p_io and the operator is
 // applied to it; x, alpha, beta are not touched.
+template <typename ST, int GEO> struct ax_geo_type { typedef ST type; };
+template <typename ST> struct ax_geo_type<ST, SEMB_GEO_F32> { typedef float type; };
 template <typename ST> struct ax_pcg_args_t { const ST* zsrc; const ST* dinv; ST* p_io; ST* x; double scale; int plain; };
 typedef ax_pcg_args_t<double> ax_pcg_args;
 
@@ -210,9 +234,9 @@ __device__ __forceinline__ void ax_prefetch_l2(const ST* ptr, int count)
 // blockIdx.x * EPB + el with its own shared-memory tiles; groups past the end recompute the last element and write nothing.
 // ST: STORAGE type of the vectors and geometric factors in global memory (double, or float for the multigrid levels:
 // PAPER.md:L102 runs the preconditioner in FP32 "to save on memory bandwidth"); the arithmetic is fp64 either way.
-template <int n1, int MODE, int MINB, int EPB, typename ST>
+template <int n1, int MODE, int MINB, int EPB, typename ST, int GEO>
 __global__ void __launch_bounds__(n1 * n1 * EPB, MINB)
-k_axhelm_line(int64_t E, int64_t n, const ST* __restrict__ geo, double lambda,
+k_axhelm_line(int64_t E, int64_t n, const void* __restrict__ geo_v, double lambda,
               const double* __restrict__ lam0, const double* __restrict__ lam1,
               const ST* __restrict__ u, ST* __restrict__ w,
               const semb_scalars* __restrict__ scal, double* __restrict__ dot_out, ax_pcg_args_t<ST> pcg, int pf_dist, int nfields)
@@ -220,6 +244,9 @@ k_axhelm_line(int64_t E, int64_t n, const ST* __restrict__ geo, double lambda,
     constexpr int n2 = n1 * n1, Np = n1 * n1 * n1;
     constexpr bool HELM = MODE & 1, VAR = MODE & 2, FUSE = MODE & 4;
     constexpr int NG = HELM ? 7 : 6;
+    constexpr bool STORED = GEO == SEMB_GEO_STORED || GEO == SEMB_GEO_F32;
+    typedef typename ax_geo_type<ST, GEO>::type GT;             // what the stored factors are read as
+    const GT* __restrict__ geo = (const GT*)geo_v;
     using T = ax_tile<n1>;
     typedef ST CT;                    // float storage => float arithmetic and 32-bit tiles (the fp64-arithmetic float-storage
                                       // kernel was bound by its 64-bit transposes at 138 GDOF/s: profiles/r1_v6_fp32_levels.md)
@@ -245,7 +272,7 @@ k_axhelm_line(int64_t E, int64_t n, const ST* __restrict__ geo, double lambda,
     // the resident blocks are in their compute phase, and that block's loads hit L2.
     if (pf_dist > 0 && tl == 0 && valid && e + pf_dist < E) {
         const int64_t ep = e + pf_dist;
-        ax_prefetch_l2(geo + ep * 7 * (int64_t)Np, NG * Np);
+        if (STORED) ax_prefetch_l2(geo + ep * 7 * (int64_t)Np, NG * Np);
         if (FUSE) {
             ax_prefetch_l2(pcg.zsrc + ep * Np, Np);
             if (pcg.dinv) ax_prefetch_l2(pcg.dinv + ep * Np, Np);
@@ -255,8 +282,8 @@ k_axhelm_line(int64_t E, int64_t n, const ST* __restrict__ geo, double lambda,
         if (VAR && lam1) ax_prefetch_l2(lam1 + ep * Np, Np);
     }
     ST* __restrict__ we = w + f * n + e * Np + tl;
-    const ST* __restrict__ g = geo + e * 7 * (int64_t)Np + tl;
-    CT ru[n1], G[NG][n1];
+    const GT* __restrict__ g = geo + e * 7 * (int64_t)Np + tl;
+    CT ru[n1], G[STORED ? NG : 1][STORED ? n1 : 1];
     if (FUSE) {
         const int64_t l0 = e * Np + tl;
         const bool plain = pcg.plain != 0;
@@ -293,10 +320,34 @@ k_axhelm_line(int64_t E, int64_t n, const ST* __restrict__ geo, double lambda,
         for (int k = 0; k < n1; ++k) ru[k] = ue[k * n2];
     }
     // ---- global loads, t-line layout: lane -> consecutive nodes of plane k (coalesced 64-bit)
+    if (STORED) {
 #pragma unroll
-    for (int k = 0; k < n1; ++k) {
+        for (int k = 0; k < n1; ++k) {
 #pragma unroll
-        for (int c = 0; c < NG; ++c) G[c][k] = __ldg(g + c * Np + k * n2);
+            for (int c = 0; c < NG; ++c) G[c][k] = (CT)__ldg(g + c * Np + k * n2);
+        }
+    }
+    // on-the-fly modes: element constants (uniform loads) and the thread's part of W = rho_i rho_j rho_k
+    double gc[GEO == SEMB_GEO_AFFINE ? 7 : 1], wab = 0.0;
+    double tA[GEO == SEMB_GEO_TRILINEAR ? 3 : 1][5];      // per coordinate: x_r = tA0 + tA1 t, x_s = tA2 + tA3 t, x_t = tA4
+    if (GEO == SEMB_GEO_AFFINE) {
+        const double* __restrict__ ge = (const double*)geo_v + e * 8;
+#pragma unroll
+        for (int c = 0; c < 7; ++c) gc[c] = __ldg(ge + c);
+        wab = c_rho[n1 - 1][a] * c_rho[n1 - 1][b];
+    }
+    if (GEO == SEMB_GEO_TRILINEAR) {
+        const double* __restrict__ ce = (const double*)geo_v + e * 24;
+        const double r = c_xi[n1 - 1][a], sx = c_xi[n1 - 1][b];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const double c1 = __ldg(ce + c * 8 + 1), c2 = __ldg(ce + c * 8 + 2), c3 = __ldg(ce + c * 8 + 3), c4 = __ldg(ce + c * 8 + 4),
+                         c5 = __ldg(ce + c * 8 + 5), c6 = __ldg(ce + c * 8 + 6), c7 = __ldg(ce + c * 8 + 7);
+            tA[c][0] = fma(c4, sx, c1); tA[c][1] = fma(c7, sx, c5);
+            tA[c][2] = fma(c4, r, c2);  tA[c][3] = fma(c7, r, c6);
+            tA[c][4] = fma(fma(c7, sx, c5), r, fma(c6, sx, c3));
+        }
+        wab = c_rho[n1 - 1][a] * c_rho[n1 - 1][b];
     }
 #pragma unroll
     for (int k = 0; k < n1; ++k) Su[AX_I(k, b, a)] = ru[k];
@@ -320,15 +371,41 @@ k_axhelm_line(int64_t E, int64_t n, const ST* __restrict__ geo, double lambda,
     __syncthreads();
     // ---- geometric factors at the nodes of the t-line
     CT gt[n1];
+    double Bk[(HELM && !STORED) ? n1 : 1];                 // mass factor W J of the on-the-fly modes
 #pragma unroll
     for (int k = 0; k < n1; ++k) {
         const int s = AX_I(k, b, a), sB = AX_IB(k, b, a);
         const CT ur = Sr[s], us = Ss[sB];
-        CT Grr = G[0][k], Grs = G[1][k], Grt = G[2][k], Gss = G[3][k], Gst = G[4][k], Gtt = G[5][k];
-        if (VAR && lam0) { const CT c = (CT)lam0[e * Np + k * n2 + tl]; Grr *= c; Grs *= c; Grt *= c; Gss *= c; Gst *= c; Gtt *= c; }
-        Sr[s] = Grr * ur + Grs * us + Grt * ut[k];
-        Ss[sB] = Grs * ur + Gss * us + Gst * ut[k];
-        gt[k] = Grt * ur + Gst * us + Gtt * ut[k];
+        if (STORED) {
+            CT Grr = G[0][k], Grs = G[1][k], Grt = G[2][k], Gss = G[3][k], Gst = G[4][k], Gtt = G[5][k];
+            if (VAR && lam0) { const CT c = (CT)lam0[e * Np + k * n2 + tl]; Grr *= c; Grs *= c; Grt *= c; Gss *= c; Gst *= c; Gtt *= c; }
+            Sr[s] = Grr * ur + Grs * us + Grt * ut[k];
+            Ss[sB] = Grs * ur + Gss * us + Gst * ut[k];
+            gt[k] = Grt * ur + Gst * us + Gtt * ut[k];
+        } else if (GEO == SEMB_GEO_AFFINE) {
+            const double W = wab * c_rho[n1 - 1][k];
+            Sr[s] = (CT)(W * (gc[0] * ur + gc[1] * us + gc[2] * ut[k]));
+            Ss[sB] = (CT)(W * (gc[1] * ur + gc[3] * us + gc[4] * ut[k]));
+            gt[k] = (CT)(W * (gc[2] * ur + gc[4] * us + gc[5] * ut[k]));
+            if (HELM) Bk[k] = W * gc[6];
+        } else {
+            const double t = c_xi[n1 - 1][k];
+            const double xr = fma(tA[0][1], t, tA[0][0]), xs = fma(tA[0][3], t, tA[0][2]), xt = tA[0][4];
+            const double yr = fma(tA[1][1], t, tA[1][0]), ys = fma(tA[1][3], t, tA[1][2]), yt = tA[1][4];
+            const double zr = fma(tA[2][1], t, tA[2][0]), zs = fma(tA[2][3], t, tA[2][2]), zt = tA[2][4];
+            // cofactor rows C_r = x_s x x_t, C_s = x_t x x_r, C_t = x_r x x_s
+            const double rx = ys * zt - yt * zs, ry = zs * xt - zt * xs, rz = xs * yt - xt * ys;
+            const double sx_ = yt * zr - yr * zt, sy_ = zt * xr - zr * xt, sz_ = xt * yr - xr * yt;
+            const double tx = yr * zs - ys * zr, ty = zr * xs - zs * xr, tz = xr * ys - xs * yr;
+            const double J = xr * rx + yr * ry + zr * rz;
+            const double W = wab * c_rho[n1 - 1][k];
+            const double sc = W * ax_rcp(J);
+            const double vx = rx * ur + sx_ * us + tx * ut[k], vy = ry * ur + sy_ * us + ty * ut[k], vz = rz * ur + sz_ * us + tz * ut[k];
+            Sr[s] = (CT)(sc * (rx * vx + ry * vy + rz * vz));
+            Ss[sB] = (CT)(sc * (sx_ * vx + sy_ * vy + sz_ * vz));
+            gt[k] = (CT)(sc * (tx * vx + ty * vy + tz * vz));
+            if (HELM) Bk[k] = W * J;
+        }
     }
     __syncthreads();
     // ---- transposed contractions
@@ -351,7 +428,7 @@ k_axhelm_line(int64_t E, int64_t n, const ST* __restrict__ geo, double lambda,
 #pragma unroll
         for (int k = 0; k < n1; ++k) {
             const CT lam = (VAR && lam1) ? (CT)lam1[e * Np + k * n2 + tl] : (CT)lambda;
-            wt[k] += lam * G[NG - 1][k] * ru[k];
+            wt[k] += lam * (STORED ? G[STORED ? NG - 1 : 0][STORED ? k : 0] : (CT)Bk[(HELM && !STORED) ? k : 0]) * ru[k];
         }
     }
     __syncthreads();
@@ -372,7 +449,7 @@ k_axhelm_line(int64_t E, int64_t n, const ST* __restrict__ geo, double lambda,
 
 // Sum of the per-block partials dot_in[0..count) in a fixed order (two stages, last block by ticket), then
 // the PCG scalars: p.Ap, alpha = rho / p.Ap, breakdown detection.
-__global__ void __launch_bounds__(256)
+static __global__ void __launch_bounds__(256)
 k_ax_dot_finish(int64_t count, const double* __restrict__ dot_in, semb_scalars* __restrict__ scal, double* __restrict__ partials)
 {
     __shared__ double red[32];

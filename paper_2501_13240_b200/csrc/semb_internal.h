@@ -48,6 +48,12 @@ struct semb_mesh {
     double   period[3] = {0.0, 0.0, 0.0};
     double*  geo = nullptr;        // [E][7][Np]  canonical layout (semb_info.geo)
     double*  geoK = nullptr;       // kernel-native layout of the same data (axhelm.cu), may alias geo
+    // geometry representation the fp64 axhelm launches read (semb_set_geometry_mode; geomode.cu)
+    int      geo_mode = 0;         // SEMB_GEO_STORED | _F32 | _AFFINE | _TRILINEAR
+    float*   geoF = nullptr;       // [E][7][Np] float copy of geo (mode 1)
+    double*  geoC = nullptr;       // [E][8]  affine element constants (mode 2)
+    double*  geoT = nullptr;       // [E][3][8] trilinear coefficients (mode 3)
+    double   geo_dev[2] = {-1.0, -1.0};   // measured: max deviation of the nodes from the trilinear / affine map of the corners, relative to max |coordinate|
     int32_t* gid = nullptr;        // [n]
     double*  invmult = nullptr;    // [n]
     int32_t* gs_off = nullptr;     // [n_gs+1]

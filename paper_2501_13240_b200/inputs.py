@@ -104,6 +104,40 @@ def box_mesh(nx, ny, nz, N, xi, periodic=(False, False, False), deform=0.0, zstr
                 dict(nx=nx, ny=ny, nz=nz, periodic=tuple(periodic), deform=deform, zstretch=zstretch))
 
 
+def trilinear_box_mesh(nx, ny, nz, N, xi, jitter=0.2, seed=BASE_SEED + 77, zstretch=0.0, name="box_trilinear"):
+    """Unit cube of nx*ny*nz hexahedra with STRAIGHT edges that are not parallelepipeds: the interior lattice vertices are
+    displaced by jitter * h * U[-1,1) per coordinate (seeded, counter RNG on the vertex index; boundary vertices stay), and
+    every node is the trilinear interpolant of its element's 8 vertices at the GLL parameters -- the class of elements whose
+    geometric factors can be rebuilt from 8 vertices.  jitter = 0 gives affine bricks."""
+    n1 = N + 1
+    a = (np.asarray(xi, dtype=np.float64) + 1.0) * 0.5
+    zb = tanh_layers(nz, zstretch) if zstretch > 0.0 else np.arange(nz + 1, dtype=np.float64) / nz
+    V = np.empty((nz + 1, ny + 1, nx + 1, 3))
+    V[..., 0] = (np.arange(nx + 1, dtype=np.float64) / nx)[None, None, :]
+    V[..., 1] = (np.arange(ny + 1, dtype=np.float64) / ny)[None, :, None]
+    V[..., 2] = zb[:, None, None]
+    if jitter != 0.0:
+        hmin = np.array([1.0 / nx, 1.0 / ny, np.diff(zb).min()])
+        d = uniform(seed, V.size).reshape(V.shape) * (jitter * hmin)[None, None, None, :]
+        d[0] = 0; d[-1] = 0; d[:, 0] = 0; d[:, -1] = 0; d[:, :, 0] = 0; d[:, :, -1] = 0
+        V = V + d
+    w = np.stack([1.0 - a, a])                                                   # [2, n1]
+    out = []
+    for c in range(3):
+        acc = np.zeros((nz, ny, nx, n1, n1, n1))
+        for vk in range(2):
+            for vj in range(2):
+                for vi in range(2):
+                    corner = V[vk:vk + nz, vj:vj + ny, vi:vi + nx, c]
+                    acc += corner[..., None, None, None] * (w[vk][:, None, None] * w[vj][None, :, None] * w[vi][None, None, :])
+        out.append(acc.reshape(-1))
+    ft = np.zeros((nz, ny, nx, 6), dtype=np.int32)
+    ft[:, :, 0, 0] = 2; ft[:, :, nx - 1, 1] = 2; ft[:, 0, :, 2] = 2; ft[:, ny - 1, :, 3] = 2
+    ft[0, :, :, 4] = 1; ft[nz - 1, :, :, 5] = 1
+    return Mesh(nx * ny * nz, N, out[0], out[1], out[2], ft.reshape(-1), [0.0, 0.0, 0.0], name,
+                dict(nx=nx, ny=ny, nz=nz, jitter=jitter, zstretch=zstretch))
+
+
 def _east_block(zeta, eta, c, R):
     """point(zeta, eta) = (1-zeta) (c, c eta) + zeta R (cos(pi eta/4), sin(pi eta/4))."""
     px = (1.0 - zeta) * c + zeta * R * np.cos(np.pi * eta / 4.0)

@@ -11,7 +11,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libsemb200.so")
+LIB_PATH = os.environ.get("SEMB_LIB") or os.path.join(_HERE, "libsemb200.so")       # SEMB_LIB: an A/B build of the same sources
 
 SEMB_OK, SEMB_MAXIT = 0, 1
 ERRORS = {-1: "SEMB_EINVAL", -2: "SEMB_ENOMEM", -3: "SEMB_ECUDA", -4: "SEMB_EGEOM", -5: "SEMB_EBREAKDOWN",
@@ -19,9 +19,9 @@ ERRORS = {-1: "SEMB_EINVAL", -2: "SEMB_ENOMEM", -3: "SEMB_ECUDA", -4: "SEMB_EGEO
 
 # every symbol include/semb200.h declares (tests check that the library exports all of them)
 SYMBOLS = ["semb_gll", "semb_setup", "semb_destroy", "semb_last_error", "semb_mesh_info", "semb_apply_axhelm",
-           "semb_gather_scatter", "semb_apply_mask", "semb_assemble_rhs", "semb_apply_operator", "semb_jacobi_diag",
+           "semb_set_geometry_mode", "semb_gather_scatter", "semb_apply_mask", "semb_assemble_rhs", "semb_apply_operator", "semb_jacobi_diag",
            "semb_pcg_solve", "semb_step_solve", "semb_mg_vcycle", "semb_mg_transfer", "semb_mg_level_size", "semb_estimate_lmax", "semb_cheb_jacobi", "semb_publish_field", "semb_publish_state",
-           "semb_export_field", "semb_field_minmax_hist", "semb_apply_axhelm_host", "semb_pcg_solve_host", "semb_read_device", "semb_version"]
+           "semb_export_field", "semb_field_minmax_hist", "semb_apply_axhelm_host", "semb_pcg_solve_host", "semb_read_device", "semb_stream_probe", "semb_version"]
 
 
 class SembError(RuntimeError):
@@ -218,6 +218,13 @@ class Mesh:
                                             C.c_int(nfields), _stream()))
         return w
 
+    def set_geometry_mode(self, mode, tol=0.0):
+        """0 stored fp64 factors, 1 float-stored factors, 2 affine elements, 3 trilinear elements (semb_set_geometry_mode).
+        Returns the measured (trilinear, affine) deviations, (-1, -1) if they were never measured."""
+        dev = (C.c_double * 2)(-1.0, -1.0)
+        self._check(lib().semb_set_geometry_mode(self._h, C.c_int(mode), C.c_double(tol), dev if mode >= 2 else None, _stream()))
+        return dev[0], dev[1]
+
     def gather_scatter(self, w, nfields=1):
         self._check(lib().semb_gather_scatter(self._h, _dp(w), C.c_int(nfields), _stream()))
         return w
@@ -342,6 +349,13 @@ class Mesh:
         self._check(lib().semb_apply_axhelm_host(self._h, C.c_double(lam), u_host.ctypes.data_as(C.c_void_p),
                                                  w_host.ctypes.data_as(C.c_void_p)))
         return w_host
+
+
+def stream_probe(src, dst, nread):
+    """measurement aid: dst[l] = sum_c src[c*n + l] (semb_stream_probe)"""
+    rc = lib().semb_stream_probe(_dp(src), _dp(dst), C.c_int64(dst.numel()), C.c_int(nread), _stream())
+    if rc:
+        raise SembError(rc, "semb_stream_probe")
 
 
 def field_minmax_hist(desc, nbins, lo, hi, minmax_dev, hist_dev):
