@@ -331,6 +331,47 @@ def ten_steps(torch, G, m, nsteps, variants):
     return out
 
 
+def image_section(torch, semb, G, m, ms_step):
+    """SURVEY.md §8 f-4 / PAPER.md:L371-373: the parts of the paper's overview scene as CUDA kernels on the exported
+    temperature field, each a 4096 x 2048 image: two slices next to the walls, two vertical slices, one isocontour."""
+    n = m.n
+    T = torch.from_numpy((1.0 - m.z) + 0.05 * I.uniform(I.seed_for(3, 31), n)).cuda()
+    G.publish_field("temperature", T)
+    G.publish_state(1, 0.0)
+    d = G.export_field("temperature")
+    W, H = 4096, 2048
+    key = torch.zeros(W * H, dtype=torch.int64, device="cuda"); rgba = torch.zeros(W * H, dtype=torch.int32, device="cuda")
+    cw = [(59, 76, 192), (141, 176, 254), (221, 221, 221), (244, 154, 123), (180, 4, 38)]
+    cm = semb.colormap(0.0, 1.0, cw)
+    lo = [float(min(a.min() for a in (m.x, m.y))), float(m.z.min())]
+    ext = float(max(m.x.max(), m.y.max())) - lo[0]
+    views = {"slice_horizontal_lower_boundary_layer": semb.image_view(W, H, (lo[0], lo[0], 0.02), (1, 0, 0), (0, 1, 0), ext / W, ext / H),
+             "slice_horizontal_upper_boundary_layer": semb.image_view(W, H, (lo[0], lo[0], 0.98), (1, 0, 0), (0, 1, 0), ext / W, ext / H),
+             "slice_vertical_x": semb.image_view(W, H, (lo[0] + 0.5 * ext, lo[0], 0.0), (0, 1, 0), (0, 0, 1), ext / W, 1.0 / H),
+             "slice_vertical_y": semb.image_view(W, H, (lo[0], lo[0] + 0.5 * ext, 0.0), (1, 0, 0), (0, 0, 1), ext / W, 1.0 / H)}
+    out = {"pixels": [W, H]}
+    total = 0.0
+    for name, vw in views.items():
+        t = timed(torch, lambda: G.image_slice(d, vw, cm, key, rgba), 5, warm=1)
+        hit = int(((key >> 32) != 0xffffffff).sum().item())
+        out[name] = {"ms": t, "pixels_hit": hit}
+        total += t
+    # isocontour T = 0.5 seen from above at an angle, coloured by the temperature
+    u = np.array([1.0, 0.0, 0.0]); v = np.array([0.0, 0.8, 0.6]); w = np.cross(u, v)
+    o = np.array([lo[0] - 0.1 * ext, lo[0] - 0.3 * ext, -0.2]) - 2.0 * w
+    vw = semb.image_view(W, H, o, u, v, 1.2 * ext / W, 1.6 * ext / H, 0.0, 6.0)
+    t = timed(torch, lambda: G.image_isosurface(d, 0.5, d, vw, cm, (0.0, 0.6, 0.8), key, rgba), 5, warm=1)
+    out["isocontour_T_0.5"] = {"ms": t, "pixels_hit": int(((key >> 32) != 0xffffffff).sum().item())}
+    total += t
+    out["overview_scene_ms"] = total
+    out["overhead_vs_pcg_iteration_pct"] = {str(nv): 100.0 * ((total + nv * ms_step) / (nv * ms_step) - 1.0) for nv in (10, 100, 1000)}
+    out["note"] = ("five 4096 x 2048 partial images of the paper's overview scene (PAPER.md:L371: two wall slices, two vertical slices, one "
+                   "isocontour) from the zero-copy exported field; the paper's ASCENT/VTK-m pipeline takes 4-5 s per part on 3360 A100 "
+                   "(Table 5, L412-424: context, other hardware and a 350x larger mesh)")
+    del T, key, rgba
+    return out
+
+
 def geometry_section(torch, semb, G3, m3, peak):
     """the same operator from fewer bytes.  (a) the float-stored factors on the cfg3 mesh (curved
     elements); (b) a 64^3, N = 7 box with tanh-stretched layers -- the paper's own mesh class, every
@@ -580,13 +621,17 @@ def main():
     solve_tts = None
     if not args.no_solve and single:
         variants = [("pmg_pcg", dict(precond=3, mg_smooth=1, mg_coarse=64, mg_coarse_frac=0.003)),
-                    ("pmg_fp32_pcg", dict(precond=3, mg_smooth=1, mg_coarse=64, mg_coarse_frac=0.003, mg_fp32=True)),
-                    ("jacobi_pcg", dict(precond=1))]
+                    ("pmg_fp32_pcg", dict(precond=3, mg_smooth=1, mg_coarse=64, mg_coarse_frac=0.003, mg_fp32=True))]
         if isinstance(ne, tuple):
-            variants = [("pmg_pcg", dict(precond=3)), ("pmg_fp32_pcg", dict(precond=3, mg_fp32=True)), ("jacobi_pcg", dict(precond=1))]
+            variants = [("pmg_pcg", dict(precond=3)), ("pmg_fp32_pcg", dict(precond=3, mg_fp32=True))]
+        if args.full_solves:                  # ~4200 iterations, 14 s on cfg3: not in the default run
+            variants.append(("jacobi_pcg", dict(precond=1)))
         solve_tts = time_to_solution(torch, G, b, variants, args.solve_maxit)
-        solve_tts["speedup"] = solve_tts["jacobi_pcg"]["seconds"] / solve_tts["pmg_pcg"]["seconds"]
-        solve_tts["speedup_fp32_levels"] = solve_tts["jacobi_pcg"]["seconds"] / solve_tts["pmg_fp32_pcg"]["seconds"]
+        if args.full_solves:
+            solve_tts["speedup"] = solve_tts["jacobi_pcg"]["seconds"] / solve_tts["pmg_pcg"]["seconds"]
+            solve_tts["speedup_fp32_levels"] = solve_tts["jacobi_pcg"]["seconds"] / solve_tts["pmg_fp32_pcg"]["seconds"]
+        else:
+            solve_tts["jacobi_pcg_seconds_at_the_measured_iteration_time"] = "iterations x ms_per_step; run with --full-solves to measure (4196 iterations, 13.97 s at r2 start)"
 
     # ---- configs[3]: zero-copy export of temperature and velocity magnitude to the in-device min/max/256-bin histogram
     #      consumer (PAPER.md:L138-159 hand-off; overhead formula of PAPER.md:L375 against the PCG iteration time)
@@ -639,6 +684,11 @@ def main():
                           "note": "ONE operator application with host buffers: bound by the two PCIe copies (8 B/node each way), "
                                   "the kernel itself is %.1f %% of the call" % (100.0 * sweep["poisson"]["ms"] * 1e-3 / dt)}
         del bh, xh
+
+    # ---- the in-situ image consumer on the exported field
+    images = None
+    if single and not args.no_export:
+        images = image_section(torch, semb, G, m, ms_step)
 
     # ---- reduced-traffic geometry representations (part on this mesh, part on an affine box built below)
     geo_modes = geo_state = None
@@ -700,6 +750,7 @@ def main():
         "axhelm_sweep": sweep,
         "time_to_solution": solve_tts,
         "export": export,
+        "image_consumer": images,
         "cfg1_batched_axhelm_gs": cfg1,
         "geometry_modes": geo_modes,
         "configs": configs,

@@ -275,6 +275,50 @@ SEMB_API int semb_export_field(semb_handle h, const char* name, semb_field_desc*
 SEMB_API int semb_field_minmax_hist(const semb_field_desc* f, int nbins, double lo, double hi,
                            double* minmax_dev, uint64_t* hist_dev, void* stream);
 
+/* ---- in-situ IMAGE consumer (§5.3: the overview scene = "two slices on the walls,
+ * two vertical slices in the background and an isocontour", 4096 pixels on the longest side, 2048 on the other).
+ * The paper renders with ASCENT / VTK-m; no graphics API exists here, so the primitives are CUDA kernels on the mesh of
+ * hexahedral SUB-CELLS between neighbouring GLL nodes, trilinear inside a cell (reading R24), fed by the
+ * descriptors of semb_export_field.  Sub-cell id = e*N^3 + (k*N + j)*N + i.
+ *
+ * View: pixel (px, py) has the centre origin + ((px + 0.5) du) u + ((py + 0.5) dv) v, u and v unit vectors; w = u x v is the
+ * viewing direction and (X - origin).w the depth of a point; depth_lo < depth_hi bound the scene along w (iso-surface only).
+ * Colour map: s = clamp((val - lo) / (hi - lo), 0, 1) (ncolors - 1), linear between control points m = floor(s) and m + 1,
+ * channel = floor(c + 0.5), alpha 255; packed r | g << 8 | b << 16 | a << 24.
+ * key_dev device [width*height] uint64 (caller-owned scratch that doubles as output), rgba_dev device [width*height] or NULL.
+ * Asynchronous on stream; nothing is allocated; images are reproducible bit for bit (atomicMin on order-independent keys). */
+typedef struct {
+    int32_t width, height;
+    double  origin[3], u[3], v[3];
+    double  du, dv;
+    double  depth_lo, depth_hi;
+} semb_image_view;
+
+typedef struct {
+    double   lo, hi;
+    int32_t  ncolors;          /* 2..16 control points */
+    uint8_t  rgb[16][3];
+    uint32_t background;       /* packed RGBA of pixels nothing covers */
+} semb_colormap;
+
+/* rgba_dev[l] = colour of val_dev[l] (device arrays of n entries). */
+SEMB_API int semb_colormap_apply(const semb_colormap* cm, const double* val_dev, int64_t n, uint32_t* rgba_dev, void* stream);
+
+/* Planar slice: the image plane itself cuts the mesh.  Every sub-cell whose corners lie on both sides of the plane (or on
+ * it) claims the pixels whose centres it contains (Newton inversion of its trilinear map: <= 12 steps, step <= 1e-13, inside
+ * = |r|, |s|, |t| <= 1 + 1e-9); where several cells contain a centre the smallest id wins.  key = cell id << 32 | RGBA, cell
+ * id 0xffffffff where nothing was hit. */
+SEMB_API int semb_image_slice(semb_handle h, const semb_field_desc* field, const semb_image_view* view, const semb_colormap* cmap,
+                     uint64_t* key_dev, uint32_t* rgba_dev, void* stream);
+
+/* Iso-surface {field = iso} seen orthographically along w: marching tetrahedra (6 per sub-cell around the diagonal corner
+ * 0 - corner 7, corner q = a + 2b + 4c) on the linear interpolant, flat shading 0.25 + 0.75 |n . light| (light HOST [3], unit)
+ * of the colour the map gives to color_or_null's value (NULL: to iso), nearest surface per pixel.
+ * key = depth quantised to 2^-32 of [depth_lo, depth_hi] << 32 | RGBA, depth 0xffffffff where nothing was hit. */
+SEMB_API int semb_image_isosurface(semb_handle h, const semb_field_desc* field, double iso, const semb_field_desc* color_or_null,
+                          const semb_image_view* view, const semb_colormap* cmap, const double* light, uint64_t* key_dev,
+                          uint32_t* rgba_dev, void* stream);
+
 /* ---- convenience: the same calls with HOST buffers (copies inside; used for end-to-end timing) */
 SEMB_API int semb_apply_axhelm_host(semb_handle h, double lambda, const double* u_host, double* w_host);
 /* pcg_solve with b and x in HOST memory (pinned memory makes the copies asynchronous): b is copied to the

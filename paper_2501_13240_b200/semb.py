@@ -21,7 +21,7 @@ ERRORS = {-1: "SEMB_EINVAL", -2: "SEMB_ENOMEM", -3: "SEMB_ECUDA", -4: "SEMB_EGEO
 SYMBOLS = ["semb_gll", "semb_setup", "semb_destroy", "semb_last_error", "semb_mesh_info", "semb_apply_axhelm",
            "semb_set_geometry_mode", "semb_gather_scatter", "semb_apply_mask", "semb_assemble_rhs", "semb_apply_operator", "semb_jacobi_diag",
            "semb_pcg_solve", "semb_step_solve", "semb_mg_vcycle", "semb_mg_transfer", "semb_mg_level_size", "semb_estimate_lmax", "semb_cheb_jacobi", "semb_publish_field", "semb_publish_state",
-           "semb_export_field", "semb_field_minmax_hist", "semb_apply_axhelm_host", "semb_pcg_solve_host", "semb_read_device", "semb_stream_probe", "semb_version"]
+           "semb_export_field", "semb_field_minmax_hist", "semb_colormap_apply", "semb_image_slice", "semb_image_isosurface", "semb_apply_axhelm_host", "semb_pcg_solve_host", "semb_read_device", "semb_stream_probe", "semb_version"]
 
 
 class SembError(RuntimeError):
@@ -107,6 +107,33 @@ class TorchAllocator:
 class FieldDesc(C.Structure):
     _fields_ = [("name", C.c_char_p), ("ptr", C.c_void_p), ("dtype", C.c_int32), ("memspace", C.c_int32),
                 ("count", C.c_int64), ("stride", C.c_int64), ("cycle", C.c_int64), ("time", C.c_double)]
+
+
+class ImageView(C.Structure):
+    _fields_ = [("width", C.c_int32), ("height", C.c_int32), ("origin", C.c_double * 3), ("u", C.c_double * 3),
+                ("v", C.c_double * 3), ("du", C.c_double), ("dv", C.c_double), ("depth_lo", C.c_double), ("depth_hi", C.c_double)]
+
+
+class Colormap(C.Structure):
+    _fields_ = [("lo", C.c_double), ("hi", C.c_double), ("ncolors", C.c_int32), ("rgb", (C.c_uint8 * 3) * 16),
+                ("background", C.c_uint32)]
+
+
+def image_view(width, height, origin, u, v, du, dv, depth_lo=0.0, depth_hi=1.0):
+    vw = ImageView(width, height)
+    for c in range(3):
+        vw.origin[c], vw.u[c], vw.v[c] = float(origin[c]), float(u[c]), float(v[c])
+    vw.du, vw.dv, vw.depth_lo, vw.depth_hi = float(du), float(dv), float(depth_lo), float(depth_hi)
+    return vw
+
+
+def colormap(lo, hi, colors, background=0xff000000):
+    cm = Colormap(float(lo), float(hi), len(colors))
+    for m, col in enumerate(colors):
+        for c in range(3):
+            cm.rgb[m][c] = int(col[c])
+    cm.background = int(background)
+    return cm
 
 
 _lib = None
@@ -344,6 +371,15 @@ class Mesh:
         self._check(lib().semb_export_field(self._h, name.encode(), C.byref(d)))
         return d
 
+    def image_slice(self, desc, view, cmap, key, rgba=None):
+        """planar slice of an exported field into key (uint64/int64 [H*W]) and rgba (int32/uint32 [H*W] or None)"""
+        self._check(lib().semb_image_slice(self._h, C.byref(desc), C.byref(view), C.byref(cmap), _dp(key), _dp(rgba), _stream()))
+
+    def image_isosurface(self, desc, iso, color_desc, view, cmap, light, key, rgba=None):
+        lt = (C.c_double * 3)(*[float(v) for v in light])
+        self._check(lib().semb_image_isosurface(self._h, C.byref(desc), C.c_double(iso), C.byref(color_desc) if color_desc is not None else None,
+                                                C.byref(view), C.byref(cmap), lt, _dp(key), _dp(rgba), _stream()))
+
     def apply_axhelm_host(self, u_host, w_host, lam=0.0):
         """End-to-end call with HOST numpy buffers (copies inside the library)."""
         self._check(lib().semb_apply_axhelm_host(self._h, C.c_double(lam), u_host.ctypes.data_as(C.c_void_p),
@@ -356,6 +392,12 @@ def stream_probe(src, dst, nread):
     rc = lib().semb_stream_probe(_dp(src), _dp(dst), C.c_int64(dst.numel()), C.c_int(nread), _stream())
     if rc:
         raise SembError(rc, "semb_stream_probe")
+
+
+def colormap_apply(cmap, val, rgba):
+    rc = lib().semb_colormap_apply(C.byref(cmap), _dp(val), C.c_int64(val.numel()), _dp(rgba), _stream())
+    if rc:
+        raise SembError(rc, "semb_colormap_apply")
 
 
 def field_minmax_hist(desc, nbins, lo, hi, minmax_dev, hist_dev):
