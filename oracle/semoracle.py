@@ -15,7 +15,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "semoracle.c")
-_SRCS = [_SRC, os.path.join(_HERE, "semimage.c")]
+_SRCS = [_SRC, os.path.join(_HERE, "semimage.c"), os.path.join(_HERE, "semflow.c")]
 _LIB = os.path.join(_HERE, "libsemoracle.so")
 _lib = None
 
@@ -44,6 +44,7 @@ def lib():
         _lib.orc_dot.restype = C.c_double
         _lib.orc_geo.restype = C.c_int64
         _lib.orc_numbering.restype = C.c_int64
+        _lib.orc_metrics.restype = C.c_int64
     return _lib
 
 
