@@ -319,6 +319,48 @@ SEMB_API int semb_image_isosurface(semb_handle h, const semb_field_desc* field, 
                           const semb_image_view* view, const semb_colormap* cmap, const double* light, uint64_t* key_dev,
                           uint32_t* rgba_dev, void* stream);
 
+/* ---- the rest of a Boussinesq time step around the solves (Eqs. (1)-(3), L238, L272).
+ * The paper states the equations only; the discrete step is DESIGN.md reading R25:  nu = sqrt(Pr/Ra), kappa = 1/sqrt(Ra Pr),
+ * theta = T - (1 - z); order 1 on the first step (beta0 = 1, b = [1], a = [1]), then BDF2 / EXT2 (3/2, [2, -1/2], [2, -1]):
+ *   (i)   N_c = -(u.grad)u_c + delta_cz T + f_c,  N_theta = -(u.grad)theta + u_z + f_theta  (collocation, per element);
+ *         omega = curl u;  omega_bar = QQ^T(B omega) / QQ^T(B);  C = curl omega_bar
+ *   (ii)  u~ = sum_k b_k u^(n+1-k) + dt sum_k a_k N^(n+1-k);  g = u~/dt - nu sum_k a_k C^(n+1-k);
+ *         A p = QQ^T wdiv(g), all Neumann, zero mean (null_mean)
+ *   (iii) (A + beta0/(nu dt) B) u_c^(n+1) = M QQ^T B (u~_c - dt dp/dx_c) / (nu dt), started from u_c^n; the same for theta with kappa.
+ * Building blocks, each element-local and asynchronous on stream (arrays device [n]): */
+/* collocation gradient of a nodal field: g_b = sum_a (dr_a/dx_b) dphi/dr_a (discontinuous across elements) */
+SEMB_API int semb_gradient(semb_handle h, const double* phi, double* gx, double* gy, double* gz, void* stream);
+/* weak divergence, the transpose of the gradient in the GLL inner product: out_i = int grad(phi_i) . g  (unassembled) */
+SEMB_API int semb_weak_divergence(semb_handle h, const double* gx, const double* gy, const double* gz, double* out, void* stream);
+/* step (i): N4 device [4][n] = N_x, N_y, N_z, N_theta; omega3 device [3][n] = the averaged vorticity omega_bar.
+ * forcing_or_null HOST array of 4 device pointers (each may be NULL). */
+SEMB_API int semb_flow_explicit_terms(semb_handle h, const double* ux, const double* uy, const double* uz, const double* theta,
+                             const double* const* forcing_or_null, double* N4, double* omega3, void* stream);
+
+typedef struct {
+    double   Ra, Pr, dt;
+    uint32_t tags_u, tags_T;      /* Dirichlet tag sets of the velocity (no-slip walls) and of theta (isothermal plates) */
+    double   rtol;                /* of every solve; <= 0 => 1e-10 */
+    int32_t  precond_p, precond_u;/* semb_pcg_opts.precond of the pressure solve (0 => 3, p-multigrid) and of the Helmholtz solves (0 => 1, Jacobi) */
+    int32_t  mg_fp32, maxit;      /* maxit <= 0 => 20000 */
+    const double* forcing[4];     /* optional body forces f_x, f_y, f_z, f_theta at time level n, device [n] each, or NULL */
+} semb_flow_opts;
+
+typedef struct {                  /* every array device [n], caller-owned */
+    double* u[3]; double* theta; double* p;      /* in: level n (p: unused); out: level n+1                    */
+    double* u1[3]; double* theta1;               /* in: level n-1;            out: level n                      */
+    double* N1[4];                               /* in: explicit terms of level n-1; out: of level n            */
+    double* C1[3];                               /* in: curl curl u of level n-1;    out: of level n            */
+    int64_t step_index;                          /* 0 on the first call (histories are then ignored); incremented */
+} semb_flow_state;
+
+typedef struct { int32_t iters[5], status[5]; } semb_flow_stats;    /* pressure, u_x, u_y, u_z, theta */
+
+/* One time step.  Returns the worst status of the five solves (SEMB_OK, SEMB_MAXIT) or an error.  The metrics (72 B/node)
+ * and 21 work vectors are allocated on the first call and owned by the handle. */
+SEMB_API int semb_boussinesq_step(semb_handle h, const semb_flow_opts* opts, semb_flow_state* state, semb_flow_stats* stats_or_null,
+                         void* stream);
+
 /* ---- convenience: the same calls with HOST buffers (copies inside; used for end-to-end timing) */
 SEMB_API int semb_apply_axhelm_host(semb_handle h, double lambda, const double* u_host, double* w_host);
 /* pcg_solve with b and x in HOST memory (pinned memory makes the copies asynchronous): b is copied to the

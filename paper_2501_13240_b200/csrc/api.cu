@@ -69,6 +69,7 @@ int semb_destroy(semb_handle h)
     semb_dev_free(h, h->geo); semb_dev_free(h, h->gid); semb_dev_free(h, h->invmult); semb_dev_free(h, h->gs_code); semb_dev_free(h, h->gs_hi);
     if (h->geoK && h->geoK != h->geo) semb_dev_free(h, h->geoK);
     semb_dev_free(h, h->geoF); semb_dev_free(h, h->geoC); semb_dev_free(h, h->geoT);
+    semb_dev_free(h, h->flow_met); semb_dev_free(h, h->flow_D); semb_dev_free(h, h->flow_work); semb_dev_free(h, (void*)h->flow_tab);
     semb_dev_free(h, h->gs_off); semb_dev_free(h, h->gs_ids); semb_dev_free(h, h->face_tag_dev);
     for (auto& kv : h->masks) semb_dev_free(h, kv.second.list);
     for (auto& en : h->dinvs) semb_dev_free(h, en.d);

@@ -26,6 +26,7 @@ struct semb_mask_entry {
 };
 
 #define SEMB_DINV_CACHE 8
+#define SEMB_FLOW_WORK 21      // N(4) omega(3) curl-curl(3) u~(3) g(3) b_p(1) grad p(3) rhs(1)
 struct semb_dinv_entry { uint32_t tags; double lambda; double* d; uint64_t stamp; };
 
 struct semb_field_entry {
@@ -69,6 +70,11 @@ struct semb_mesh {
     // (tags, lambda) pairs only, so a variable time step (lambda = c / dt) neither leaks memory nor re-runs the setup.
     double* diagA = nullptr; double* diagB = nullptr;
     std::vector<semb_dinv_entry> dinvs; uint64_t dinv_clock = 0;
+    // flow operators of the Boussinesq step (flow.cu), built on first use
+    double* flow_met = nullptr;         // [E][9][Np] dr_a/dx_b
+    double* flow_D = nullptr;           // D on the device
+    double* flow_work = nullptr;        // [SEMB_FLOW_WORK][n]
+    const double** flow_tab = nullptr;  // device pointer tables (8 slots x 16)
     // solver workspace
     double* work = nullptr; int64_t work_vecs = 0;
     double* partials = nullptr;         // block partial sums [4][SEMB_MAX_BLOCKS]
@@ -183,6 +189,9 @@ int semb_mg_vcycle_run(semb_mesh* h, const semb_mg_ctx& ctx, int level, const do
 int semb_mg_transfer_run(semb_mesh* h, const semb_mg_ctx& ctx, int level, int restrict_, const double* in, double* out, cudaStream_t s);
 int64_t semb_mg_level_n(const semb_mg_ctx& ctx, int level);
 void semb_mg_destroy_all(semb_mesh* h);
+
+// ---- flow.cu
+int semb_flow_prepare(semb_mesh* h, cudaStream_t s);
 
 // ---- export.cu
 int semb_vmag_launch(const double* vx, const double* vy, const double* vz, double* out, int64_t n, cudaStream_t s);

@@ -21,7 +21,7 @@ ERRORS = {-1: "SEMB_EINVAL", -2: "SEMB_ENOMEM", -3: "SEMB_ECUDA", -4: "SEMB_EGEO
 SYMBOLS = ["semb_gll", "semb_setup", "semb_destroy", "semb_last_error", "semb_mesh_info", "semb_apply_axhelm",
            "semb_set_geometry_mode", "semb_gather_scatter", "semb_apply_mask", "semb_assemble_rhs", "semb_apply_operator", "semb_jacobi_diag",
            "semb_pcg_solve", "semb_step_solve", "semb_mg_vcycle", "semb_mg_transfer", "semb_mg_level_size", "semb_estimate_lmax", "semb_cheb_jacobi", "semb_publish_field", "semb_publish_state",
-           "semb_export_field", "semb_field_minmax_hist", "semb_colormap_apply", "semb_image_slice", "semb_image_isosurface", "semb_apply_axhelm_host", "semb_pcg_solve_host", "semb_read_device", "semb_stream_probe", "semb_version"]
+           "semb_export_field", "semb_field_minmax_hist", "semb_gradient", "semb_weak_divergence", "semb_flow_explicit_terms", "semb_boussinesq_step", "semb_colormap_apply", "semb_image_slice", "semb_image_isosurface", "semb_apply_axhelm_host", "semb_pcg_solve_host", "semb_read_device", "semb_stream_probe", "semb_version"]
 
 
 class SembError(RuntimeError):
@@ -107,6 +107,39 @@ class TorchAllocator:
 class FieldDesc(C.Structure):
     _fields_ = [("name", C.c_char_p), ("ptr", C.c_void_p), ("dtype", C.c_int32), ("memspace", C.c_int32),
                 ("count", C.c_int64), ("stride", C.c_int64), ("cycle", C.c_int64), ("time", C.c_double)]
+
+
+class FlowOpts(C.Structure):
+    _fields_ = [("Ra", C.c_double), ("Pr", C.c_double), ("dt", C.c_double), ("tags_u", C.c_uint32), ("tags_T", C.c_uint32),
+                ("rtol", C.c_double), ("precond_p", C.c_int32), ("precond_u", C.c_int32), ("mg_fp32", C.c_int32), ("maxit", C.c_int32),
+                ("forcing", C.c_void_p * 4)]
+
+
+class FlowStateC(C.Structure):
+    _fields_ = [("u", C.c_void_p * 3), ("theta", C.c_void_p), ("p", C.c_void_p), ("u1", C.c_void_p * 3), ("theta1", C.c_void_p),
+                ("N1", C.c_void_p * 4), ("C1", C.c_void_p * 3), ("step_index", C.c_int64)]
+
+
+class FlowStats(C.Structure):
+    _fields_ = [("iters", C.c_int32 * 5), ("status", C.c_int32 * 5)]
+
+
+class FlowState:
+    """device arrays of a Boussinesq run (semb_flow_state): torch owns the memory, the library the arithmetic"""
+
+    def __init__(self, n):
+        import torch
+        z = lambda: torch.zeros(n, dtype=torch.float64, device="cuda")
+        self.u = [z() for _ in range(3)]; self.theta = z(); self.p = z()
+        self.u1 = [z() for _ in range(3)]; self.theta1 = z()
+        self.N1 = [z() for _ in range(4)]; self.C1 = [z() for _ in range(3)]
+        self.c = FlowStateC()
+        for i in range(3):
+            self.c.u[i] = self.u[i].data_ptr(); self.c.u1[i] = self.u1[i].data_ptr(); self.c.C1[i] = self.C1[i].data_ptr()
+        for i in range(4):
+            self.c.N1[i] = self.N1[i].data_ptr()
+        self.c.theta, self.c.p, self.c.theta1 = self.theta.data_ptr(), self.p.data_ptr(), self.theta1.data_ptr()
+        self.c.step_index = 0
 
 
 class ImageView(C.Structure):
@@ -370,6 +403,25 @@ class Mesh:
         d = FieldDesc()
         self._check(lib().semb_export_field(self._h, name.encode(), C.byref(d)))
         return d
+
+    def gradient(self, phi, gx, gy, gz):
+        self._check(lib().semb_gradient(self._h, _dp(phi), _dp(gx), _dp(gy), _dp(gz), _stream()))
+
+    def weak_divergence(self, gx, gy, gz, out):
+        self._check(lib().semb_weak_divergence(self._h, _dp(gx), _dp(gy), _dp(gz), _dp(out), _stream()))
+
+    def flow_explicit_terms(self, ux, uy, uz, theta, N4, omega3, forcing=None):
+        f = (C.c_void_p * 4)(*[(t.data_ptr() if t is not None else None) for t in (forcing or [None] * 4)])
+        self._check(lib().semb_flow_explicit_terms(self._h, _dp(ux), _dp(uy), _dp(uz), _dp(theta), f if forcing else None, _dp(N4), _dp(omega3), _stream()))
+
+    def boussinesq_step(self, state, Ra, Pr, dt, tags_u, tags_T, rtol=1e-10, precond_p=3, precond_u=1, mg_fp32=False, maxit=0, forcing=None):
+        """one time step on `state` (FlowState); returns (status, iterations of the pressure, u_x, u_y, u_z, theta solves)"""
+        o = FlowOpts(Ra, Pr, dt, tags_u, tags_T, rtol, precond_p, precond_u, 1 if mg_fp32 else 0, maxit)
+        for i, t in enumerate(forcing or []):
+            o.forcing[i] = t.data_ptr() if t is not None else None
+        st = FlowStats()
+        rc = self._check(lib().semb_boussinesq_step(self._h, C.byref(o), C.byref(state.c), C.byref(st), _stream()))
+        return int(rc), [int(v) for v in st.iters]
 
     def image_slice(self, desc, view, cmap, key, rgba=None):
         """planar slice of an exported field into key (uint64/int64 [H*W]) and rgba (int32/uint32 [H*W] or None)"""
