@@ -423,6 +423,35 @@ def geometry_section_affine(torch, semb, out, u, w, sweep, peak):
     return out
 
 
+def boussinesq_section(torch, semb, G, m, nsteps):
+    """configs[4] as a REAL time step (Eqs. (1)-(3)): no-slip walls, isothermal plates T(z=0) = 1,
+    T(z=1) = 0, adiabatic side wall, started from the conduction state plus a seeded perturbation of theta,
+    dt = 5e-4 (configs[4]), Ra = 1e8, Pr = 0.7; pressure by p-multigrid PCG on FP32 levels, Helmholtz solves by Jacobi-PCG."""
+    n = m.n
+    st = semb.FlowState(n)
+    th0 = torch.from_numpy(0.05 * I.uniform(I.seed_for(4, 7), n) * np.sin(np.pi * m.z)).cuda()
+    G.gather_scatter(th0)                       # continuous start field: QQ^T, then the inverse multiplicity through a unit field
+    ones = torch.ones(n, dtype=torch.float64, device="cuda"); G.gather_scatter(ones)
+    th0.div_(ones); G.apply_mask(th0, 0b10)
+    st.theta.copy_(th0)
+    del th0, ones
+    secs, its = [], []
+    for s in range(nsteps):
+        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(); t0.record()
+        rc, it = G.boussinesq_step(st, 1e8, 0.7, 5e-4, 0b110, 0b10, rtol=1e-10, mg_fp32=True)
+        t1.record(); torch.cuda.synchronize()
+        secs.append(t0.elapsed_time(t1) * 1e-3); its.append(it)
+    umax = max(float(c.abs().max()) for c in st.u)
+    out = {"steps_run": nsteps, "seconds_per_step": secs, "iterations_per_step_p_ux_uy_uz_theta": its, "status": rc, "max_abs_velocity": umax,
+           "points_per_second_per_gpu": n / secs[-1],
+           "note": "one full Boussinesq step (explicit terms, curl-curl pressure Poisson with mean projection, 3 velocity + 1 temperature "
+                   "Helmholtz solves); step 1 builds the multigrid levels and the metrics.  Paper context: 34-36 M points per second per "
+                   "A100 for the whole NekRS step at p = 7, 9 (Table 4, L279-285; other hardware, other preconditioner)"}
+    del st
+    return out
+
+
 def config_section(torch, semb, name, peak, args):
     """build -> 20 Jacobi-PCG iterations -> stand-alone axhelm -> time to solution (-> ten steps on cfg4) -> destroy"""
     m, G = build_problem(torch, semb, WORKLOADS[name])
@@ -448,6 +477,7 @@ def config_section(torch, semb, name, peak, args):
             if args.full_solves:
                 sv.append(("jacobi_pcg_all_solves", dict(precond=1)))
             steps = ten_steps(torch, G, m, args.cfg4_steps, sv)
+            sec["boussinesq_steps"] = boussinesq_section(torch, semb, G, m, 3)
     del b
     G.close()
     torch.cuda.empty_cache()
@@ -465,10 +495,11 @@ def export_section(torch, semb, G, m, ms_step):
     mm = torch.zeros(2, dtype=torch.float64, device="cuda"); hist = torch.zeros(256, dtype=torch.int64, device="cuda")
 
     def analysis_step(cycle):
-        G.publish_state(cycle, 1e-3 * cycle)                     # refreshes |v| (one kernel: 24 B read + 8 B written per node)
-        dT = G.export_field("temperature"); dV = G.export_field("velocity_magnitude")
-        semb.field_minmax_hist(dT, 256, 0.0, 1.0, mm, hist)      # one pass: 8 B/node
-        semb.field_minmax_hist(dV, 256, 0.0, 0.0, mm, hist)      # range found on the device: two passes, 16 B/node
+        G.publish_state(cycle, 1e-3 * cycle)                     # no kernel: nobody asked for the derived field's buffer
+        dT = G.export_field("temperature")
+        dv = [G.export_field(nm) for nm in ("velocity_x", "velocity_y", "velocity_z")]
+        semb.field_minmax_hist(dT, 256, 0.0, 1.0, mm, hist)      # range given: one pass, 8 B/node
+        semb.vector_magnitude_minmax_hist(dv[0], dv[1], dv[2], 256, 0.0, 5.2, mm, hist)   # |v| on the fly, range given: one pass, 24 B/node
         return dT
     dT = analysis_step(0)
     torch.cuda.synchronize()
@@ -480,12 +511,13 @@ def export_section(torch, semb, G, m, ms_step):
         analysis_step(c + 1)
     x1.record(); torch.cuda.synchronize()
     t_an = x0.elapsed_time(x1) / reps
-    nbytes = (24 + 8 + 8 + 16) * n
-    out = {"ms_per_analysis_step": t_an, "bytes_per_node": 56, "gbs": nbytes / (t_an * 1e-3) / 1e9,
+    nbytes = (8 + 24) * n
+    out = {"ms_per_analysis_step": t_an, "bytes_per_node": 32, "gbs": nbytes / (t_an * 1e-3) / 1e9,
            "pointer_identity": bool(dT.ptr == T.data_ptr()), "bytes_allocated": int(free0 - torch.cuda.mem_get_info()[0]),
            "overhead_vs_pcg_iteration_pct": {str(nv): 100.0 * ((t_an + nv * ms_step) / (nv * ms_step) - 1.0) for nv in (1, 10, 100)},
-           "note": "overhead = (t_vis + (n_vis - 1) t_novis) / (n_vis t_novis) - 1 with t_vis = t_novis + analysis step, "
-                   "t_novis = one PCG iteration (PAPER.md:L375)"}
+           "note": "min / max / 256-bin histogram of T (8 B/node) and of |v| computed on the fly from its components (24 B/node), each one "
+                   "pass with a given range; overhead = (t_vis + (n_vis - 1) t_novis) / (n_vis t_novis) - 1 with t_vis = t_novis + analysis "
+                   "step, t_novis = one PCG iteration (PAPER.md:L375)"}
     del T, vel
     return out
 

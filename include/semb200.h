@@ -263,17 +263,26 @@ typedef struct {
 /* Register a device array under a name once.  Names "velocity_x|y|z" additionally
  * define the derived field "velocity_magnitude" (library-owned buffer, allocated here, not later). */
 SEMB_API int semb_publish_field(semb_handle h, const char* name, double* dev_ptr, int64_t count);
-/* Per analysis step: records cycle/time and refreshes derived fields with one
- * kernel on stream.  Steps that do no analysis simply do not call it. */
+/* Per analysis step: records cycle/time and refreshes, with one kernel on stream, those derived fields
+ * that a consumer has asked for through semb_export_field before (none otherwise: nothing unused is paid for).
+ * Steps that do no analysis simply do not call it.  A derived field's buffer is current from the first publish_state AFTER
+ * its first export_field on. */
 SEMB_API int semb_publish_state(semb_handle h, int64_t cycle, double time, void* stream);
 /* No copy, no allocation, no synchronisation, no launch. */
 SEMB_API int semb_export_field(semb_handle h, const char* name, semb_field_desc* out);
 /* In-device consumer: min, max and an nbins histogram of the field over [lo, hi] (values outside go
  * to the end bins); bin = min(nbins-1, floor((v - lo) * (nbins / (hi - lo)))).
  * minmax_dev device [2], hist_dev device [nbins] (uint64).  Results stay on the device.
- * If lo >= hi the range [min, max] found by the first pass is used (two passes). */
+ * lo < hi: ONE pass over the field (min, max and counts together, 8 B/node).  If lo >= hi the range [min, max] found by a
+ * first pass is used (two passes). */
 SEMB_API int semb_field_minmax_hist(const semb_field_desc* f, int nbins, double lo, double hi,
                            double* minmax_dev, uint64_t* hist_dev, void* stream);
+
+/* The same statistics of the magnitude of a vector field given by its three exported components, |v| = sqrt(fma(vz, vz,
+ * fma(vy, vy, vx vx))) (reading R11) computed ON THE FLY: nothing is written, 24 B/node per pass.  One pass when
+ * lo < hi, two when the range is to be found.  The three descriptors must agree in count and stride. */
+SEMB_API int semb_vector_magnitude_minmax_hist(const semb_field_desc* vx, const semb_field_desc* vy, const semb_field_desc* vz,
+                                      int nbins, double lo, double hi, double* minmax_dev, uint64_t* hist_dev, void* stream);
 
 /* ---- in-situ IMAGE consumer (§5.3: the overview scene = "two slices on the walls,
  * two vertical slices in the background and an isocontour", 4096 pixels on the longest side, 2048 on the other).

@@ -306,7 +306,7 @@ int semb_publish_state(semb_handle h, int64_t cycle, double time, void* stream)
     if (!h) return SEMB_EINVAL;
     h->cycle = cycle; h->time = time;
     semb_field_entry* vm = find_field(h, "velocity_magnitude");
-    if (vm) {
+    if (vm && vm->wanted) {           // refreshed only once a consumer has asked for the pointer (pay for nothing unused)
         semb_field_entry *vx = find_field(h, "velocity_x"), *vy = find_field(h, "velocity_y"), *vz = find_field(h, "velocity_z");
         if (semb_vmag_launch(vx->ptr, vy->ptr, vz->ptr, vm->ptr, vm->count, (cudaStream_t)stream))
             return semb_fail(h, SEMB_ECUDA, "velocity_magnitude kernel: %s", cudaGetErrorString(cudaGetLastError()));
@@ -319,6 +319,11 @@ int semb_export_field(semb_handle h, const char* name, semb_field_desc* out)
     if (!h || !name || !out) return SEMB_EINVAL;
     semb_field_entry* f = find_field(h, name);
     if (!f) return SEMB_ENOTFOUND;
+    if (f->derived && !f->wanted) {
+        // first request of a derived field: from now on publish_state refreshes it; the content is current from the NEXT
+        // publish_state on (this call itself launches nothing)
+        f->wanted = true;
+    }
     out->name = f->name.c_str(); out->ptr = f->ptr; out->dtype = SEMB_F64; out->memspace = SEMB_MEM_DEVICE;
     out->count = f->count; out->stride = 1; out->cycle = h->cycle; out->time = h->time;
     return SEMB_OK;
@@ -329,8 +334,18 @@ int semb_field_minmax_hist(const semb_field_desc* f, int nbins, double lo, doubl
 {
     if (!f || !f->ptr || !minmax_dev || !hist_dev) return SEMB_EINVAL;
     if (f->memspace != SEMB_MEM_DEVICE || f->dtype != SEMB_F64) return SEMB_EINVAL;
-    return semb_minmax_hist_launch((const double*)f->ptr, f->count, f->stride, nbins, lo, hi, minmax_dev, hist_dev,
+    return semb_minmax_hist_launch((const double*)f->ptr, nullptr, nullptr, f->count, f->stride, nbins, lo, hi, minmax_dev, hist_dev,
                                    (cudaStream_t)stream);
+}
+
+int semb_vector_magnitude_minmax_hist(const semb_field_desc* fx, const semb_field_desc* fy, const semb_field_desc* fz, int nbins,
+                                      double lo, double hi, double* minmax_dev, uint64_t* hist_dev, void* stream)
+{
+    if (!fx || !fy || !fz || !fx->ptr || !fy->ptr || !fz->ptr || !minmax_dev || !hist_dev) return SEMB_EINVAL;
+    for (const semb_field_desc* f : {fx, fy, fz})
+        if (f->memspace != SEMB_MEM_DEVICE || f->dtype != SEMB_F64 || f->count != fx->count || f->stride != fx->stride) return SEMB_EINVAL;
+    return semb_minmax_hist_launch((const double*)fx->ptr, (const double*)fy->ptr, (const double*)fz->ptr, fx->count, fx->stride, nbins,
+                                   lo, hi, minmax_dev, hist_dev, (cudaStream_t)stream);
 }
 
 int semb_apply_axhelm_host(semb_handle h, double lambda, const double* u_host, double* w_host)

@@ -35,6 +35,10 @@ static __constant__ double c_xi[SEMB_MAX_N + 1][SEMB_MAXN1], c_rho[SEMB_MAX_N + 
 //          C_t = x_r x x_s and J = x_r . C_r are recomputed per node and G applied in factored form
 //          g_a = (W / J) C_a . (C_r u_r + C_s u_s + C_t u_t)                                        192 B/element
 
+#ifndef SEMB_AX_SPLIT_N1
+#define SEMB_AX_SPLIT_N1 99          // off by default until measured
+#endif
+
 // 1 / d for d > 0 in the normal range: hardware seed (2^-23) + two Newton steps (2^-46, 2^-92 -> rounding level)
 __device__ __forceinline__ double ax_rcp(double d)
 {
@@ -320,9 +324,13 @@ k_axhelm_line(int64_t E, int64_t n, const void* __restrict__ geo_v, double lambd
         for (int k = 0; k < n1; ++k) ru[k] = ue[k * n2];
     }
     // ---- global loads, t-line layout: lane -> consecutive nodes of plane k (coalesced 64-bit)
+    // KH: how many k-planes of factors a thread loads up front.  For n1 >= SEMB_AX_SPLIT_N1 (N = 9, 10) the 6 x n1 factors of a
+    // thread are 120+ registers on their own; loading the second half of the planes only after the second barrier (they are L2
+    // hits by then: the bulk prefetch brought the element in) halves that footprint and lets one more block reside on the SM.
+    constexpr int KH = (STORED && sizeof(ST) == 8 && n1 >= SEMB_AX_SPLIT_N1) ? (n1 + 1) / 2 : n1;
     if (STORED) {
 #pragma unroll
-        for (int k = 0; k < n1; ++k) {
+        for (int k = 0; k < KH; ++k) {
 #pragma unroll
             for (int c = 0; c < NG; ++c) G[c][k] = (CT)__ldg(g + c * Np + k * n2);
         }
@@ -369,6 +377,13 @@ k_axhelm_line(int64_t E, int64_t n, const void* __restrict__ geo_v, double lambd
     CT ut[n1];
     ax_line<n1, 0, CT>(ru, ut);
     __syncthreads();
+    if (STORED && KH < n1) {
+#pragma unroll
+        for (int k = KH; k < n1; ++k) {
+#pragma unroll
+            for (int c = 0; c < NG; ++c) G[c][k] = (CT)__ldg(g + c * Np + k * n2);
+        }
+    }
     // ---- geometric factors at the nodes of the t-line
     CT gt[n1];
     double Bk[(HELM && !STORED) ? n1 : 1];                 // mass factor W J of the on-the-fly modes

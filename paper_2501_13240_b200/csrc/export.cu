@@ -64,9 +64,10 @@ k_minmax(int64_t n, int64_t stride, const double* __restrict__ v, unsigned long 
 
 // bin = min(nbins-1, floor((v - lo) * scale)), scale = nbins / (hi - lo); v < lo -> bin 0.
 // The subtraction and the multiplication are rounded separately (no fused multiply-add).
+template <int NV>
 __global__ void __launch_bounds__(256)
-k_hist(int64_t n, int64_t stride, const double* __restrict__ v, int nbins, double lo, double hi,
-       const double* __restrict__ range_dev, unsigned long long* __restrict__ hist)
+k_hist(int64_t n, int64_t stride, const double* __restrict__ v, const double* __restrict__ v1, const double* __restrict__ v2, int nbins,
+       double lo, double hi, const double* __restrict__ range_dev, unsigned long long* __restrict__ hist)
 {
     extern __shared__ unsigned int sh[];
     for (int b = threadIdx.x; b < nbins; b += blockDim.x) sh[b] = 0u;
@@ -74,7 +75,9 @@ k_hist(int64_t n, int64_t stride, const double* __restrict__ v, int nbins, doubl
     const double scale = __ddiv_rn((double)nbins, __dsub_rn(hi, lo));
     __syncthreads();
     for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
-        const double t = __dsub_rn(v[l * stride], lo);
+        double a = v[l * stride];
+        if (NV == 3) { const double b = v1[l * stride], c = v2[l * stride]; a = sqrt(fma(c, c, fma(b, b, __dmul_rn(a, a)))); }
+        const double t = __dsub_rn(a, lo);
         const double sc = __dmul_rn(t, scale);
         long long b = (sc < 0.0) ? 0ll : (long long)floor(sc);
         if (b > nbins - 1) b = nbins - 1;
@@ -84,20 +87,89 @@ k_hist(int64_t n, int64_t stride, const double* __restrict__ v, int nbins, doubl
     for (int b = threadIdx.x; b < nbins; b += blockDim.x) if (sh[b]) atomicAdd(&hist[b], (unsigned long long)sh[b]);
 }
 
-int semb_minmax_hist_launch(const double* v, int64_t n, int64_t stride, int nbins, double lo, double hi,
+// One pass over the data when the range is known: min, max and the histogram together.  NV = 1: a scalar field; NV = 3: the
+// magnitude of a vector field computed on the fly, sqrt(fma(vz, vz, fma(vy, vy, vx vx))) (reading R11), never written to memory.
+template <int NV>
+__global__ void __launch_bounds__(256)
+k_minmax_hist(int64_t n, int64_t stride, const double* __restrict__ v0, const double* __restrict__ v1, const double* __restrict__ v2,
+              int nbins, double lo, double hi, unsigned long long* __restrict__ mm, unsigned long long* __restrict__ hist)
+{
+    extern __shared__ unsigned int sh[];
+    for (int b = threadIdx.x; b < nbins; b += blockDim.x) sh[b] = 0u;
+    const double scale = __ddiv_rn((double)nbins, __dsub_rn(hi, lo));
+    __syncthreads();
+    double mn = INFINITY, mx = -INFINITY;
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
+        double a = v0[l * stride];
+        if (NV == 3) { const double b = v1[l * stride], c = v2[l * stride]; a = sqrt(fma(c, c, fma(b, b, __dmul_rn(a, a)))); }
+        mn = fmin(mn, a); mx = fmax(mx, a);
+        const double sc = __dmul_rn(__dsub_rn(a, lo), scale);
+        long long b = (sc < 0.0) ? 0ll : (long long)floor(sc);
+        if (b > nbins - 1) b = nbins - 1;
+        atomicAdd(&sh[b], 1u);
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        mn = fmin(mn, __shfl_xor_sync(0xffffffffu, mn, o));
+        mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    }
+    __shared__ double smn[8], smx[8];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane == 0) { smn[wid] = mn; smx[wid] = mx; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 8; ++w) { mn = fmin(mn, smn[w]); mx = fmax(mx, smx[w]); }
+        atomicMin(&mm[0], enc(mn)); atomicMax(&mm[1], enc(mx));
+    }
+    for (int b = threadIdx.x; b < nbins; b += blockDim.x) if (sh[b]) atomicAdd(&hist[b], (unsigned long long)sh[b]);
+}
+
+// min / max of |v| alone (first pass when the histogram range is to be found on the device)
+__global__ void __launch_bounds__(256)
+k_minmax_vmag(int64_t n, int64_t stride, const double* __restrict__ v0, const double* __restrict__ v1, const double* __restrict__ v2,
+              unsigned long long* __restrict__ mm)
+{
+    double mn = INFINITY, mx = -INFINITY;
+    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
+        const double a0 = v0[l * stride], b = v1[l * stride], c = v2[l * stride];
+        const double a = sqrt(fma(c, c, fma(b, b, __dmul_rn(a0, a0))));
+        mn = fmin(mn, a); mx = fmax(mx, a);
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        mn = fmin(mn, __shfl_xor_sync(0xffffffffu, mn, o));
+        mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    }
+    __shared__ double smn[8], smx[8];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane == 0) { smn[wid] = mn; smx[wid] = mx; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 8; ++w) { mn = fmin(mn, smn[w]); mx = fmax(mx, smx[w]); }
+        atomicMin(&mm[0], enc(mn)); atomicMax(&mm[1], enc(mx));
+    }
+}
+
+// v1 == NULL: scalar field v0; else the magnitude of (v0, v1, v2) computed on the fly
+int semb_minmax_hist_launch(const double* v, const double* v1, const double* v2, int64_t n, int64_t stride, int nbins, double lo, double hi,
                             double* minmax_dev, uint64_t* hist_dev, cudaStream_t s)
 {
     if (nbins < 1 || nbins > 8192 || n < 1 || stride < 1) return SEMB_EINVAL;
     // each block's shared counters are 32-bit: keep every block's share of the input below 2^32
     int64_t blocks = (n + 2047) / 2048; if (blocks > semb_sm_count() * 8) blocks = semb_sm_count() * 8; if (blocks < 1) blocks = 1;
     unsigned long long* mm = (unsigned long long*)minmax_dev;
+    unsigned long long* hist = (unsigned long long*)hist_dev;
     k_mm_init<<<1, 1, 0, s>>>(mm);
-    k_minmax<<<(unsigned)blocks, 256, 0, s>>>(n, stride, v, mm);
-    k_mm_decode<<<1, 1, 0, s>>>(mm);
     if (cudaMemsetAsync(hist_dev, 0, sizeof(uint64_t) * nbins, s) != cudaSuccess) return SEMB_ECUDA;
-    const bool own_range = !(lo < hi);
-    k_hist<<<(unsigned)blocks, 256, sizeof(unsigned int) * nbins, s>>>(n, stride, v, nbins, lo, hi,
-                                                                      own_range ? minmax_dev : nullptr,
-                                                                      (unsigned long long*)hist_dev);
+    const size_t smem = sizeof(unsigned int) * nbins;
+    if (lo < hi) {                       // range given: ONE pass (8 B/node for a scalar, 24 B/node for a magnitude)
+        if (v1) k_minmax_hist<3><<<(unsigned)blocks, 256, smem, s>>>(n, stride, v, v1, v2, nbins, lo, hi, mm, hist);
+        else    k_minmax_hist<1><<<(unsigned)blocks, 256, smem, s>>>(n, stride, v, nullptr, nullptr, nbins, lo, hi, mm, hist);
+        k_mm_decode<<<1, 1, 0, s>>>(mm);
+    } else {                             // range = [min, max] found by a first pass
+        if (v1) k_minmax_vmag<<<(unsigned)blocks, 256, 0, s>>>(n, stride, v, v1, v2, mm);
+        else    k_minmax<<<(unsigned)blocks, 256, 0, s>>>(n, stride, v, mm);
+        k_mm_decode<<<1, 1, 0, s>>>(mm);
+        if (v1) k_hist<3><<<(unsigned)blocks, 256, smem, s>>>(n, stride, v, v1, v2, nbins, lo, hi, minmax_dev, hist);
+        else    k_hist<1><<<(unsigned)blocks, 256, smem, s>>>(n, stride, v, nullptr, nullptr, nbins, lo, hi, minmax_dev, hist);
+    }
     return cudaGetLastError() == cudaSuccess ? SEMB_OK : SEMB_ECUDA;
 }

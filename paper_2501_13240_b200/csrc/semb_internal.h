@@ -34,6 +34,7 @@ struct semb_field_entry {
     double* ptr = nullptr;
     int64_t count = 0;
     bool derived = false;
+    bool wanted = false;       // derived fields: a consumer has asked for the pointer, so publish_state keeps the buffer current
 };
 
 struct semb_mg;
@@ -195,5 +196,5 @@ int semb_flow_prepare(semb_mesh* h, cudaStream_t s);
 
 // ---- export.cu
 int semb_vmag_launch(const double* vx, const double* vy, const double* vz, double* out, int64_t n, cudaStream_t s);
-int semb_minmax_hist_launch(const double* v, int64_t n, int64_t stride, int nbins, double lo, double hi,
+int semb_minmax_hist_launch(const double* v, const double* v1, const double* v2, int64_t n, int64_t stride, int nbins, double lo, double hi,
                             double* minmax_dev, uint64_t* hist_dev, cudaStream_t s);

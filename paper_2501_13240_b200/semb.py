@@ -21,7 +21,7 @@ ERRORS = {-1: "SEMB_EINVAL", -2: "SEMB_ENOMEM", -3: "SEMB_ECUDA", -4: "SEMB_EGEO
 SYMBOLS = ["semb_gll", "semb_setup", "semb_destroy", "semb_last_error", "semb_mesh_info", "semb_apply_axhelm",
            "semb_set_geometry_mode", "semb_gather_scatter", "semb_apply_mask", "semb_assemble_rhs", "semb_apply_operator", "semb_jacobi_diag",
            "semb_pcg_solve", "semb_step_solve", "semb_mg_vcycle", "semb_mg_transfer", "semb_mg_level_size", "semb_estimate_lmax", "semb_cheb_jacobi", "semb_publish_field", "semb_publish_state",
-           "semb_export_field", "semb_field_minmax_hist", "semb_gradient", "semb_weak_divergence", "semb_flow_explicit_terms", "semb_boussinesq_step", "semb_colormap_apply", "semb_image_slice", "semb_image_isosurface", "semb_apply_axhelm_host", "semb_pcg_solve_host", "semb_read_device", "semb_stream_probe", "semb_version"]
+           "semb_export_field", "semb_field_minmax_hist", "semb_vector_magnitude_minmax_hist", "semb_gradient", "semb_weak_divergence", "semb_flow_explicit_terms", "semb_boussinesq_step", "semb_colormap_apply", "semb_image_slice", "semb_image_isosurface", "semb_apply_axhelm_host", "semb_pcg_solve_host", "semb_read_device", "semb_stream_probe", "semb_version"]
 
 
 class SembError(RuntimeError):
@@ -444,6 +444,14 @@ def stream_probe(src, dst, nread):
     rc = lib().semb_stream_probe(_dp(src), _dp(dst), C.c_int64(dst.numel()), C.c_int(nread), _stream())
     if rc:
         raise SembError(rc, "semb_stream_probe")
+
+
+def vector_magnitude_minmax_hist(dx, dy, dz, nbins, lo, hi, minmax_dev, hist_dev):
+    """min / max / histogram of |v| from the three component descriptors, computed on the fly (nothing written)"""
+    rc = lib().semb_vector_magnitude_minmax_hist(C.byref(dx), C.byref(dy), C.byref(dz), C.c_int(nbins), C.c_double(lo), C.c_double(hi),
+                                                 _dp(minmax_dev), _dp(hist_dev), _stream())
+    if rc:
+        raise SembError(rc, "semb_vector_magnitude_minmax_hist")
 
 
 def colormap_apply(cmap, val, rgba):

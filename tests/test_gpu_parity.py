@@ -336,6 +336,13 @@ def test_export_is_zero_copy_and_consumer_is_exact(torch_cuda, semb, cases, orc)
     G.publish_field("temperature", dT)
     for name, t in zip(("velocity_x", "velocity_y", "velocity_z"), dv):
         G.publish_field(name, t)
+    G.export_field("velocity_magnitude")             # a consumer asks for the derived field: publish_state keeps it current from now on
+    # one untimed pass first: the driver loads kernel images lazily and grows the context's local-memory pool on the first launch
+    # of a kernel with a stack frame -- context growth, not an allocation of the call
+    warm_mm = torch.zeros(2, dtype=torch.float64, device="cuda"); warm_h = torch.zeros(256, dtype=torch.int64, device="cuda")
+    G.publish_state(0, 0.0)
+    semb.field_minmax_hist(G.export_field("temperature"), 256, 0.0, 1.0, warm_mm, warm_h)
+    semb.field_minmax_hist(G.export_field("temperature"), 256, 0.0, 0.0, warm_mm, warm_h)
     torch.cuda.synchronize()
     free0 = torch.cuda.mem_get_info()[0]
     G.publish_state(17, 0.25)
@@ -355,5 +362,13 @@ def test_export_is_zero_copy_and_consumer_is_exact(torch_cuda, semb, cases, orc)
     mn, mx, h = orc.minmax_hist(vm_ref, 64, vm_ref.min(), vm_ref.max())
     assert mm[0].item() == mn and mm[1].item() == mx
     assert np.array_equal(hist[:64].cpu().numpy().astype(np.uint64), h)
+    # the same statistics from the three components, |v| computed on the fly (nothing written): one pass with a given range,
+    # two when the range is to be found; both exactly the oracle's counts
+    dx, dy, dz = (G.export_field(nm) for nm in ("velocity_x", "velocity_y", "velocity_z"))
+    for lo, hi in ((0.0, 1.8), (0.0, 0.0)):
+        semb.vector_magnitude_minmax_hist(dx, dy, dz, 64, lo, hi, mm, hist[:64])
+        mn, mx, h = orc.minmax_hist(vm_ref, 64, lo if lo < hi else vm_ref.min(), hi if lo < hi else vm_ref.max())
+        assert mm[0].item() == mn and mm[1].item() == mx
+        assert np.array_equal(hist[:64].cpu().numpy().astype(np.uint64), h)
     with pytest.raises(semb.SembError):
         G.export_field("no_such_field")
