@@ -189,6 +189,11 @@ typedef struct {
                                  the class sums of the gather-scatter accumulate in fp64); the PCG around the cycle, its
                                  residual and its solution stay fp64
                                  (reading R21: same iteration counts, fp64 true residual <= 2e-10)          */
+    int32_t  mg_schwarz;      /* 1: every level of order >= 2 except the last is smoothed by the fourth-kind Chebyshev polynomial
+                                 (degree mg_smooth_degree) in S A, S the overlapping Schwarz smoother of PAPER.md:L102 -- element
+                                 closures as subdomains, fast-diagonalisation subdomain solves (reading R26); lambda_max(S A)
+                                 estimated by 10 preconditioned Lanczos steps x 1.1 and cached.  0: Chebyshev-Jacobi (R19) */
+    int32_t  pad2_;
 } semb_pcg_opts;
 
 typedef struct {
@@ -244,6 +249,10 @@ SEMB_API int64_t semb_mg_level_size(semb_handle h, const semb_pcg_opts* opts, in
 /* z = Chebyshev-Jacobi(k) preconditioner applied to r (device [n] each, z != r). */
 SEMB_API int semb_cheb_jacobi(semb_handle h, double lambda, uint32_t dirichlet_tags, int k, double lmax,
                      const double* r, double* z, void* stream);
+
+/* out = S r, the Schwarz smoother of reading R26 for the operator (lambda, dirichlet_tags) on the handle's own mesh (order >= 2):
+ * S r = M QQ^T [ w o A~_e^-1 (w o r) ], w = sqrt(1 / multiplicity).  r, out device [n], r continuous and masked, out != r. */
+SEMB_API int semb_schwarz_apply(semb_handle h, double lambda, uint32_t dirichlet_tags, const double* r, double* out, void* stream);
 
 /* ---- in-situ hand-off ---------------------------------------- */
 #define SEMB_F64          1

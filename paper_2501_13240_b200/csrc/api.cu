@@ -65,6 +65,7 @@ int semb_destroy(semb_handle h)
     if (!h) return SEMB_OK;
     cudaDeviceSynchronize();
     semb_mg_destroy_all(h);
+    semb_schwarz_free(h);
     semb_dev_free(h, h->xyz);
     semb_dev_free(h, h->geo); semb_dev_free(h, h->gid); semb_dev_free(h, h->invmult); semb_dev_free(h, h->gs_code); semb_dev_free(h, h->gs_hi);
     if (h->geoK && h->geoK != h->geo) semb_dev_free(h, h->geoK);
@@ -263,6 +264,13 @@ int64_t semb_mg_level_size(semb_handle h, const semb_pcg_opts* o, int level)
     if (level < 0 || level >= nlev) return semb_fail(h, SEMB_EINVAL, "mg_level_size: level %d of %d", level, nlev);
     const int64_t n1 = orders[level] + 1;
     return h->E * n1 * n1 * n1;
+}
+
+int semb_schwarz_apply(semb_handle h, double lambda, uint32_t tags, const double* r, double* out, void* stream)
+{
+    if (!h) return SEMB_EINVAL;
+    if (!r || !out || r == out) return semb_fail(h, SEMB_EINVAL, "schwarz_apply: bad argument");
+    return semb_schwarz_apply_run(h, tags, lambda, r, out, (cudaStream_t)stream);
 }
 
 int semb_cheb_jacobi(semb_handle h, double lambda, uint32_t tags, int k, double lmax, const double* r, double* z, void* stream)

@@ -31,7 +31,7 @@ struct semb_mg {
     bool f32_ready = false;
     float* geoF[8] = {nullptr};          // [E][7][Np]
     float* invmultF[8] = {nullptr};
-    float* WF[8][5] = {{nullptr}};       // Chebyshev work (res, d, Ad), residual, scratch
+    float* WF[8][6] = {{nullptr}};       // Chebyshev work (res, d, Ad), residual, scratch
     float* rF[8] = {nullptr};            // level l: right-hand side (level 0: the converted PCG residual)
     float* zF[8] = {nullptr};            // level l: result
     // float copies of the level diagonals for the MG_DINVF_CACHE most recently used (tags, lambda) pairs, owned
@@ -151,9 +151,9 @@ static void mg_free(semb_mesh* h, semb_mg* g)
     for (int l = 0; l < 8; ++l) {
         semb_dev_free(h, g->J[l]); semb_dev_free(h, g->rc[l]); semb_dev_free(h, g->ec[l]);
         for (int w = 0; w < 6; ++w) semb_dev_free(h, g->W[l][w]);
-        for (int w = 0; w < 5; ++w) semb_dev_free(h, g->WF[l][w]);
+        for (int w = 0; w < 6; ++w) semb_dev_free(h, g->WF[l][w]);
         semb_dev_free(h, g->geoF[l]); semb_dev_free(h, g->invmultF[l]); semb_dev_free(h, g->rF[l]); semb_dev_free(h, g->zF[l]);
-        if (l >= 1 && g->lev[l]) semb_destroy(g->lev[l]);
+        if (l >= 1 && g->lev[l]) semb_destroy(g->lev[l]);        // frees the level's Schwarz data too
     }
     for (auto& en : g->dinvF) for (float* p : en.d) semb_dev_free(h, p);
     delete g;
@@ -286,6 +286,27 @@ int semb_mg_prepare(semb_mesh* h, const semb_pcg_opts* o, semb_mg_ctx* ctx, cuda
         if (g->lmax_cache.size() >= MG_LMAX_CACHE) g->lmax_cache.clear();
         g->lmax_cache[key] = est;
     }
+    // Schwarz smoother (reading R26) on every level of order >= 2 but the last: subdomain data and lambda_max(S A)
+    ctx->schwarz = o->mg_schwarz ? 1 : 0;
+    for (int l = 0; l < 8; ++l) { ctx->sz[l] = nullptr; ctx->sz_lmax[l] = 0.0; }
+    if (ctx->schwarz) {
+        for (int l = 0; l + 1 < nlev; ++l) {
+            semb_mesh* L = g->lev[l];
+            if (L->N < 2) continue;
+            semb_mask_entry ml;
+            int rc = semb_get_mask(L, o->dirichlet_tags, &ml, s);
+            if (!rc) rc = semb_schwarz_get(L, o->dirichlet_tags, o->mg_fp32 != 0, &ctx->sz[l], s);
+            if (!rc) {
+                double* v0 = g->W[l][5];
+                k_mg_random<<<mg_grid(L->n), 256, 0, s>>>(L->n, MG_LMAX_SEED + (unsigned long long)l, v0);
+                rc = semb_gs_launch(L, v0, 1, s);
+                if (!rc) rc = semb_mask_launch(L, ml, v0, 1, s);
+                double* wk[5] = { g->W[l][0], g->W[l][1], g->W[l][2], g->W[l][3], g->W[l][4] };
+                if (!rc) rc = semb_schwarz_lmax(L, ctx->sz[l], o->lambda, ml, v0, 10, wk, &ctx->sz_lmax[l], s);
+            }
+            if (rc) return semb_fail(h, rc, "multigrid: Schwarz smoother of level %d: %s", l, semb_last_error(L));
+        }
+    }
     // masks and diagonals of every level for this operator (cached in the level handles)
     for (int l = 0; l < nlev; ++l) {
         semb_mask_entry m; double* dinv;
@@ -342,7 +363,10 @@ int semb_mg_vcycle_run(semb_mesh* h, const semb_mg_ctx& ctx, int l, const double
     semb_mesh* C = g->lev[l + 1];
     semb_mask_entry mc;
     rc = semb_get_mask(C, ctx.tags, &mc, s); if (rc) return rc;
-    rc = semb_cheb_apply(L, ctx.lambda, m, dinv, ctx.k_smooth, cc, r, z, cres, cd, cAd, scal, false, s); if (rc) return rc;   // z = S r
+    double* spare = g->W[l][5];
+    if (ctx.sz[l]) rc = semb_schwarz_cheb4(L, ctx.sz[l], ctx.lambda, m, ctx.k_smooth, ctx.sz_lmax[l], r, z, cres, cd, cAd, spare, scal, s, false);
+    else rc = semb_cheb_apply(L, ctx.lambda, m, dinv, ctx.k_smooth, cc, r, z, cres, cd, cAd, scal, false, s);                 // z = S r
+    if (rc) return rc;
     rc = semb_residual_launch(L, ctx.lambda, m, z, r, res, t1, scal, s); if (rc) return rc;                                  // res = r - A z
     interp3_launch<double>(L->E, L->n1, C->n1, g->J[l], 1, res, (const double*)L->invmult, g->rc[l + 1], 0, scal, s);               // R res
     rc = semb_gs_launch(C, g->rc[l + 1], 1, s); if (rc) return rc;
@@ -352,7 +376,9 @@ int semb_mg_vcycle_run(semb_mesh* h, const semb_mg_ctx& ctx, int l, const double
     (void)lc0;
     interp3_launch<double>(L->E, C->n1, L->n1, g->J[l], 0, (const double*)g->ec[l + 1], (const double*)nullptr, z, 1, scal, s);                    // z += P e
     rc = semb_residual_launch(L, ctx.lambda, m, z, r, res, t1, scal, s); if (rc) return rc;                                  // res = r - A z
-    rc = semb_cheb_apply(L, ctx.lambda, m, dinv, ctx.k_smooth, cc, res, z, cres, cd, cAd, scal, false, s, true); if (rc) return rc; // z += S res
+    if (ctx.sz[l]) rc = semb_schwarz_cheb4(L, ctx.sz[l], ctx.lambda, m, ctx.k_smooth, ctx.sz_lmax[l], res, z, cres, cd, cAd, spare, scal, s, true);
+    else rc = semb_cheb_apply(L, ctx.lambda, m, dinv, ctx.k_smooth, cc, res, z, cres, cd, cAd, scal, false, s, true);         // z += S res
+    if (rc) return rc;
     L->launches += 2;
     if (L != h) h->launches += L->launches - l0;
     SEMB_CUDA(h, cudaGetLastError());
@@ -381,7 +407,7 @@ static int mg_f32_prepare(semb_mesh* h, const semb_mg_ctx& ctx, cudaStream_t s)
             g->rF[l] = (float*)semb_dev_alloc(h, sizeof(float) * (size_t)n);
             g->zF[l] = (float*)semb_dev_alloc(h, sizeof(float) * (size_t)n);
             bool ok = g->geoF[l] && g->invmultF[l] && g->rF[l] && g->zF[l];
-            for (int w = 0; w < 5; ++w) { g->WF[l][w] = (float*)semb_dev_alloc(h, sizeof(float) * (size_t)n); ok = ok && g->WF[l][w]; }
+            for (int w = 0; w < 6; ++w) { g->WF[l][w] = (float*)semb_dev_alloc(h, sizeof(float) * (size_t)n); ok = ok && g->WF[l][w]; }
             if (!ok) return semb_fail(h, SEMB_ENOMEM, "multigrid: fp32 data of level %d", l);
             k_mg_convert<double, float><<<mg_grid(ng), 256, 0, s>>>(ng, L->geo, g->geoF[l], nullptr);
             k_mg_convert<double, float><<<mg_grid(n), 256, 0, s>>>(n, L->invmult, g->invmultF[l], nullptr);
@@ -438,7 +464,10 @@ static int mg_vcycle_f32(semb_mesh* h, const semb_mg_ctx& ctx, int l, const floa
     semb_mesh* C = g->lev[l + 1];
     semb_mask_entry mc;
     rc = semb_get_mask(C, ctx.tags, &mc, s); if (rc) return rc;
-    rc = semb_cheb_apply_f(L, ctx.lambda, geo, m, dinv, ctx.k_smooth, cc, r, z, cres, cd, cAd, scal, s, false); if (rc) return rc;   // z = S r
+    float* spare = g->WF[l][5];
+    if (ctx.sz[l]) rc = semb_schwarz_cheb4_f(L, ctx.sz[l], ctx.lambda, geo, m, ctx.k_smooth, ctx.sz_lmax[l], r, z, cres, cd, cAd, spare, scal, s, false);
+    else rc = semb_cheb_apply_f(L, ctx.lambda, geo, m, dinv, ctx.k_smooth, cc, r, z, cres, cd, cAd, scal, s, false);           // z = S r
+    if (rc) return rc;
     rc = semb_residual_launch_f(L, ctx.lambda, geo, m, z, r, res, t1, scal, s); if (rc) return rc;                                  // res = r - A z
     interp3_launch<float>(L->E, L->n1, C->n1, g->J[l], 1, res, g->invmultF[l], g->rF[l + 1], 0, scal, s);                           // R res
     rc = semb_gs_launch_f(C, g->rF[l + 1], s); if (rc) return rc;
@@ -446,7 +475,9 @@ static int mg_vcycle_f32(semb_mesh* h, const semb_mg_ctx& ctx, int l, const floa
     rc = mg_vcycle_f32(h, ctx, l + 1, g->rF[l + 1], g->zF[l + 1], scal, s); if (rc) return rc;
     interp3_launch<float>(L->E, C->n1, L->n1, g->J[l], 0, (const float*)g->zF[l + 1], (const float*)nullptr, z, 1, scal, s);        // z += P e
     rc = semb_residual_launch_f(L, ctx.lambda, geo, m, z, r, res, t1, scal, s); if (rc) return rc;                                  // res = r - A z
-    rc = semb_cheb_apply_f(L, ctx.lambda, geo, m, dinv, ctx.k_smooth, cc, res, z, cres, cd, cAd, scal, s, true); if (rc) return rc; // z += S res
+    if (ctx.sz[l]) rc = semb_schwarz_cheb4_f(L, ctx.sz[l], ctx.lambda, geo, m, ctx.k_smooth, ctx.sz_lmax[l], res, z, cres, cd, cAd, spare, scal, s, true);
+    else rc = semb_cheb_apply_f(L, ctx.lambda, geo, m, dinv, ctx.k_smooth, cc, res, z, cres, cd, cAd, scal, s, true);          // z += S res
+    if (rc) return rc;
     L->launches += 2;
     if (L != h) h->launches += L->launches - l0;
     SEMB_CUDA(h, cudaGetLastError());

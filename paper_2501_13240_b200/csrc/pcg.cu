@@ -487,6 +487,8 @@ int semb_cheb_run(semb_mesh* h, double lambda, uint32_t tags, int k, double lmax
 }
 
 // largest eigenvalue of the symmetric tridiagonal (a[0..m), b[0..m-1)) by bisection on the Sturm count
+static double tridiag_lmax(int m, const double* a, const double* b);
+double semb_tridiag_lmax(int m, const double* a, const double* b) { return tridiag_lmax(m, a, b); }
 static double tridiag_lmax(int m, const double* a, const double* b)
 {
     double lo = a[0], hi = a[0];

@@ -38,6 +38,7 @@ struct semb_field_entry {
 };
 
 struct semb_mg;
+struct semb_schwarz;
 
 struct semb_mesh {
     int64_t E = 0; int N = 0, n1 = 0; int64_t Np = 0, n = 0;
@@ -87,6 +88,7 @@ struct semb_mesh {
     int64_t launches = 0;               // kernels launched through this handle (bench.py reports it)
     std::vector<cudaEvent_t> prof_ev;   // event pairs around axhelm launches (opts.profile)
     std::vector<semb_mg*> mgs;          // p-multigrid hierarchies built so far (mg.cu), owned
+    std::vector<semb_schwarz*> schwarz; // Schwarz subdomain data of this (level) mesh per Dirichlet tag set (schwarz.cu), owned
     // export
     std::vector<semb_field_entry> fields;
     int64_t cycle = 0; double time = 0.0;
@@ -183,13 +185,26 @@ int semb_cheb_apply_f(semb_mesh* h, double lambda, const float* geo, const semb_
 int semb_dot_rz_launch(semb_mesh* h, const double* r, const double* z, semb_scalars* scal, cudaStream_t s);
 
 // ---- mg.cu: p-multigrid V-cycle
-struct semb_mg_ctx { semb_mg* mg; double lambda; uint32_t tags; int k_smooth, k_coarse, kind, fp32; double coarse_frac; double lmax[8]; };
+struct semb_mg_ctx { semb_mg* mg; double lambda; uint32_t tags; int k_smooth, k_coarse, kind, fp32; double coarse_frac; double lmax[8];
+                     int schwarz; semb_schwarz* sz[8]; double sz_lmax[8]; };
 int semb_mg_orders(semb_mesh* h, const semb_pcg_opts* o, int* nlev_out, int* orders);
 int semb_mg_prepare(semb_mesh* h, const semb_pcg_opts* o, semb_mg_ctx* ctx, cudaStream_t s);
 int semb_mg_vcycle_run(semb_mesh* h, const semb_mg_ctx& ctx, int level, const double* r, double* z, semb_scalars* scal, cudaStream_t s);
 int semb_mg_transfer_run(semb_mesh* h, const semb_mg_ctx& ctx, int level, int restrict_, const double* in, double* out, cudaStream_t s);
 int64_t semb_mg_level_n(const semb_mg_ctx& ctx, int level);
 void semb_mg_destroy_all(semb_mesh* h);
+
+// ---- schwarz.cu: overlapping Schwarz smoother of the multigrid levels (reading R26)
+void semb_schwarz_free(semb_mesh* L);
+int semb_schwarz_get(semb_mesh* L, uint32_t tags, bool want_float, semb_schwarz** out, cudaStream_t s);
+int semb_schwarz_lmax(semb_mesh* L, semb_schwarz* zd, double lambda, const semb_mask_entry& m, const double* v0, int steps, double* const* work,
+                      double* lmax, cudaStream_t s);
+int semb_schwarz_apply_run(semb_mesh* L, uint32_t tags, double lambda, const double* r, double* out, cudaStream_t s);
+// z (+)= W_k-Chebyshev (fourth kind) in S A applied to r; res, d, sr, t: work vectors of the level
+int semb_schwarz_cheb4(semb_mesh* L, semb_schwarz* zd, double lambda, const semb_mask_entry& m, int k, double lmax, const double* r, double* z,
+                       double* res, double* d, double* sr, double* t, semb_scalars* scal, cudaStream_t s, bool zacc);
+int semb_schwarz_cheb4_f(semb_mesh* L, semb_schwarz* zd, double lambda, const float* geo, const semb_mask_entry& m, int k, double lmax, const float* r,
+                         float* z, float* res, float* d, float* sr, float* t, semb_scalars* scal, cudaStream_t s, bool zacc);
 
 // ---- flow.cu
 int semb_flow_prepare(semb_mesh* h, cudaStream_t s);

@@ -20,7 +20,7 @@ ERRORS = {-1: "SEMB_EINVAL", -2: "SEMB_ENOMEM", -3: "SEMB_ECUDA", -4: "SEMB_EGEO
 # every symbol include/semb200.h declares (tests check that the library exports all of them)
 SYMBOLS = ["semb_gll", "semb_setup", "semb_destroy", "semb_last_error", "semb_mesh_info", "semb_apply_axhelm",
            "semb_set_geometry_mode", "semb_gather_scatter", "semb_apply_mask", "semb_assemble_rhs", "semb_apply_operator", "semb_jacobi_diag",
-           "semb_pcg_solve", "semb_step_solve", "semb_mg_vcycle", "semb_mg_transfer", "semb_mg_level_size", "semb_estimate_lmax", "semb_cheb_jacobi", "semb_publish_field", "semb_publish_state",
+           "semb_pcg_solve", "semb_step_solve", "semb_mg_vcycle", "semb_mg_transfer", "semb_mg_level_size", "semb_estimate_lmax", "semb_cheb_jacobi", "semb_schwarz_apply", "semb_publish_field", "semb_publish_state",
            "semb_export_field", "semb_field_minmax_hist", "semb_vector_magnitude_minmax_hist", "semb_gradient", "semb_weak_divergence", "semb_flow_explicit_terms", "semb_boussinesq_step", "semb_colormap_apply", "semb_image_slice", "semb_image_isosurface", "semb_apply_axhelm_host", "semb_pcg_solve_host", "semb_read_device", "semb_stream_probe", "semb_version"]
 
 
@@ -43,7 +43,7 @@ class PcgOpts(C.Structure):
                 ("maxit", C.c_int32), ("x0_is_zero", C.c_int32), ("check_every", C.c_int32), ("profile", C.c_int32),
                 ("mg_nlevels", C.c_int32), ("mg_orders", C.c_int32 * 8), ("mg_smooth_degree", C.c_int32),
                 ("mg_coarse_degree", C.c_int32), ("mg_lmax", C.c_double * 8), ("mg_smoother_kind", C.c_int32), ("pad_", C.c_int32),
-                ("mg_coarse_lmin_frac", C.c_double), ("null_mean", C.c_int32), ("mg_fp32", C.c_int32)]
+                ("mg_coarse_lmin_frac", C.c_double), ("null_mean", C.c_int32), ("mg_fp32", C.c_int32), ("mg_schwarz", C.c_int32), ("pad2_", C.c_int32)]
 
 
 def _mg_fill(o, mg_orders=None, mg_smooth=0, mg_coarse=0, mg_lmax=None, mg_kind=1, mg_coarse_frac=0.0):
@@ -307,13 +307,14 @@ class Mesh:
 
     def pcg_solve(self, b, x, lam=0.0, tags=0, precond=1, cheb_degree=2, cheb_lmax=0.0, rtol=1e-10, atol=0.0,
                   maxit=10000, x0_is_zero=True, check_every=0, hist_len=0, profile=False, mg_orders=None, mg_smooth=0,
-                  mg_coarse=0, mg_lmax=None, mg_kind=1, mg_coarse_frac=0.0, null_mean=False, mg_fp32=False):
+                  mg_coarse=0, mg_lmax=None, mg_kind=1, mg_coarse_frac=0.0, null_mean=False, mg_fp32=False, mg_schwarz=False):
         """Returns dict(iters, status, b_norm, r0_norm, r_norm, lmax_used, hist).  precond: 0 none, 1 Jacobi,
         2 Chebyshev-Jacobi, 3 p-multigrid V-cycle (mg_orders e.g. [7, 3, 1]; None = default)."""
         o = PcgOpts(lam, tags, precond, cheb_degree, cheb_lmax, rtol, atol, maxit, 1 if x0_is_zero else 0, check_every, 1 if profile else 0)
         _mg_fill(o, mg_orders, mg_smooth, mg_coarse, mg_lmax, mg_kind, mg_coarse_frac)
         o.null_mean = 1 if null_mean else 0
         o.mg_fp32 = 1 if mg_fp32 else 0
+        o.mg_schwarz = 1 if mg_schwarz else 0
         hist = np.zeros(max(hist_len, 1))
         st = PcgStats()
         st.hist = hist.ctypes.data_as(C.c_void_p).value if hist_len > 0 else None
@@ -337,6 +338,7 @@ class Mesh:
                      sv.get("mg_coarse_frac", 0.0))
             o.null_mean = 1 if sv.get("null_mean", False) else 0
             o.mg_fp32 = 1 if sv.get("mg_fp32", False) else 0
+            o.mg_schwarz = 1 if sv.get("mg_schwarz", False) else 0
             items[i].opts = o
             items[i].b = _dp(sv["b"]).value
             items[i].x = _dp(sv["x"]).value
@@ -350,11 +352,16 @@ class Mesh:
         o = PcgOpts(lam, tags, 3, 0, 0.0, 0.0, 0.0, 0, 1, 0, 0)
         return _mg_fill(o, mg_orders, mg_smooth, mg_coarse, mg_lmax, mg_kind, mg_coarse_frac)
 
+    def schwarz_apply(self, r, out, lam=0.0, tags=0):
+        self._check(lib().semb_schwarz_apply(self._h, C.c_double(lam), C.c_uint32(tags), _dp(r), _dp(out), _stream()))
+        return out
+
     def mg_vcycle(self, r, z, lam=0.0, tags=0, mg_orders=None, mg_smooth=0, mg_coarse=0, mg_lmax=None, mg_kind=1,
-                  mg_coarse_frac=0.0, mg_fp32=False):
+                  mg_coarse_frac=0.0, mg_fp32=False, mg_schwarz=False):
         """z = one p-multigrid V-cycle applied to r; returns the Chebyshev bounds used per level."""
         o = self._mg_opts(lam, tags, mg_orders, mg_smooth, mg_coarse, mg_lmax, mg_kind, mg_coarse_frac)
         o.mg_fp32 = 1 if mg_fp32 else 0
+        o.mg_schwarz = 1 if mg_schwarz else 0
         used = (C.c_double * 8)()
         self._check(lib().semb_mg_vcycle(self._h, C.byref(o), _dp(r), _dp(z), used, _stream()))
         nl = len(mg_orders) if mg_orders is not None else 8
