@@ -14,7 +14,12 @@
 
 #include <vector>
 
+#include "axhelm_kernels.cuh"      // ax_tile<n1>: the conflict-free shared-memory layouts of the element tile
 #include "semb_internal.h"
+
+#ifndef SEMB_SZ_LINE
+#define SEMB_SZ_LINE 1
+#endif
 
 struct semb_schwarz {             // per (level mesh, Dirichlet tag set); owned by the level mesh
     uint32_t tags = 0;
@@ -203,6 +208,132 @@ k_sz_apply(int n1, double lambda, const ST* __restrict__ Sm, const ST* __restric
     }
 }
 
+// ---- apply, production form: one thread per LINE, as in the axhelm kernel (axhelm_kernels.cuh).  Thread (a, b) of an element owns
+// the t-line (i=a, j=b, k=*), an r-line and an s-line; a line is transformed in registers by the element's own n1 x n1 matrix,
+// whose rows come from shared memory as 128-bit BROADCAST loads (every thread of the block reads the same row), and shared memory
+// otherwise only transposes the tile between the three line orientations (32-bit tiles for the FP32 levels, the swizzled
+// conflict-free layout for n1 = 8).  Passes: r, s forward; t forward, diagonal inverse, t backward in registers; s, r backward.
+template <int n1, typename ST> struct sz_cfg {
+    static constexpr int VL = 16 / (int)sizeof(ST);                       // elements per 128-bit load
+    static constexpr int RL = (n1 + VL - 1) / VL * VL;                    // padded row length
+    static constexpr int EPB = (n1 <= 3) ? 14 : (n1 == 4) ? 8 : (n1 <= 6) ? 3 : 1;
+};
+
+template <int n1, typename ST>
+__device__ __forceinline__ void sz_line(const ST* __restrict__ M, const ST (&x)[sz_cfg<n1, ST>::RL], ST (&y)[n1])
+{
+    constexpr int RL = sz_cfg<n1, ST>::RL, VL = sz_cfg<n1, ST>::VL;
+#pragma unroll
+    for (int o = 0; o < n1; ++o) {
+        ST acc = (ST)0;
+#pragma unroll
+        for (int q = 0; q < RL; q += VL) {
+            if (sizeof(ST) == 4) {
+                const float4 m4 = *reinterpret_cast<const float4*>(reinterpret_cast<const float*>(M) + o * RL + q);
+                acc += (ST)m4.x * x[q] + (ST)m4.y * x[q + 1] + (ST)m4.z * x[q + 2] + (ST)m4.w * x[q + 3];
+            } else {
+                const double2 m2 = *reinterpret_cast<const double2*>(reinterpret_cast<const double*>(M) + o * RL + q);
+                acc += (ST)m2.x * x[q] + (ST)m2.y * x[q + 1];
+            }
+        }
+        y[o] = acc;
+    }
+}
+
+template <int n1, typename ST>
+__global__ void __launch_bounds__(n1 * n1 * sz_cfg<n1, ST>::EPB)
+k_sz_line(int64_t E, double lambda, const ST* __restrict__ Sm, const ST* __restrict__ lamv, const ST* __restrict__ w, const ST* __restrict__ r,
+          ST* __restrict__ out, const semb_scalars* __restrict__ scal)
+{
+    using T = ax_tile<n1>;
+    using C = sz_cfg<n1, ST>;
+    constexpr int n2 = n1 * n1, Np = n2 * n1, RL = C::RL, EPB = C::EPB;
+    constexpr bool W32 = sizeof(ST) == 4;
+#define SZ_I(k, j, i) (W32 ? T::idx32(k, j, i) : T::idx(k, j, i))
+    __shared__ __align__(16) ST tileA[EPB * T::size];
+    __shared__ __align__(16) ST mat[EPB][3][2][n1 * RL];                  // [direction][0: S^T (forward), 1: S (backward)][row][padded column]
+    __shared__ ST lam[EPB][3][n1];
+    if (scal && *(volatile const int32_t*)&scal->done) return;
+    const int el = (EPB > 1) ? threadIdx.x / n2 : 0, tl = (EPB > 1) ? threadIdx.x - el * n2 : threadIdx.x;
+    int64_t e = blockIdx.x * (int64_t)EPB + el;
+    const bool valid = e < E;
+    if (!valid) e = E - 1;
+    ST* __restrict__ Su = tileA + el * T::size;
+    const int a = tl % n1, b = tl / n1;
+    // the element's matrices: S_d[node][mode] -> forward rows [mode][node], backward rows [node][mode], zero padded
+    for (int t = tl; t < 3 * n1 * RL; t += n2) {
+        const int d = t / (n1 * RL), row = (t / RL) % n1, col = t % RL;
+        const bool in = col < n1;
+        mat[el][d][0][row * RL + col] = in ? Sm[(e * 3 + d) * n2 + col * n1 + row] : (ST)0;
+        mat[el][d][1][row * RL + col] = in ? Sm[(e * 3 + d) * n2 + row * n1 + col] : (ST)0;
+    }
+    for (int t = tl; t < 3 * n1; t += n2) lam[el][t / n1][t % n1] = lamv[e * 3 * n1 + t];
+    ST wv[n1];
+#pragma unroll
+    for (int k = 0; k < n1; ++k) {
+        wv[k] = w[e * Np + k * n2 + tl];
+        Su[SZ_I(k, b, a)] = wv[k] * r[e * Np + k * n2 + tl];
+    }
+    __syncthreads();
+    ST x[RL], y[n1];
+#pragma unroll
+    for (int q = n1; q < RL; ++q) x[q] = (ST)0;
+    // forward r: line (i = *, j = a, k = b)
+#pragma unroll
+    for (int i = 0; i < n1; ++i) x[i] = Su[SZ_I(b, a, i)];
+    sz_line<n1, ST>(mat[el][0][0], x, y);
+#pragma unroll
+    for (int i = 0; i < n1; ++i) Su[SZ_I(b, a, i)] = y[i];
+    __syncthreads();
+    // forward s: line (i = a, j = *, k = b)
+#pragma unroll
+    for (int j = 0; j < n1; ++j) x[j] = Su[SZ_I(b, j, a)];
+    sz_line<n1, ST>(mat[el][1][0], x, y);
+#pragma unroll
+    for (int j = 0; j < n1; ++j) Su[SZ_I(b, j, a)] = y[j];
+    __syncthreads();
+    // t: forward, diagonal inverse, backward on the thread's own t-line (i = a, j = b, k = *); modes (a, b) of r and s
+#pragma unroll
+    for (int k = 0; k < n1; ++k) x[k] = Su[SZ_I(k, b, a)];
+    sz_line<n1, ST>(mat[el][2][0], x, y);
+    {
+        ST big = (ST)lambda;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { ST mx = (ST)0; for (int q = 0; q < n1; ++q) mx = fmax(mx, lam[el][d][q]); big += mx; }
+        const ST tiny = big * (ST)(W32 ? 1e-5 : 1e-12), lab = lam[el][0][a] + lam[el][1][b] + (ST)lambda;
+#pragma unroll
+        for (int c = 0; c < n1; ++c) { const ST den = lam[el][2][c] + lab; x[c] = (den > tiny) ? y[c] / den : (ST)0; }
+    }
+    sz_line<n1, ST>(mat[el][2][1], x, y);
+#pragma unroll
+    for (int k = 0; k < n1; ++k) Su[SZ_I(k, b, a)] = y[k];
+    __syncthreads();
+    // backward s
+#pragma unroll
+    for (int j = 0; j < n1; ++j) x[j] = Su[SZ_I(b, j, a)];
+    sz_line<n1, ST>(mat[el][1][1], x, y);
+#pragma unroll
+    for (int j = 0; j < n1; ++j) Su[SZ_I(b, j, a)] = y[j];
+    __syncthreads();
+    // backward r
+#pragma unroll
+    for (int i = 0; i < n1; ++i) x[i] = Su[SZ_I(b, a, i)];
+    sz_line<n1, ST>(mat[el][0][1], x, y);
+#pragma unroll
+    for (int i = 0; i < n1; ++i) Su[SZ_I(b, a, i)] = y[i];
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < n1; ++k) if (valid) out[e * Np + k * n2 + tl] = wv[k] * Su[SZ_I(k, b, a)];
+#undef SZ_I
+}
+
+template <int n1, typename ST>
+static void sz_line_launch(semb_mesh* L, double lambda, const ST* S, const ST* lam, const ST* w, const ST* v, ST* out, semb_scalars* scal, cudaStream_t s)
+{
+    constexpr int EPB = sz_cfg<n1, ST>::EPB;
+    k_sz_line<n1, ST><<<(unsigned)((L->E + EPB - 1) / EPB), n1 * n1 * EPB, 0, s>>>(L->E, lambda, S, lam, w, v, out, scal);
+}
+
 // d = c1 d + c2 sr (first: d = c2 sr);  z = z + d (zset: z = d)
 template <typename ST>
 __global__ void k_sz_update(int64_t n, double c1, double c2, const ST* __restrict__ sr, ST* __restrict__ d, ST* __restrict__ z, int first, int zset,
@@ -222,6 +353,55 @@ __global__ void k_sz_axpy(int64_t n, double a, const ST* __restrict__ x, const S
     if (scal && *(volatile const int32_t*)&scal->done) return;
     const ST k = (ST)a;
     for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) out[l] = y[l] + k * x[l];
+}
+
+// Gather form of QQ^T for a vector that is consumed once (as in pcg.cu): code -1 = no copy; <= -2: one partner at local index
+// -(code + 2); >= 3: the class was summed in place by k_gs_hi.  Four nodes per thread in lock-step keep four partner loads in flight.
+template <typename ST>
+__device__ __forceinline__ void sz_gather4(const ST* __restrict__ v, const int32_t* __restrict__ code, int64_t l0, int64_t n, int64_t stride, ST (&val)[4])
+{
+    int32_t c[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { const int64_t l = l0 + u * stride; c[u] = (l < n) ? code[l] : -1; }
+    ST own[4], pv[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { const int64_t l = l0 + u * stride; own[u] = (l < n) ? v[l] : (ST)0; pv[u] = (c[u] <= -2) ? v[-(c[u] + 2)] : (ST)0; }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) val[u] = own[u] + pv[u];
+}
+// d = c1 d + c2 QQ^T sr (first: d = c2 QQ^T sr);  z = z + d (zset: z = d)
+template <typename ST>
+__global__ void __launch_bounds__(256)
+k_sz_update_g(int64_t n, double c1, double c2, const ST* __restrict__ sr, const int32_t* __restrict__ code, ST* __restrict__ d, ST* __restrict__ z,
+              int first, int zset, const semb_scalars* __restrict__ scal)
+{
+    if (scal && *(volatile const int32_t*)&scal->done) return;
+    const ST k1 = (ST)c1, k2 = (ST)c2;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t l0 = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l0 < n; l0 += 4 * stride) {
+        ST sv[4];
+        sz_gather4<ST>(sr, code, l0, n, stride, sv);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int64_t l = l0 + u * stride;
+            if (l < n) { const ST dn = first ? k2 * sv[u] : k1 * d[l] + k2 * sv[u]; d[l] = dn; z[l] = zset ? dn : z[l] + dn; }
+        }
+    }
+}
+// out = y - QQ^T x
+template <typename ST>
+__global__ void __launch_bounds__(256)
+k_sz_resid_g(int64_t n, const ST* __restrict__ x, const int32_t* __restrict__ code, const ST* __restrict__ y, ST* __restrict__ out,
+             const semb_scalars* __restrict__ scal)
+{
+    if (scal && *(volatile const int32_t*)&scal->done) return;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t l0 = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l0 < n; l0 += 4 * stride) {
+        ST sv[4];
+        sz_gather4<ST>(x, code, l0, n, stride, sv);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { const int64_t l = l0 + u * stride; if (l < n) out[l] = y[l] - sv[u]; }
+    }
 }
 
 static unsigned sz_grid(int64_t n) { int64_t b = (n + 1023) / 1024, cap = (int64_t)semb_sm_count() * 8; return (unsigned)(b < 1 ? 1 : (b > cap ? cap : b)); }
@@ -300,19 +480,40 @@ static inline int sz_gs(semb_mesh* L, double* v, cudaStream_t s) { return semb_g
 static inline int sz_gs(semb_mesh* L, float* v, cudaStream_t s) { return semb_gs_launch_f(L, v, s); }
 static inline int sz_mask(semb_mesh* L, const semb_mask_entry& m, double* v, cudaStream_t s) { return semb_mask_launch(L, m, v, 1, s); }
 static inline int sz_mask(semb_mesh* L, const semb_mask_entry& m, float* v, cudaStream_t s) { return semb_mask_launch_f(L, m, v, s); }
+static inline int sz_gs_hi(semb_mesh* L, double* v, semb_scalars* scal, cudaStream_t s) { return semb_gs_hi_launch(L, v, scal, s); }
+static inline int sz_gs_hi(semb_mesh* L, float* v, semb_scalars* scal, cudaStream_t s) { return semb_gs_hi_launch_f(L, v, scal, s); }
 static inline int sz_axhelm(semb_mesh* L, double lambda, const double*, const double* u, double* w, semb_scalars* scal, cudaStream_t s)
 { (void)scal; return semb_axhelm_launch(L, lambda, nullptr, nullptr, u, w, 1, nullptr, s); }
 static inline int sz_axhelm(semb_mesh* L, double lambda, const float* geo, const float* u, float* w, semb_scalars* scal, cudaStream_t s)
 { return semb_axhelm_launch_f(L, lambda, geo, u, w, scal, s); }
 
-// out = S v = M QQ^T [w o A~^-1 (w o v)]
+// out = S v = M QQ^T [w o A~^-1 (w o v)];  local_only: stop before QQ^T (the consumer applies it in gather form after k_gs_hi)
 template <typename ST>
-static int sz_apply(semb_mesh* L, const semb_schwarz* z, double lambda, const semb_mask_entry& m, const ST* v, ST* out, semb_scalars* scal, cudaStream_t s)
+static int sz_apply(semb_mesh* L, const semb_schwarz* z, double lambda, const semb_mask_entry& m, const ST* v, ST* out, semb_scalars* scal, cudaStream_t s,
+                    bool local_only = false)
 {
     const int n1 = L->n1;
-    const size_t smem = sizeof(ST) * (2 * (size_t)L->Np + 3 * n1 * n1 + 3 * n1);
-    k_sz_apply<ST><<<(unsigned)L->E, 128, smem, s>>>(n1, lambda, sz_S(z, ST()), sz_lam(z, ST()), sz_w(z, ST()), v, out, scal);
+    const ST *S = sz_S(z, ST()), *lm = sz_lam(z, ST()), *w = sz_w(z, ST());
+    switch (SEMB_SZ_LINE ? n1 : 0) {
+        case 3:  sz_line_launch<3, ST>(L, lambda, S, lm, w, v, out, scal, s); break;
+        case 4:  sz_line_launch<4, ST>(L, lambda, S, lm, w, v, out, scal, s); break;
+        case 5:  sz_line_launch<5, ST>(L, lambda, S, lm, w, v, out, scal, s); break;
+        case 6:  sz_line_launch<6, ST>(L, lambda, S, lm, w, v, out, scal, s); break;
+        case 7:  sz_line_launch<7, ST>(L, lambda, S, lm, w, v, out, scal, s); break;
+        case 8:  sz_line_launch<8, ST>(L, lambda, S, lm, w, v, out, scal, s); break;
+        case 9:  sz_line_launch<9, ST>(L, lambda, S, lm, w, v, out, scal, s); break;
+        case 10: sz_line_launch<10, ST>(L, lambda, S, lm, w, v, out, scal, s); break;
+        case 11: sz_line_launch<11, ST>(L, lambda, S, lm, w, v, out, scal, s); break;
+        default: {                       // the plain six-pass kernel (run-time order; kept as the A/B reference: -DSEMB_SZ_LINE=0)
+            const size_t smem = sizeof(ST) * (2 * (size_t)L->Np + 3 * n1 * n1 + 3 * n1);
+            k_sz_apply<ST><<<(unsigned)L->E, 128, smem, s>>>(n1, lambda, S, lm, w, v, out, scal);
+        }
+    }
     L->launches += 1;
+    if (local_only) {
+        int rc = sz_mask(L, m, out, s); if (rc) return rc;
+        return sz_gs_hi(L, out, scal, s);
+    }
     int rc = sz_gs(L, out, s); if (rc) return rc;
     return sz_mask(L, m, out, s);
 }
@@ -323,17 +524,19 @@ static int sz_cheb4(semb_mesh* L, const semb_schwarz* zd, double lambda, const S
                     const ST* r, ST* z, ST* res, ST* d, ST* sr, ST* t, semb_scalars* scal, cudaStream_t s, bool zacc)
 {
     const int64_t n = L->n;
-    int rc = sz_apply<ST>(L, zd, lambda, m, r, sr, scal, s); if (rc) return rc;
-    k_sz_update<ST><<<sz_grid(n), 256, 0, s>>>(n, 0.0, 4.0 / (3.0 * lmax), sr, d, z, 1, zacc ? 0 : 1, scal);
+    // every assembled vector of the recurrence is consumed exactly once, so QQ^T is applied in gather form by the consumer
+    // (k_gs_hi for the edge / corner classes, the face partner inside the streaming kernel) instead of a read-modify-write pass
+    int rc = sz_apply<ST>(L, zd, lambda, m, r, sr, scal, s, true); if (rc) return rc;
+    k_sz_update_g<ST><<<sz_grid(n), 256, 0, s>>>(n, 0.0, 4.0 / (3.0 * lmax), sr, L->gs_code, d, z, 1, zacc ? 0 : 1, scal);
     const ST* rin = r;
     for (int i = 1; i <= k; ++i) {
-        rc = sz_axhelm(L, lambda, geo, d, t, scal, s); if (rc) return rc;             // t = A d
+        rc = sz_axhelm(L, lambda, geo, d, t, scal, s); if (rc) return rc;             // t = A_L d
         rc = sz_mask(L, m, t, s); if (rc) return rc;
-        rc = sz_gs(L, t, s); if (rc) return rc;
-        k_sz_axpy<ST><<<sz_grid(n), 256, 0, s>>>(n, -1.0, t, rin, res, scal);         // res = res - A d
+        rc = sz_gs_hi(L, t, scal, s); if (rc) return rc;
+        k_sz_resid_g<ST><<<sz_grid(n), 256, 0, s>>>(n, t, L->gs_code, rin, res, scal);  // res = res - QQ^T A_L d
         rin = res;
-        rc = sz_apply<ST>(L, zd, lambda, m, res, sr, scal, s); if (rc) return rc;
-        k_sz_update<ST><<<sz_grid(n), 256, 0, s>>>(n, (2.0 * i - 1.0) / (2.0 * i + 3.0), (8.0 * i + 4.0) / ((2.0 * i + 3.0) * lmax), sr, d, z, 0, 0, scal);
+        rc = sz_apply<ST>(L, zd, lambda, m, res, sr, scal, s, true); if (rc) return rc;
+        k_sz_update_g<ST><<<sz_grid(n), 256, 0, s>>>(n, (2.0 * i - 1.0) / (2.0 * i + 3.0), (8.0 * i + 4.0) / ((2.0 * i + 3.0) * lmax), sr, L->gs_code, d, z, 0, 0, scal);
         L->launches += 2;
     }
     L->launches += 1;
