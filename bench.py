@@ -426,7 +426,7 @@ def geometry_section_affine(torch, semb, out, u, w, sweep, peak):
 def boussinesq_section(torch, semb, G, m, nsteps):
     """configs[4] as a REAL time step (Eqs. (1)-(3)): no-slip walls, isothermal plates T(z=0) = 1,
     T(z=1) = 0, adiabatic side wall, started from the conduction state plus a seeded perturbation of theta,
-    dt = 5e-4 (configs[4]), Ra = 1e8, Pr = 0.7; pressure by p-multigrid PCG on FP32 levels, Helmholtz solves by Jacobi-PCG."""
+    dt = 5e-4 (configs[4]), Ra = 1e8, Pr = 0.7; pressure by p-multigrid PCG on FP32 levels with Chebyshev-Schwarz smoothing, Helmholtz solves by Jacobi-PCG."""
     n = m.n
     st = semb.FlowState(n)
     th0 = torch.from_numpy(0.05 * I.uniform(I.seed_for(4, 7), n) * np.sin(np.pi * m.z)).cuda()
@@ -439,7 +439,7 @@ def boussinesq_section(torch, semb, G, m, nsteps):
     for s in range(nsteps):
         t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         torch.cuda.synchronize(); t0.record()
-        rc, it = G.boussinesq_step(st, 1e8, 0.7, 5e-4, 0b110, 0b10, rtol=1e-10, mg_fp32=True)
+        rc, it = G.boussinesq_step(st, 1e8, 0.7, 5e-4, 0b110, 0b10, rtol=1e-10, mg_fp32=True, mg_schwarz=True)
         t1.record(); torch.cuda.synchronize()
         secs.append(t0.elapsed_time(t1) * 1e-3); its.append(it)
     umax = max(float(c.abs().max()) for c in st.u)
@@ -468,14 +468,15 @@ def config_section(torch, semb, name, peak, args):
         sec["chebyshev2_jacobi_pcg_iteration_ms"] = iteration_numbers(torch, G, m, b, 20, 3, peak, precond=2, cheb_degree=2)["ms"]
     steps = None
     if not args.no_solve:
-        variants = [("pmg_fp32_pcg", dict(precond=3, mg_fp32=True))]
+        variants = [("pmg_fp32_pcg", dict(precond=3, mg_fp32=True)),
+                    ("pmg_fp32_schwarz_pcg", dict(precond=3, mg_fp32=True, mg_schwarz=True, mg_smooth=1, mg_kind=4))]
         if args.full_solves:
             variants += [("pmg_pcg", dict(precond=3)), ("jacobi_pcg", dict(precond=1))]
         sec["time_to_solution"] = time_to_solution(torch, G, b, variants, args.solve_maxit)
         if cfg == 4 and args.cfg4_steps > 0:
-            sv = [("pmg_fp32_pcg_all_solves", dict(precond=3, mg_fp32=True))]
+            sv = [("pmg_fp32_schwarz_pcg_all_solves", dict(precond=3, mg_fp32=True, mg_schwarz=True, mg_smooth=1, mg_kind=4))]
             if args.full_solves:
-                sv.append(("jacobi_pcg_all_solves", dict(precond=1)))
+                sv += [("pmg_fp32_pcg_all_solves", dict(precond=3, mg_fp32=True)), ("jacobi_pcg_all_solves", dict(precond=1))]
             steps = ten_steps(torch, G, m, args.cfg4_steps, sv)
             sec["boussinesq_steps"] = boussinesq_section(torch, semb, G, m, 3)
     del b
@@ -730,9 +731,9 @@ def main():
     # ---- configs[4] ten-step recipe when cfg4 IS the workload (otherwise inside the configs section below)
     steps10 = None
     if args.workload.startswith("cfg4") and not args.no_solve and single and args.cfg4_steps > 0:
-        sv = [("pmg_fp32_pcg_all_solves", dict(precond=3, mg_fp32=True))]
+        sv = [("pmg_fp32_schwarz_pcg_all_solves", dict(precond=3, mg_fp32=True, mg_schwarz=True, mg_smooth=1, mg_kind=4))]
         if args.full_solves:
-            sv.append(("jacobi_pcg_all_solves", dict(precond=1)))
+            sv += [("pmg_fp32_pcg_all_solves", dict(precond=3, mg_fp32=True)), ("jacobi_pcg_all_solves", dict(precond=1))]
         steps10 = ten_steps(torch, G, m, args.cfg4_steps, sv)
 
     launches = st["launches"]

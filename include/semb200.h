@@ -361,6 +361,7 @@ typedef struct {
     double   rtol;                /* of every solve; <= 0 => 1e-10 */
     int32_t  precond_p, precond_u;/* semb_pcg_opts.precond of the pressure solve (0 => 3, p-multigrid) and of the Helmholtz solves (0 => 1, Jacobi) */
     int32_t  mg_fp32, maxit;      /* maxit <= 0 => 20000 */
+    int32_t  mg_schwarz, pad_;    /* 1: the p-multigrid solves smooth with the Chebyshev-Schwarz smoother (semb_pcg_opts.mg_schwarz) */
     const double* forcing[4];     /* optional body forces f_x, f_y, f_z, f_theta at time level n, device [n] each, or NULL */
 } semb_flow_opts;
 

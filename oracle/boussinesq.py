@@ -18,6 +18,9 @@ the oracle's primitives (semflow.c: grad, wdiv; semoracle.c: gs, mask, PCG), in 
     (iii) u^_c    = u~_c - dt dp/dx_c (collocation);   (A + beta0/(nu dt) B) u_c^(n+1) = M QQ^T (B u^_c) / (nu dt),  start u_c^n
           theta~  = sum_k b_k theta^(n+1-k) + dt sum_k a_k N_theta^(n+1-k)
           (A + beta0/(kappa dt) B) theta^(n+1) = M QQ^T (B theta~) / (kappa dt),  start theta^n
+
+Pins (tests/test_oracle_flow.py): the conduction state is a fixed point; second order in time on a manufactured solution whose
+forcing sympy derives from Eqs. (1)-(3).  Parity unpinned: none.
 """
 import ctypes as C
 

@@ -20,6 +20,9 @@ exactly the assembled operator restricted to the element's nodes (the pin).
 Smoother:  S r = M QQ^T [ w o A~_e^-1 ( w o r ) ],  w = sqrt(1 / multiplicity)  -- symmetric positive semi-definite.
 A~_e^-1 = (S_t x S_s x S_r) [Lam_r (+) Lam_s (+) Lam_t + lambda]^-1 (S_t x S_s x S_r)^T with A_d S_d = B_d S_d Lam_d,
 S_d^T B_d S_d = I (numpy.linalg.eigh on B^-1/2 A B^-1/2: a library primitive as one step).
+
+Pins (tests/test_oracle_schwarz.py): exact restricted inverse on tensor boxes, dense symmetric positive S, closed-form fourth-kind
+polynomial in S A, Lanczos bound.  Parity unpinned: none.
 """
 import numpy as np
 

@@ -5,6 +5,8 @@
  * DESIGN.md reading R25 and is assembled from these pieces in oracle/boussinesq.py.
  *
  * TEST INFRASTRUCTURE ONLY.  Plain C, fp64, the definitions written out; shares no code with csrc/.
+ * Pins (tests/test_oracle_flow.py): closed-form metrics of a sheared affine mesh, exact gradients of polynomials, analytic integrals for
+ * the weak divergence, grad(linear) exact on curved meshes, wdiv = grad^T, QQ^T wdiv o grad = A.  Parity unpinned: none.
  *
  *   metrics   J = d(x,y,z)/d(r,s,t) by applying D to the coordinates (as c-3); met[e][9][Np] = dr_a/dx_b,
  *             a = r,s,t (rows), b = x,y,z: the inverse of J, entry (a,b) at index 3a + b.

@@ -4,6 +4,8 @@
  * isocontour.  4096 pixels were used ... for the longest side", 2048 for the shorter one).
  *
  * TEST INFRASTRUCTURE ONLY: used by tests/, __graft_entry__.smoke() and bench.py's cpu_baseline leg.  Plain C, fp64, loops in
+ * Pins (tests/test_oracle_image.py): colour ramps in closed form; the claiming sub-cell against a numpy search of the node planes and
+ * the value of a linear field; the disc footprint of the cylinder; iso-plane exact, iso-sphere to second order.  Parity unpinned: none.
  * the order the definitions below state; shares no code with the CUDA path (csrc/image.cu).
  *
  * The paper renders with ASCENT / VTK-m, which see the spectral-element field as an unstructured mesh of hexahedral

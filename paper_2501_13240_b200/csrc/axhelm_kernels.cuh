@@ -237,7 +237,8 @@ __device__ __forceinline__ void ax_prefetch_l2(const ST* ptr, int count)
 // N = 1 level of the multigrid ran at 1 TB/s): thread group el = tl / n1^2 works on element
 // blockIdx.x * EPB + el with its own shared-memory tiles; groups past the end recompute the last element and write nothing.
 // ST: STORAGE type of the vectors and geometric factors in global memory (double, or float for the multigrid levels:
-// PAPER.md:L102 runs the preconditioner in FP32 "to save on memory bandwidth"); the arithmetic is fp64 either way.
+// PAPER.md:L102 runs the preconditioner in FP32 "to save on memory bandwidth"); float storage computes in float with 32-bit tiles,
+// double storage in fp64 (R21).
 template <int n1, int MODE, int MINB, int EPB, typename ST, int GEO>
 __global__ void __launch_bounds__(n1 * n1 * EPB, MINB)
 k_axhelm_line(int64_t E, int64_t n, const void* __restrict__ geo_v, double lambda,

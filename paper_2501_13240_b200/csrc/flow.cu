@@ -363,7 +363,7 @@ extern "C" int semb_boussinesq_step(semb_handle h, const semb_flow_opts* o, semb
     h->launches += 5;
     semb_pcg_opts po{};
     po.lambda = 0.0; po.dirichlet_tags = 0; po.precond = o->precond_p ? o->precond_p : 3; po.cheb_degree = 2; po.rtol = o->rtol > 0.0 ? o->rtol : 1e-10;
-    po.maxit = o->maxit > 0 ? o->maxit : 20000; po.x0_is_zero = 1; po.null_mean = 1; po.mg_fp32 = o->mg_fp32;
+    po.maxit = o->maxit > 0 ? o->maxit : 20000; po.x0_is_zero = 1; po.null_mean = 1; po.mg_fp32 = o->mg_fp32; po.mg_schwarz = o->mg_schwarz; po.mg_smoother_kind = o->mg_schwarz ? 4 : 1;
     semb_pcg_stats ps{};
     rc = semb_pcg_run(h, &po, bp, st->p, &ps, s);
     if (stats) { stats->iters[0] = ps.iters; stats->status[0] = rc; }
@@ -375,7 +375,7 @@ extern "C" int semb_boussinesq_step(semb_handle h, const semb_flow_opts* o, semb
     rc = semb_get_mask(h, o->tags_u, &mu, s); if (rc) return rc;
     rc = semb_get_mask(h, o->tags_T, &mt, s); if (rc) return rc;
     semb_pcg_opts ho{};
-    ho.precond = o->precond_u ? o->precond_u : 1; ho.cheb_degree = 2; ho.rtol = po.rtol; ho.maxit = po.maxit; ho.x0_is_zero = 0; ho.mg_fp32 = o->mg_fp32;
+    ho.precond = o->precond_u ? o->precond_u : 1; ho.cheb_degree = 2; ho.rtol = po.rtol; ho.maxit = po.maxit; ho.x0_is_zero = 0; ho.mg_fp32 = o->mg_fp32; ho.mg_schwarz = o->mg_schwarz; ho.mg_smoother_kind = o->mg_schwarz ? 4 : 1;
     for (int c = 0; c < 3; ++c) {
         k_flow_rhs<<<flow_grid(n), 256, 0, s>>>(n, h->Np, h->geo, dt, nu, ut + c * n, gp + c * n, rhs);
         rc = semb_gs_launch(h, rhs, 1, s); if (rc) return rc;

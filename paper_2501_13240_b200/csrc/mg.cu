@@ -387,7 +387,8 @@ int semb_mg_vcycle_run(semb_mesh* h, const semb_mg_ctx& ctx, int l, const double
 
 
 // ---- fp32-storage levels (the preconditioner runs in FP32 "to save on memory bandwidth").  Vectors and
-// geometric factors of every level live in float, every kernel computes in fp64 registers and rounds at its stores.
+// geometric factors of every level live in float and every level kernel computes in float as well (R21; only the class sums of
+// the gather-scatter accumulate in fp64).
 template <typename TI, typename TO>
 __global__ void k_mg_convert(int64_t n, const TI* __restrict__ in, TO* __restrict__ out, const semb_scalars* __restrict__ scal)
 {

@@ -357,7 +357,7 @@ int semb_residual_launch(semb_mesh* h, double lambda, const semb_mask_entry& m, 
     return SEMB_OK;
 }
 
-// ---- fp32-storage variants for the multigrid levels (mg.cu): same kernels, float vectors, fp64 arithmetic
+// ---- fp32-storage variants for the multigrid levels (mg.cu): same kernels, float vectors, float arithmetic (R21)
 int semb_residual_launch_f(semb_mesh* h, double lambda, const float* geo, const semb_mask_entry& m, const float* z, const float* r,
                            float* res, float* tmp, semb_scalars* scal, cudaStream_t s)
 {

@@ -112,7 +112,7 @@ class FieldDesc(C.Structure):
 class FlowOpts(C.Structure):
     _fields_ = [("Ra", C.c_double), ("Pr", C.c_double), ("dt", C.c_double), ("tags_u", C.c_uint32), ("tags_T", C.c_uint32),
                 ("rtol", C.c_double), ("precond_p", C.c_int32), ("precond_u", C.c_int32), ("mg_fp32", C.c_int32), ("maxit", C.c_int32),
-                ("forcing", C.c_void_p * 4)]
+                ("mg_schwarz", C.c_int32), ("pad_", C.c_int32), ("forcing", C.c_void_p * 4)]
 
 
 class FlowStateC(C.Structure):
@@ -421,9 +421,10 @@ class Mesh:
         f = (C.c_void_p * 4)(*[(t.data_ptr() if t is not None else None) for t in (forcing or [None] * 4)])
         self._check(lib().semb_flow_explicit_terms(self._h, _dp(ux), _dp(uy), _dp(uz), _dp(theta), f if forcing else None, _dp(N4), _dp(omega3), _stream()))
 
-    def boussinesq_step(self, state, Ra, Pr, dt, tags_u, tags_T, rtol=1e-10, precond_p=3, precond_u=1, mg_fp32=False, maxit=0, forcing=None):
+    def boussinesq_step(self, state, Ra, Pr, dt, tags_u, tags_T, rtol=1e-10, precond_p=3, precond_u=1, mg_fp32=False, maxit=0, forcing=None,
+                        mg_schwarz=False):
         """one time step on `state` (FlowState); returns (status, iterations of the pressure, u_x, u_y, u_z, theta solves)"""
-        o = FlowOpts(Ra, Pr, dt, tags_u, tags_T, rtol, precond_p, precond_u, 1 if mg_fp32 else 0, maxit)
+        o = FlowOpts(Ra, Pr, dt, tags_u, tags_T, rtol, precond_p, precond_u, 1 if mg_fp32 else 0, maxit, 1 if mg_schwarz else 0, 0)
         for i, t in enumerate(forcing or []):
             o.forcing[i] = t.data_ptr() if t is not None else None
         st = FlowStats()
