@@ -656,7 +656,8 @@ def main():
         variants = [("pmg_pcg", dict(precond=3, mg_smooth=1, mg_coarse=64, mg_coarse_frac=0.003)),
                     ("pmg_fp32_pcg", dict(precond=3, mg_smooth=1, mg_coarse=64, mg_coarse_frac=0.003, mg_fp32=True))]
         if isinstance(ne, tuple):
-            variants = [("pmg_pcg", dict(precond=3)), ("pmg_fp32_pcg", dict(precond=3, mg_fp32=True))]
+            variants = [("pmg_pcg", dict(precond=3)), ("pmg_fp32_pcg", dict(precond=3, mg_fp32=True)),
+                        ("pmg_fp32_schwarz_pcg", dict(precond=3, mg_fp32=True, mg_schwarz=True, mg_smooth=1, mg_kind=4))]
         if args.full_solves:                  # ~4200 iterations, 14 s on cfg3: not in the default run
             variants.append(("jacobi_pcg", dict(precond=1)))
         solve_tts = time_to_solution(torch, G, b, variants, args.solve_maxit)
@@ -735,6 +736,9 @@ def main():
         if args.full_solves:
             sv += [("pmg_fp32_pcg_all_solves", dict(precond=3, mg_fp32=True)), ("jacobi_pcg_all_solves", dict(precond=1))]
         steps10 = ten_steps(torch, G, m, args.cfg4_steps, sv)
+    bq_main = None
+    if args.workload.startswith("cfg4") and not args.no_solve and single:
+        bq_main = boussinesq_section(torch, semb, G, m, 3)
 
     launches = st["launches"]
     del b, x
@@ -788,6 +792,7 @@ def main():
         "geometry_modes": geo_modes,
         "configs": configs,
         "cfg4_ten_steps": steps10,
+        "boussinesq_steps": bq_main if bq_main is not None else (configs or {}).get("cfg4_ogrid_N9", {}).get("boussinesq_steps"),
         "e2e": e2e, "e2e_single": e2e_single, "gpu_launches": launches, "clocks": clocks,
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
