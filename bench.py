@@ -54,7 +54,7 @@ WORKLOADS = {            # name -> elements per direction of the deformed box (B
     "cfg4_ogrid_N9": ("ogrid", 4),
 }
 TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r2_traffic.json")
-KERNEL_SOURCES = ["axhelm_kernels.cuh", "axhelm.cu", "reduce.cuh"]     # what the dominant kernel is compiled from
+KERNEL_SOURCES = ["axhelm_kernels.cuh", "axhelm_launch.cuh", "axhelm.cu", "reduce.cuh"]     # what the dominant kernel is compiled from
 
 
 def metric_name(N):
@@ -105,7 +105,7 @@ def recorded_traffic(workload):
 
 def record_traffic(args):
     """`bench.py --record-traffic RAW.csv --workload W`: read `ncu -i X.ncu-rep --page raw --csv` output, take the launches
-    of the PCG-fused axhelm kernel (k_axhelm_line<..,4|5,..>), and write their mean dram bytes into profiles/r2_traffic.json
+    of the PCG-fused axhelm kernel (k_axhelm_line<..,4|5,..>), and write their median dram bytes into profiles/r2_traffic.json
     together with the hash of the kernel sources and the commit they were captured at."""
     import csv
     with open(args.record_traffic, newline="") as f:
@@ -133,8 +133,8 @@ def record_traffic(args):
         rec = {"what": "dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, ncu --set full; "
                        "written by `python bench.py --record-traffic <raw csv> --workload <W>`", "entries": {}}
     commit = subprocess.run(["git", "rev-parse", "--short", "HEAD"], cwd=ROOT, capture_output=True, text=True).stdout.strip()
-    rec["entries"][args.workload] = {"kernel": kname, "launches_captured": len(tot), "dram_bytes_per_launch": float(np.mean(tot)),
-                                     "duration_ns_under_ncu": float(np.mean(ns)), "kernel_sources": KERNEL_SOURCES,
+    rec["entries"][args.workload] = {"kernel": kname, "launches_captured": len(tot), "dram_bytes_per_launch": float(np.median(tot)),
+                                     "duration_ns_under_ncu": float(np.median(ns)), "kernel_sources": KERNEL_SOURCES,
                                      "kernel_sources_sha256": kernel_source_hash(), "commit": commit or "unknown",
                                      "command": args.traffic_command}
     with open(TRAFFIC_JSON, "w") as f:

@@ -18,6 +18,16 @@ int semb_axhelm_upload_basis(semb_mesh* h)
     return rc;
 }
 
+int64_t semb_axhelm_dot_count(semb_mesh* h)
+{
+    switch (h->n1) {
+        case 2: return ax_dot_count_of<2>(h);  case 3: return ax_dot_count_of<3>(h);  case 4: return ax_dot_count_of<4>(h);
+        case 5: return ax_dot_count_of<5>(h);  case 6: return ax_dot_count_of<6>(h);  case 7: return ax_dot_count_of<7>(h);
+        case 8: return ax_dot_count_of<8>(h);  case 9: return ax_dot_count_of<9>(h);  case 10: return ax_dot_count_of<10>(h);
+        default: return ax_dot_count_of<11>(h);
+    }
+}
+
 int semb_axhelm_prepare_geo(semb_mesh* h, cudaStream_t) { h->geoK = h->geo; return SEMB_OK; }
 
 // every fp64 application on the handle's own geometry goes through here: the representation semb_set_geometry_mode selected

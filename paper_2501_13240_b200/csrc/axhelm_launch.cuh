@@ -113,7 +113,7 @@ static int launch_line(semb_mesh* h, const void* geo, int mode, double lambda, c
     }
 #undef SEMB_AX_LAUNCH
     h->launches += 1;
-    if (dot) {
+    if (dot && !h->defer_dot_finish) {
         // p.Ap = sum of the per-element partials, alpha = rho / p.Ap (fixed order: bit-reproducible)
         int64_t blocks = ((int64_t)grid + 2047) / 2048;
         if (blocks > 128) blocks = 128;
@@ -123,6 +123,8 @@ static int launch_line(semb_mesh* h, const void* geo, int mode, double lambda, c
     SEMB_CUDA(h, cudaGetLastError());
     return SEMB_OK;
 }
+
+template <int n1> static int64_t ax_dot_count_of(semb_mesh* h) { return (h->E + ax_epb<n1>::v - 1) / ax_epb<n1>::v; }
 
 template <typename ST, int GEO>
 static int axhelm_dispatch(semb_mesh* h, const void* geo, int mode, double lambda, const double* lam0, const double* lam1,

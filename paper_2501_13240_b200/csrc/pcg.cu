@@ -9,6 +9,8 @@
 #include <math.h>
 #include <string.h>
 
+#include <cooperative_groups.h>
+
 #include "reduce.cuh"
 #include "semb_internal.h"
 
@@ -161,6 +163,86 @@ k_update_r(int64_t n, const double* __restrict__ q, double* __restrict__ r, gs_l
         if (hist && it < hist_cap) hist[it] = scal->rnorm;
         scal->rho_old = scal->rho_new;
         if (FUSED_Z) { scal->rho_new = tot[1]; scal->rz = tot[1]; scal->beta = tot[1] / scal->rho_old; }
+        if (scal->rnorm <= scal->target) { scal->done = 1; scal->status = SEMB_OK; }
+        else if (it >= scal->maxit) { scal->done = 1; scal->status = SEMB_MAXIT; }
+    }
+}
+
+// Small meshes (n <= SEMB_SMALL_N nodes): an iteration of the loop above is five dependent launches of a few microseconds each
+// and nothing else (configs[0]: 30 us per iteration for 32 768 nodes, all of it launch latency).  ONE launch does everything that
+// follows the operator (a cluster of 8 blocks, hardware cluster barriers between the phases): p.Ap from the per-block partials and alpha; the Dirichlet mask; the class sums of the edge / corner nodes;
+// r -= alpha QQ^T q with the face partner gathered; <r,r>, <r,z>; beta and the stop test.  Block-wide barriers replace four kernel
+// boundaries; every sum has a fixed order, so the iterates are reproducible run to run.
+#define SEMB_SMALL_N 65536
+#define SMALL_BLOCK 1024
+#define SMALL_CL 8              // blocks of the thread-block cluster that shares the work (hardware cluster barrier between the phases)
+template <bool FUSED_Z>
+__global__ void __cluster_dims__(SMALL_CL, 1, 1) __launch_bounds__(SMALL_BLOCK)
+k_iter_small(int64_t n, int64_t ndot, const double* __restrict__ ax_dot, int64_t nmask, const int32_t* __restrict__ masklist,
+             int64_t n_hi, const int32_t* __restrict__ hi, const int32_t* __restrict__ off, const int32_t* __restrict__ ids,
+             double* q, double* __restrict__ r, const int32_t* __restrict__ code, const double* __restrict__ dinv,
+             semb_scalars* __restrict__ scal, double* __restrict__ partials, double* __restrict__ hist, int hist_cap)
+{
+    __shared__ double red[32];
+    namespace cg = cooperative_groups;
+    cg::cluster_group cl = cg::this_cluster();
+    if (STOPPED(scal)) return;                                     // uniform over the cluster: written only at the end of an iteration
+    const int64_t tid = blockIdx.x * (int64_t)SMALL_BLOCK + threadIdx.x, nthr = (int64_t)SMALL_CL * SMALL_BLOCK;
+    double s = 0.0;
+    for (int64_t t = threadIdx.x; t < ndot; t += SMALL_BLOCK) s += ax_dot[t];       // every block sums all partials: same order, same bits
+    const double pAp = block_sum(s, red);
+    if (!(pAp > 0.0) || !isfinite(pAp)) {
+        if (tid == 0) { scal->pAp = pAp; scal->status = SEMB_EBREAKDOWN; scal->done = 1; scal->x_pending = 0; }
+        return;
+    }
+    const double alpha = scal->rho_new / pAp;
+    for (int64_t t = tid; t < nmask; t += nthr) q[masklist[t]] = 0.0;
+    cl.sync();
+    for (int64_t t = tid; t < n_hi; t += nthr) {
+        const int32_t g = hi[t], a = off[g], b = off[g + 1];
+        double c = 0.0;
+        for (int32_t u = a; u < b; ++u) c += q[ids[u]];
+        for (int32_t u = a; u < b; ++u) q[ids[u]] = c;
+    }
+    cl.sync();
+    double rr = 0.0, rz = 0.0;
+    for (int64_t l0 = tid; l0 < n; l0 += 4 * nthr) {               // four independent nodes per pass: two exposed latencies
+        int32_t c[4]; double own[4], rv[4], dv[4], pv[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { const int64_t l = l0 + u * nthr; c[u] = (l < n) ? code[l] : -1; }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int64_t l = l0 + u * nthr;
+            own[u] = (l < n) ? q[l] : 0.0; rv[u] = (l < n) ? r[l] : 0.0; dv[u] = (FUSED_Z && dinv && l < n) ? dinv[l] : 1.0;
+            pv[u] = (c[u] <= -2) ? q[-(c[u] + 2)] : 0.0;
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int64_t l = l0 + u * nthr;
+            if (l < n) {
+                const double w = (c[u] <= -2) ? 0.5 : (c[u] >= 3) ? 1.0 / (double)c[u] : 1.0;
+                const double rl = rv[u] - alpha * (own[u] + pv[u]);
+                r[l] = rl;
+                const double t = rl * rl * w;
+                rr += t;
+                if (FUSED_Z) rz += dv[u] * t;
+            }
+        }
+    }
+    rr = block_sum(rr, red);
+    rz = block_sum(rz, red);
+    if (threadIdx.x == 0) { partials[blockIdx.x] = rr; partials[SEMB_MAX_BLOCKS + blockIdx.x] = rz; }
+    cl.sync();
+    if (tid == 0) {
+        double trr = 0.0, trz = 0.0;
+        for (int bq = 0; bq < SMALL_CL; ++bq) { trr += partials[bq]; trz += partials[SEMB_MAX_BLOCKS + bq]; }
+        scal->pAp = pAp; scal->alpha = alpha; scal->x_pending = 1;
+        const int it = scal->iter + 1;
+        scal->iter = it;
+        scal->rr = trr; scal->rnorm = sqrt(trr);
+        if (hist && it < hist_cap) hist[it] = scal->rnorm;
+        scal->rho_old = scal->rho_new;
+        if (FUSED_Z) { scal->rho_new = trz; scal->rz = trz; scal->beta = trz / scal->rho_old; }
         if (scal->rnorm <= scal->target) { scal->done = 1; scal->status = SEMB_OK; }
         else if (it >= scal->maxit) { scal->done = 1; scal->status = SEMB_MAXIT; }
     }
@@ -620,6 +702,9 @@ int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* 
     }
     const int check = o->check_every > 0 ? o->check_every : 16;
     bool finished = (o->maxit == 0);
+    // small meshes: two launches per iteration instead of five (k_iter_small)
+    const bool small = n <= SEMB_SMALL_N && o->precond <= 1 && !o->profile;
+    const int64_t ndot = small ? semb_axhelm_dot_count(h) : 0;
     for (int it0 = 0; it0 < o->maxit && !finished; it0 += check) {
         const int mbatch = (o->maxit - it0 < check) ? o->maxit - it0 : check;
         for (int i = 0; i < mbatch; ++i) {
@@ -634,8 +719,17 @@ int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* 
             }
             const int itn = it0 + i;
             if (itn < nprof) SEMB_CUDA(h, cudaEventRecord(h->prof_ev[2 * itn], s));
-            rc = semb_axhelm_pcg_launch(h, o->lambda, zsrc, dz, p, x, q, h->scal, s); if (rc) return rc;
+            h->defer_dot_finish = small;
+            rc = semb_axhelm_pcg_launch(h, o->lambda, zsrc, dz, p, x, q, h->scal, s);
+            h->defer_dot_finish = false;
+            if (rc) return rc;
             if (itn < nprof) SEMB_CUDA(h, cudaEventRecord(h->prof_ev[2 * itn + 1], s));
+            if (small) {
+                k_iter_small<true><<<SMALL_CL, SMALL_BLOCK, 0, s>>>(n, ndot, h->ax_dot, m.count, m.list, h->n_gs_hi, h->gs_hi, h->gs_off, h->gs_ids,
+                                                                    q, r, h->gs_code, dz, h->scal, h->partials, hist, want_hist);     // dz == NULL: z = r
+                h->launches += 1;
+                continue;
+            }
             rc = semb_mask_launch(h, m, q, 1, s); if (rc) return rc;     // every copy of a Dirichlet node is masked => sum 0
             rc = semb_gs_hi_launch(h, q, h->scal, s); if (rc) return rc; // edges and corners; faces in k_update_r
             const gs_lists L{h->gs_code};

@@ -81,6 +81,7 @@ struct semb_mesh {
     double* work = nullptr; int64_t work_vecs = 0;
     double* partials = nullptr;         // block partial sums [4][SEMB_MAX_BLOCKS]
     double* ax_dot = nullptr;           // per-element partials of p.Ap written by axhelm [E]
+    bool defer_dot_finish = false;      // small-mesh PCG: the partials are summed by k_iter_small, not by k_ax_dot_finish
     semb_scalars* scal = nullptr;       // device
     semb_scalars* scal_host = nullptr;  // pinned mirror
     double* hist_dev = nullptr; int hist_cap = 0;
@@ -140,6 +141,7 @@ int semb_axhelm_launch(semb_mesh* h, double lambda, const double* lam0, const do
 int semb_axhelm_pcg_launch(semb_mesh* h, double lambda, const double* zsrc, const double* dinv, double* p, double* x,
                            double* q, semb_scalars* scal, cudaStream_t s);
 
+int64_t semb_axhelm_dot_count(semb_mesh* h);       // number of per-block partials the PCG-fused launch writes into h->ax_dot
 int semb_axhelm_scaled_launch(semb_mesh* h, double lambda, const double* r, const double* dinv, double scale, double* d,
                               double* Ad, semb_scalars* scal, cudaStream_t s);
 
