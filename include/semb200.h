@@ -323,7 +323,7 @@ typedef struct {
 SEMB_API int semb_colormap_apply(const semb_colormap* cm, const double* val_dev, int64_t n, uint32_t* rgba_dev, void* stream);
 
 /* Planar slice: the image plane itself cuts the mesh.  Every sub-cell whose corners lie on both sides of the plane (or on
- * it) claims the pixels whose centres it contains (Newton inversion of its trilinear map: <= 12 steps, step <= 1e-13, inside
+ * it) claims the pixels whose centres it contains (Newton inversion of its trilinear map: <= 12 steps, step <= 1e-10, inside
  * = |r|, |s|, |t| <= 1 + 1e-9); where several cells contain a centre the smallest id wins.  key = cell id << 32 | RGBA, cell
  * id 0xffffffff where nothing was hit. */
 SEMB_API int semb_image_slice(semb_handle h, const semb_field_desc* field, const semb_image_view* view, const semb_colormap* cmap,

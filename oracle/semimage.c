@@ -22,7 +22,7 @@
  *
  * (1) slice: the image plane cuts the mesh.  For every sub-cell in ascending id whose corner distances satisfy
  *     min d <= 0 <= max d, and every pixel of the bounding box of its corners' image coordinates: invert the cell's
- *     trilinear map at P by Newton (start 0, at most 12 steps, stop when the step's max norm is <= 1e-13); the pixel is
+ *     trilinear map at P by Newton (start 0, at most 12 steps, stop when the step's max norm is <= 1e-10: Newton is quadratic, the next iterate is exact to rounding; 1e-13 is below the rounding noise of the residual on the smallest cells of a 64^3 mesh); the pixel is
  *     inside when every reference coordinate has |.| <= 1 + 1e-9; the first (= smallest id) cell claims the pixel; its
  *     value is the trilinear interpolant of the field; colour by the map (3).
  * (2) iso-surface: every sub-cell is split into the 6 tetrahedra around its diagonal corner 0 - corner 7; each tetrahedron
@@ -152,7 +152,7 @@ static int tri_invert(const double X[3][8], const double* P, double* rst)
         r -= dr; s -= ds; t -= dt;
         const double step = fmax(fabs(dr), fmax(fabs(ds), fabs(dt)));
         if (!(fabs(r) <= 4.0 && fabs(s) <= 4.0 && fabs(t) <= 4.0)) return 0;        /* diverging: not this cell */
-        if (step <= 1e-13) { rst[0] = r; rst[1] = s; rst[2] = t; return 1; }
+        if (step <= 1e-10) { rst[0] = r; rst[1] = s; rst[2] = t; return 1; }
     }
     return 0;
 }

@@ -69,7 +69,7 @@ __global__ void k_img_colormap(int64_t n, const double* __restrict__ val, semb_c
 }
 
 // Newton inversion of the trilinear map of one cell at P: start at the centre, <= 12 steps, converged when the step's
-// max norm is <= 1e-13; gives up when the iterate leaves [-4, 4]^3 or the Jacobian is singular.
+// max norm is <= 1e-10 (quadratic convergence: the iterate is then exact to rounding); gives up when the iterate leaves [-4, 4]^3 or the Jacobian is singular.
 __device__ bool img_invert(const double (&X)[3][8], const double (&P)[3], double (&rst)[3])
 {
     double r = 0.0, s = 0.0, t = 0.0;
@@ -106,7 +106,7 @@ __device__ bool img_invert(const double (&X)[3][8], const double (&P)[3], double
         r = SUB(r, dr); s = SUB(s, ds); t = SUB(t, dt);
         const double step = fmax(fabs(dr), fmax(fabs(ds), fabs(dt)));
         if (!(fabs(r) <= 4.0 && fabs(s) <= 4.0 && fabs(t) <= 4.0)) return false;
-        if (step <= 1e-13) { rst[0] = r; rst[1] = s; rst[2] = t; return true; }
+        if (step <= 1e-10) { rst[0] = r; rst[1] = s; rst[2] = t; return true; }
     }
     return false;
 }

@@ -133,6 +133,31 @@ def test_cfg3_fullsize_bench_configuration(torch_cuda, semb, orc, xi_of):
             ref = orc.axhelm(len(sample), N, geo_s, lam, u[idx])
             assert normwise(w[idx], ref) <= TOL, (lam, normwise(w[idx], ref))
             assert np.isfinite(w).all()
+        # ---- in-situ images (row f-4) at full size, bytes against the oracle: a horizontal slice through the lower boundary layer and
+        #      the iso-surface T = 0.5 of a smooth temperature field, 1024 x 512 pixels
+        T = (1.0 - m.z) + 0.1 * np.sin(2 * np.pi * m.x) * np.sin(2 * np.pi * m.y) * m.z * (1.0 - m.z)
+        Td = dev(torch, T)
+        G.publish_field("temperature", Td)
+        dT = G.export_field("temperature")
+        Wp, Hp = 1024, 512
+        key = torch.zeros(Wp * Hp, dtype=torch.int64, device="cuda"); rgba = torch.zeros(Wp * Hp, dtype=torch.int32, device="cuda")
+        cw = [(59, 76, 192), (141, 176, 254), (221, 221, 221), (244, 154, 123), (180, 4, 38)]
+        G.image_slice(dT, semb.image_view(Wp, Hp, (0.0, 0.0, 0.02), (1, 0, 0), (0, 1, 0), 1.0 / Wp, 1.0 / Hp), semb.colormap(0.0, 1.0, cw), key, rgba)
+        ref_rgba, ref_cell = orc.image_slice(m.E, N, m.x, m.y, m.z, T, orc.make_view(Wp, Hp, (0.0, 0.0, 0.02), (1, 0, 0), (0, 1, 0), 1.0 / Wp, 1.0 / Hp),
+                                             orc.make_cmap(0.0, 1.0, cw))
+        k = key.cpu().numpy().view(np.uint64).reshape(Hp, Wp)
+        cell = (k >> np.uint64(32)).astype(np.int64); cell[cell == 0xffffffff] = -1
+        assert np.array_equal(cell, ref_cell) and np.array_equal(rgba.cpu().numpy().view(np.uint32).reshape(Hp, Wp), ref_rgba)
+        assert (ref_cell >= 0).all()
+        uu, vv = np.array([1.0, 0.0, 0.0]), np.array([0.0, 0.8, 0.6])
+        oo = np.array([-0.1, -0.3, -0.2]) - 2.0 * np.cross(uu, vv)
+        light = (0.0, 0.6, 0.8)
+        G.image_isosurface(dT, 0.5, dT, semb.image_view(Wp, Hp, oo, uu, vv, 1.2 / Wp, 1.6 / Hp, 0.0, 6.0), semb.colormap(0.0, 1.0, cw), light, key, rgba)
+        ref_rgba, ref_key = orc.image_isosurface(m.E, N, m.x, m.y, m.z, T, 0.5, T, orc.make_view(Wp, Hp, oo, uu, vv, 1.2 / Wp, 1.6 / Hp),
+                                                 orc.make_cmap(0.0, 1.0, cw), light, 0.0, 6.0)
+        assert np.array_equal(key.cpu().numpy().view(np.uint64).reshape(Hp, Wp), ref_key)
+        assert ((ref_key >> np.uint64(32)) != np.uint64(0xffffffff)).sum() > 0.3 * Wp * Hp
+        del T, Td, key, rgba, ref_rgba, ref_cell, ref_key, k, cell
         # ---- gather-scatter: exact on an integer-valued continuous field, QQ^T v = mult * v
         v = ((lat * 2654435761) % 1021).astype(np.float64) - 510.0
         mult = lattice_mult(ne, N)
@@ -243,7 +268,14 @@ def test_ogrid_fullsize(torch_cuda, semb, orc, xi_of, cfg):
             P.set_operator(0.0, 0b10)
             rr = b - P.apply_A(xh)
             assert np.sqrt(P.dot(rr, rr)) <= 2e-10 * np.sqrt(P.dot(b, b))
-            print(f"cfg2 iterations: Jacobi {rj['iters']}, Chebyshev(2)-Jacobi {rc['iters']}, p-multigrid {rm['iters']}")
+            # Schwarz smoothing on FP32 levels (R26, R21): fewer iterations than Jacobi smoothing, the same oracle-verified residual
+            xs = torch.zeros(m.n, dtype=torch.float64, device="cuda")
+            rs = G.pcg_solve(dev(torch, b), xs, lam=0.0, tags=0b10, precond=3, rtol=1e-10, maxit=400, mg_fp32=True, mg_schwarz=True, mg_smooth=1, mg_kind=4)
+            assert rs["status"] == 0 and rs["iters"] <= 0.6 * rm["iters"], (rs["iters"], rm["iters"])
+            rr = b - P.apply_A(xs.cpu().numpy())
+            assert np.sqrt(P.dot(rr, rr)) <= 2e-10 * np.sqrt(P.dot(b, b))
+            assert normwise(xs.cpu().numpy(), xh) <= 2e-7
+            print(f"cfg2 iterations: Jacobi {rj['iters']}, Chebyshev(2)-Jacobi {rc['iters']}, p-multigrid {rm['iters']}, with Schwarz smoothing on FP32 levels {rs['iters']}")
         else:              # one velocity-type Helmholtz solve (lambda = 1.5/dt, no-slip on plates and side wall)
             P.set_operator(prm["lam"], 0b110)
             b = P.assemble_rhs(f)
