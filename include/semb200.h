@@ -15,7 +15,9 @@
  *     pointer, not the memory).  "host" pointers are ordinary host memory.
  *   - Mesh-derived arrays are owned by the handle until semb_destroy.
  *   - All work is enqueued on the caller's stream (a cudaStream_t passed as void*; NULL = default
- *     stream).  Only semb_setup, semb_pcg_solve, semb_estimate_lmax and the *_host calls synchronise.
+ *     stream).  Only semb_setup, the solvers (semb_pcg_solve, semb_step_solve, semb_boussinesq_step: to poll the stop flag),
+ *     semb_estimate_lmax, the first use of a multigrid hierarchy / Schwarz smoother / geometry class / flow metrics (one-off
+ *     setup work) and the *_host calls synchronise.
  *   - Layout ("(ijk) ordering on [-1,1]^3"): local node l = e*Np + k*n1*n1 + j*n1 + i,
  *     n1 = N+1, Np = n1^3, i fastest; n = E*Np local nodes; all fields fp64, indices int32.
  *   - There is no CPU fallback: with no CUDA device every compute call returns SEMB_ECUDA.

@@ -179,3 +179,22 @@ def test_fullsize_affine_and_trilinear_boxes(torch_cuda, semb, orc, xi_of):
         finally:
             G.close()
         del m
+
+
+def test_geometry_modes_on_the_smallest_meshes(torch_cuda, semb, orc, xi_of):
+    """Degenerate sizes: one element, order 1 (8 nodes) and order 2, every representation, ragged packed blocks (32 / 14 elements per block)."""
+    torch = torch_cuda
+    for N, ne in ((1, (1, 1, 1)), (1, (5, 3, 7)), (2, (1, 1, 1)), (2, (3, 5, 3))):
+        m = I.box_mesh(*ne, N, xi_of(N), zstretch=1.5)
+        P = orc.Problem(m.E, m.N, m.x, m.y, m.z, m.face_tag, m.period)
+        G = semb.Mesh(m.E, m.N, dev(torch, m.x), dev(torch, m.y), dev(torch, m.z), m.face_tag, m.period)
+        try:
+            u = I.uniform(9, m.n); ud = dev(torch, u); wd = torch.empty_like(ud)
+            for mode in (0, 1, 2, 3):
+                G.set_geometry_mode(mode)
+                geo_ref = P.geo if mode != 1 else np.ascontiguousarray(G.geo_host().astype(np.float32).astype(np.float64))
+                for lam in (0.0, 7.0):
+                    G.apply_axhelm(ud, wd, lam=lam)
+                    assert normwise(wd.cpu().numpy(), orc.axhelm(m.E, m.N, geo_ref, lam, u)) <= TOL, (N, ne, mode, lam)
+        finally:
+            G.close()

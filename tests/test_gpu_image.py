@@ -140,3 +140,34 @@ def test_colormap_and_argument_checks(torch_cuda, semb, orc, xi_of):
             G.image_slice(bad, semb.image_view(8, 8, (0, 0, 0.5), (1, 0, 0), (0, 1, 0), 0.125, 0.125), semb.colormap(0, 1, COOLWARM), key)
     finally:
         G.close()
+
+
+def test_degenerate_views(torch_cuda, semb, orc, xi_of):
+    """Edge cases: a plane that misses the mesh (all background), a 1 x 1 image, an iso value outside the field's range, and a
+    one-element mesh of order 1 (a single sub-cell)."""
+    torch = torch_cuda
+    for m in (I.box_mesh(2, 2, 2, 3, xi_of(3), deform=0.03), I.box_mesh(1, 1, 1, 1, xi_of(1))):
+        T = 1.0 - m.z + 0.1 * m.x
+        G = semb.Mesh(m.E, m.N, dev(torch, m.x), dev(torch, m.y), dev(torch, m.z), m.face_tag, m.period)
+        try:
+            Td = dev(torch, T)
+            G.publish_field("t", Td)
+            d = G.export_field("t")
+            cm_o, cm_g = orc.make_cmap(0.0, 1.0, COOLWARM, background=0xff112233), semb.colormap(0.0, 1.0, COOLWARM, background=0xff112233)
+            for W, H, o in ((16, 9, (0.0, 0.0, 1.5)), (1, 1, (0.2, 0.3, 0.5)), (7, 5, (0.0, 0.0, 1.0))):
+                key = torch.zeros(W * H, dtype=torch.int64, device="cuda"); rgba = torch.zeros(W * H, dtype=torch.int32, device="cuda")
+                G.image_slice(d, semb.image_view(W, H, o, (1, 0, 0), (0, 1, 0), 1.0 / W, 1.0 / H), cm_g, key, rgba)
+                ref_rgba, ref_cell = orc.image_slice(m.E, m.N, m.x, m.y, m.z, T, orc.make_view(W, H, o, (1, 0, 0), (0, 1, 0), 1.0 / W, 1.0 / H), cm_o)
+                assert np.array_equal(rgba.cpu().numpy().view(np.uint32).reshape(H, W), ref_rgba)
+                if o[2] > 1.0:
+                    assert np.all(ref_cell < 0) and np.all(ref_rgba == 0xff112233)
+                for iso in (5.0, 0.55):
+                    G.image_isosurface(d, iso, None, semb.image_view(W, H, (0.0, 0.0, 2.0), (0, 1, 0), (1, 0, 0), 1.0 / W, 1.0 / H, 0.0, 4.0), cm_g,
+                                       (0, 0, 1), key, rgba)
+                    rr, rk = orc.image_isosurface(m.E, m.N, m.x, m.y, m.z, T, iso, None, orc.make_view(W, H, (0.0, 0.0, 2.0), (0, 1, 0), (1, 0, 0), 1.0 / W, 1.0 / H),
+                                                  cm_o, (0, 0, 1), 0.0, 4.0)
+                    assert np.array_equal(key.cpu().numpy().view(np.uint64).reshape(H, W), rk)
+                    if iso > 2.0:
+                        assert np.all(rr == 0xff112233)
+        finally:
+            G.close()
