@@ -345,7 +345,7 @@ SEMB_API int semb_image_isosurface(semb_handle h, const semb_field_desc* field, 
  *   (i)   N_c = -(u.grad)u_c + delta_cz T + f_c,  N_theta = -(u.grad)theta + u_z + f_theta  (collocation, per element);
  *         omega = curl u;  omega_bar = QQ^T(B omega) / QQ^T(B);  C = curl omega_bar
  *   (ii)  u~ = sum_k b_k u^(n+1-k) + dt sum_k a_k N^(n+1-k);  g = u~/dt - nu sum_k a_k C^(n+1-k);
- *         A p = QQ^T wdiv(g), all Neumann, zero mean (null_mean)
+ *         A p = QQ^T wdiv(g), all Neumann, zero mean (null_mean), started from p^n
  *   (iii) (A + beta0/(nu dt) B) u_c^(n+1) = M QQ^T B (u~_c - dt dp/dx_c) / (nu dt), started from u_c^n; the same for theta with kappa.
  * Building blocks, each element-local and asynchronous on stream (arrays device [n]): */
 /* collocation gradient of a nodal field: g_b = sum_a (dr_a/dx_b) dphi/dr_a (discontinuous across elements) */
@@ -368,7 +368,7 @@ typedef struct {
 } semb_flow_opts;
 
 typedef struct {                  /* every array device [n], caller-owned */
-    double* u[3]; double* theta; double* p;      /* in: level n (p: unused); out: level n+1                    */
+    double* u[3]; double* theta; double* p;      /* in: level n (p: initial guess of the solve); out: level n+1 */
     double* u1[3]; double* theta1;               /* in: level n-1;            out: level n                      */
     double* N1[4];                               /* in: explicit terms of level n-1; out: of level n            */
     double* C1[3];                               /* in: curl curl u of level n-1;    out: of level n            */

@@ -14,7 +14,7 @@ the oracle's primitives (semflow.c: grad, wdiv; semoracle.c: gs, mask, PCG), in 
           omega   = curl u (collocation);  omega_bar = QQ^T(B omega) / QQ^T(B);  C = curl omega_bar
     (ii)  u~_c    = sum_k b_k u_c^(n+1-k) + dt sum_k a_k N_c^(n+1-k)
           g_c     = u~_c / dt - nu sum_k a_k C_c^(n+1-k)          (curl-curl form of the viscous term in the pressure equation)
-          b_p     = QQ^T wdiv(g);   A p = b_p  (all Neumann: null_mean, R20)
+          b_p     = QQ^T wdiv(g);   A p = b_p  (all Neumann: null_mean, R20), started from p^n
     (iii) u^_c    = u~_c - dt dp/dx_c (collocation);   (A + beta0/(nu dt) B) u_c^(n+1) = M QQ^T (B u^_c) / (nu dt),  start u_c^n
           theta~  = sum_k b_k theta^(n+1-k) + dt sum_k a_k N_theta^(n+1-k)
           (A + beta0/(kappa dt) B) theta^(n+1) = M QQ^T (B theta~) / (kappa dt),  start theta^n
@@ -115,7 +115,7 @@ class Boussinesq:
         ut = [b[0] * self.u[c] + b[1] * self.u1[c] + dt * (a[0] * N[c] + a[1] * self.N1[c]) for c in range(3)]
         g = [ut[c] / dt - nu * (a[0] * Cc[c] + a[1] * self.C1[c]) for c in range(3)]
         bp = O.gs(P.gid, P.n_unique, ops.wdiv(*g))
-        self.p = self.solver(P, 0.0, 0, bp, None, True)
+        self.p = self.solver(P, 0.0, 0, bp, self.p, True)          # started from the previous step's pressure (zero on the first step)
         # (iii)
         gp = ops.grad(self.p)
         un = []

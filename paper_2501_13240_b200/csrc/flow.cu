@@ -363,7 +363,7 @@ extern "C" int semb_boussinesq_step(semb_handle h, const semb_flow_opts* o, semb
     h->launches += 5;
     semb_pcg_opts po{};
     po.lambda = 0.0; po.dirichlet_tags = 0; po.precond = o->precond_p ? o->precond_p : 3; po.cheb_degree = 2; po.rtol = o->rtol > 0.0 ? o->rtol : 1e-10;
-    po.maxit = o->maxit > 0 ? o->maxit : 20000; po.x0_is_zero = 1; po.null_mean = 1; po.mg_fp32 = o->mg_fp32; po.mg_schwarz = o->mg_schwarz; po.mg_smoother_kind = o->mg_schwarz ? 4 : 1;
+    po.maxit = o->maxit > 0 ? o->maxit : 20000; po.x0_is_zero = 0; /* started from p^n (zero on the first step) */ po.null_mean = 1; po.mg_fp32 = o->mg_fp32; po.mg_schwarz = o->mg_schwarz; po.mg_smoother_kind = o->mg_schwarz ? 4 : 1;
     semb_pcg_stats ps{};
     rc = semb_pcg_run(h, &po, bp, st->p, &ps, s);
     if (stats) { stats->iters[0] = ps.iters; stats->status[0] = rc; }
