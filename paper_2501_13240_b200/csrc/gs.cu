@@ -47,6 +47,22 @@ __global__ void k_gs_hi(int64_t n_hi, const int32_t* __restrict__ hi, const int3
     if (q >= n_hi) return;
     const int32_t g = hi[q];
     const int32_t a = off[g], b = off[g + 1];
+    // A class of a hexahedral mesh has 3..8 members (more only at irregular points): the member ids and then the member values are
+    // fetched as two batches of independent loads (two exposed latencies per class instead of two per member); the sum keeps the
+    // ascending order of k_gs.
+    if (b - a <= 8) {
+        int32_t id[8]; double v[8];
+#pragma unroll
+        for (int t = 0; t < 8; ++t) id[t] = (a + t < b) ? ids[a + t] : -1;
+#pragma unroll
+        for (int t = 0; t < 8; ++t) v[t] = (id[t] >= 0) ? semb_wide(w[id[t]]) : 0.0;
+        double s = 0.0;
+#pragma unroll
+        for (int t = 0; t < 8; ++t) if (id[t] >= 0) s += v[t];
+#pragma unroll
+        for (int t = 0; t < 8; ++t) if (id[t] >= 0) w[id[t]] = (ST)s;
+        return;
+    }
     double s = 0.0;
     for (int32_t t = a; t < b; ++t) s += semb_wide(w[ids[t]]);
     for (int32_t t = a; t < b; ++t) w[ids[t]] = (ST)s;

@@ -200,9 +200,22 @@ k_iter_small(int64_t n, int64_t ndot, const double* __restrict__ ax_dot, int64_t
     cl.sync();
     for (int64_t t = tid; t < n_hi; t += nthr) {
         const int32_t g = hi[t], a = off[g], b = off[g + 1];
-        double c = 0.0;
-        for (int32_t u = a; u < b; ++u) c += q[ids[u]];
-        for (int32_t u = a; u < b; ++u) q[ids[u]] = c;
+        if (b - a <= 8) {                                          // member ids, then member values, as two batches of independent loads
+            int32_t id[8]; double v[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) id[u] = (a + u < b) ? ids[a + u] : -1;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) v[u] = (id[u] >= 0) ? q[id[u]] : 0.0;
+            double c = 0.0;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) if (id[u] >= 0) c += v[u];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) if (id[u] >= 0) q[id[u]] = c;
+        } else {
+            double c = 0.0;
+            for (int32_t u = a; u < b; ++u) c += q[ids[u]];
+            for (int32_t u = a; u < b; ++u) q[ids[u]] = c;
+        }
     }
     cl.sync();
     double rr = 0.0, rz = 0.0;
