@@ -35,6 +35,9 @@ static __constant__ double c_xi[SEMB_MAX_N + 1][SEMB_MAXN1], c_rho[SEMB_MAX_N + 
 //          C_t = x_r x x_s and J = x_r . C_r are recomputed per node and G applied in factored form
 //          g_a = (W / J) C_a . (C_r u_r + C_s u_s + C_t u_t)                                        192 B/element
 
+#ifndef SEMB_AX_RELOAD_N1
+#define SEMB_AX_RELOAD_N1 10
+#endif
 #ifndef SEMB_AX_SPLIT_N1
 #define SEMB_AX_SPLIT_N1 99          // off by default until measured
 #endif
@@ -440,11 +443,17 @@ k_axhelm_line(int64_t E, int64_t n, const void* __restrict__ geo_v, double lambd
     }
     CT wt[n1];
     ax_line<n1, 1, CT>(gt, wt);
+    // RELOAD (n1 >= SEMB_AX_RELOAD_N1, i.e. N = 9, 10): the thread's own u values are read back from the Su tile (never overwritten)
+    // where the epilogue needs them, instead of staying in 2 n1 registers across both contraction phases.  Measured on B200, N = 9,
+    // 46.7 M nodes: spills 88-132 -> 8-52 bytes; Poisson 5.50 -> 5.70 TB/s, Helmholtz 5.65 -> 6.41, PCG-fused 6.69 -> 6.87; N = 7
+    // unchanged within noise (left off there).  Computing the t-contraction after the barrier from a reloaded u changed nothing.
+    constexpr bool RELOAD = n1 >= SEMB_AX_RELOAD_N1;
     if (HELM) {
 #pragma unroll
         for (int k = 0; k < n1; ++k) {
             const CT lam = (VAR && lam1) ? (CT)lam1[e * Np + k * n2 + tl] : (CT)lambda;
-            wt[k] += lam * (STORED ? G[STORED ? NG - 1 : 0][STORED ? k : 0] : (CT)Bk[(HELM && !STORED) ? k : 0]) * ru[k];
+            const CT uk = RELOAD ? Su[AX_I(k, b, a)] : ru[k];
+            wt[k] += lam * (STORED ? G[STORED ? NG - 1 : 0][STORED ? k : 0] : (CT)Bk[(HELM && !STORED) ? k : 0]) * uk;
         }
     }
     __syncthreads();
@@ -452,7 +461,8 @@ k_axhelm_line(int64_t E, int64_t n, const void* __restrict__ geo_v, double lambd
 #pragma unroll
     for (int k = 0; k < n1; ++k) {
         const CT wv = wt[k] + Sr[AX_I(k, b, a)] + Ss[AX_IB(k, b, a)];
-        if (valid) { we[k * n2] = wv; dot += (double)ru[k] * (double)wv; }
+        const CT uk = RELOAD ? Su[AX_I(k, b, a)] : ru[k];
+        if (valid) { we[k * n2] = wv; dot += (double)uk * (double)wv; }
     }
     if (dot_out) {
         __shared__ double red[32];
