@@ -64,6 +64,7 @@ template <int n1> struct ax_tile {
     static constexpr int P2 = (n1 == 4) ? 19 : (n1 == 10) ? 103 : n1 * n1;                        // Su, Sr
     static constexpr int P2B = (n1 == 4) ? 19 : (n1 == 7) ? 57 : (n1 == 10) ? 101 : n1 * n1;       // Ss
     static constexpr int size = n1 * (P2 > P2B ? P2 : P2B);
+    static constexpr int sizeA = (n1 - 1) * P2 + n1 * n1, sizeB = (n1 - 1) * P2B + n1 * n1;     // what idx / idxB really reach
     // measured on B200 (A/B in one session): N = 6 +5 %, N = 9 +3 % (Poisson) / +10 % (Helmholtz), N = 10 +7 %;
     // n1 = 9 was 3 % slower with its best permuted layout and n1 <= 6 within noise: those keep thread = line.
     static constexpr bool permuted = (n1 == 7) || (n1 >= 10);
@@ -74,7 +75,7 @@ template <int n1> struct ax_tile {
 // n1 = 8: XOR swizzle, conflict-free in all three orientations without padding:
 //   slot mod 16 = ((j^k)&1)*8 + (i ^ (((j>>1)&3) | ((k&1)<<2)))
 template <> struct ax_tile<8> {
-    static constexpr int size = 512;
+    static constexpr int size = 512, sizeA = 512, sizeB = 512;
     static constexpr int P1 = 8, P2 = 64, P2B = 64;
     static constexpr bool permuted = false;
     __device__ static __forceinline__ int idx(int k, int j, int i)
@@ -261,10 +262,10 @@ k_axhelm_line(int64_t E, int64_t n, const void* __restrict__ geo_v, double lambd
     constexpr bool W32 = sizeof(CT) == 4;
 #define AX_I(k, j, i) (W32 ? T::idx32(k, j, i) : T::idx(k, j, i))
 #define AX_IB(k, j, i) (W32 ? T::idx32(k, j, i) : T::idxB(k, j, i))
-    __shared__ CT SuA[EPB * T::size], SrA[EPB * T::size], SsA[EPB * T::size];
+    __shared__ __align__(8) CT SuA[EPB * T::sizeA], SrA[EPB * T::sizeA], SsA[EPB * (W32 ? T::sizeA : T::sizeB)];
     if (scal && *(volatile const int32_t*)&scal->done) return;
     const int el = (EPB > 1) ? threadIdx.x / n2 : 0, tl = (EPB > 1) ? threadIdx.x - el * n2 : threadIdx.x;
-    CT* __restrict__ Su = SuA + el * T::size; CT* __restrict__ Sr = SrA + el * T::size; CT* __restrict__ Ss = SsA + el * T::size;
+    CT* __restrict__ Su = SuA + el * T::sizeA; CT* __restrict__ Sr = SrA + el * T::sizeA; CT* __restrict__ Ss = SsA + el * (W32 ? T::sizeA : T::sizeB);
     const int64_t nef = E * (int64_t)nfields;
     int64_t ef = blockIdx.x * (int64_t)EPB + el;
     const bool valid = ef < nef;
@@ -465,13 +466,164 @@ k_axhelm_line(int64_t E, int64_t n, const void* __restrict__ geo_v, double lambd
         if (valid) { we[k * n2] = wv; dot += (double)uk * (double)wv; }
     }
     if (dot_out) {
-        __shared__ double red[32];
+        // two N = 9 elements per block fill the 48 KB of static shared memory: the reduction scratch then lives in the Sr tile
+        constexpr bool ALIAS = sizeof(CT) * EPB * (2 * T::sizeA + (W32 ? T::sizeA : T::sizeB)) + 256 > 48 * 1024;
+        __shared__ double red_own[ALIAS ? 1 : 32];
+        double* red = ALIAS ? reinterpret_cast<double*>(SrA) : red_own;
+        if (ALIAS) __syncthreads();
         dot = block_sum(dot, red);
         if (threadIdx.x == 0) dot_out[blockIdx.x] = dot;
     }
 }
 #undef AX_I
 #undef AX_IB
+
+// ---- N = 9 stand-alone operator, factors staged through shared memory by the TMA unit -------------------------------------
+// k_axhelm_line at n1 = 10 holds 6 x 10 factors per thread in registers (168 registers, 3 blocks of 4 warps per SM) and its
+// blocks wait for their own loads: 0.71 ms per launch on the cfg4 mesh whatever the byte count (Poisson 5.7 TB/s).  Here a
+// block is persistent (3 per SM, elements blockIdx.x, + gridDim.x, ...), the six factors of its NEXT element are copied into a
+// 48 KB shared-memory buffer by one cp.async.bulk issued as soon as the current element's factor phase has released the
+// buffer, and consumed in place (conflict-free: slot = plane + thread).  The element body is a __noinline__ function so that
+// ptxas cannot hoist the constant-bank operands of the contractions out of the element loop.
+// Only n1 = 10: the bulk copy needs 16-byte aligned element starts (7 Np doubles per element: Np even).
+template <int n1> struct ax_stage_smem {
+    using T = ax_tile<n1>;
+    static constexpr int Np = n1 * n1 * n1;
+    static constexpr int oSu = 6 * Np, oSr = oSu + T::sizeA, oSs = oSr + T::sizeA, oBar = oSs + T::sizeB;     // in doubles
+    static constexpr size_t bytes = (size_t)(oBar + 2) * sizeof(double);
+};
+__device__ __forceinline__ unsigned ax_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void ax_stage_issue(double* dst, uint64_t* bar, const double* src, unsigned bytes)
+{
+    const unsigned d = ax_smem_u32(dst), m = ax_smem_u32(bar);
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");       // the buffer's last generic-proxy reads precede the async write
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(m), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(d), "l"(src), "r"(bytes), "r"(m) : "memory");
+}
+__device__ __forceinline__ void ax_stage_wait(uint64_t* bar, unsigned phase)
+{
+    const unsigned m = ax_smem_u32(bar);
+    asm volatile("{\n\t.reg .pred p;\n\tAX_WAIT:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@p bra AX_DONE;\n\tbra AX_WAIT;\n\tAX_DONE:\n\t}"
+                 :: "r"(m), "r"(phase) : "memory");
+}
+
+template <int n1, bool HELM>
+__device__ __noinline__ void ax_stage_element(int64_t ef, int64_t ef_next, int64_t E, int64_t n, const double* __restrict__ geo,
+                                              double lambda, const double* __restrict__ u, double* __restrict__ w, unsigned phase)
+{
+    constexpr int n2 = n1 * n1, Np = n2 * n1;
+    using T = ax_tile<n1>; using L = ax_stage_smem<n1>;
+    extern __shared__ __align__(128) double ax_dyn[];
+    double* __restrict__ Gs = ax_dyn; double* __restrict__ Su = ax_dyn + L::oSu; double* __restrict__ Sr = ax_dyn + L::oSr;
+    double* __restrict__ Ss = ax_dyn + L::oSs; uint64_t* bar = reinterpret_cast<uint64_t*>(ax_dyn + L::oBar);
+    const int tl = threadIdx.x, a = tl % n1, b = tl / n1;
+    int ra = a, rb = b, sa = a, sb = b;
+    if (T::permuted) {
+        const int rq = c_perm[n1 - 1][0][tl], sq = c_perm[n1 - 1][1][tl];
+        ra = rq % n1; rb = rq / n1; sa = sq % n1; sb = sq / n1;
+    }
+    const int64_t e = ef % E, f = ef / E;
+    if (tl == 0 && ef_next >= 0) {                     // what the next element reads with plain loads goes to L2 now
+        const int64_t ep = ef_next % E, fp = ef_next / E;
+        ax_prefetch_l2(u + fp * n + ep * Np, Np);
+        if (HELM) ax_prefetch_l2(geo + (ep * 7 + 6) * (int64_t)Np, Np);
+    }
+    const double* __restrict__ ue = u + f * n + e * Np + tl;
+    double ut[n1];
+    {
+        double ru[n1];
+#pragma unroll
+        for (int k = 0; k < n1; ++k) ru[k] = ue[k * n2];
+#pragma unroll
+        for (int k = 0; k < n1; ++k) Su[T::idx(k, b, a)] = ru[k];
+        ax_line<n1, 0, double>(ru, ut);
+    }
+    double Bf[HELM ? n1 : 1];
+    if (HELM) {
+        const double* __restrict__ gB = geo + (e * 7 + 6) * (int64_t)Np + tl;
+#pragma unroll
+        for (int k = 0; k < n1; ++k) Bf[k] = __ldg(gB + k * n2);
+    }
+    __syncthreads();
+    {
+        double ln[n1], out[n1];
+#pragma unroll
+        for (int i = 0; i < n1; ++i) ln[i] = Su[T::idx(rb, ra, i)];
+        ax_line<n1, 0, double>(ln, out);
+#pragma unroll
+        for (int i = 0; i < n1; ++i) Sr[T::idx(rb, ra, i)] = out[i];
+#pragma unroll
+        for (int j = 0; j < n1; ++j) ln[j] = Su[T::idx(sb, j, sa)];
+        ax_line<n1, 0, double>(ln, out);
+#pragma unroll
+        for (int j = 0; j < n1; ++j) Ss[T::idxB(sb, j, sa)] = out[j];
+    }
+    __syncthreads();
+    ax_stage_wait(bar, phase);                         // the factors of this element have landed
+    double gt[n1];
+#pragma unroll
+    for (int k = 0; k < n1; ++k) {
+        const int s = T::idx(k, b, a), sB = T::idxB(k, b, a), g = k * n2 + tl;
+        const double ur = Sr[s], us = Ss[sB];
+        const double Grr = Gs[g], Grs = Gs[Np + g], Grt = Gs[2 * Np + g], Gss = Gs[3 * Np + g], Gst = Gs[4 * Np + g], Gtt = Gs[5 * Np + g];
+        Sr[s] = Grr * ur + Grs * us + Grt * ut[k];
+        Ss[sB] = Grs * ur + Gss * us + Gst * ut[k];
+        gt[k] = Grt * ur + Gst * us + Gtt * ut[k];
+    }
+    __syncthreads();
+    if (tl == 0 && ef_next >= 0)                       // every thread is past its last read of Gs
+        ax_stage_issue(Gs, bar, geo + (ef_next % E) * 7 * (int64_t)Np, (unsigned)(6 * Np * sizeof(double)));
+    {
+        double ln[n1], out[n1];
+#pragma unroll
+        for (int i = 0; i < n1; ++i) ln[i] = Sr[T::idx(rb, ra, i)];
+        ax_line<n1, 1, double>(ln, out);
+#pragma unroll
+        for (int i = 0; i < n1; ++i) Sr[T::idx(rb, ra, i)] = out[i];
+#pragma unroll
+        for (int j = 0; j < n1; ++j) ln[j] = Ss[T::idxB(sb, j, sa)];
+        ax_line<n1, 1, double>(ln, out);
+#pragma unroll
+        for (int j = 0; j < n1; ++j) Ss[T::idxB(sb, j, sa)] = out[j];
+    }
+    double wt[n1];
+    ax_line<n1, 1, double>(gt, wt);
+    if (HELM) {
+#pragma unroll
+        for (int k = 0; k < n1; ++k) wt[k] += lambda * Bf[HELM ? k : 0] * Su[T::idx(k, b, a)];
+    }
+    __syncthreads();
+    double* __restrict__ we = w + f * n + e * Np + tl;
+#pragma unroll
+    for (int k = 0; k < n1; ++k) we[k * n2] = wt[k] + Sr[T::idx(k, b, a)] + Ss[T::idxB(k, b, a)];
+}
+
+template <int n1, bool HELM>
+__global__ void __launch_bounds__(n1 * n1, 3)
+k_axhelm_stage(int64_t E, int64_t n, const double* __restrict__ geo, double lambda, const double* __restrict__ u, double* __restrict__ w, int nfields)
+{
+    constexpr int Np = n1 * n1 * n1;
+    using L = ax_stage_smem<n1>;
+    extern __shared__ __align__(128) double ax_dyn[];
+    uint64_t* bar = reinterpret_cast<uint64_t*>(ax_dyn + L::oBar);
+    const int64_t nef = E * (int64_t)nfields, stride = gridDim.x;
+    int64_t ef = blockIdx.x;
+    if (ef >= nef) return;
+    if (threadIdx.x == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(ax_smem_u32(bar)) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        ax_stage_issue(ax_dyn, bar, geo + (ef % E) * 7 * (int64_t)Np, (unsigned)(6 * Np * sizeof(double)));
+    }
+    __syncthreads();
+    unsigned phase = 0;
+#pragma unroll 1
+    for (; ef < nef; ef += stride) {
+        const int64_t nx = ef + stride < nef ? ef + stride : -1;
+        ax_stage_element<n1, HELM>(ef, nx, E, n, geo, lambda, u, w, phase);
+        phase ^= 1u;
+    }
+}
 
 // Sum of the per-block partials dot_in[0..count) in a fixed order (two stages, last block by ticket), then
 // the PCG scalars: p.Ap, alpha = rho / p.Ap, breakdown detection.

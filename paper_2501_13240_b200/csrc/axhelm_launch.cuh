@@ -1,7 +1,11 @@
 // Launch machinery of the axhelm kernels, shared by the translation units that instantiate them (one per geometry
 // representation, so that they compile in parallel; every unit has its own copy of the __constant__ tables and uploads it).
 #pragma once
+#include <cstdlib>
 #include "axhelm_kernels.cuh"
+#ifndef SEMB_AX_STAGE
+#define SEMB_AX_STAGE 1          // N = 9 stand-alone launches use k_axhelm_stage (env SEMB_AX_STAGE=0/1 overrides at run time)
+#endif
 
 // one translation unit per on-the-fly / reduced-precision geometry representation
 #define SEMB_AX_GEO_TU(G) \
@@ -70,7 +74,10 @@ static int ax_upload_basis_tu(semb_mesh* h)
 #define SEMB_EPB7 1
 #define SEMB_MINB7 4
 #endif
-template <int n1> struct ax_epb { static constexpr int v = (n1 == 2) ? 32 : (n1 == 3) ? 14 : (n1 == 4) ? 8 : (n1 == 5) ? SEMB_EPB5 : (n1 == 6) ? SEMB_EPB6 : (n1 == 7) ? SEMB_EPB7 : 1; };
+#ifndef SEMB_EPB10
+#define SEMB_EPB10 1
+#endif
+template <int n1> struct ax_epb { static constexpr int v = (n1 == 2) ? 32 : (n1 == 3) ? 14 : (n1 == 4) ? 8 : (n1 == 5) ? SEMB_EPB5 : (n1 == 6) ? SEMB_EPB6 : (n1 == 7) ? SEMB_EPB7 : (n1 == 10) ? SEMB_EPB10 : 1; };
 #ifndef SEMB_MINB8_G3
 #define SEMB_MINB8_G3 8
 #endif
@@ -102,6 +109,29 @@ static int launch_line(semb_mesh* h, const void* geo, int mode, double lambda, c
     const int64_t bytes_per_elem = (int64_t)n1 * n1 * n1 * (((mode & 4) ? (pcg.plain ? 80 : 104) : (mode & 2) ? 88 : (mode & 1) ? 72 : 64) - gsub)
                                    * (int64_t)sizeof(ST) / 8;
     const int pf = (int)(((int64_t)8 << 20) / bytes_per_elem);
+    // N = 9, fp64 stored factors, stand-alone Poisson / Helmholtz: the persistent kernel with TMA-staged factors
+    if constexpr (n1 == 10 && sizeof(ST) == 8 && GEO == SEMB_GEO_STORED) {
+        static const int stage_on = [] { const char* v = getenv("SEMB_AX_STAGE"); return v ? atoi(v) : SEMB_AX_STAGE; }();
+        if (stage_on && !scal && (mode == 0 || mode == 1) && ((uintptr_t)geo & 15) == 0) {
+            constexpr size_t smem = ax_stage_smem<n1>::bytes;
+            auto kern = (mode & 1) ? k_axhelm_stage<n1, true> : k_axhelm_stage<n1, false>;
+            static int per_sm[2][64] = {{0}};                      // per device: the opt-in shared-memory size is a per-device attribute
+            int devid = 0;
+            SEMB_CUDA(h, cudaGetDevice(&devid));
+            int& nb_dev = per_sm[mode & 1][devid & 63];
+            if (!nb_dev) {
+                SEMB_CUDA(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                int nb = 0;
+                SEMB_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, n1 * n1, smem));
+                nb_dev = nb > 0 ? nb : 1;
+            }
+            const int64_t nef = h->E * (int64_t)nfields, cap = (int64_t)nb_dev * semb_sm_count();
+            kern<<<(unsigned)(nef < cap ? nef : cap), n1 * n1, smem, s>>>(h->E, h->n, (const double*)geo, lambda, (const double*)u, (double*)w, nfields);
+            h->launches += 1;
+            SEMB_CUDA(h, cudaGetLastError());
+            return SEMB_OK;
+        }
+    }
 #define SEMB_AX_LAUNCH(M) k_axhelm_line<n1, M, MB, EPB, ST, GEO><<<grid, n1 * n1 * EPB, 0, s>>>(h->E, h->n, geo, lambda, lam0, lam1, u, w, scal, dot, pcg, pf, nfields)
     switch (mode) {
         case 0: SEMB_AX_LAUNCH(0); break;

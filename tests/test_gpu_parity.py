@@ -155,6 +155,26 @@ def test_axhelm_batched_and_variable_coefficients(torch_cuda, cases, orc, name):
     assert normwise(w.cpu().numpy(), orc.axhelm(m.E, m.N, P.geo, 0.0, U[0], lam0=lam0, lam1=lam1)) <= TOL
 
 
+def test_axhelm_order9_persistent_blocks(torch_cuda, semb, orc, xi_of):
+    """N = 9 stand-alone launches run k_axhelm_stage: persistent blocks (3 per SM on B200 = 444) that walk over the elements
+    blockIdx.x + i * gridDim.x with the factors of their next element in flight (TMA into shared memory).  9 x 8 x 7 = 504 elements
+    x 2 fields = 1008 block-elements: two full rounds and a ragged third one; then a single element (one block, no next element)."""
+    for dims, nf in (((9, 8, 7), 2), ((1, 1, 1), 1)):
+        m = I.box_mesh(*dims, 9, xi_of(9), deform=0.04)
+        P, G = oracle_problem(orc, m), gpu_mesh(torch_cuda, semb, m)
+        U = np.stack([I.uniform(I.seed_for(1, 40 + f), m.n) for f in range(nf)])
+        for lam in (0.0, 1e4):
+            W = torch_cuda.full((nf, m.n), np.nan, dtype=torch_cuda.float64, device="cuda")
+            G.apply_axhelm(dev(torch_cuda, U), W, lam=lam, nfields=nf)
+            for f in range(nf):
+                ref = orc.axhelm(m.E, m.N, P.geo, lam, U[f])
+                w = W[f].cpu().numpy()
+                assert normwise(w, ref) <= TOL
+                per_elem = np.abs((w - ref).reshape(m.E, -1)).max(1) / np.abs(ref.reshape(m.E, -1)).max(1)
+                assert per_elem.max() <= TOL
+        G.close()
+
+
 def test_axhelm_host_entry_point(torch_cuda, cases, orc):
     m, P, G = cases("cfg0")
     u = I.uniform(3, m.n); w = np.zeros(m.n)
