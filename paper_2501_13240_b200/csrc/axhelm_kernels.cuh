@@ -509,7 +509,7 @@ __device__ __forceinline__ void ax_stage_wait(uint64_t* bar, unsigned phase)
 }
 
 template <int n1, bool HELM>
-__device__ __noinline__ void ax_stage_element(int64_t ef, int64_t ef_next, int64_t E, int64_t n, const double* __restrict__ geo,
+__device__ __noinline__ void ax_stage_element(int64_t e, int64_t f, int64_t ep, int64_t fp, int64_t n, const double* __restrict__ geo,
                                               double lambda, const double* __restrict__ u, double* __restrict__ w, unsigned phase)
 {
     constexpr int n2 = n1 * n1, Np = n2 * n1;
@@ -523,9 +523,7 @@ __device__ __noinline__ void ax_stage_element(int64_t ef, int64_t ef_next, int64
         const int rq = c_perm[n1 - 1][0][tl], sq = c_perm[n1 - 1][1][tl];
         ra = rq % n1; rb = rq / n1; sa = sq % n1; sb = sq / n1;
     }
-    const int64_t e = ef % E, f = ef / E;
-    if (tl == 0 && ef_next >= 0) {                     // what the next element reads with plain loads goes to L2 now
-        const int64_t ep = ef_next % E, fp = ef_next / E;
+    if (tl == 0 && ep >= 0) {                          // what the next element (ep, field fp) reads with plain loads goes to L2 now
         ax_prefetch_l2(u + fp * n + ep * Np, Np);
         if (HELM) ax_prefetch_l2(geo + (ep * 7 + 6) * (int64_t)Np, Np);
     }
@@ -572,8 +570,8 @@ __device__ __noinline__ void ax_stage_element(int64_t ef, int64_t ef_next, int64
         gt[k] = Grt * ur + Gst * us + Gtt * ut[k];
     }
     __syncthreads();
-    if (tl == 0 && ef_next >= 0)                       // every thread is past its last read of Gs
-        ax_stage_issue(Gs, bar, geo + (ef_next % E) * 7 * (int64_t)Np, (unsigned)(6 * Np * sizeof(double)));
+    if (tl == 0 && ep >= 0)                            // every thread is past its last read of Gs
+        ax_stage_issue(Gs, bar, geo + ep * 7 * (int64_t)Np, (unsigned)(6 * Np * sizeof(double)));
     {
         double ln[n1], out[n1];
 #pragma unroll
@@ -610,17 +608,20 @@ k_axhelm_stage(int64_t E, int64_t n, const double* __restrict__ geo, double lamb
     const int64_t nef = E * (int64_t)nfields, stride = gridDim.x;
     int64_t ef = blockIdx.x;
     if (ef >= nef) return;
+    int64_t e = ef % E, f = ef / E;
     if (threadIdx.x == 0) {
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(ax_smem_u32(bar)) : "memory");
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        ax_stage_issue(ax_dyn, bar, geo + (ef % E) * 7 * (int64_t)Np, (unsigned)(6 * Np * sizeof(double)));
+        ax_stage_issue(ax_dyn, bar, geo + e * 7 * (int64_t)Np, (unsigned)(6 * Np * sizeof(double)));
     }
     __syncthreads();
     unsigned phase = 0;
 #pragma unroll 1
     for (; ef < nef; ef += stride) {
-        const int64_t nx = ef + stride < nef ? ef + stride : -1;
-        ax_stage_element<n1, HELM>(ef, nx, E, n, geo, lambda, u, w, phase);
+        int64_t ep = -1, fp = f;
+        if (ef + stride < nef) { ep = e + stride; while (ep >= E) { ep -= E; ++fp; } }
+        ax_stage_element<n1, HELM>(e, f, ep, fp, n, geo, lambda, u, w, phase);
+        e = ep; f = fp;
         phase ^= 1u;
     }
 }
