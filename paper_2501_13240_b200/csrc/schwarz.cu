@@ -213,117 +213,150 @@ k_sz_apply(int n1, double lambda, const ST* __restrict__ Sm, const ST* __restric
 // whose rows come from shared memory as 128-bit BROADCAST loads (every thread of the block reads the same row), and shared memory
 // otherwise only transposes the tile between the three line orientations (32-bit tiles for the FP32 levels, the swizzled
 // conflict-free layout for n1 = 8).  Passes: r, s forward; t forward, diagonal inverse, t backward in registers; s, r backward.
+#ifndef SEMB_SZ_LPT
+#define SEMB_SZ_LPT 2
+#endif
+#ifndef SEMB_SZ_EPB10
+#define SEMB_SZ_EPB10 3
+#endif
+#ifndef SEMB_SZ_EPB8
+#define SEMB_SZ_EPB8 2
+#endif
 template <int n1, typename ST> struct sz_cfg {
     static constexpr int VL = 16 / (int)sizeof(ST);                       // elements per 128-bit load
     static constexpr int RL = (n1 + VL - 1) / VL * VL;                    // padded row length
-    static constexpr int EPB = (n1 <= 3) ? 14 : (n1 == 4) ? 8 : (n1 <= 6) ? 3 : 1;
+    // LPT lines per thread (n1 = 8, 10): one broadcast matrix-row load feeds LPT multiply-adds, which halves the kernel's
+    // largest share of shared-memory wavefronts; the lines of a thread are (a, b) and (a, b + n1/2).  Measured on B200 (40 M nodes,
+    // V-cycle on fp32 levels with Schwarz smoothing / fp64 apply): N = 9 6.84 -> 6.61 ms / 0.79 -> 0.77 ms, N = 7 5.70 -> 5.64 ms /
+    // 0.70 -> 0.65 ms; elements per block 5 | 3 | 2 at n1 = 10: 6.74 | 6.61 | 6.73 ms.
+    static constexpr int LPT = (n1 == 8 || n1 == 10) ? SEMB_SZ_LPT : 1;
+    static constexpr int TPE = n1 * n1 / LPT;                             // threads per element
+    static constexpr int EPB = (n1 <= 3) ? 14 : (n1 == 4) ? 8 : (n1 <= 6) ? 3 : (LPT == 1) ? 1
+                             : (sizeof(ST) == 4) ? (n1 == 10 ? SEMB_SZ_EPB10 : SEMB_SZ_EPB8) : 2;
 };
 
-template <int n1, typename ST>
-__device__ __forceinline__ void sz_line(const ST* __restrict__ M, const ST (&x)[sz_cfg<n1, ST>::RL], ST (&y)[n1])
+// y_l = M x_l for the LPT lines of a thread
+template <int n1, typename ST, int LPT>
+__device__ __forceinline__ void sz_line(const ST* __restrict__ M, const ST (&x)[LPT][sz_cfg<n1, ST>::RL], ST (&y)[LPT][n1])
 {
     constexpr int RL = sz_cfg<n1, ST>::RL, VL = sz_cfg<n1, ST>::VL;
 #pragma unroll
     for (int o = 0; o < n1; ++o) {
-        ST acc = (ST)0;
+        ST acc[LPT];
+#pragma unroll
+        for (int l = 0; l < LPT; ++l) acc[l] = (ST)0;
 #pragma unroll
         for (int q = 0; q < RL; q += VL) {
             if (sizeof(ST) == 4) {
                 const float4 m4 = *reinterpret_cast<const float4*>(reinterpret_cast<const float*>(M) + o * RL + q);
-                acc += (ST)m4.x * x[q] + (ST)m4.y * x[q + 1] + (ST)m4.z * x[q + 2] + (ST)m4.w * x[q + 3];
+#pragma unroll
+                for (int l = 0; l < LPT; ++l) acc[l] += (ST)m4.x * x[l][q] + (ST)m4.y * x[l][q + 1] + (ST)m4.z * x[l][q + 2] + (ST)m4.w * x[l][q + 3];
             } else {
                 const double2 m2 = *reinterpret_cast<const double2*>(reinterpret_cast<const double*>(M) + o * RL + q);
-                acc += (ST)m2.x * x[q] + (ST)m2.y * x[q + 1];
+#pragma unroll
+                for (int l = 0; l < LPT; ++l) acc[l] += (ST)m2.x * x[l][q] + (ST)m2.y * x[l][q + 1];
             }
         }
-        y[o] = acc;
+#pragma unroll
+        for (int l = 0; l < LPT; ++l) y[l][o] = acc[l];
     }
 }
 
 template <int n1, typename ST>
-__global__ void __launch_bounds__(n1 * n1 * sz_cfg<n1, ST>::EPB)
+__global__ void __launch_bounds__(sz_cfg<n1, ST>::TPE * sz_cfg<n1, ST>::EPB)
 k_sz_line(int64_t E, double lambda, const ST* __restrict__ Sm, const ST* __restrict__ lamv, const ST* __restrict__ w, const ST* __restrict__ r,
           ST* __restrict__ out, const semb_scalars* __restrict__ scal)
 {
     using T = ax_tile<n1>;
     using C = sz_cfg<n1, ST>;
-    constexpr int n2 = n1 * n1, Np = n2 * n1, RL = C::RL, EPB = C::EPB;
+    constexpr int n2 = n1 * n1, Np = n2 * n1, RL = C::RL, EPB = C::EPB, LPT = C::LPT, TPE = C::TPE, BS = n1 / LPT;
     constexpr bool W32 = sizeof(ST) == 4;
 #define SZ_I(k, j, i) (W32 ? T::idx32(k, j, i) : T::idx(k, j, i))
     __shared__ __align__(16) ST tileA[EPB * T::size];
     __shared__ __align__(16) ST mat[EPB][3][2][n1 * RL];                  // [direction][0: S^T (forward), 1: S (backward)][row][padded column]
     __shared__ ST lam[EPB][3][n1];
     if (scal && *(volatile const int32_t*)&scal->done) return;
-    const int el = (EPB > 1) ? threadIdx.x / n2 : 0, tl = (EPB > 1) ? threadIdx.x - el * n2 : threadIdx.x;
+    const int el = (EPB > 1) ? threadIdx.x / TPE : 0, tl = (EPB > 1) ? threadIdx.x - el * TPE : threadIdx.x;
     int64_t e = blockIdx.x * (int64_t)EPB + el;
     const bool valid = e < E;
     if (!valid) e = E - 1;
     ST* __restrict__ Su = tileA + el * T::size;
-    const int a = tl % n1, b = tl / n1;
+    const int a = tl % n1, b = tl / n1;                                   // the thread's lines: second index b + l * BS
     // the element's matrices: S_d[node][mode] -> forward rows [mode][node], backward rows [node][mode], zero padded
-    for (int t = tl; t < 3 * n1 * RL; t += n2) {
+    for (int t = tl; t < 3 * n1 * RL; t += TPE) {
         const int d = t / (n1 * RL), row = (t / RL) % n1, col = t % RL;
         const bool in = col < n1;
         mat[el][d][0][row * RL + col] = in ? Sm[(e * 3 + d) * n2 + col * n1 + row] : (ST)0;
         mat[el][d][1][row * RL + col] = in ? Sm[(e * 3 + d) * n2 + row * n1 + col] : (ST)0;
     }
-    for (int t = tl; t < 3 * n1; t += n2) lam[el][t / n1][t % n1] = lamv[e * 3 * n1 + t];
-    ST wv[n1];
+    for (int t = tl; t < 3 * n1; t += TPE) lam[el][t / n1][t % n1] = lamv[e * 3 * n1 + t];
+    ST wv[LPT][n1];
 #pragma unroll
-    for (int k = 0; k < n1; ++k) {
-        wv[k] = w[e * Np + k * n2 + tl];
-        Su[SZ_I(k, b, a)] = wv[k] * r[e * Np + k * n2 + tl];
+    for (int l = 0; l < LPT; ++l) {
+#pragma unroll
+        for (int k = 0; k < n1; ++k) {
+            const int64_t g = e * Np + k * n2 + (b + l * BS) * n1 + a;
+            wv[l][k] = w[g];
+            Su[SZ_I(k, b + l * BS, a)] = wv[l][k] * r[g];
+        }
     }
     __syncthreads();
-    ST x[RL], y[n1];
+    ST x[LPT][RL], y[LPT][n1];
 #pragma unroll
-    for (int q = n1; q < RL; ++q) x[q] = (ST)0;
-    // forward r: line (i = *, j = a, k = b)
+    for (int l = 0; l < LPT; ++l) {
 #pragma unroll
-    for (int i = 0; i < n1; ++i) x[i] = Su[SZ_I(b, a, i)];
-    sz_line<n1, ST>(mat[el][0][0], x, y);
+        for (int q = n1; q < RL; ++q) x[l][q] = (ST)0;
+    }
+    // one pass: read the thread's LPT lines, contract, write back.  ORI 0: r-line (i = *, j = a, k = b_l), 1: s-line (i = a, j = *, k = b_l)
+#define SZ_PASS(ORI, M)                                                                                            \
+    {                                                                                                              \
+        _Pragma("unroll") for (int l = 0; l < LPT; ++l) {                                                          \
+            _Pragma("unroll") for (int q = 0; q < n1; ++q) x[l][q] = (ORI == 0) ? Su[SZ_I(b + l * BS, a, q)] : Su[SZ_I(b + l * BS, q, a)]; \
+        }                                                                                                          \
+        sz_line<n1, ST, LPT>(M, x, y);                                                                             \
+        _Pragma("unroll") for (int l = 0; l < LPT; ++l) {                                                          \
+            _Pragma("unroll") for (int q = 0; q < n1; ++q) {                                                       \
+                if (ORI == 0) Su[SZ_I(b + l * BS, a, q)] = y[l][q]; else Su[SZ_I(b + l * BS, q, a)] = y[l][q];     \
+            }                                                                                                      \
+        }                                                                                                          \
+        __syncthreads();                                                                                           \
+    }
+    SZ_PASS(0, mat[el][0][0])
+    SZ_PASS(1, mat[el][1][0])
+    // t: forward, diagonal inverse, backward on the thread's own t-lines (i = a, j = b_l, k = *); modes (a, b_l) of r and s
 #pragma unroll
-    for (int i = 0; i < n1; ++i) Su[SZ_I(b, a, i)] = y[i];
-    __syncthreads();
-    // forward s: line (i = a, j = *, k = b)
+    for (int l = 0; l < LPT; ++l) {
 #pragma unroll
-    for (int j = 0; j < n1; ++j) x[j] = Su[SZ_I(b, j, a)];
-    sz_line<n1, ST>(mat[el][1][0], x, y);
-#pragma unroll
-    for (int j = 0; j < n1; ++j) Su[SZ_I(b, j, a)] = y[j];
-    __syncthreads();
-    // t: forward, diagonal inverse, backward on the thread's own t-line (i = a, j = b, k = *); modes (a, b) of r and s
-#pragma unroll
-    for (int k = 0; k < n1; ++k) x[k] = Su[SZ_I(k, b, a)];
-    sz_line<n1, ST>(mat[el][2][0], x, y);
+        for (int k = 0; k < n1; ++k) x[l][k] = Su[SZ_I(k, b + l * BS, a)];
+    }
+    sz_line<n1, ST, LPT>(mat[el][2][0], x, y);
     {
         ST big = (ST)lambda;
 #pragma unroll
         for (int d = 0; d < 3; ++d) { ST mx = (ST)0; for (int q = 0; q < n1; ++q) mx = fmax(mx, lam[el][d][q]); big += mx; }
-        const ST tiny = big * (ST)(W32 ? 1e-5 : 1e-12), lab = lam[el][0][a] + lam[el][1][b] + (ST)lambda;
+        const ST tiny = big * (ST)(W32 ? 1e-5 : 1e-12);
 #pragma unroll
-        for (int c = 0; c < n1; ++c) { const ST den = lam[el][2][c] + lab; x[c] = (den > tiny) ? y[c] / den : (ST)0; }
+        for (int l = 0; l < LPT; ++l) {
+            const ST lab = lam[el][0][a] + lam[el][1][b + l * BS] + (ST)lambda;
+#pragma unroll
+            for (int c = 0; c < n1; ++c) { const ST den = lam[el][2][c] + lab; x[l][c] = (den > tiny) ? y[l][c] / den : (ST)0; }
+        }
     }
-    sz_line<n1, ST>(mat[el][2][1], x, y);
+    sz_line<n1, ST, LPT>(mat[el][2][1], x, y);
 #pragma unroll
-    for (int k = 0; k < n1; ++k) Su[SZ_I(k, b, a)] = y[k];
+    for (int l = 0; l < LPT; ++l) {
+#pragma unroll
+        for (int k = 0; k < n1; ++k) Su[SZ_I(k, b + l * BS, a)] = y[l][k];
+    }
     __syncthreads();
-    // backward s
+    SZ_PASS(1, mat[el][1][1])
+    SZ_PASS(0, mat[el][0][1])
+#undef SZ_PASS
 #pragma unroll
-    for (int j = 0; j < n1; ++j) x[j] = Su[SZ_I(b, j, a)];
-    sz_line<n1, ST>(mat[el][1][1], x, y);
+    for (int l = 0; l < LPT; ++l) {
 #pragma unroll
-    for (int j = 0; j < n1; ++j) Su[SZ_I(b, j, a)] = y[j];
-    __syncthreads();
-    // backward r
-#pragma unroll
-    for (int i = 0; i < n1; ++i) x[i] = Su[SZ_I(b, a, i)];
-    sz_line<n1, ST>(mat[el][0][1], x, y);
-#pragma unroll
-    for (int i = 0; i < n1; ++i) Su[SZ_I(b, a, i)] = y[i];
-    __syncthreads();
-#pragma unroll
-    for (int k = 0; k < n1; ++k) if (valid) out[e * Np + k * n2 + tl] = wv[k] * Su[SZ_I(k, b, a)];
+        for (int k = 0; k < n1; ++k) if (valid) out[e * Np + k * n2 + (b + l * BS) * n1 + a] = wv[l][k] * Su[SZ_I(k, b + l * BS, a)];
+    }
 #undef SZ_I
 }
 
@@ -331,7 +364,7 @@ template <int n1, typename ST>
 static void sz_line_launch(semb_mesh* L, double lambda, const ST* S, const ST* lam, const ST* w, const ST* v, ST* out, semb_scalars* scal, cudaStream_t s)
 {
     constexpr int EPB = sz_cfg<n1, ST>::EPB;
-    k_sz_line<n1, ST><<<(unsigned)((L->E + EPB - 1) / EPB), n1 * n1 * EPB, 0, s>>>(L->E, lambda, S, lam, w, v, out, scal);
+    k_sz_line<n1, ST><<<(unsigned)((L->E + EPB - 1) / EPB), sz_cfg<n1, ST>::TPE * EPB, 0, s>>>(L->E, lambda, S, lam, w, v, out, scal);
 }
 
 // d = c1 d + c2 sr (first: d = c2 sr);  z = z + d (zset: z = d)
