@@ -295,6 +295,21 @@ SEMB_API int semb_field_minmax_hist(const semb_field_desc* f, int nbins, double 
 SEMB_API int semb_vector_magnitude_minmax_hist(const semb_field_desc* vx, const semb_field_desc* vy, const semb_field_desc* vz,
                                       int nbins, double lo, double hi, double* minmax_dev, uint64_t* hist_dev, void* stream);
 
+/* The same consumer for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): semb_field_minmax_hist with identical arguments and bit-identical results, but the call allocates NOTHING -- no
+ * cudaMalloc, cudaFree, cudaMemset or allocating library routine -- and the outputs are written once, with their final values, by
+ * the last thread block to finish.  Its accumulators (order-encoded min / max words, 64-bit bin counters, completion ticket) live
+ * in one file-scope device array of 8 + SEMB_NOALLOC_MAX_BINS 64-bit words = 32 832 bytes, which every GPU that loads the
+ * library holds until the process exits.  Limit: nbins <= SEMB_NOALLOC_MAX_BINS, else SEMB_EINVAL (the message names the limit).
+ * Every call SHARES that array: each call clears it with a launch of its own first, so calls ordered on one stream (or by events)
+ * are independent, but calls that OVERLAP on the GPU -- different streams or host threads with no ordering -- race on it and give
+ * wrong counts.  One array per device: calls on different GPUs do not interact.  Asynchronous on stream (3-4 launches). */
+#define SEMB_NOALLOC_MAX_BINS 4096
+SEMB_API int semb_field_minmax_hist_noalloc(const semb_field_desc* f, int nbins, double lo, double hi,
+                                   double* minmax_dev, uint64_t* hist_dev, void* stream);
+/* Message of the last error of semb_field_minmax_hist_noalloc on the calling thread ("" if none).  Owned by the library. */
+SEMB_API const char* semb_noalloc_last_error(void);
+
 /* ---- in-situ IMAGE consumer (§5.3: the overview scene = "two slices on the walls,
  * two vertical slices in the background and an isocontour", 4096 pixels on the longest side, 2048 on the other).
  * The paper renders with ASCENT / VTK-m; no graphics API exists here, so the primitives are CUDA kernels on the mesh of

@@ -21,7 +21,8 @@ ERRORS = {-1: "SEMB_EINVAL", -2: "SEMB_ENOMEM", -3: "SEMB_ECUDA", -4: "SEMB_EGEO
 SYMBOLS = ["semb_gll", "semb_setup", "semb_destroy", "semb_last_error", "semb_mesh_info", "semb_apply_axhelm",
            "semb_set_geometry_mode", "semb_gather_scatter", "semb_apply_mask", "semb_assemble_rhs", "semb_apply_operator", "semb_jacobi_diag",
            "semb_pcg_solve", "semb_step_solve", "semb_mg_vcycle", "semb_mg_transfer", "semb_mg_level_size", "semb_estimate_lmax", "semb_cheb_jacobi", "semb_schwarz_apply", "semb_publish_field", "semb_publish_state",
-           "semb_export_field", "semb_field_minmax_hist", "semb_vector_magnitude_minmax_hist", "semb_gradient", "semb_weak_divergence", "semb_flow_explicit_terms", "semb_boussinesq_step", "semb_colormap_apply", "semb_image_slice", "semb_image_isosurface", "semb_apply_axhelm_host", "semb_pcg_solve_host", "semb_read_device", "semb_stream_probe", "semb_version"]
+           "semb_export_field", "semb_field_minmax_hist", "semb_vector_magnitude_minmax_hist", "semb_gradient", "semb_weak_divergence", "semb_flow_explicit_terms", "semb_boussinesq_step", "semb_colormap_apply", "semb_image_slice", "semb_image_isosurface", "semb_apply_axhelm_host", "semb_pcg_solve_host", "semb_read_device", "semb_stream_probe", "semb_version",
+           "semb_field_minmax_hist_noalloc", "semb_noalloc_last_error"]
 
 
 class SembError(RuntimeError):
@@ -474,3 +475,17 @@ def field_minmax_hist(desc, nbins, lo, hi, minmax_dev, hist_dev):
                                       _dp(hist_dev), _stream())
     if rc:
         raise SembError(rc, "semb_field_minmax_hist")
+
+
+NOALLOC_MAX_BINS = 4096          # include/semb200.h: SEMB_NOALLOC_MAX_BINS
+
+
+def field_minmax_hist_noalloc(desc, nbins, lo, hi, minmax_dev, hist_dev):
+    """field_minmax_hist through the entry point that allocates nothing (static device scratch, nbins <= NOALLOC_MAX_BINS;
+    calls that overlap on the GPU race on that scratch: include/semb200.h)."""
+    L = lib()
+    L.semb_noalloc_last_error.restype = C.c_char_p
+    rc = L.semb_field_minmax_hist_noalloc(C.byref(desc), C.c_int(nbins), C.c_double(lo), C.c_double(hi), _dp(minmax_dev),
+                                          _dp(hist_dev), _stream())
+    if rc:
+        raise SembError(rc, L.semb_noalloc_last_error().decode())
