@@ -76,6 +76,7 @@ int semb_destroy(semb_handle h)
     for (auto& en : h->dinvs) semb_dev_free(h, en.d);
     semb_dev_free(h, h->diagA); semb_dev_free(h, h->diagB);
     semb_dev_free(h, h->work); semb_dev_free(h, h->partials); semb_dev_free(h, h->ax_dot); semb_dev_free(h, h->scal); semb_dev_free(h, h->hist_dev); semb_dev_free(h, h->stage);
+    semb_dev_free(h, h->pp_noff); semb_dev_free(h, h->pp_rlist); semb_dev_free(h, h->pp_msk); semb_dev_free(h, h->pp_part);
     if (h->scal_host) cudaFreeHost(h->scal_host);
     for (cudaEvent_t ev : h->prof_ev) cudaEventDestroy(ev);
     for (auto& f : h->fields) if (f.derived) semb_dev_free(h, f.ptr);

@@ -11,6 +11,7 @@
 
 #include <cooperative_groups.h>
 
+#include <cstdlib>
 #include "reduce.cuh"
 #include "semb_internal.h"
 
@@ -718,6 +719,18 @@ int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* 
     // small meshes: two launches per iteration instead of five (k_iter_small)
     const bool small = n <= SEMB_SMALL_N && o->precond <= 1 && !o->profile;
     const int64_t ndot = small ? semb_axhelm_dot_count(h) : 0;
+    // ... and where one block per element fits on the device at once, the whole loop is ONE cooperative launch (pcg_persist.cu)
+    const char* persist_env = getenv("SEMB_PCG_PERSIST");          // "0": keep the launch-per-phase loop (A/B runs, tests of that path)
+    const bool persist_on = persist_env ? atoi(persist_env) != 0 : true;
+    if (small && persist_on && !finished) {
+        rc = semb_pcg_persist_run(h, o->lambda, m, o->dirichlet_tags, dz, r, x, p, q, hist, want_hist, s);
+        if (rc < 0) return rc;
+        if (rc == 1) {
+            SEMB_CUDA(h, cudaMemcpyAsync(h->scal_host, h->scal, sizeof(semb_scalars), cudaMemcpyDeviceToHost, s));
+            SEMB_CUDA(h, cudaStreamSynchronize(s));
+            finished = true;
+        }
+    }
     for (int it0 = 0; it0 < o->maxit && !finished; it0 += check) {
         const int mbatch = (o->maxit - it0 < check) ? o->maxit - it0 : check;
         for (int i = 0; i < mbatch; ++i) {

@@ -85,6 +85,9 @@ struct semb_mesh {
     semb_scalars* scal = nullptr;       // device
     semb_scalars* scal_host = nullptr;  // pinned mirror
     double* hist_dev = nullptr; int hist_cap = 0;
+    // persistent small-mesh PCG (pcg_persist.cu): remote-copy lists of the shared nodes, Dirichlet flags of the last tag set, per-block partials + barrier
+    int32_t* pp_noff = nullptr; int32_t* pp_rlist = nullptr; int pp_maxcnt = 0;
+    unsigned char* pp_msk = nullptr; double* pp_part = nullptr; uint32_t pp_msk_tags = 0; bool pp_msk_valid = false;
     double* stage = nullptr;            // device staging of the *_host entry points [2][n]
     int64_t launches = 0;               // kernels launched through this handle (bench.py reports it)
     std::vector<cudaEvent_t> prof_ev;   // event pairs around axhelm launches (opts.profile)
@@ -125,6 +128,10 @@ int semb_setup_geo(semb_mesh* h, const double* x, const double* y, const double*
 int semb_setup_numbering(semb_mesh* h, const double* x, const double* y, const double* z,
                          const double* period, const int32_t* gid_in, cudaStream_t s);
 int semb_get_mask(semb_mesh* h, uint32_t tags, semb_mask_entry* out, cudaStream_t s);
+// Jacobi / unpreconditioned PCG iterations of a small mesh in ONE cooperative launch, from the state k_pcg_init left (r, scal).
+// Returns 1 if launched (scal->done is then set by the kernel), 0 if the mesh is not eligible, < 0 on error.
+int semb_pcg_persist_run(semb_mesh* h, double lambda, const semb_mask_entry& m, uint32_t tags, const double* dinv, double* r, double* x, double* p,
+                         double* q, double* hist, int hist_cap, cudaStream_t s);
 int semb_get_dinv(semb_mesh* h, double lambda, uint32_t tags, double** out, cudaStream_t s);
 int semb_diag_local(semb_mesh* h, double lambda, double* d, cudaStream_t s);
 
