@@ -722,7 +722,7 @@ int semb_pcg_run(semb_mesh* h, const semb_pcg_opts* o, const double* b, double* 
     // ... and where one block per element fits on the device at once, the whole loop is ONE cooperative launch (pcg_persist.cu)
     const char* persist_env = getenv("SEMB_PCG_PERSIST");          // "0": keep the launch-per-phase loop (A/B runs, tests of that path)
     const bool persist_on = persist_env ? atoi(persist_env) != 0 : true;
-    if (small && persist_on && !finished) {
+    if (persist_on && o->precond <= 1 && !o->profile && !finished) {        // eligibility (elements, residency) is decided in there
         rc = semb_pcg_persist_run(h, o->lambda, m, o->dirichlet_tags, dz, r, x, p, q, hist, want_hist, s);
         if (rc < 0) return rc;
         if (rc == 1) {

@@ -311,7 +311,9 @@ int semb_pcg_persist_run(semb_mesh* h, double lambda, const semb_mask_entry& m, 
                          double* q, double* hist, int hist_cap, cudaStream_t s)
 {
     const int64_t n = h->n, E = h->E;
-    if (h->geo_mode != 0 || h->n1 < 3) return 0;                         // stored fp64 factors; blocks of at least 9 threads
+    // stored fp64 factors; blocks of at least 16 threads; a barrier over at most 768 blocks (measured on B200, ~30 000-node boxes:
+    // N = 3, 512 elements 21.8 -> 14.8 us per iteration, N = 2, 1000 elements 23.8 -> 51 us: those stay on the launch-per-phase loop)
+    if (h->geo_mode != 0 || h->n1 < 4 || E > 768) return 0;
     if (!h->pp_noff) {
         int rc = ax_upload_basis_tu(h); if (rc) return rc;               // this translation unit's copy of the constant tables
         rc = pp_build_lists(h, s); if (rc) return rc;
