@@ -689,6 +689,31 @@ def main():
                 "note": "axhelm (72 B/node) + stand-alone gather-scatter on 3 fields; working set about the size of L2"}
         G1.close(); del U, Wv
 
+    # ---- configs[0] (64 elements, N = 7, 32 768 nodes): the latency regime.  One persistent cooperative kernel runs the whole solve
+    #      (csrc/pcg_persist.cu); SEMB_PCG_PERSIST=0 selects the launch-per-phase loop for comparison.
+    cfg0 = None
+    if not args.no_cfg1 and single:
+        m0, _ = I.config_mesh(0, lambda N: semb.gll(N)[0])
+        G0 = semb.Mesh(m0.E, m0.N, *(torch.from_numpy(a).cuda() for a in (m0.x, m0.y, m0.z)), m0.face_tag, m0.period)
+        f0 = torch.from_numpy(I.uniform(I.seed_for(0, 2), m0.n)).cuda(); b0 = torch.empty_like(f0); G0.assemble_rhs(f0, b0, 0b10)
+        x0 = torch.zeros_like(b0)
+        cfg0 = {"local_nodes": m0.n, "elements": m0.E, "N": m0.N}
+        for key, env in (("launch_per_phase", "0"), ("persistent_kernel", "1")):
+            os.environ["SEMB_PCG_PERSIST"] = env
+            G0.pcg_solve(b0, x0, tags=0b10, precond=1, rtol=0.0, maxit=20, check_every=20)
+            x0.zero_()
+            t0 = timed(torch, lambda: G0.pcg_solve(b0, x0, tags=0b10, precond=1, rtol=0.0, maxit=500, check_every=500), 1)
+            x0.zero_()
+            e0_, e1_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize(); e0_.record()
+            st0 = G0.pcg_solve(b0, x0, tags=0b10, precond=1, rtol=1e-10, maxit=5000)
+            e1_.record(); torch.cuda.synchronize()
+            cfg0[key] = {"us_per_iteration": 1e3 * t0 / 500,
+                         "solve_to_1e-10": {"iters": st0["iters"], "ms": e0_.elapsed_time(e1_), "launches": st0["launches"]}}
+            x0.zero_()
+        os.environ.pop("SEMB_PCG_PERSIST", None)
+        G0.close(); del f0, b0, x0
+
     # ---- end to end through the C ABI with HOST buffers (pinned): b H2D, K iterations, x D2H
     e2e = e2e_single = None
     if not args.no_e2e:
@@ -789,6 +814,7 @@ def main():
         "export": export,
         "image_consumer": images,
         "cfg1_batched_axhelm_gs": cfg1,
+        "cfg0_small_mesh_pcg": cfg0,
         "geometry_modes": geo_modes,
         "configs": configs,
         "cfg4_ten_steps": steps10,

@@ -17,6 +17,8 @@
 
 #include "axhelm_launch.cuh"
 
+#define PP_FACE   (1 << 28)
+#define PP_SHARED (1 << 29)
 #define PP_CH 10          // remote copies a thread fetches per batch: one batch covers 10 n1^2 entries (a hexahedron inside a box mesh needs ~9 n1^2)
 
 struct pp_args {
@@ -34,6 +36,28 @@ struct pp_args {
 // Measured and rejected on B200 (configs[0], 64 blocks): publishing each partial in self-validating {phase : half of the double}
 // words that all threads poll, so that the poll is the data load (one round trip instead of three): 15.4 -> 18.8 us per
 // iteration -- 4096 polling threads delay the very stores they wait for.
+// K block-wide sums with one pair of barriers (block_sum of reduce.cuh, K values at a time; the same fixed order per value)
+template <int K>
+__device__ __forceinline__ void pp_block_sum(double (&v)[K], double* red)
+{
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    const int live = min(32, (int)blockDim.x - (wid << 5));
+#pragma unroll
+    for (int k = 0; k < K; ++k) v[k] = warp_sum_live(v[k], lane, live);
+    __syncthreads();                       // red may still be read from a previous call
+    if (lane == 0) {
+#pragma unroll
+        for (int k = 0; k < K; ++k) red[k * 32 + wid] = v[k];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        double t = 0.0;
+        for (int w = 0; w < nw; ++w) t += red[k * 32 + w];
+        v[k] = t;
+    }
+}
+
 template <int K>
 __device__ __forceinline__ void pp_allsum(double* part, unsigned* bar, int64_t E, const double (&v)[K], double (&tot)[K], unsigned phase, double* red)
 {
@@ -56,8 +80,9 @@ __device__ __forceinline__ void pp_allsum(double* part, unsigned* bar, int64_t E
 #pragma unroll
         for (int k = 0; k < K; ++k) s[k] += __ldcg(part + k * E + t);
     }
+    pp_block_sum<K>(s, red);
 #pragma unroll
-    for (int k = 0; k < K; ++k) tot[k] = block_sum(s[k], red);
+    for (int k = 0; k < K; ++k) tot[k] = s[k];
 }
 
 template <int n1, bool HELM>
@@ -71,8 +96,8 @@ k_pcg_persist(pp_args A)
     double* __restrict__ Su = Gs + NG * Np;
     double* __restrict__ Sr = Su + T::sizeA;
     double* __restrict__ Ss = Sr + T::sizeA;
-    double* red = Ss + T::sizeB;                           // 32 doubles
-    double* __restrict__ Sg = red + 32;                    // the remote copies this element needs in the assembly (<= max over elements)
+    double* red = Ss + T::sizeB;                           // 2 x 32 doubles
+    double* __restrict__ Sg = red + 64;                    // the remote copies this element needs in the assembly (<= max over elements)
     semb_scalars* __restrict__ scal = A.scal;
     if (*(volatile const int32_t*)&scal->done) return;     // set before the launch only (k_pcg_init): uniform over the grid
     const int tl = threadIdx.x, a = tl % n1, b = tl / n1;
@@ -92,7 +117,8 @@ k_pcg_persist(pp_args A)
         }
     }
     double r[n1], p[n1], x[n1], dv[n1];
-    int32_t cd[n1], pos[n1];                               // pos: start of the node's entries in Sg | number of entries << 20
+    double wq[n1];                                         // 1 / multiplicity: weight of the node in sums over local nodes
+    int32_t pos[n1];                                       // start of the node's entries in Sg | number of entries << 20 | PP_FACE | PP_SHARED
     unsigned mbits = 0u;
     const int32_t ebase = __ldg(A.noff + e * Np), ecnt = __ldg(A.noff + (e + 1) * Np) - ebase;
 #pragma unroll
@@ -100,10 +126,11 @@ k_pcg_persist(pp_args A)
         const int64_t l = l0 + k * n2;
         r[k] = A.r[l]; x[k] = A.x[l]; p[k] = 0.0;
         dv[k] = A.dinv ? A.dinv[l] : 1.0;
-        cd[k] = A.code[l];
+        const int32_t cd = A.code[l];
+        wq[k] = (cd <= -2) ? 0.5 : (cd >= 3) ? 1.0 / (double)cd : 1.0;
         const int32_t n0 = __ldg(A.noff + l), nn = __ldg(A.noff + l + 1) - n0;
-        pos[k] = (n0 - ebase) | (nn << 20);
-        if (A.msk[l]) { mbits |= 1u << k; pos[k] = 0; }    // Dirichlet node: w = 0 and nothing is added
+        pos[k] = (n0 - ebase) | (nn << 20) | (cd <= -2 ? PP_FACE : 0) | (cd != -1 ? PP_SHARED : 0);
+        if (A.msk[l]) { mbits |= 1u << k; pos[k] &= PP_SHARED; }    // Dirichlet node: w = 0 is published, nothing is added
     }
     double rho = scal->rho_new, beta = 0.0, alpha = 0.0, pAp = 0.0, rnorm = scal->rnorm, trr = scal->rr;
     const double target = scal->target, lambda = A.lambda;
@@ -169,7 +196,7 @@ k_pcg_persist(pp_args A)
             w[k] += Sr[T::idx(k, b, a)] + Ss[T::idxB(k, b, a)];
             dot += p[k] * w[k];                            // p is continuous and zero at Dirichlet nodes: sum over elements = p.Ap
             if (mbits >> k & 1u) w[k] = 0.0;               // Dirichlet mask before the assembly
-            if (cd[k] != -1) __stcg(A.q + l0 + k * n2, w[k]);
+            if (pos[k] & PP_SHARED) __stcg(A.q + l0 + k * n2, w[k]);
         }
         {
             const double v[1] = { block_sum(dot, red) };
@@ -195,9 +222,9 @@ k_pcg_persist(pp_args A)
         __syncthreads();
 #pragma unroll
         for (int k = 0; k < n1; ++k) {
-            const int st = pos[k] & 0xfffff, cnt = pos[k] >> 20;
+            const int st = pos[k] & 0xfffff, cnt = (pos[k] >> 20) & 0xff;
             if (cnt) {
-                double c = (cd[k] <= -2) ? w[k] : 0.0;     // face: own + partner;  class: its members in list order, the same bits in every copy
+                double c = (pos[k] & PP_FACE) ? w[k] : 0.0;     // face: own + partner;  class: its members in list order, the same bits in every copy
                 for (int u = 0; u < cnt; ++u) c += Sg[st + u];
                 w[k] = c;
             }
@@ -205,15 +232,15 @@ k_pcg_persist(pp_args A)
         double rr = 0.0, rz = 0.0;
 #pragma unroll
         for (int k = 0; k < n1; ++k) {
-            const double wq = (cd[k] <= -2) ? 0.5 : (cd[k] >= 3) ? 1.0 / (double)cd[k] : 1.0;
             x[k] += alpha * p[k];
             r[k] -= alpha * w[k];
-            const double t = r[k] * r[k] * wq;
+            const double t = r[k] * r[k] * wq[k];
             rr += t; rz += dv[k] * t;
         }
         double trz;
         {
-            const double v[2] = { block_sum(rr, red), block_sum(rz, red) };
+            double v[2] = { rr, rz };
+            pp_block_sum<2>(v, red);
             double tot[2];
             pp_allsum<2>(partB, A.bar, E, v, tot, ++phase, red);
             trr = tot[0]; trz = tot[1];
@@ -244,7 +271,7 @@ static __global__ void k_pp_mask(int64_t count, const int32_t* __restrict__ list
 template <int n1> static size_t pp_smem(bool helm, int maxcnt)
 {
     using T = ax_tile<n1>;
-    return sizeof(double) * ((size_t)(helm ? 7 : 6) * n1 * n1 * n1 + 2 * T::sizeA + T::sizeB + 32 + (size_t)maxcnt);
+    return sizeof(double) * ((size_t)(helm ? 7 : 6) * n1 * n1 * n1 + 2 * T::sizeA + T::sizeB + 64 + (size_t)maxcnt);
 }
 
 // 1: launched;  0: not eligible (the caller runs the launch-per-phase loop);  < 0: error
@@ -294,6 +321,7 @@ static int pp_build_lists(semb_mesh* h, cudaStream_t s)
     int maxcnt = 0;
     for (int64_t e = 0; e < h->E; ++e) { const int c = noff[(e + 1) * Np] - noff[e * Np]; if (c > maxcnt) maxcnt = c; }
     if (maxcnt >= (1 << 20)) return semb_fail(h, SEMB_EINVAL, "persistent PCG: %d remote copies in one element", maxcnt);
+    for (int64_t l = 0; l < n; ++l) if (code[l] > 255) { h->pp_maxcnt = -1; return SEMB_OK; }      // a class of more than 255 copies: not eligible
     h->pp_maxcnt = maxcnt;
     h->pp_noff = (int32_t*)semb_dev_alloc(h, sizeof(int32_t) * ((size_t)n + 1));
     h->pp_rlist = (int32_t*)semb_dev_alloc(h, sizeof(int32_t) * rl.size());
@@ -314,10 +342,11 @@ int semb_pcg_persist_run(semb_mesh* h, double lambda, const semb_mask_entry& m, 
     // stored fp64 factors; blocks of at least 16 threads; a barrier over at most 768 blocks (measured on B200, ~30 000-node boxes:
     // N = 3, 512 elements 21.8 -> 14.8 us per iteration, N = 2, 1000 elements 23.8 -> 51 us: those stay on the launch-per-phase loop)
     if (h->geo_mode != 0 || h->n1 < 4 || E > 768) return 0;
-    if (!h->pp_noff) {
+    if (!h->pp_noff && h->pp_maxcnt >= 0) {
         int rc = ax_upload_basis_tu(h); if (rc) return rc;               // this translation unit's copy of the constant tables
         rc = pp_build_lists(h, s); if (rc) return rc;
     }
+    if (h->pp_maxcnt < 0) return 0;
     if (!h->pp_msk_valid || h->pp_msk_tags != tags) {
         SEMB_CUDA(h, cudaMemsetAsync(h->pp_msk, 0, (size_t)n, s));
         if (m.count > 0) k_pp_mask<<<(unsigned)((m.count + 255) / 256), 256, 0, s>>>(m.count, m.list, h->pp_msk);
