@@ -66,6 +66,7 @@ int semb_destroy(semb_handle h)
     cudaDeviceSynchronize();
     semb_mg_destroy_all(h);
     semb_schwarz_free(h);
+    semb_coarse_free(h);
     semb_dev_free(h, h->xyz);
     semb_dev_free(h, h->geo); semb_dev_free(h, h->gid); semb_dev_free(h, h->invmult); semb_dev_free(h, h->gs_code); semb_dev_free(h, h->gs_hi);
     if (h->geoK && h->geoK != h->geo) semb_dev_free(h, h->geoK);

@@ -355,7 +355,11 @@ int semb_mg_vcycle_run(semb_mesh* h, const semb_mg_ctx& ctx, int l, const double
     double *cres = g->W[l][0], *cd = g->W[l][1], *cAd = g->W[l][2], *res = g->W[l][3], *t1 = g->W[l][4];
     const int64_t l0 = L->launches;
     if (l == g->nlevels - 1) {
-        rc = semb_cheb_apply(L, ctx.lambda, m, dinv, ctx.k_coarse, semb_cheb_coefficients(ctx.k_coarse, ctx.lmax[l], ctx.kind, ctx.coarse_frac), r, z, cres, cd, cAd, scal, false, s);
+        const semb_cheb_coef cl = semb_cheb_coefficients(ctx.k_coarse, ctx.lmax[l], ctx.kind, ctx.coarse_frac);
+        semb_coarse* ca = nullptr;
+        rc = semb_coarse_get(L, &ca, s); if (rc) return rc;
+        if (ca) rc = semb_coarse_cheb(L, ca, ctx.lambda, ctx.tags, m, dinv, ctx.k_coarse, cl, r, z, scal, s);       // assembled operator: one launch per step
+        else rc = semb_cheb_apply(L, ctx.lambda, m, dinv, ctx.k_coarse, cl, r, z, cres, cd, cAd, scal, false, s);
         if (L != h) { h->launches += L->launches - l0; }
         return rc;
     }
@@ -456,8 +460,11 @@ static int mg_vcycle_f32(semb_mesh* h, const semb_mg_ctx& ctx, int l, const floa
     float *cres = g->WF[l][0], *cd = g->WF[l][1], *cAd = g->WF[l][2], *res = g->WF[l][3], *t1 = g->WF[l][4];
     const int64_t l0 = L->launches;
     if (l == g->nlevels - 1) {
-        rc = semb_cheb_apply_f(L, ctx.lambda, geo, m, dinv, ctx.k_coarse, semb_cheb_coefficients(ctx.k_coarse, ctx.lmax[l], ctx.kind, ctx.coarse_frac),
-                               r, z, cres, cd, cAd, scal, s, false);
+        const semb_cheb_coef cl = semb_cheb_coefficients(ctx.k_coarse, ctx.lmax[l], ctx.kind, ctx.coarse_frac);
+        semb_coarse* ca = nullptr;
+        rc = semb_coarse_get(L, &ca, s); if (rc) return rc;
+        if (ca) rc = semb_coarse_cheb_f(L, ca, ctx.lambda, ctx.tags, m, dinv, ctx.k_coarse, cl, r, z, scal, s);
+        else rc = semb_cheb_apply_f(L, ctx.lambda, geo, m, dinv, ctx.k_coarse, cl, r, z, cres, cd, cAd, scal, s, false);
         if (L != h) h->launches += L->launches - l0;
         return rc;
     }

@@ -39,6 +39,7 @@ struct semb_field_entry {
 
 struct semb_mg;
 struct semb_schwarz;
+struct semb_coarse;
 
 struct semb_mesh {
     int64_t E = 0; int N = 0, n1 = 0; int64_t Np = 0, n = 0;
@@ -93,6 +94,7 @@ struct semb_mesh {
     std::vector<cudaEvent_t> prof_ev;   // event pairs around axhelm launches (opts.profile)
     std::vector<semb_mg*> mgs;          // p-multigrid hierarchies built so far (mg.cu), owned
     std::vector<semb_schwarz*> schwarz; // Schwarz subdomain data of this (level) mesh per Dirichlet tag set (schwarz.cu), owned
+    semb_coarse* coarse = nullptr;      // assembled operator of this mesh when it is the order-1 last level of a multigrid hierarchy (coarse.cu), owned
     // export
     std::vector<semb_field_entry> fields;
     int64_t cycle = 0; double time = 0.0;
@@ -202,6 +204,14 @@ int semb_mg_vcycle_run(semb_mesh* h, const semb_mg_ctx& ctx, int level, const do
 int semb_mg_transfer_run(semb_mesh* h, const semb_mg_ctx& ctx, int level, int restrict_, const double* in, double* out, cudaStream_t s);
 int64_t semb_mg_level_n(const semb_mg_ctx& ctx, int level);
 void semb_mg_destroy_all(semb_mesh* h);
+
+// ---- coarse.cu: the order-1 last level on its assembled operator (one launch per Chebyshev step)
+void semb_coarse_free(semb_mesh* L);
+int semb_coarse_get(semb_mesh* L, semb_coarse** out, cudaStream_t s);       // *out = NULL: not eligible, stay matrix-free
+int semb_coarse_cheb(semb_mesh* L, semb_coarse* c, double lambda, uint32_t tags, const semb_mask_entry& m, const double* dinv, int k,
+                     const semb_cheb_coef& cf, const double* r, double* z, semb_scalars* scal, cudaStream_t s);
+int semb_coarse_cheb_f(semb_mesh* L, semb_coarse* c, double lambda, uint32_t tags, const semb_mask_entry& m, const float* dinv, int k,
+                       const semb_cheb_coef& cf, const float* r, float* z, semb_scalars* scal, cudaStream_t s);
 
 // ---- schwarz.cu: overlapping Schwarz smoother of the multigrid levels (reading R26)
 void semb_schwarz_free(semb_mesh* L);
