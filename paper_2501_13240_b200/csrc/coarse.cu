@@ -9,6 +9,9 @@
 // k_c + 2 launches per V-cycle instead of 4 k_c + 1.  The element matrices are what the level's own operator kernel returns for the
 // eight unit vectors, so the assembled operator IS the matrix-free one up to the order of the sums.  Vectors and matrix entries
 // are stored in the level's storage type (float with mg_fp32, R21), the arithmetic is fp64.
+// Measured on B200 (V-cycle, k_c = 64): 32^3-element box 2.99 -> 2.15 ms (fp64 levels), 2.32 -> 1.60 ms (FP32 levels), a coarse step
+// 19.3 / 17.5 -> 6.1 us; cfg2 O-grid 5.57 -> 4.34 ms and 3.87 -> 2.97 ms.  Measured and rejected: all k_c steps in ONE cooperative
+// launch with a grid barrier per step (1124 blocks): 6.15-6.45 us per step -- the barrier costs what the launch gap did.
 #include <cstdlib>
 #include <vector>
 

@@ -249,3 +249,48 @@ def test_fp32_storage_levels(torch_cuda, cases, orc, name):
     assert normwise(xg, ro["x"]) <= 2e-7
     res = b - P.apply_A(xg)
     assert np.sqrt(P.dot(res, res)) <= 2e-10 * np.sqrt(P.dot(b, b))
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_last_level_assembled_operator_against_matrix_free(torch_cuda, cases, orc, name):
+    """csrc/coarse.cu: the order-1 last level works on its assembled operator (one launch per Chebyshev step).  The element matrices
+    come from the level's own operator kernel, so the two forms are the same operator up to the order of the sums: V-cycles agree
+    to rounding (fp64 levels 1e-12; FP32 levels: both within the 2e-6 of reading R21 of the oracle, and 2e-6 of each other), also
+    after the Dirichlet tag set changes on the same hierarchy.  SEMB_MG_COARSE_ASSEMBLED=0 keeps the matrix-free form."""
+    import os
+    torch = torch_cuda
+    m, mg, G, orders, lam, tags = cases(name)
+    P = mg.levels[0]
+    r = dev(torch, cont(orc, P, 61))
+    out = {}
+    for fp32 in (False, True):
+        for env in ("0", "1"):
+            os.environ["SEMB_MG_COARSE_ASSEMBLED"] = env
+            try:
+                z = torch.empty(P.n, dtype=torch.float64, device="cuda")
+                G.mg_vcycle(r, z, lam, tags, orders, 2, 32, mg.lmax, mg_coarse_frac=0.02, mg_fp32=fp32)
+                out[(fp32, env)] = z.cpu().numpy()
+            finally:
+                os.environ.pop("SEMB_MG_COARSE_ASSEMBLED", None)
+    assert normwise(out[(False, "1")], out[(False, "0")]) <= 1e-12
+    assert normwise(out[(True, "1")], out[(True, "0")]) <= 2e-6
+    assert normwise(out[(True, "1")], out[(False, "1")]) <= 2e-6
+    # another tag set on the same hierarchy (the level's free-node flags are rebuilt), then the first one again
+    other = 0b110 if name.startswith("ogrid") else (0b10 if tags == 0 else 0)
+    if other == 0 and lam == 0.0:
+        return                                              # all-Neumann Poisson is singular: covered by the null_mean tests
+    Po = orc.Problem(m.E, m.N, m.x, m.y, m.z, m.face_tag, m.period, lam=lam, dirichlet_tags=other)
+    ro = dev(torch, cont(orc, Po, 62))
+    zz = {}
+    for env in ("0", "1"):
+        os.environ["SEMB_MG_COARSE_ASSEMBLED"] = env
+        try:
+            z = torch.empty(P.n, dtype=torch.float64, device="cuda")
+            G.mg_vcycle(ro, z, lam, other, orders, 2, 32, None, mg_coarse_frac=0.02)
+            zz[env] = z.cpu().numpy()
+        finally:
+            os.environ.pop("SEMB_MG_COARSE_ASSEMBLED", None)
+    assert normwise(zz["1"], zz["0"]) <= 1e-12 and np.all(zz["1"][Po.mask == 0] == 0)
+    z = torch.empty(P.n, dtype=torch.float64, device="cuda")
+    G.mg_vcycle(r, z, lam, tags, orders, 2, 32, mg.lmax, mg_coarse_frac=0.02)
+    assert np.array_equal(z.cpu().numpy(), out[(False, "1")])
