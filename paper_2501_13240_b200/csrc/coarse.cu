@@ -10,7 +10,7 @@
 // eight unit vectors, so the assembled operator IS the matrix-free one up to the order of the sums.  Vectors and matrix entries
 // are stored in the level's storage type (float with mg_fp32, R21), the arithmetic is fp64.
 // Measured on B200 (V-cycle, k_c = 64): 32^3-element box 2.99 -> 2.15 ms (fp64 levels), 2.32 -> 1.60 ms (FP32 levels), a coarse step
-// 19.3 / 17.5 -> 6.1 us; cfg2 O-grid 5.57 -> 4.34 ms and 3.87 -> 2.97 ms.  Measured and rejected: all k_c steps in ONE cooperative
+// 19.3 / 17.5 -> 6.1 us; cfg2 O-grid 5.57 -> 4.34 ms and 3.87 -> 2.97 ms; cfg3 (64^3 elements) pressure solve 0.344 -> 0.296 s and 0.242 -> 0.219 s.  Measured and rejected: all k_c steps in ONE cooperative
 // launch with a grid barrier per step (1124 blocks): 6.15-6.45 us per step -- the barrier costs what the launch gap did.
 #include <cstdlib>
 #include <vector>
@@ -18,7 +18,9 @@
 #include "semb_internal.h"
 
 #define CU_WMAX 64            // rows with more entries than this (a vertex shared by very many elements): the level stays matrix-free
-#define CU_EMAX 150000        // elements; the assembly runs on the host, once per level
+#ifndef CU_EMAX
+#define CU_EMAX 300000        // elements; the assembly runs on the host, once per level (262 144 elements: ~3 s)
+#endif
 
 struct semb_coarse {
     bool eligible = false;
