@@ -11,8 +11,6 @@
 // i.e. two grid-wide synchronisations per iteration, each fused with the sum it exists for (pp_allsum below); the cooperative
 // launch guarantees that all blocks are resident.  Values written by other blocks are read with ld.global.cg (L1 is not coherent).
 // All sums have a fixed order: iterates are reproducible run to run.
-#include <cooperative_groups.h>
-
 #include <vector>
 
 #include "axhelm_launch.cuh"
