@@ -87,6 +87,15 @@ k_hist(int64_t n, int64_t stride, const double* __restrict__ v, const double* __
     for (int b = threadIdx.x; b < nbins; b += blockDim.x) if (sh[b]) atomicAdd(&hist[b], (unsigned long long)sh[b]);
 }
 
+#ifndef MH_BPS
+#define MH_BPS 8           // blocks per SM of the consumer's grids
+#endif
+#ifndef MH_U1
+#define MH_U1 8
+#endif
+#ifndef MH_U3
+#define MH_U3 4
+#endif
 // One pass over the data when the range is known: min, max and the histogram together.  NV = 1: a scalar field; NV = 3: the
 // magnitude of a vector field computed on the fly, sqrt(fma(vz, vz, fma(vy, vy, vx vx))) (reading R11), never written to memory.
 template <int NV>
@@ -99,14 +108,30 @@ k_minmax_hist(int64_t n, int64_t stride, const double* __restrict__ v0, const do
     const double scale = __ddiv_rn((double)nbins, __dsub_rn(hi, lo));
     __syncthreads();
     double mn = INFINITY, mx = -INFINITY;
-    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
-        double a = v0[l * stride];
-        if (NV == 3) { const double b = v1[l * stride], c = v2[l * stride]; a = sqrt(fma(c, c, fma(b, b, __dmul_rn(a, a)))); }
-        mn = fmin(mn, a); mx = fmax(mx, a);
-        const double sc = __dmul_rn(__dsub_rn(a, lo), scale);
-        long long b = (sc < 0.0) ? 0ll : (long long)floor(sc);
-        if (b > nbins - 1) b = nbins - 1;
-        atomicAdd(&sh[b], 1u);
+    // MH_U values per thread and pass, all loads issued before the first use: with one 64-bit load in flight per thread the kernel
+    // was latency bound at 60 % of the DRAM peak (profiles/r2_consumers_flow.md)
+    constexpr int U = (NV == 3) ? MH_U3 : MH_U1;
+    for (int64_t c0 = blockIdx.x * (int64_t)(256 * U); c0 < n; c0 += (int64_t)gridDim.x * (256 * U)) {
+        double a[U], b3[NV == 3 ? U : 1], c3[NV == 3 ? U : 1];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int64_t l = c0 + u * 256 + threadIdx.x;
+            const bool ok = l < n;
+            a[u] = ok ? v0[l * stride] : 0.0;
+            if (NV == 3) { b3[u] = ok ? v1[l * stride] : 0.0; c3[u] = ok ? v2[l * stride] : 0.0; }
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            if (c0 + u * 256 + threadIdx.x < n) {
+                double x = a[u];
+                if (NV == 3) x = sqrt(fma(c3[NV == 3 ? u : 0], c3[NV == 3 ? u : 0], fma(b3[NV == 3 ? u : 0], b3[NV == 3 ? u : 0], __dmul_rn(x, x))));
+                mn = fmin(mn, x); mx = fmax(mx, x);
+                const double sc = __dmul_rn(__dsub_rn(x, lo), scale);
+                long long b = (sc < 0.0) ? 0ll : (long long)floor(sc);
+                if (b > nbins - 1) b = nbins - 1;
+                atomicAdd(&sh[b], 1u);
+            }
+        }
     }
     for (int o = 16; o > 0; o >>= 1) {
         mn = fmin(mn, __shfl_xor_sync(0xffffffffu, mn, o));
@@ -154,7 +179,7 @@ int semb_minmax_hist_launch(const double* v, const double* v1, const double* v2,
 {
     if (nbins < 1 || nbins > 8192 || n < 1 || stride < 1) return SEMB_EINVAL;
     // each block's shared counters are 32-bit: keep every block's share of the input below 2^32
-    int64_t blocks = (n + 2047) / 2048; if (blocks > semb_sm_count() * 8) blocks = semb_sm_count() * 8; if (blocks < 1) blocks = 1;
+    int64_t blocks = (n + 2047) / 2048; if (blocks > semb_sm_count() * MH_BPS) blocks = semb_sm_count() * MH_BPS; if (blocks < 1) blocks = 1;
     unsigned long long* mm = (unsigned long long*)minmax_dev;
     unsigned long long* hist = (unsigned long long*)hist_dev;
     k_mm_init<<<1, 1, 0, s>>>(mm);
