@@ -213,8 +213,11 @@ k_sz_apply(int n1, double lambda, const ST* __restrict__ Sm, const ST* __restric
 // whose rows come from shared memory as 128-bit BROADCAST loads (every thread of the block reads the same row), and shared memory
 // otherwise only transposes the tile between the three line orientations (32-bit tiles for the FP32 levels, the swizzled
 // conflict-free layout for n1 = 8).  Passes: r, s forward; t forward, diagonal inverse, t backward in registers; s, r backward.
-#ifndef SEMB_SZ_LPT
-#define SEMB_SZ_LPT 2
+#ifndef SEMB_SZ_LPT8
+#define SEMB_SZ_LPT8 2
+#endif
+#ifndef SEMB_SZ_LPT10
+#define SEMB_SZ_LPT10 2
 #endif
 #ifndef SEMB_SZ_EPB10
 #define SEMB_SZ_EPB10 3
@@ -229,7 +232,7 @@ template <int n1, typename ST> struct sz_cfg {
     // largest share of shared-memory wavefronts; the lines of a thread are (a, b) and (a, b + n1/2).  Measured on B200 (40 M nodes,
     // V-cycle on fp32 levels with Schwarz smoothing / fp64 apply): N = 9 6.84 -> 6.61 ms / 0.79 -> 0.77 ms, N = 7 5.70 -> 5.64 ms /
     // 0.70 -> 0.65 ms; elements per block 5 | 3 | 2 at n1 = 10: 6.74 | 6.61 | 6.73 ms.
-    static constexpr int LPT = (n1 == 8 || n1 == 10) ? SEMB_SZ_LPT : 1;
+    static constexpr int LPT = (n1 == 8) ? SEMB_SZ_LPT8 : (n1 == 10) ? SEMB_SZ_LPT10 : 1;
     static constexpr int TPE = n1 * n1 / LPT;                             // threads per element
     static constexpr int EPB = (n1 <= 3) ? 14 : (n1 == 4) ? 8 : (n1 <= 6) ? 3 : (LPT == 1) ? 1
                              : (sizeof(ST) == 4) ? (n1 == 10 ? SEMB_SZ_EPB10 : SEMB_SZ_EPB8) : 2;
