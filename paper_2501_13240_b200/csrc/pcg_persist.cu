@@ -325,7 +325,11 @@ static int pp_build_lists(semb_mesh* h, cudaStream_t s)
     h->pp_rlist = (int32_t*)semb_dev_alloc(h, sizeof(int32_t) * rl.size());
     h->pp_msk = (unsigned char*)semb_dev_alloc(h, (size_t)n);
     h->pp_part = (double*)semb_dev_alloc(h, sizeof(double) * (3 * (size_t)h->E + 2));
-    if (!h->pp_noff || !h->pp_rlist || !h->pp_msk || !h->pp_part) return semb_fail(h, SEMB_ENOMEM, "persistent PCG: node tables");
+    if (!h->pp_noff || !h->pp_rlist || !h->pp_msk || !h->pp_part) {
+        semb_dev_free(h, h->pp_noff); semb_dev_free(h, h->pp_rlist); semb_dev_free(h, h->pp_msk); semb_dev_free(h, h->pp_part);
+        h->pp_noff = h->pp_rlist = nullptr; h->pp_msk = nullptr; h->pp_part = nullptr;
+        return semb_fail(h, SEMB_ENOMEM, "persistent PCG: node tables");
+    }
     SEMB_CUDA(h, cudaMemcpyAsync(h->pp_noff, noff.data(), sizeof(int32_t) * ((size_t)n + 1), cudaMemcpyHostToDevice, s));
     SEMB_CUDA(h, cudaMemcpyAsync(h->pp_rlist, rl.data(), sizeof(int32_t) * rl.size(), cudaMemcpyHostToDevice, s));
     SEMB_CUDA(h, cudaStreamSynchronize(s));                              // the host vectors go out of scope
