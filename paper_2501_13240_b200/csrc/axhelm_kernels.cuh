@@ -38,6 +38,9 @@ static __constant__ double c_xi[SEMB_MAX_N + 1][SEMB_MAXN1], c_rho[SEMB_MAX_N + 
 #ifndef SEMB_AX_RELOAD_N1
 #define SEMB_AX_RELOAD_N1 10
 #endif
+#ifndef SEMB_AX_FIELD_FAST
+#define SEMB_AX_FIELD_FAST 1          // measured on B200, 3 fields: N = 7 112 -> 141 GDOF/s (Helmholtz 100 -> 137), N = 5 106 -> 123, N = 3 101 -> 157
+#endif
 #ifndef SEMB_AX_SPLIT_N1
 #define SEMB_AX_SPLIT_N1 99          // off by default until measured
 #endif
@@ -276,12 +279,16 @@ k_axhelm_line(int64_t E, int64_t n, const void* __restrict__ geo_v, double lambd
         const int rq = c_perm[n1 - 1][0][tl], sq = c_perm[n1 - 1][1][tl];
         ra = rq % n1; rb = rq / n1; sa = sq % n1; sb = sq / n1;
     }
+#if SEMB_AX_FIELD_FAST
+    const int64_t e = ef / nfields, f = ef - e * nfields;           // the fields of an element in neighbouring blocks: its factors are read from DRAM once
+#else
     const int64_t e = ef % E, f = ef / E;
+#endif
     // The element that a block pf_dist launches later will work on is pulled into L2 now: DRAM stays busy while
     // the resident blocks are in their compute phase, and that block's loads hit L2.
     if (pf_dist > 0 && tl == 0 && valid && e + pf_dist < E) {
         const int64_t ep = e + pf_dist;
-        if (STORED) ax_prefetch_l2(geo + ep * 7 * (int64_t)Np, NG * Np);
+        if (STORED && (!SEMB_AX_FIELD_FAST || f == 0)) ax_prefetch_l2(geo + ep * 7 * (int64_t)Np, NG * Np);
         if (FUSE) {
             ax_prefetch_l2(pcg.zsrc + ep * Np, Np);
             if (pcg.dinv) ax_prefetch_l2(pcg.dinv + ep * Np, Np);
@@ -510,8 +517,12 @@ __device__ __forceinline__ void ax_stage_wait(uint64_t* bar, unsigned phase)
 
 template <int n1, bool HELM>
 __device__ __noinline__ void ax_stage_element(int64_t e, int64_t f, int64_t ep, int64_t fp, int64_t n, const double* __restrict__ geo,
-                                              double lambda, const double* __restrict__ u, double* __restrict__ w, unsigned phase)
+                                              double lambda, const double* __restrict__ u, double* __restrict__ w, unsigned phase,
+                                              int do_wait, int64_t e_issue)
 {
+    // (e, f): the element and field applied now; (ep, fp): what this block applies next (its u goes to L2 now), ep < 0: nothing;
+    // do_wait: the first field of the element -- its factors may still be in flight; e_issue >= 0: the last field -- once the factor
+    // phase is over, the factors of element e_issue are copied into the buffer
     constexpr int n2 = n1 * n1, Np = n2 * n1;
     using T = ax_tile<n1>; using L = ax_stage_smem<n1>;
     extern __shared__ __align__(128) double ax_dyn[];
@@ -525,7 +536,7 @@ __device__ __noinline__ void ax_stage_element(int64_t e, int64_t f, int64_t ep, 
     }
     if (tl == 0 && ep >= 0) {                          // what the next element (ep, field fp) reads with plain loads goes to L2 now
         ax_prefetch_l2(u + fp * n + ep * Np, Np);
-        if (HELM) ax_prefetch_l2(geo + (ep * 7 + 6) * (int64_t)Np, Np);
+        if (HELM && ep != e) ax_prefetch_l2(geo + (ep * 7 + 6) * (int64_t)Np, Np);
     }
     const double* __restrict__ ue = u + f * n + e * Np + tl;
     double ut[n1];
@@ -558,7 +569,7 @@ __device__ __noinline__ void ax_stage_element(int64_t e, int64_t f, int64_t ep, 
         for (int j = 0; j < n1; ++j) Ss[T::idxB(sb, j, sa)] = out[j];
     }
     __syncthreads();
-    ax_stage_wait(bar, phase);                         // the factors of this element have landed
+    if (do_wait) ax_stage_wait(bar, phase);            // the factors of this element have landed
     double gt[n1];
 #pragma unroll
     for (int k = 0; k < n1; ++k) {
@@ -570,8 +581,8 @@ __device__ __noinline__ void ax_stage_element(int64_t e, int64_t f, int64_t ep, 
         gt[k] = Grt * ur + Gst * us + Gtt * ut[k];
     }
     __syncthreads();
-    if (tl == 0 && ep >= 0)                            // every thread is past its last read of Gs
-        ax_stage_issue(Gs, bar, geo + ep * 7 * (int64_t)Np, (unsigned)(6 * Np * sizeof(double)));
+    if (tl == 0 && e_issue >= 0)                       // every thread is past its last read of Gs
+        ax_stage_issue(Gs, bar, geo + e_issue * 7 * (int64_t)Np, (unsigned)(6 * Np * sizeof(double)));
     {
         double ln[n1], out[n1];
 #pragma unroll
@@ -597,6 +608,8 @@ __device__ __noinline__ void ax_stage_element(int64_t e, int64_t f, int64_t ep, 
     for (int k = 0; k < n1; ++k) we[k * n2] = wt[k] + Sr[T::idx(k, b, a)] + Ss[T::idxB(k, b, a)];
 }
 
+// Several fields (semb_apply_axhelm with nfields > 1, BASELINE.json configs[1]): a block applies its element to ALL fields before it
+// moves on, so the factors cross DRAM -> shared memory once per element: 48 + 16 nfields bytes per node instead of 64 nfields.
 template <int n1, bool HELM>
 __global__ void __launch_bounds__(n1 * n1, 3)
 k_axhelm_stage(int64_t E, int64_t n, const double* __restrict__ geo, double lambda, const double* __restrict__ u, double* __restrict__ w, int nfields)
@@ -605,10 +618,9 @@ k_axhelm_stage(int64_t E, int64_t n, const double* __restrict__ geo, double lamb
     using L = ax_stage_smem<n1>;
     extern __shared__ __align__(128) double ax_dyn[];
     uint64_t* bar = reinterpret_cast<uint64_t*>(ax_dyn + L::oBar);
-    const int64_t nef = E * (int64_t)nfields, stride = gridDim.x;
-    int64_t ef = blockIdx.x;
-    if (ef >= nef) return;
-    int64_t e = ef % E, f = ef / E;
+    const int64_t stride = gridDim.x;
+    int64_t e = blockIdx.x;
+    if (e >= E) return;
     if (threadIdx.x == 0) {
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(ax_smem_u32(bar)) : "memory");
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -617,11 +629,13 @@ k_axhelm_stage(int64_t E, int64_t n, const double* __restrict__ geo, double lamb
     __syncthreads();
     unsigned phase = 0;
 #pragma unroll 1
-    for (; ef < nef; ef += stride) {
-        int64_t ep = -1, fp = f;
-        if (ef + stride < nef) { ep = e + stride; while (ep >= E) { ep -= E; ++fp; } }
-        ax_stage_element<n1, HELM>(e, f, ep, fp, n, geo, lambda, u, w, phase);
-        e = ep; f = fp;
+    for (; e < E; e += stride) {
+        const int64_t en = (e + stride < E) ? e + stride : -1;
+#pragma unroll 1
+        for (int f = 0; f < nfields; ++f) {
+            const bool lastf = f == nfields - 1;
+            ax_stage_element<n1, HELM>(e, f, lastf ? en : e, lastf ? 0 : f + 1, n, geo, lambda, u, w, phase, f == 0, lastf ? en : -1);
+        }
         phase ^= 1u;
     }
 }

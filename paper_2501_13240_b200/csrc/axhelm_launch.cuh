@@ -110,9 +110,9 @@ static int launch_line(semb_mesh* h, const void* geo, int mode, double lambda, c
                                    * (int64_t)sizeof(ST) / 8;
     const int pf = (int)(((int64_t)8 << 20) / bytes_per_elem);
     // N = 9, fp64 stored factors, stand-alone Poisson / Helmholtz: the persistent kernel with TMA-staged factors
-    if constexpr (n1 == 10 && sizeof(ST) == 8 && GEO == SEMB_GEO_STORED) {
+    if constexpr ((n1 == 10 || n1 == 8) && sizeof(ST) == 8 && GEO == SEMB_GEO_STORED) {
         static const int stage_on = [] { const char* v = getenv("SEMB_AX_STAGE"); return v ? atoi(v) : SEMB_AX_STAGE; }();
-        if (stage_on && !scal && (mode == 0 || mode == 1) && ((uintptr_t)geo & 15) == 0) {
+        if (stage_on && !scal && (mode == 0 || mode == 1) && ((uintptr_t)geo & 15) == 0 && (n1 == 10 || nfields >= 2)) {       // N = 7: several fields only
             constexpr size_t smem = ax_stage_smem<n1>::bytes;
             auto kern = (mode & 1) ? k_axhelm_stage<n1, true> : k_axhelm_stage<n1, false>;
             static int per_sm[2][64] = {{0}};                      // per device: the opt-in shared-memory size is a per-device attribute
@@ -125,7 +125,7 @@ static int launch_line(semb_mesh* h, const void* geo, int mode, double lambda, c
                 SEMB_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, n1 * n1, smem));
                 nb_dev = nb > 0 ? nb : 1;
             }
-            const int64_t nef = h->E * (int64_t)nfields, cap = (int64_t)nb_dev * semb_sm_count();
+            const int64_t nef = h->E, cap = (int64_t)nb_dev * semb_sm_count();                  // one block walks over elements, all fields of each
             kern<<<(unsigned)(nef < cap ? nef : cap), n1 * n1, smem, s>>>(h->E, h->n, (const double*)geo, lambda, (const double*)u, (double*)w, nfields);
             h->launches += 1;
             SEMB_CUDA(h, cudaGetLastError());

@@ -156,11 +156,13 @@ def test_axhelm_batched_and_variable_coefficients(torch_cuda, cases, orc, name):
 
 
 def test_axhelm_order9_persistent_blocks(torch_cuda, semb, orc, xi_of):
-    """N = 9 stand-alone launches run k_axhelm_stage: persistent blocks (3 per SM on B200 = 444) that walk over the elements
-    blockIdx.x + i * gridDim.x with the factors of their next element in flight (TMA into shared memory).  9 x 8 x 7 = 504 elements
-    x 2 fields = 1008 block-elements: two full rounds and a ragged third one; then a single element (one block, no next element)."""
-    for dims, nf in (((9, 8, 7), 2), ((1, 1, 1), 1)):
-        m = I.box_mesh(*dims, 9, xi_of(9), deform=0.04)
+    """N = 9 stand-alone launches (and N = 7 launches on several fields) run k_axhelm_stage: persistent blocks (3 per SM on B200 = 444
+    at N = 9) that walk over the elements blockIdx.x + i * gridDim.x, apply each to all fields, with the factors of their next element in
+    flight (TMA into shared memory).  9 x 8 x 7 = 504 elements: a full round and a ragged one; then a single element (one block, no
+    next element)."""
+    for dims, nf, N in (((9, 8, 7), 2, 9), ((1, 1, 1), 1, 9), ((10, 10, 10), 3, 7), ((1, 1, 1), 2, 7)):
+        # N = 7: several fields only (888 resident blocks: 1000 elements = one full round and a ragged one, all 3 fields per element)
+        m = I.box_mesh(*dims, N, xi_of(N), deform=0.04)
         P, G = oracle_problem(orc, m), gpu_mesh(torch_cuda, semb, m)
         U = np.stack([I.uniform(I.seed_for(1, 40 + f), m.n) for f in range(nf)])
         for lam in (0.0, 1e4):
