@@ -39,8 +39,8 @@ static __constant__ double c_xi[SEMB_MAX_N + 1][SEMB_MAXN1], c_rho[SEMB_MAX_N + 
 #define SEMB_AX_RELOAD_N1 10
 #endif
 #ifndef SEMB_AX_FIELD_FAST
-#define SEMB_AX_FIELD_FAST 1          // measured on B200, 3 fields: N = 7 112 -> 141 GDOF/s (Helmholtz 100 -> 137), N = 5 106 -> 123, N = 3 101 -> 157
-#endif
+#define SEMB_AX_FIELD_FAST 1          // launches on several fields use the MODE | 8 instantiations; measured on B200, 3 fields:
+#endif                                // N = 7 112 -> 141 GDOF/s (Helmholtz 100 -> 137), N = 5 106 -> 123, N = 3 101 -> 157
 #ifndef SEMB_AX_SPLIT_N1
 #define SEMB_AX_SPLIT_N1 99          // off by default until measured
 #endif
@@ -279,16 +279,15 @@ k_axhelm_line(int64_t E, int64_t n, const void* __restrict__ geo_v, double lambd
         const int rq = c_perm[n1 - 1][0][tl], sq = c_perm[n1 - 1][1][tl];
         ra = rq % n1; rb = rq / n1; sa = sq % n1; sb = sq / n1;
     }
-#if SEMB_AX_FIELD_FAST
-    const int64_t e = ef / nfields, f = ef - e * nfields;           // the fields of an element in neighbouring blocks: its factors are read from DRAM once
-#else
-    const int64_t e = ef % E, f = ef / E;
-#endif
+    // MODE bit 3 (launches on several fields): the fields of an element sit in neighbouring blocks, so its factors cross DRAM once and
+    // the other fields read them from L2.  Single-field launches keep the instantiation without the bit: their code is unchanged.
+    constexpr bool FF = (MODE & 8) != 0;
+    const int64_t e = FF ? ef / nfields : ef % E, f = FF ? ef - (ef / nfields) * nfields : ef / E;
     // The element that a block pf_dist launches later will work on is pulled into L2 now: DRAM stays busy while
     // the resident blocks are in their compute phase, and that block's loads hit L2.
     if (pf_dist > 0 && tl == 0 && valid && e + pf_dist < E) {
         const int64_t ep = e + pf_dist;
-        if (STORED && (!SEMB_AX_FIELD_FAST || f == 0)) ax_prefetch_l2(geo + ep * 7 * (int64_t)Np, NG * Np);
+        if (STORED && (!FF || f == 0)) ax_prefetch_l2(geo + ep * 7 * (int64_t)Np, NG * Np);
         if (FUSE) {
             ax_prefetch_l2(pcg.zsrc + ep * Np, Np);
             if (pcg.dinv) ax_prefetch_l2(pcg.dinv + ep * Np, Np);

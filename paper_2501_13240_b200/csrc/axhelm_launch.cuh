@@ -134,8 +134,8 @@ static int launch_line(semb_mesh* h, const void* geo, int mode, double lambda, c
     }
 #define SEMB_AX_LAUNCH(M) k_axhelm_line<n1, M, MB, EPB, ST, GEO><<<grid, n1 * n1 * EPB, 0, s>>>(h->E, h->n, geo, lambda, lam0, lam1, u, w, scal, dot, pcg, pf, nfields)
     switch (mode) {
-        case 0: SEMB_AX_LAUNCH(0); break;
-        case 1: SEMB_AX_LAUNCH(1); break;
+        case 0: if (SEMB_AX_FIELD_FAST && nfields > 1) SEMB_AX_LAUNCH(8); else SEMB_AX_LAUNCH(0); break;
+        case 1: if (SEMB_AX_FIELD_FAST && nfields > 1) SEMB_AX_LAUNCH(9); else SEMB_AX_LAUNCH(1); break;
         case 3: if constexpr (GEO == SEMB_GEO_STORED) { SEMB_AX_LAUNCH(3); break; } else return semb_fail(h, SEMB_EINVAL, "axhelm: coefficient fields need stored fp64 factors");
         case 4: SEMB_AX_LAUNCH(4); break;
         case 5: SEMB_AX_LAUNCH(5); break;
