@@ -107,13 +107,21 @@ k_na_hist(int64_t n, int64_t stride, const double* __restrict__ v, int nbins, do
     const double scale = __ddiv_rn((double)nbins, __dsub_rn(hi, lo));
     __syncthreads();
     double mn = INFINITY, mx = -INFINITY;
-    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
-        const double a = v[l * stride];
-        if (!FROM_DATA) { mn = fmin(mn, a); mx = fmax(mx, a); }
-        const double s = __dmul_rn(__dsub_rn(a, lo), scale);
-        long long b = (s < 0.0) ? 0ll : (long long)floor(s);
-        if (b > nbins - 1) b = nbins - 1;
-        atomicAdd(&sh[b], 1u);
+    constexpr int U = 8;                                   // values per thread and pass, all loads issued before the first use (export.cu)
+    for (int64_t c0 = blockIdx.x * (int64_t)(256 * U); c0 < n; c0 += (int64_t)gridDim.x * (256 * U)) {
+        double a[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) { const int64_t l = c0 + u * 256 + threadIdx.x; a[u] = (l < n) ? v[l * stride] : 0.0; }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            if (c0 + u * 256 + threadIdx.x < n) {
+                if (!FROM_DATA) { mn = fmin(mn, a[u]); mx = fmax(mx, a[u]); }
+                const double s = __dmul_rn(__dsub_rn(a[u], lo), scale);
+                long long b = (s < 0.0) ? 0ll : (long long)floor(s);
+                if (b > nbins - 1) b = nbins - 1;
+                atomicAdd(&sh[b], 1u);
+            }
+        }
     }
     if (!FROM_DATA) {
         for (int o = 16; o > 0; o >>= 1) {
