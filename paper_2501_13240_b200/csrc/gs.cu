@@ -4,6 +4,10 @@
 // index and writes the sum back to every copy, so the result is deterministic.
 #include "semb_internal.h"
 
+#ifndef SEMB_GS_BATCH
+#define SEMB_GS_BATCH 1
+#endif
+
 // ST: storage type of the vector (double; float on the fp32 multigrid levels); sums in fp64
 template <typename ST>
 __global__ void k_gs(int64_t n_gs, int64_t n, const int32_t* __restrict__ off, const int32_t* __restrict__ ids,
@@ -13,6 +17,21 @@ __global__ void k_gs(int64_t n_gs, int64_t n, const int32_t* __restrict__ off, c
     if (g >= n_gs) return;
     ST* __restrict__ wf = w + blockIdx.y * n;
     const int32_t a = off[g], b = off[g + 1];
+#if SEMB_GS_BATCH
+    if (b - a <= 8) {                                      // member ids, then member values, as two batches of independent loads (as k_gs_hi)
+        int32_t id[8]; double v[8];
+#pragma unroll
+        for (int t = 0; t < 8; ++t) id[t] = (a + t < b) ? ids[a + t] : -1;
+#pragma unroll
+        for (int t = 0; t < 8; ++t) v[t] = (id[t] >= 0) ? semb_wide(wf[id[t]]) : 0.0;
+        double s = 0.0;
+#pragma unroll
+        for (int t = 0; t < 8; ++t) if (id[t] >= 0) s += v[t];                  // ascending local index: the order of the plain loop
+#pragma unroll
+        for (int t = 0; t < 8; ++t) if (id[t] >= 0) wf[id[t]] = (ST)s;
+        return;
+    }
+#endif
     double s = 0.0;
     for (int32_t t = a; t < b; ++t) s += semb_wide(wf[ids[t]]);
     for (int32_t t = a; t < b; ++t) wf[ids[t]] = (ST)s;
