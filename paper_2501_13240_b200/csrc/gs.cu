@@ -8,40 +8,46 @@
 #define SEMB_GS_BATCH 1
 #endif
 
-// ST: storage type of the vector (double; float on the fp32 multigrid levels); sums in fp64
+// ST: storage type of the vector (double; float on the fp32 multigrid levels); sums in fp64.  nfields vectors [nfields][n]: a
+// thread fetches the member ids of its class once and sums field after field.
 template <typename ST>
 __global__ void k_gs(int64_t n_gs, int64_t n, const int32_t* __restrict__ off, const int32_t* __restrict__ ids,
-                     ST* __restrict__ w)
+                     ST* __restrict__ w, int nfields)
 {
     const int64_t g = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (g >= n_gs) return;
-    ST* __restrict__ wf = w + blockIdx.y * n;
     const int32_t a = off[g], b = off[g + 1];
 #if SEMB_GS_BATCH
     if (b - a <= 8) {                                      // member ids, then member values, as two batches of independent loads (as k_gs_hi)
-        int32_t id[8]; double v[8];
+        int32_t id[8];
 #pragma unroll
         for (int t = 0; t < 8; ++t) id[t] = (a + t < b) ? ids[a + t] : -1;
+        for (int f = 0; f < nfields; ++f) {
+            ST* __restrict__ wf = w + f * n;
+            double v[8];
 #pragma unroll
-        for (int t = 0; t < 8; ++t) v[t] = (id[t] >= 0) ? semb_wide(wf[id[t]]) : 0.0;
-        double s = 0.0;
+            for (int t = 0; t < 8; ++t) v[t] = (id[t] >= 0) ? semb_wide(wf[id[t]]) : 0.0;
+            double s = 0.0;
 #pragma unroll
-        for (int t = 0; t < 8; ++t) if (id[t] >= 0) s += v[t];                  // ascending local index: the order of the plain loop
+            for (int t = 0; t < 8; ++t) if (id[t] >= 0) s += v[t];              // ascending local index: the order of the plain loop
 #pragma unroll
-        for (int t = 0; t < 8; ++t) if (id[t] >= 0) wf[id[t]] = (ST)s;
+            for (int t = 0; t < 8; ++t) if (id[t] >= 0) wf[id[t]] = (ST)s;
+        }
         return;
     }
 #endif
-    double s = 0.0;
-    for (int32_t t = a; t < b; ++t) s += semb_wide(wf[ids[t]]);
-    for (int32_t t = a; t < b; ++t) wf[ids[t]] = (ST)s;
+    for (int f = 0; f < nfields; ++f) {
+        ST* __restrict__ wf = w + f * n;
+        double s = 0.0;
+        for (int32_t t = a; t < b; ++t) s += semb_wide(wf[ids[t]]);
+        for (int32_t t = a; t < b; ++t) wf[ids[t]] = (ST)s;
+    }
 }
 
 int semb_gs_launch(semb_mesh* h, double* w, int nfields, cudaStream_t s)
 {
     if (h->n_gs == 0) return SEMB_OK;
-    dim3 grid((unsigned)((h->n_gs + 255) / 256), (unsigned)nfields);
-    k_gs<double><<<grid, 256, 0, s>>>(h->n_gs, h->n, h->gs_off, h->gs_ids, w);
+    k_gs<double><<<(unsigned)((h->n_gs + 255) / 256), 256, 0, s>>>(h->n_gs, h->n, h->gs_off, h->gs_ids, w, nfields);
     h->launches += 1;
     SEMB_CUDA(h, cudaGetLastError());
     return SEMB_OK;
@@ -49,7 +55,7 @@ int semb_gs_launch(semb_mesh* h, double* w, int nfields, cudaStream_t s)
 int semb_gs_launch_f(semb_mesh* h, float* w, cudaStream_t s)
 {
     if (h->n_gs == 0) return SEMB_OK;
-    k_gs<float><<<(unsigned)((h->n_gs + 255) / 256), 256, 0, s>>>(h->n_gs, h->n, h->gs_off, h->gs_ids, w);
+    k_gs<float><<<(unsigned)((h->n_gs + 255) / 256), 256, 0, s>>>(h->n_gs, h->n, h->gs_off, h->gs_ids, w, 1);
     h->launches += 1;
     SEMB_CUDA(h, cudaGetLastError());
     return SEMB_OK;
