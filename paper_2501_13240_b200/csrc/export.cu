@@ -5,6 +5,17 @@
 
 #include "semb_internal.h"
 
+// values per thread and pass, all loads issued before the first use (scalar field / three components); blocks per SM of the grids
+#ifndef MH_BPS
+#define MH_BPS 8
+#endif
+#ifndef MH_U1
+#define MH_U1 8
+#endif
+#ifndef MH_U3
+#define MH_U3 4
+#endif
+
 // |v| = sqrt(fma(vz, vz, fma(vy, vy, vx*vx)))  (reading R11: the fma form is part of the definition)
 __global__ void k_vmag(int64_t n, const double* __restrict__ vx, const double* __restrict__ vy,
                        const double* __restrict__ vz, double* __restrict__ out)
@@ -44,9 +55,12 @@ __global__ void __launch_bounds__(256)
 k_minmax(int64_t n, int64_t stride, const double* __restrict__ v, unsigned long long* __restrict__ mm)
 {
     double mn = INFINITY, mx = -INFINITY;
-    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
-        const double a = v[l * stride];
-        mn = fmin(mn, a); mx = fmax(mx, a);
+    for (int64_t c0 = blockIdx.x * (int64_t)(256 * MH_U1); c0 < n; c0 += (int64_t)gridDim.x * (256 * MH_U1)) {       // batched loads, as k_minmax_hist
+        double a[MH_U1];
+#pragma unroll
+        for (int u = 0; u < MH_U1; ++u) { const int64_t l = c0 + u * 256 + threadIdx.x; a[u] = (l < n) ? v[l * stride] : NAN; }
+#pragma unroll
+        for (int u = 0; u < MH_U1; ++u) if (c0 + u * 256 + threadIdx.x < n) { mn = fmin(mn, a[u]); mx = fmax(mx, a[u]); }
     }
     for (int o = 16; o > 0; o >>= 1) {
         mn = fmin(mn, __shfl_xor_sync(0xffffffffu, mn, o));
@@ -74,28 +88,29 @@ k_hist(int64_t n, int64_t stride, const double* __restrict__ v, const double* __
     if (range_dev) { lo = range_dev[0]; hi = range_dev[1]; }
     const double scale = __ddiv_rn((double)nbins, __dsub_rn(hi, lo));
     __syncthreads();
-    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
-        double a = v[l * stride];
-        if (NV == 3) { const double b = v1[l * stride], c = v2[l * stride]; a = sqrt(fma(c, c, fma(b, b, __dmul_rn(a, a)))); }
-        const double t = __dsub_rn(a, lo);
-        const double sc = __dmul_rn(t, scale);
-        long long b = (sc < 0.0) ? 0ll : (long long)floor(sc);
-        if (b > nbins - 1) b = nbins - 1;
-        atomicAdd(&sh[b], 1u);
+    constexpr int U = (NV == 3) ? MH_U3 : MH_U1;
+    for (int64_t c0 = blockIdx.x * (int64_t)(256 * U); c0 < n; c0 += (int64_t)gridDim.x * (256 * U)) {
+        double a[U], b3[NV == 3 ? U : 1], c3[NV == 3 ? U : 1];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int64_t l = c0 + u * 256 + threadIdx.x; const bool ok = l < n;
+            a[u] = ok ? v[l * stride] : 0.0;
+            if (NV == 3) { b3[u] = ok ? v1[l * stride] : 0.0; c3[u] = ok ? v2[l * stride] : 0.0; }
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) if (c0 + u * 256 + threadIdx.x < n) {
+            double x = a[u];
+            if (NV == 3) x = sqrt(fma(c3[NV == 3 ? u : 0], c3[NV == 3 ? u : 0], fma(b3[NV == 3 ? u : 0], b3[NV == 3 ? u : 0], __dmul_rn(x, x))));
+            const double sc = __dmul_rn(__dsub_rn(x, lo), scale);
+            long long b = (sc < 0.0) ? 0ll : (long long)floor(sc);
+            if (b > nbins - 1) b = nbins - 1;
+            atomicAdd(&sh[b], 1u);
+        }
     }
     __syncthreads();
     for (int b = threadIdx.x; b < nbins; b += blockDim.x) if (sh[b]) atomicAdd(&hist[b], (unsigned long long)sh[b]);
 }
 
-#ifndef MH_BPS
-#define MH_BPS 8           // blocks per SM of the consumer's grids
-#endif
-#ifndef MH_U1
-#define MH_U1 8
-#endif
-#ifndef MH_U3
-#define MH_U3 4
-#endif
 // One pass over the data when the range is known: min, max and the histogram together.  NV = 1: a scalar field; NV = 3: the
 // magnitude of a vector field computed on the fly, sqrt(fma(vz, vz, fma(vy, vy, vx vx))) (reading R11), never written to memory.
 template <int NV>
@@ -154,10 +169,18 @@ k_minmax_vmag(int64_t n, int64_t stride, const double* __restrict__ v0, const do
               unsigned long long* __restrict__ mm)
 {
     double mn = INFINITY, mx = -INFINITY;
-    for (int64_t l = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) {
-        const double a0 = v0[l * stride], b = v1[l * stride], c = v2[l * stride];
-        const double a = sqrt(fma(c, c, fma(b, b, __dmul_rn(a0, a0))));
-        mn = fmin(mn, a); mx = fmax(mx, a);
+    for (int64_t c0 = blockIdx.x * (int64_t)(256 * MH_U3); c0 < n; c0 += (int64_t)gridDim.x * (256 * MH_U3)) {
+        double a0[MH_U3], b[MH_U3], c[MH_U3];
+#pragma unroll
+        for (int u = 0; u < MH_U3; ++u) {
+            const int64_t l = c0 + u * 256 + threadIdx.x; const bool ok = l < n;
+            a0[u] = ok ? v0[l * stride] : 0.0; b[u] = ok ? v1[l * stride] : 0.0; c[u] = ok ? v2[l * stride] : 0.0;
+        }
+#pragma unroll
+        for (int u = 0; u < MH_U3; ++u) if (c0 + u * 256 + threadIdx.x < n) {
+            const double a = sqrt(fma(c[u], c[u], fma(b[u], b[u], __dmul_rn(a0[u], a0[u]))));
+            mn = fmin(mn, a); mx = fmax(mx, a);
+        }
     }
     for (int o = 16; o > 0; o >>= 1) {
         mn = fmin(mn, __shfl_xor_sync(0xffffffffu, mn, o));
